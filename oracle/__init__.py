@@ -1,0 +1,187 @@
+"""TEST INFRASTRUCTURE ONLY — ctypes face of the CPU oracle (oracle/wg_oracle.cpp).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product package
+``paper_2606_11871_b200`` never does, and this package never imports it.
+
+The oracle is built with plain ``g++ -O2`` (no -march, no intrinsics) into
+``oracle/libwg_oracle.so``.  All arrays are numpy, host memory.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "wg_oracle.cpp"
+_HDR = _HERE / "wg_oracle.h"
+_LIB = _HERE / "libwg_oracle.so"
+
+KIND_PROTECTED_RETURN = 0
+KIND_PROTECTED_FORWARD = 1
+KIND_FIXED_EDGE = 2
+KIND_UNSUPPORTED = 3
+KIND_PROFILE_EXCLUDED = 4
+KIND_FALLBACK = 5
+KIND_NO_SURFACE = 6
+KIND_COUNT = 7
+MODE_DETECT = 0
+MODE_ENFORCE = 1
+
+COUNTER_FIELDS = (
+    ["events_total", "events_empty", "events_unknown_site", "events_misrouted"]
+    + [f"events_by_kind_{k}" for k in range(7)]
+    + ["ret_checks", "fwd_checks", "ret_lanes", "fwd_lanes", "ret_viol", "fwd_viol",
+       "ret_viol_events", "fwd_viol_events", "blocked_lanes", "blocked_events",
+       "first_violation_key", "signed_lanes", "sign_skipped_events", "policy_digest", "last_mode"]
+)
+assert len(COUNTER_FIELDS) == 26
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle if the library is missing or older than its sources."""
+    newest = max(_SRC.stat().st_mtime, _HDR.stat().st_mtime)
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < newest:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        cmd = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-Wall", "-Wextra",
+               "-o", str(tmp), str(_SRC)]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(str(build()))
+        u64, u32, vp = C.c_uint64, C.c_uint32, C.c_void_p
+        L.wgo_siphash24.restype = u64
+        L.wgo_siphash24.argtypes = [u64, u64, C.c_char_p, C.c_size_t]
+        L.wgo_mac.restype = u64
+        L.wgo_mac.argtypes = [u64, u64, u32, u64, u64]
+        L.wgo_lane_ctx.restype = u64
+        L.wgo_lane_ctx.argtypes = [u64, u32]
+        L.wgo_validate_policy.restype = C.c_int
+        L.wgo_validate_policy.argtypes = [u32, vp, vp, vp]
+        L.wgo_create.restype = vp
+        L.wgo_create.argtypes = [u32, vp, vp, vp, u64, u64, u64]
+        L.wgo_destroy.restype = None
+        L.wgo_destroy.argtypes = [vp]
+        L.wgo_reset_counters.restype = None
+        L.wgo_reset_counters.argtypes = [vp]
+        L.wgo_set_binary_search.restype = None
+        L.wgo_set_binary_search.argtypes = [vp, C.c_int]
+        L.wgo_sign.restype = None
+        L.wgo_sign.argtypes = [vp, vp, vp, vp, u64]
+        L.wgo_check.restype = None
+        L.wgo_check.argtypes = [vp, vp, vp, vp, vp, u64, C.c_int]
+        L.wgo_read_counters.restype = None
+        L.wgo_read_counters.argtypes = [vp, vp, vp]
+        _lib = L
+    return _lib
+
+
+def siphash24(k0: int, k1: int, msg: bytes) -> int:
+    return int(lib().wgo_siphash24(k0, k1, msg, len(msg)))
+
+
+def mac(k0: int, k1: int, site_id: int, value: int, context_id: int) -> int:
+    return int(lib().wgo_mac(k0, k1, site_id, value, context_id))
+
+
+def lane_ctx(context_base: int, lane: int) -> int:
+    return int(lib().wgo_lane_ctx(context_base, lane))
+
+
+def _ptr(a: np.ndarray | None):
+    return None if a is None else a.ctypes.data
+
+
+def _c(a, dtype) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a), dtype=dtype)
+
+
+def validate_policy(kind, tgt_off, tgts) -> int:
+    kind = _c(kind, np.uint8)
+    tgt_off = _c(tgt_off, np.uint32)
+    tgts = _c(tgts, np.uint64)
+    assert tgt_off.size == kind.size + 1
+    return int(lib().wgo_validate_policy(kind.size, _ptr(kind), _ptr(tgt_off), _ptr(tgts)))
+
+
+def _hdr_bytes(hdr: np.ndarray) -> np.ndarray:
+    """Accept [n,2] (u)int64 rows (site | mask<<32, context_base) and return them as raw rows."""
+    h = np.ascontiguousarray(hdr)
+    assert h.ndim == 2 and h.shape[1] == 2 and h.dtype.itemsize == 8, (h.shape, h.dtype)
+    return h.view(np.uint64)
+
+
+class Oracle:
+    """One loaded policy + key + counters (the oracle's analogue of wg_engine)."""
+
+    def __init__(self, kind, tgt_off, tgts, k0: int, k1: int, policy_digest: int = 0):
+        self.kind = _c(kind, np.uint8)
+        self.tgt_off = _c(tgt_off, np.uint32)
+        self.tgts = _c(tgts, np.uint64)
+        assert self.tgt_off.size == self.kind.size + 1
+        self.n_sites = int(self.kind.size)
+        self._h = lib().wgo_create(self.n_sites, _ptr(self.kind), _ptr(self.tgt_off), _ptr(self.tgts),
+                                   k0, k1, policy_digest)
+        if not self._h:
+            raise ValueError("oracle rejected the policy (wgo_validate_policy = %d)"
+                             % validate_policy(self.kind, self.tgt_off, self.tgts))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().wgo_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # interpreter shutdown
+            pass
+
+    def reset_counters(self):
+        lib().wgo_reset_counters(self._h)
+
+    def set_binary_search(self, on: bool):
+        lib().wgo_set_binary_search(self._h, int(bool(on)))
+
+    def sign(self, hdr: np.ndarray, val: np.ndarray) -> np.ndarray:
+        h = _hdr_bytes(hdr)
+        n = h.shape[0]
+        v = np.ascontiguousarray(val).view(np.uint64).reshape(n, 32)
+        tag = np.empty((n, 32), dtype=np.uint64)
+        lib().wgo_sign(self._h, _ptr(h), _ptr(v), _ptr(tag), n)
+        return tag
+
+    def check(self, hdr: np.ndarray, val: np.ndarray, tag: np.ndarray | None, mode: int) -> np.ndarray:
+        """Returns [n,2] uint32: (viol_mask, allow_mask).  tag=None is the forward entry point."""
+        h = _hdr_bytes(hdr)
+        n = h.shape[0]
+        v = np.ascontiguousarray(val).view(np.uint64).reshape(n, 32)
+        t = None if tag is None else np.ascontiguousarray(tag).view(np.uint64).reshape(n, 32)
+        out = np.empty((n, 2), dtype=np.uint32)
+        lib().wgo_check(self._h, _ptr(h), _ptr(v), _ptr(t), _ptr(out), n, int(mode))
+        return out
+
+    def verify(self, hdr, val, tag, mode):
+        assert tag is not None
+        return self.check(hdr, val, tag, mode)
+
+    def check_forward(self, hdr, val, mode):
+        return self.check(hdr, val, None, mode)
+
+    def read_counters(self, per_site: bool = True):
+        g = np.zeros(26, dtype=np.uint64)
+        s = np.zeros((self.n_sites, 4), dtype=np.uint64) if per_site else None
+        lib().wgo_read_counters(self._h, _ptr(g), _ptr(s))
+        return {k: int(v) for k, v in zip(COUNTER_FIELDS, g)}, s

@@ -1,0 +1,298 @@
+// wg_oracle.cpp — TEST INFRASTRUCTURE ONLY (see wg_oracle.h).
+//
+// Plain single-threaded C++17.  No intrinsics, no blocking, no fusion, no
+// reordering: SipHash-2-4 lane by lane, linear-scan set membership, counters
+// updated event by event in stream order.  Written so that a reader can check
+// each function against the cited passage by eye.
+
+#include "wg_oracle.h"
+
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+inline uint64_t rotl64(uint64_t x, unsigned b) { return (x << b) | (x >> (64u - b)); }
+
+// One SipRound (Aumasson & Bernstein, "SipHash: a fast short-input PRF", §2.1
+// figure of the ARX network; restated in SURVEY.md §8(c)).
+inline void sipround(uint64_t& v0, uint64_t& v1, uint64_t& v2, uint64_t& v3) {
+  v0 += v1;
+  v1 = rotl64(v1, 13);
+  v1 ^= v0;
+  v0 = rotl64(v0, 32);
+  v2 += v3;
+  v3 = rotl64(v3, 16);
+  v3 ^= v2;
+  v0 += v3;
+  v3 = rotl64(v3, 21);
+  v3 ^= v0;
+  v2 += v1;
+  v1 = rotl64(v1, 17);
+  v1 ^= v2;
+  v2 = rotl64(v2, 32);
+}
+
+inline uint64_t load_le64(const uint8_t* p) {
+  uint64_t w = 0;
+  for (int i = 0; i < 8; ++i) w |= static_cast<uint64_t>(p[i]) << (8 * i);
+  return w;
+}
+
+inline void store_le64(uint8_t* p, uint64_t w) {
+  for (int i = 0; i < 8; ++i) p[i] = static_cast<uint8_t>(w >> (8 * i));
+}
+
+inline unsigned popcount32(uint32_t x) {
+  unsigned c = 0;
+  for (int i = 0; i < 32; ++i) c += (x >> i) & 1u;
+  return c;
+}
+
+inline unsigned lowest_set_lane(uint32_t x) {  // x != 0
+  unsigned i = 0;
+  while (((x >> i) & 1u) == 0) ++i;
+  return i;
+}
+
+}  // namespace
+
+struct wgo_engine {
+  uint32_t n_sites = 0;
+  std::vector<uint8_t> kind;
+  std::vector<uint32_t> tgt_off;
+  std::vector<uint64_t> tgts;
+  uint64_t k0 = 0, k1 = 0;
+  uint64_t seq = 0;  // running event index over check calls (R12)
+  int use_binary_search = 0;
+  wgo_counters g;
+  std::vector<wgo_site_counters> site;
+};
+
+extern "C" {
+
+// SipHash-c-d with c = 2 compression rounds and d = 4 finalisation rounds,
+// 64-bit output.  Initialisation constants are the ASCII of
+// "somepseudorandomlygeneratedbytes"; the last word carries the message
+// length mod 256 in its top byte.
+uint64_t wgo_siphash24(uint64_t k0, uint64_t k1, const uint8_t* msg, size_t len) {
+  uint64_t v0 = k0 ^ 0x736f6d6570736575ULL;
+  uint64_t v1 = k1 ^ 0x646f72616e646f6dULL;
+  uint64_t v2 = k0 ^ 0x6c7967656e657261ULL;
+  uint64_t v3 = k1 ^ 0x7465646279746573ULL;
+
+  const size_t full_words = len / 8;
+  for (size_t i = 0; i < full_words; ++i) {
+    const uint64_t m = load_le64(msg + 8 * i);
+    v3 ^= m;
+    sipround(v0, v1, v2, v3);
+    sipround(v0, v1, v2, v3);
+    v0 ^= m;
+  }
+
+  uint64_t last = static_cast<uint64_t>(len & 0xff) << 56;
+  const size_t tail = len % 8;
+  for (size_t i = 0; i < tail; ++i) last |= static_cast<uint64_t>(msg[8 * full_words + i]) << (8 * i);
+  v3 ^= last;
+  sipround(v0, v1, v2, v3);
+  sipround(v0, v1, v2, v3);
+  v0 ^= last;
+
+  v2 ^= 0xff;
+  sipround(v0, v1, v2, v3);
+  sipround(v0, v1, v2, v3);
+  sipround(v0, v1, v2, v3);
+  sipround(v0, v1, v2, v3);
+  return v0 ^ v1 ^ v2 ^ v3;
+}
+
+// Backward token (binds expected return, callsite
+// identifier, depth / thread slot / epoch and key material).  DESIGN.md R2-R4:
+// message = LE64(zero-extended site_id) || LE64(continuation) || LE64(context_id).
+uint64_t wgo_mac(uint64_t k0, uint64_t k1, uint32_t site_id, uint64_t value, uint64_t context_id) {
+  uint8_t msg[24];
+  store_le64(msg + 0, static_cast<uint64_t>(site_id));
+  store_le64(msg + 8, value);
+  store_le64(msg + 16, context_id);
+  return wgo_siphash24(k0, k1, msg, sizeof msg);
+}
+
+// DESIGN.md R2: the caller's context_base has its low five bits reserved for
+// the lane, so a lane's token cannot be replayed in another lane (the paper's
+// per-thread-slot binding).
+uint64_t wgo_lane_ctx(uint64_t context_base, uint32_t lane) {
+  return (context_base & ~static_cast<uint64_t>(31)) | static_cast<uint64_t>(lane & 31u);
+}
+
+// Load-time policy validation.  "A binding mismatch becomes an abort ... rather
+// than a wider allowed target set"; "missing ... target evidence
+// receive[s] an unsupported outcome".  DESIGN.md R16.
+int wgo_validate_policy(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off,
+                        const uint64_t* tgts) {
+  for (uint32_t s = 0; s < n_sites; ++s)
+    if (kind[s] >= WGO_KIND_COUNT) return WGO_POLICY_BAD_KIND;
+  if (tgt_off[0] != 0) return WGO_POLICY_BAD_OFFSETS;
+  for (uint32_t s = 0; s < n_sites; ++s)
+    if (tgt_off[s + 1] < tgt_off[s]) return WGO_POLICY_BAD_OFFSETS;
+  for (uint32_t s = 0; s < n_sites; ++s) {
+    const uint32_t lo = tgt_off[s], hi = tgt_off[s + 1];
+    if (kind[s] == WGO_PROTECTED_FORWARD) {
+      if (hi == lo) return WGO_POLICY_EMPTY_FORWARD;
+    } else if (hi != lo) {
+      return WGO_POLICY_STRAY_SET;
+    }
+    for (uint32_t i = lo; i + 1 < hi; ++i)
+      if (!(tgts[i] < tgts[i + 1])) return WGO_POLICY_UNSORTED_SET;
+  }
+  return WGO_POLICY_OK;
+}
+
+void wgo_reset_counters(wgo_engine* e) {
+  const uint64_t digest = e->g.policy_digest;  // echoed policy binding, not a counter
+  std::memset(&e->g, 0, sizeof e->g);
+  e->g.policy_digest = digest;
+  e->g.first_violation_key = ~static_cast<uint64_t>(0);
+  std::fill(e->site.begin(), e->site.end(), wgo_site_counters{0, 0, 0, 0});
+  e->seq = 0;
+}
+
+wgo_engine* wgo_create(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off,
+                       const uint64_t* tgts, uint64_t k0, uint64_t k1, uint64_t policy_digest) {
+  if (wgo_validate_policy(n_sites, kind, tgt_off, tgts) != WGO_POLICY_OK) return nullptr;
+  wgo_engine* e = new (std::nothrow) wgo_engine;
+  if (!e) return nullptr;
+  e->n_sites = n_sites;
+  e->kind.assign(kind, kind + n_sites);
+  e->tgt_off.assign(tgt_off, tgt_off + n_sites + 1);
+  e->tgts.assign(tgts, tgts + tgt_off[n_sites]);
+  e->k0 = k0;
+  e->k1 = k1;
+  e->site.resize(n_sites);
+  e->g.policy_digest = policy_digest;
+  wgo_reset_counters(e);
+  return e;
+}
+
+void wgo_destroy(wgo_engine* e) { delete e; }
+
+void wgo_set_binary_search(wgo_engine* e, int use_binary_search) {
+  e->use_binary_search = use_binary_search;
+}
+
+// Backward push (PAPER.md:228 push(site, expected_ret, guard); 248 "writes the
+// authenticated record").  Guard-false lanes are no-ops: tag 0.
+void wgo_sign(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, uint64_t* tag,
+              uint64_t n) {
+  for (uint64_t ev = 0; ev < n; ++ev) {
+    const uint32_t s = hdr[ev].site_id;
+    const uint32_t a = hdr[ev].active_mask;
+    const bool protected_return = s < e->n_sites && e->kind[s] == WGO_PROTECTED_RETURN;
+    for (uint32_t lane = 0; lane < 32; ++lane) {
+      const bool active = (a >> lane) & 1u;
+      uint64_t t = 0;
+      if (protected_return && active)
+        t = wgo_mac(e->k0, e->k1, s, val[ev * 32 + lane], wgo_lane_ctx(hdr[ev].context_base, lane));
+      tag[ev * 32 + lane] = t;
+    }
+    if (protected_return)
+      e->g.signed_lanes += popcount32(a);
+    else
+      e->g.sign_skipped_events += 1;
+  }
+}
+
+static bool member_linear(const wgo_engine* e, uint32_t s, uint64_t target) {
+  for (uint32_t i = e->tgt_off[s]; i < e->tgt_off[s + 1]; ++i)
+    if (e->tgts[i] == target) return true;  // exact 64-bit equality, R8
+  return false;
+}
+
+static bool member_bsearch(const wgo_engine* e, uint32_t s, uint64_t target) {
+  return std::binary_search(e->tgts.begin() + e->tgt_off[s], e->tgts.begin() + e->tgt_off[s + 1],
+                            target);
+}
+
+// check_ret(site, observed_ret, guard) and the forward check (site, target,
+// guard); verdict rules PAPER.md:264; accounting
+// PAPER.md:113, 127, 224.  Follows SURVEY.md §8(c) "CHECK" line by line.
+void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, const uint64_t* tag,
+               wgo_verdict* out, uint64_t n, int mode) {
+  for (uint64_t ev = 0; ev < n; ++ev) {
+    const uint64_t seq = e->seq++;
+    const uint32_t s = hdr[ev].site_id;
+    const uint32_t a = hdr[ev].active_mask;
+    uint32_t viol = 0;
+    e->g.events_total += 1;
+
+    if (s >= e->n_sites) {
+      // unknown site: fail closed, outside every denominator (R13)
+      viol = a;
+      e->g.events_unknown_site += 1;
+    } else {
+      const uint8_t k = e->kind[s];
+      e->g.events_by_kind[k] += 1;
+      e->site[s].events += 1;
+      if (a == 0) {
+        // fully predicated-off instruction: no helper ran (R22)
+        e->g.events_empty += 1;
+      } else if (k == WGO_PROTECTED_RETURN && tag != nullptr) {
+        for (uint32_t lane = 0; lane < 32; ++lane) {
+          if (!((a >> lane) & 1u)) continue;  // inactive lanes are never judged
+          const uint64_t expect =
+              wgo_mac(e->k0, e->k1, s, val[ev * 32 + lane], wgo_lane_ctx(hdr[ev].context_base, lane));
+          if (expect != tag[ev * 32 + lane]) viol |= (1u << lane);
+        }
+        e->g.ret_checks += 1;
+        e->g.ret_lanes += popcount32(a);
+        e->g.ret_viol += popcount32(viol);
+        e->g.ret_viol_events += (viol != 0);
+        e->site[s].lanes_checked += popcount32(a);
+        e->site[s].lanes_violation += popcount32(viol);
+      } else if (k == WGO_PROTECTED_RETURN) {
+        // handed to the forward entry point: no tag, cannot authenticate (R14)
+        viol = a;
+        e->g.events_misrouted += 1;
+      } else if (k == WGO_PROTECTED_FORWARD) {
+        for (uint32_t lane = 0; lane < 32; ++lane) {
+          if (!((a >> lane) & 1u)) continue;
+          const uint64_t target = val[ev * 32 + lane];
+          const bool ok = e->use_binary_search ? member_bsearch(e, s, target) : member_linear(e, s, target);
+          if (!ok) viol |= (1u << lane);
+        }
+        e->g.fwd_checks += 1;
+        e->g.fwd_lanes += popcount32(a);
+        e->g.fwd_viol += popcount32(viol);
+        e->g.fwd_viol_events += (viol != 0);
+        e->site[s].lanes_checked += popcount32(a);
+        e->site[s].lanes_violation += popcount32(viol);
+      } else {
+        // fixed-edge / unsupported / profile-excluded / fallback / no-surface:
+        // counted above, never judged (R17)
+      }
+    }
+
+    const uint32_t allow = (mode == WGO_ENFORCE) ? (a & ~viol) : a;
+    if (mode == WGO_ENFORCE && viol != 0) {
+      e->g.blocked_lanes += popcount32(viol);
+      e->g.blocked_events += 1;
+      if (s < e->n_sites) e->site[s].lanes_blocked += popcount32(viol);
+    }
+    if (viol != 0) {
+      const uint64_t key = (seq << 5) | lowest_set_lane(viol);
+      if (key < e->g.first_violation_key) e->g.first_violation_key = key;
+    }
+    out[ev].viol_mask = viol;
+    out[ev].allow_mask = allow;
+  }
+  if (n != 0) e->g.last_mode = static_cast<uint64_t>(mode);
+}
+
+void wgo_read_counters(const wgo_engine* e, wgo_counters* global, wgo_site_counters* per_site) {
+  if (global) *global = e->g;
+  if (per_site)
+    for (uint32_t s = 0; s < e->n_sites; ++s) per_site[s] = e->site[s];
+}
+
+}  // extern "C"

@@ -1,0 +1,129 @@
+/* wg_oracle.h — TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, single-threaded CPU oracle for the WarpGuard protected-site CFI
+ * check path (arxiv/paper_2606_11871).  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load this library.
+ * The product (paper_2606_11871_b200/, include/warpguard.h) shares no code,
+ * header, table or constant with it; the layouts below are re-declared here on
+ * purpose.
+ *
+ * Everything the oracle computes is an integer function of (policy, key,
+ * events, mode, call order), so there is exactly one correct result and the
+ * CUDA path must match it bit for bit (SURVEY.md §8(c) "Nature of the result").
+ *
+ * Passages followed (PAPER.md line numbers):
+ *   backward push / check_ret ..... 162-168 (§4.4), 228 (§5.3), 242-248 (§5.5), 258 (§5.6)
+ *   forward membership ............ 172-180 (§4.5), 250-252 (§5.5)
+ *   lane granularity, guards ...... 190 (§4.7), 230 (§5.3)
+ *   detect / enforce .............. 196-198 (§4.8), 264-266 (§5.7)
+ *   accounting .................... 113 (§3), 127 (§4.1), 145-158 (Table 2), 224 (§5.2)
+ *   MAC primitive ................. the paper's formula is lost in extraction
+ *                                   (PAPER.md:164-166, 244-246); reading R1
+ *                                   takes SipHash-2-4 as BASELINE.json states.
+ *
+ * Pins (tests/test_oracle_*.py): SipHash known answers and an OpenSSL
+ * EVP_MAC("SIPHASH") cross-check; brute-force Python-set membership; the
+ * sign/verify, tamper, replay, guard, mode and accounting invariants.
+ * No function in this file is "parity unpinned".
+ */
+#ifndef WG_ORACLE_H
+#define WG_ORACLE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wgo_engine wgo_engine;
+
+/* Site outcome kinds, PAPER.md:145-154 (Table 2) with "protected" split by edge
+ * direction as BASELINE.json's policy table does. */
+enum {
+  WGO_PROTECTED_RETURN = 0,
+  WGO_PROTECTED_FORWARD = 1,
+  WGO_FIXED_EDGE = 2,
+  WGO_UNSUPPORTED = 3,
+  WGO_PROFILE_EXCLUDED = 4,
+  WGO_FALLBACK = 5,
+  WGO_NO_SURFACE = 6,
+  WGO_KIND_COUNT = 7
+};
+enum { WGO_DETECT = 0, WGO_ENFORCE = 1 };
+
+/* policy validation result */
+enum {
+  WGO_POLICY_OK = 0,
+  WGO_POLICY_BAD_KIND = 1,       /* kind >= 7                                        */
+  WGO_POLICY_BAD_OFFSETS = 2,    /* tgt_off[0] != 0 or decreasing                    */
+  WGO_POLICY_UNSORTED_SET = 3,   /* a set not strictly ascending                     */
+  WGO_POLICY_EMPTY_FORWARD = 4,  /* protected-forward site with no target evidence   */
+  WGO_POLICY_STRAY_SET = 5       /* a non-forward site that owns targets             */
+};
+
+typedef struct {
+  uint32_t site_id;
+  uint32_t active_mask;
+  uint64_t context_base;
+} wgo_event_hdr; /* 16 bytes */
+
+typedef struct {
+  uint32_t viol_mask;
+  uint32_t allow_mask;
+} wgo_verdict; /* 8 bytes */
+
+typedef struct {
+  uint64_t events_total, events_empty, events_unknown_site, events_misrouted;
+  uint64_t events_by_kind[7];
+  uint64_t ret_checks, fwd_checks;
+  uint64_t ret_lanes, fwd_lanes;
+  uint64_t ret_viol, fwd_viol;
+  uint64_t ret_viol_events, fwd_viol_events;
+  uint64_t blocked_lanes, blocked_events;
+  uint64_t first_violation_key;
+  uint64_t signed_lanes, sign_skipped_events;
+  uint64_t policy_digest, last_mode;
+} wgo_counters; /* 26 x u64 */
+
+typedef struct {
+  uint64_t events, lanes_checked, lanes_violation, lanes_blocked;
+} wgo_site_counters;
+
+/* SipHash-2-4, 64-bit output, arbitrary length — the plain definition. */
+uint64_t wgo_siphash24(uint64_t k0, uint64_t k1, const uint8_t* msg, size_t len);
+
+/* token = SipHash-2-4_key( LE64(site_id) || LE64(value) || LE64(context_id) ) */
+uint64_t wgo_mac(uint64_t k0, uint64_t k1, uint32_t site_id, uint64_t value, uint64_t context_id);
+
+/* context id of one lane: low five bits of context_base replaced by the lane */
+uint64_t wgo_lane_ctx(uint64_t context_base, uint32_t lane);
+
+int wgo_validate_policy(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off,
+                        const uint64_t* tgts);
+
+/* NULL when the policy is rejected (nothing is loaded). Arrays are copied. */
+wgo_engine* wgo_create(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off,
+                       const uint64_t* tgts, uint64_t k0, uint64_t k1, uint64_t policy_digest);
+void wgo_destroy(wgo_engine* e);
+void wgo_reset_counters(wgo_engine* e);
+
+/* use_binary_search != 0 switches membership to std::binary_search (config 5
+ * timing only; tests prove both agree).  Default is the linear scan. */
+void wgo_set_binary_search(wgo_engine* e, int use_binary_search);
+
+void wgo_sign(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val /*[n][32]*/,
+              uint64_t* tag /*[n][32] out*/, uint64_t n);
+
+/* tag == NULL is the forward entry point (wg_check_forward); non-NULL is
+ * wg_verify_continuations. */
+void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, const uint64_t* tag,
+               wgo_verdict* out, uint64_t n, int mode);
+
+void wgo_read_counters(const wgo_engine* e, wgo_counters* global,
+                       wgo_site_counters* per_site /* [n_sites] or NULL */);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
