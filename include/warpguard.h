@@ -1,0 +1,174 @@
+/* warpguard.h — C ABI of the B200-native protected-site CFI check engine (libwarpguard.so).
+ *
+ * What it computes: the runtime check path of WarpGuard (arxiv/paper_2606_11871), re-cast from an inline
+ * helper called by every instrumented SASS CALL / RET / indirect branch into a batched engine over a stream
+ * of per-warp check events.  The three helper calls of PAPER.md:228 (§5.3)
+ *     push(site, expected_ret, guard)   check_ret(site, observed_ret, guard)   forward check (site, target, guard)
+ * become wg_sign_continuations, wg_verify_continuations and wg_check_forward; `guard` is the event's 32-bit
+ * active-lane mask ("lanes with P0=false ... must not be checked").
+ *
+ * Passages: backward token sign / verify PAPER.md:162-168 (§4.4), 242-248 (§5.5), 258 (§5.6); forward
+ * membership PAPER.md:172-180 (§4.5), 250-252 (§5.5); lane granularity PAPER.md:190 (§4.7); detect / enforce and
+ * fail closed PAPER.md:196-198 (§4.8), 264-266 (§5.7); outcome kinds and the protected denominator
+ * PAPER.md:113 (§3), 127 (§4.1), 145-158 (Table 2), 224 (§5.2).  Where the paper is silent or garbled (the MAC
+ * formula is lost at PAPER.md:164-166 and 244-246) the readings R1-R25 of DESIGN.md §2 apply: the token is
+ * SipHash-2-4 under the 128-bit backend key over the 24-byte message
+ *     LE64(zero-extended site_id) || LE64(continuation) || LE64((context_base & ~31) | lane).
+ *
+ * General rules
+ *  - Every call returns a wg_status; nothing throws or aborts.  Data-dependent conditions (unknown site,
+ *    tampered tag, out-of-set target) are never errors: they are verdicts and counters.
+ *  - `d_*` arguments are caller-owned DEVICE pointers on the engine's device, 16-byte aligned, valid until
+ *    `cuda_stream` has executed the call's work; the engine neither frees nor keeps them.  `h_*` / `desc`
+ *    arguments are HOST pointers.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *  - Policy tables, the key and all counters live in engine-owned device memory ("backend-private state",
+ *    PAPER.md:256 §5.6; Table A3): the caller never gets their addresses.
+ *  - Sign / verify / check enqueue work on `cuda_stream` and return without waiting.  Counters accumulate across
+ *    calls until wg_reset_counters or the next successful wg_load_policy.
+ *  - There is no CPU fallback: without a CUDA device every call that needs one returns WG_ERR_CUDA.
+ */
+#ifndef WARPGUARD_H
+#define WARPGUARD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wg_engine wg_engine; /* opaque; owns device tables, key, counters */
+
+typedef enum {
+  WG_OK = 0,
+  WG_ERR_INVALID_ARG = 1, /* NULL / misaligned pointer, bad mode, bad device                         */
+  WG_ERR_BAD_POLICY = 2,  /* policy rejected at load; nothing was loaded                             */
+  WG_ERR_NO_POLICY = 3,   /* engine handle is NULL or holds no policy                                */
+  WG_ERR_CUDA = 4,        /* a CUDA runtime call failed (wg_last_cuda_error gives the code)          */
+  WG_ERR_OOM = 5          /* host or device allocation failed                                        */
+} wg_status;
+
+/* Site outcome kinds: PAPER.md:145-154 (Table 2), "protected" split by edge direction. */
+typedef enum {
+  WG_KIND_PROTECTED_RETURN = 0,
+  WG_KIND_PROTECTED_FORWARD = 1,
+  WG_KIND_FIXED_EDGE = 2,
+  WG_KIND_UNSUPPORTED = 3,
+  WG_KIND_PROFILE_EXCLUDED = 4,
+  WG_KIND_FALLBACK = 5,
+  WG_KIND_NO_SURFACE = 6,
+  WG_KIND_COUNT = 7
+} wg_kind;
+
+/* PAPER.md:264 (§5.7): detect-only records and continues; enforce blocks the violating transfer. */
+typedef enum { WG_MODE_DETECT = 0, WG_MODE_ENFORCE = 1 } wg_mode;
+
+/* Policy description — HOST pointers, copied by wg_load_policy; the caller keeps ownership.
+ * Forward record of PAPER.md:250 {site_id, token, target_count, allowed_targets} as CSR. */
+typedef struct {
+  uint32_t n_sites;        /* site_id in events is a dense index 0 .. n_sites-1 (R5)      */
+  const uint8_t* kind;     /* [n_sites] wg_kind                                                      */
+  const uint32_t* tgt_off; /* [n_sites + 1] CSR offsets, tgt_off[0] == 0, non-decreasing             */
+  const uint64_t* tgts;    /* [tgt_off[n_sites]] per site strictly ascending; may be NULL if empty   */
+  uint64_t key[2];         /* k0, k1 = little-endian 64-bit halves of the 128-bit backend key (R20)  */
+  uint64_t policy_digest;  /* stored and echoed by wg_read_counters; not checked (R25)               */
+} wg_policy_desc;
+
+/* One per-warp check event (16 bytes, little-endian).  context_base packs the caller's epoch / depth /
+ * warp slot; its low five bits are reserved: the engine binds lane l to (context_base & ~31) | l (R2). */
+typedef struct {
+  uint32_t site_id;
+  uint32_t active_mask;
+  uint64_t context_base;
+} wg_event_hdr;
+
+/* Per-event result.  viol_mask: active lanes that failed their check.  allow_mask: lanes whose transfer is
+ * released — the active mask in detect mode, active & ~viol in enforce mode. */
+typedef struct {
+  uint32_t viol_mask;
+  uint32_t allow_mask;
+} wg_verdict;
+
+/* Global outcome counters, all u64 (26 words).  Only non-empty events at protected sites enter
+ * ret_checks / fwd_checks (events) and ret_lanes / fwd_lanes (lane verdicts): the protected denominator
+ * of PAPER.md:113, 127, 224.  Names follow the paper's ret_viol / fwd_viol counters (Table 3, Table 5). */
+typedef struct {
+  uint64_t events_total, events_empty, events_unknown_site, events_misrouted;
+  uint64_t events_by_kind[7];
+  uint64_t ret_checks, fwd_checks;
+  uint64_t ret_lanes, fwd_lanes;
+  uint64_t ret_viol, fwd_viol; /* violating lanes */
+  uint64_t ret_viol_events, fwd_viol_events;
+  uint64_t blocked_lanes, blocked_events; /* enforce mode only */
+  uint64_t first_violation_key;           /* min((seq << 5) | lane) over violations; UINT64_MAX if none (R12) */
+  uint64_t signed_lanes, sign_skipped_events;
+  uint64_t policy_digest, last_mode;
+} wg_counters;
+
+typedef struct {
+  uint64_t events, lanes_checked, lanes_violation, lanes_blocked;
+} wg_site_counters;
+
+/* Load (or replace) the policy, PAPER.md:186 (§4.6), 260 (§5.6): validated BEFORE any state is touched; on
+ * failure nothing is loaded and an existing engine keeps its previous policy.
+ *   eng     in: address of NULL (create) or of an existing handle (replace); out: the handle.
+ *   device  CUDA device ordinal.
+ * WG_ERR_BAD_POLICY for: kind >= 7; tgt_off[0] != 0 or decreasing; a set not strictly ascending; a
+ * protected-forward site with an empty set; a non-forward site owning targets (R16).
+ * A successful load zeroes all counters and the event sequence number. */
+wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc);
+
+/* Backward push: d_tag[e][l] = token(site, d_val[e][l], lane context) for every active
+ * lane of every event whose site is protected-return, 0 for every other lane (R10).
+ *   d_hdr [n] wg_event_hdr, d_val [n][32] u64 in, d_tag [n][32] u64 out.  n == 0 is a no-op. */
+wg_status wg_sign_continuations(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                                uint64_t* d_tag, uint64_t n, void* cuda_stream);
+
+/* Backward check_ret over a stream that may interleave events of ANY site kind: the engine
+ * dispatches on the policy's kind (protected-return: recompute the token over the observed continuation and
+ * compare with d_tag; protected-forward: membership, tag row ignored; other kinds: counted only, R17).
+ *   d_out [n] wg_verdict out.  mode: WG_MODE_DETECT or WG_MODE_ENFORCE. */
+wg_status wg_verify_continuations(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                                  const uint64_t* d_tag, wg_verdict* d_out, uint64_t n, wg_mode mode,
+                                  void* cuda_stream);
+
+/* Forward check: observed target must be a member of the site's set (exact
+ * 64-bit equality, R8).  A protected-return event given to this entry point has no tag and fails closed (R14). */
+wg_status wg_check_forward(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                           wg_verdict* d_out, uint64_t n, wg_mode mode, void* cuda_stream);
+
+/* Synchronises `cuda_stream`, then copies the counters to HOST memory (diagnostic only,
+ * they never feed a verdict).  h_per_site may be NULL, else [n_sites]. */
+wg_status wg_read_counters(wg_engine* eng, wg_counters* h_global, wg_site_counters* h_per_site,
+                           void* cuda_stream);
+
+/* ---- lifecycle helpers beside the five ---- */
+wg_status wg_reset_counters(wg_engine* eng, void* cuda_stream); /* also restarts the event sequence (R12) */
+void wg_destroy(wg_engine* eng);                                /* NULL is allowed */
+const char* wg_strerror(wg_status s);
+int wg_last_cuda_error(const wg_engine* eng); /* cudaError_t of the last WG_ERR_CUDA, 0 if none */
+
+/* ---- HOST-buffer entry points (end-to-end path) ----
+ * Same semantics as the calls above but every array is in HOST memory (pinned memory gives full PCIe speed,
+ * pageable works).  The engine streams the events through its own double-buffered device staging in chunks,
+ * runs the same kernels, and returns after the results are back in h_tag / h_out (synchronous). */
+wg_status wg_sign_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                                     uint64_t* h_tag, uint64_t n);
+wg_status wg_verify_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                                       const uint64_t* h_tag, wg_verdict* h_out, uint64_t n, wg_mode mode);
+wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                                wg_verdict* h_out, uint64_t n, wg_mode mode);
+
+/* ---- measurement helpers (no part of the check path) ----
+ * wg_probe_int_pipe: runs a register-only integer micro-benchmark on `device` and returns, in *ops_per_s, the
+ * achieved 32-bit integer lane-operations per second (DESIGN.md §6 "integer-pipe peak").
+ *   mix: 0 = IADD3 only, 1 = LOP3 only, 2 = SHF only, 3 = IMAD only, 4 = IMAD.WIDE.U32 only,
+ *        5 = ALU:FMA 1:1 (LOP3 + IMAD), 6 = SipRound-shaped ALU mix (IADD3 / LOP3 / SHF, 8:8:8),
+ *        7 = IMAD.HI.U32 only, 8 = ALU:FMA 2:1 (LOP3, SHF + IMAD).
+ * wg_launch_count: kernels this library has launched since it was loaded (bench.py's gpu_launches). */
+wg_status wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms);
+uint64_t wg_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WARPGUARD_H */
