@@ -1,0 +1,234 @@
+"""Thin ctypes face of the C-ABI library ``libwarpguard.so`` (include/warpguard.h), same names.
+
+Argument marshalling only: ``tensor.data_ptr()``, sizes and the current CUDA stream are handed to the
+library; every step of the check path (MAC, membership, verdicts, counters) runs in its CUDA kernels.
+There is no CPU fallback: a missing library, or a box without a CUDA device, raises.
+
+Tensors follow ``streams.py``: ``hdr`` int64 [n, 2] (the little-endian image of ``wg_event_hdr``),
+``val`` / ``tag`` int64 [n, 32], ``out`` int32 [n, 2] = (viol_mask, allow_mask).
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+import torch
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libwarpguard.so"
+
+WG_OK, WG_ERR_INVALID_ARG, WG_ERR_BAD_POLICY, WG_ERR_NO_POLICY, WG_ERR_CUDA, WG_ERR_OOM = range(6)
+WG_MODE_DETECT, WG_MODE_ENFORCE = 0, 1
+
+EXPORTS = [
+    "wg_load_policy", "wg_sign_continuations", "wg_verify_continuations", "wg_check_forward", "wg_read_counters",
+    "wg_reset_counters", "wg_destroy", "wg_strerror", "wg_last_cuda_error",
+    "wg_sign_continuations_host", "wg_verify_continuations_host", "wg_check_forward_host",
+    "wg_probe_int_pipe", "wg_launch_count",
+]
+
+COUNTER_FIELDS = (
+    ["events_total", "events_empty", "events_unknown_site", "events_misrouted"]
+    + [f"events_by_kind_{k}" for k in range(7)]
+    + ["ret_checks", "fwd_checks", "ret_lanes", "fwd_lanes", "ret_viol", "fwd_viol",
+       "ret_viol_events", "fwd_viol_events", "blocked_lanes", "blocked_events",
+       "first_violation_key", "signed_lanes", "sign_skipped_events", "policy_digest", "last_mode"]
+)
+
+
+class WgError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        super().__init__(f"{what}: wg_status {status} ({strerror(status)})")
+
+
+class _PolicyDesc(C.Structure):
+    _fields_ = [("n_sites", C.c_uint32), ("kind", C.c_void_p), ("tgt_off", C.c_void_p), ("tgts", C.c_void_p),
+                ("key", C.c_uint64 * 2), ("policy_digest", C.c_uint64)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads libwarpguard.so (built in-tree by ``python -m paper_2606_11871_b200.build``).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_11871_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(str(LIB_PATH))
+        vp, u64, i = C.c_void_p, C.c_uint64, C.c_int
+        L.wg_load_policy.argtypes = [C.POINTER(vp), i, C.POINTER(_PolicyDesc)]
+        L.wg_sign_continuations.argtypes = [vp, vp, vp, vp, u64, vp]
+        L.wg_verify_continuations.argtypes = [vp, vp, vp, vp, vp, u64, i, vp]
+        L.wg_check_forward.argtypes = [vp, vp, vp, vp, u64, i, vp]
+        L.wg_read_counters.argtypes = [vp, vp, vp, vp]
+        L.wg_reset_counters.argtypes = [vp, vp]
+        L.wg_destroy.argtypes = [vp]
+        L.wg_destroy.restype = None
+        L.wg_strerror.argtypes = [i]
+        L.wg_strerror.restype = C.c_char_p
+        L.wg_last_cuda_error.argtypes = [vp]
+        L.wg_sign_continuations_host.argtypes = [vp, vp, vp, vp, u64]
+        L.wg_verify_continuations_host.argtypes = [vp, vp, vp, vp, vp, u64, i]
+        L.wg_check_forward_host.argtypes = [vp, vp, vp, vp, u64, i]
+        L.wg_probe_int_pipe.argtypes = [i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.wg_launch_count.argtypes = []
+        L.wg_launch_count.restype = u64
+        for name in EXPORTS:
+            if name not in ("wg_destroy", "wg_strerror", "wg_launch_count"):
+                getattr(L, name).restype = i
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return lib().wg_strerror(int(status)).decode()
+
+
+def _chk(status: int, what: str) -> None:
+    if status != WG_OK:
+        raise WgError(status, what)
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev(t: torch.Tensor, what: str, cols: int, itemsize: int) -> int:
+    if not t.is_cuda:
+        raise ValueError(f"{what} must be a CUDA tensor (use the *_host calls for host buffers)")
+    if not t.is_contiguous() or t.element_size() != itemsize or (t.dim() != 2 or t.shape[1] != cols):
+        raise ValueError(f"{what}: expected a contiguous [n, {cols}] tensor of {itemsize}-byte elements, "
+                         f"got {tuple(t.shape)} {t.dtype}")
+    return t.data_ptr()
+
+
+def _host(t: torch.Tensor, what: str, cols: int, itemsize: int) -> int:
+    if t.is_cuda:
+        raise ValueError(f"{what} must be a host tensor")
+    if not t.is_contiguous() or t.element_size() != itemsize or (t.dim() != 2 or t.shape[1] != cols):
+        raise ValueError(f"{what}: expected a contiguous [n, {cols}] tensor of {itemsize}-byte elements")
+    return t.data_ptr()
+
+
+class Engine:
+    """Owner of one ``wg_engine*``.  Method names are the C-ABI's."""
+
+    def __init__(self, device: int | None = None):
+        self._h = C.c_void_p(None)
+        self.device = torch.cuda.current_device() if device is None else int(device)
+        self.n_sites = 0
+
+    # -- wg_load_policy ---------------------------------------------------------------------------
+    def wg_load_policy(self, kind, tgt_off, tgts, k0: int, k1: int, policy_digest: int = 0) -> None:
+        kind = np.ascontiguousarray(kind, dtype=np.uint8)
+        tgt_off = np.ascontiguousarray(tgt_off, dtype=np.uint32)
+        tgts = np.ascontiguousarray(tgts, dtype=np.uint64)
+        if tgt_off.size != kind.size + 1:
+            raise ValueError("tgt_off must have n_sites + 1 entries")
+        d = _PolicyDesc()
+        d.n_sites = kind.size
+        d.kind = kind.ctypes.data if kind.size else None
+        d.tgt_off = tgt_off.ctypes.data
+        d.tgts = tgts.ctypes.data if tgts.size else None
+        d.key[0] = k0 & (2**64 - 1)
+        d.key[1] = k1 & (2**64 - 1)
+        d.policy_digest = policy_digest & (2**64 - 1)
+        _chk(lib().wg_load_policy(C.byref(self._h), self.device, C.byref(d)), "wg_load_policy")
+        self.n_sites = int(kind.size)
+
+    def load(self, policy) -> "Engine":
+        self.wg_load_policy(policy.kind, policy.tgt_off, policy.tgts, policy.k0, policy.k1, policy.policy_digest)
+        return self
+
+    # -- device-buffer calls ----------------------------------------------------------------------
+    def wg_sign_continuations(self, hdr, val, tag=None, stream=None) -> torch.Tensor:
+        n = hdr.shape[0]
+        if tag is None:
+            tag = torch.empty((n, 32), dtype=torch.int64, device=hdr.device)
+        _chk(lib().wg_sign_continuations(self._h, _dev(hdr, "hdr", 2, 8), _dev(val, "val", 32, 8),
+                                         _dev(tag, "tag", 32, 8), n, _stream_ptr(stream)), "wg_sign_continuations")
+        return tag
+
+    def wg_verify_continuations(self, hdr, val, tag, mode: int, out=None, stream=None) -> torch.Tensor:
+        n = hdr.shape[0]
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32, device=hdr.device)
+        _chk(lib().wg_verify_continuations(self._h, _dev(hdr, "hdr", 2, 8), _dev(val, "val", 32, 8),
+                                           _dev(tag, "tag", 32, 8), _dev(out, "out", 2, 4), n, int(mode),
+                                           _stream_ptr(stream)), "wg_verify_continuations")
+        return out
+
+    def wg_check_forward(self, hdr, val, mode: int, out=None, stream=None) -> torch.Tensor:
+        n = hdr.shape[0]
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32, device=hdr.device)
+        _chk(lib().wg_check_forward(self._h, _dev(hdr, "hdr", 2, 8), _dev(val, "val", 32, 8),
+                                    _dev(out, "out", 2, 4), n, int(mode), _stream_ptr(stream)), "wg_check_forward")
+        return out
+
+    # -- host-buffer calls (end-to-end path) ------------------------------------------------------
+    def wg_sign_continuations_host(self, hdr, val, tag=None) -> torch.Tensor:
+        n = hdr.shape[0]
+        if tag is None:
+            tag = torch.empty((n, 32), dtype=torch.int64)
+        _chk(lib().wg_sign_continuations_host(self._h, _host(hdr, "hdr", 2, 8), _host(val, "val", 32, 8),
+                                              _host(tag, "tag", 32, 8), n), "wg_sign_continuations_host")
+        return tag
+
+    def wg_verify_continuations_host(self, hdr, val, tag, mode: int, out=None) -> torch.Tensor:
+        n = hdr.shape[0]
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32)
+        _chk(lib().wg_verify_continuations_host(self._h, _host(hdr, "hdr", 2, 8), _host(val, "val", 32, 8),
+                                                _host(tag, "tag", 32, 8), _host(out, "out", 2, 4), n, int(mode)),
+             "wg_verify_continuations_host")
+        return out
+
+    def wg_check_forward_host(self, hdr, val, mode: int, out=None) -> torch.Tensor:
+        n = hdr.shape[0]
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32)
+        _chk(lib().wg_check_forward_host(self._h, _host(hdr, "hdr", 2, 8), _host(val, "val", 32, 8),
+                                         _host(out, "out", 2, 4), n, int(mode)), "wg_check_forward_host")
+        return out
+
+    # -- counters ---------------------------------------------------------------------------------
+    def wg_read_counters(self, per_site: bool = True, stream=None):
+        g = np.zeros(26, dtype=np.uint64)
+        s = np.zeros((self.n_sites, 4), dtype=np.uint64) if per_site else None
+        _chk(lib().wg_read_counters(self._h, g.ctypes.data, None if s is None or s.size == 0 else s.ctypes.data,
+                                    _stream_ptr(stream)), "wg_read_counters")
+        return {k: int(v) for k, v in zip(COUNTER_FIELDS, g)}, s
+
+    def wg_reset_counters(self, stream=None) -> None:
+        _chk(lib().wg_reset_counters(self._h, _stream_ptr(stream)), "wg_reset_counters")
+
+    def wg_destroy(self) -> None:
+        if self._h:
+            lib().wg_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    close = wg_destroy
+
+    def __del__(self):
+        try:
+            self.wg_destroy()
+        except Exception:  # interpreter shutdown
+            pass
+
+
+def wg_probe_int_pipe(device: int, mix: int) -> tuple[float, float]:
+    """(int32 lane-ops per second, milliseconds) of the register-only integer probe; see warpguard.h."""
+    ops, ms = C.c_double(0), C.c_double(0)
+    _chk(lib().wg_probe_int_pipe(int(device), int(mix), C.byref(ops), C.byref(ms)), "wg_probe_int_pipe")
+    return ops.value, ms.value
+
+
+def wg_launch_count() -> int:
+    return int(lib().wg_launch_count())

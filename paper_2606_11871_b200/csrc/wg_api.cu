@@ -1,0 +1,445 @@
+// wg_api.cu — the C-ABI of include/warpguard.h: argument checks, policy validation (a bad
+// policy loads nothing), engine-owned device tables, launches, counter read-out, and the HOST-buffer entry
+// points that stream events through a double-buffered device staging area.  No verdict, MAC or membership
+// arithmetic happens on the host: every step of the path runs in the kernels of wg_kernels.cu.
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/warpguard.h"
+#include "wg_internal.h"
+
+struct wg_engine {
+  int device = 0;
+  int sm_count = 0;
+  bool loaded = false;
+  uint32_t n_sites = 0;
+  uint64_t n_tgts = 0;
+  wg::SiteRow* d_rows = nullptr;
+  uint64_t* d_tgts = nullptr;
+  unsigned long long* d_glob = nullptr;  // [C_WORDS]
+  unsigned long long* d_site = nullptr;  // [n_sites][4]
+  uint64_t v_init[4] = {0, 0, 0, 0};     // key ^ SipHash constants
+  uint64_t digest = 0;
+  uint64_t seq = 0;        // running event index over check calls (R12), assigned at call time
+  uint64_t last_mode = 0;  // mode of the last non-empty check call
+  int last_cuda_error = 0;
+  // staging for the *_host entry points (allocated on first use)
+  uint64_t stage_cap = 0;  // events per buffer
+  void* d_stage[2] = {nullptr, nullptr};
+  cudaStream_t st[2] = {nullptr, nullptr};
+  cudaEvent_t ev_done[2] = {nullptr, nullptr};
+};
+
+namespace {
+
+std::atomic<uint64_t> g_launches{0};
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) return;
+    ok = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+wg_status cuda_fail(wg_engine* e, cudaError_t err) {
+  if (e) e->last_cuda_error = static_cast<int>(err);
+  cudaGetLastError();  // clear the sticky-free error state
+  return err == cudaErrorMemoryAllocation ? WG_ERR_OOM : WG_ERR_CUDA;
+}
+
+#define WG_CUDA(e, call)                                  \
+  do {                                                    \
+    cudaError_t err__ = (call);                           \
+    if (err__ != cudaSuccess) return cuda_fail(e, err__); \
+  } while (0)
+
+bool aligned(const void* p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+
+// R16: everything that would widen or blur an allowed set is rejected before any state is touched.
+bool policy_ok(const wg_policy_desc* d) {
+  const uint32_t n = d->n_sites;
+  if (d->tgt_off[0] != 0) return false;
+  for (uint32_t s = 0; s < n; ++s) {
+    if (d->kind[s] >= WG_KIND_COUNT) return false;
+    const uint32_t a = d->tgt_off[s], b = d->tgt_off[s + 1];
+    if (b < a) return false;
+    const bool fwd = d->kind[s] == WG_KIND_PROTECTED_FORWARD;
+    if (fwd && a == b) return false;   // no target evidence: must have been labelled unsupported
+    if (!fwd && a != b) return false;  // a set nobody may consult
+    if (a != b && d->tgts == nullptr) return false;
+    for (uint32_t i = a + 1; i < b; ++i)
+      if (!(d->tgts[i - 1] < d->tgts[i])) return false;  // strictly ascending: sorted, no duplicates
+  }
+  return true;
+}
+
+void free_tables(wg_engine* e) {
+  cudaFree(e->d_rows);
+  cudaFree(e->d_tgts);
+  cudaFree(e->d_glob);
+  cudaFree(e->d_site);
+  e->d_rows = nullptr;
+  e->d_tgts = nullptr;
+  e->d_glob = nullptr;
+  e->d_site = nullptr;
+  e->loaded = false;
+}
+
+void free_staging(wg_engine* e) {
+  for (int i = 0; i < 2; ++i) {
+    if (e->d_stage[i]) cudaFree(e->d_stage[i]);
+    if (e->st[i]) cudaStreamDestroy(e->st[i]);
+    if (e->ev_done[i]) cudaEventDestroy(e->ev_done[i]);
+    e->d_stage[i] = nullptr;
+    e->st[i] = nullptr;
+    e->ev_done[i] = nullptr;
+  }
+  e->stage_cap = 0;
+}
+
+wg_status zero_counters(wg_engine* e, cudaStream_t st) {
+  WG_CUDA(e, cudaMemsetAsync(e->d_glob, 0, sizeof(unsigned long long) * wg::C_WORDS, st));
+  WG_CUDA(e, cudaMemsetAsync(e->d_glob + wg::C_FIRST_VIOLATION, 0xff, sizeof(unsigned long long), st));
+  if (e->n_sites)
+    WG_CUDA(e, cudaMemsetAsync(e->d_site, 0, sizeof(unsigned long long) * 4 * e->n_sites, st));
+  e->seq = 0;
+  e->last_mode = 0;
+  return WG_OK;
+}
+
+wg::Params base_params(const wg_engine* e) {
+  wg::Params p;
+  std::memset(&p, 0, sizeof(p));
+  p.rows = e->d_rows;
+  p.tgts = e->d_tgts;
+  p.glob = e->d_glob;
+  p.site = e->d_site;
+  p.n_sites = e->n_sites;
+  p.v0 = e->v_init[0];
+  p.v1 = e->v_init[1];
+  p.v2 = e->v_init[2];
+  p.v3 = e->v_init[3];
+  return p;
+}
+
+wg_status check_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d_val, const uint64_t* d_tag,
+                       bool has_tag, wg_verdict* d_out, uint64_t n, wg_mode mode, cudaStream_t st) {
+  if (!e || !e->loaded) return WG_ERR_NO_POLICY;
+  if (mode != WG_MODE_DETECT && mode != WG_MODE_ENFORCE) return WG_ERR_INVALID_ARG;
+  if (n == 0) return WG_OK;  // R24: nothing changes
+  if (!d_hdr || !d_val || !d_out || (has_tag && !d_tag)) return WG_ERR_INVALID_ARG;
+  if (!aligned(d_hdr, 16) || !aligned(d_val, 16) || !aligned(d_out, 8) || (has_tag && !aligned(d_tag, 16)))
+    return WG_ERR_INVALID_ARG;
+  if (n > (1ull << 58)) return WG_ERR_INVALID_ARG;  // (seq << 5) must not wrap
+  DeviceGuard g(e->device);
+  if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
+  wg::Params p = base_params(e);
+  p.hdr = reinterpret_cast<const uint4*>(d_hdr);
+  p.val = d_val;
+  p.tag = has_tag ? d_tag : nullptr;
+  p.out = reinterpret_cast<uint2*>(d_out);
+  p.n = n;
+  p.seq_base = e->seq;
+  p.mode = static_cast<uint32_t>(mode);
+  WG_CUDA(e, wg::launch_check(p, e->sm_count, st));
+  e->seq += n;
+  e->last_mode = static_cast<uint64_t>(mode);
+  return WG_OK;
+}
+
+wg_status sign_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d_val, uint64_t* d_tag,
+                      uint64_t n, cudaStream_t st) {
+  if (!e || !e->loaded) return WG_ERR_NO_POLICY;
+  if (n == 0) return WG_OK;
+  if (!d_hdr || !d_val || !d_tag) return WG_ERR_INVALID_ARG;
+  if (!aligned(d_hdr, 16) || !aligned(d_val, 16) || !aligned(d_tag, 16)) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(e->device);
+  if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
+  wg::Params p = base_params(e);
+  p.hdr = reinterpret_cast<const uint4*>(d_hdr);
+  p.val = d_val;
+  p.tag_out = d_tag;
+  p.n = n;
+  WG_CUDA(e, wg::launch_sign(p, e->sm_count, st));
+  return WG_OK;
+}
+
+// ---- host-buffer streaming -------------------------------------------------------------------------
+constexpr uint64_t kStageEvents = 1ull << 18;  // 256 Ki events per buffer: 4 MiB hdr + 64 MiB val + 64 MiB tag + 2 MiB out
+constexpr uint64_t kBytesPerStagedEvent = 16 + 256 + 256 + 8;
+
+wg_status ensure_staging(wg_engine* e) {
+  if (e->stage_cap) return WG_OK;
+  for (int i = 0; i < 2; ++i) {
+    WG_CUDA(e, cudaMalloc(&e->d_stage[i], kStageEvents * kBytesPerStagedEvent));
+    WG_CUDA(e, cudaStreamCreateWithFlags(&e->st[i], cudaStreamNonBlocking));
+    WG_CUDA(e, cudaEventCreateWithFlags(&e->ev_done[i], cudaEventDisableTiming));
+  }
+  e->stage_cap = kStageEvents;
+  return WG_OK;
+}
+
+struct StageView {
+  wg_event_hdr* hdr;
+  uint64_t* val;
+  uint64_t* tag;
+  wg_verdict* out;
+};
+StageView stage_view(void* base) {
+  char* b = static_cast<char*>(base);
+  StageView v;
+  v.hdr = reinterpret_cast<wg_event_hdr*>(b);
+  v.val = reinterpret_cast<uint64_t*>(b + kStageEvents * 16);
+  v.tag = reinterpret_cast<uint64_t*>(b + kStageEvents * (16 + 256));
+  v.out = reinterpret_cast<wg_verdict*>(b + kStageEvents * (16 + 256 + 256));
+  return v;
+}
+
+enum HostOp { OP_SIGN, OP_VERIFY, OP_FORWARD };
+
+wg_status host_common(wg_engine* e, HostOp op, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                      const uint64_t* h_tag_in, uint64_t* h_tag_out, wg_verdict* h_out, uint64_t n, wg_mode mode) {
+  if (!e || !e->loaded) return WG_ERR_NO_POLICY;
+  if (op != OP_SIGN && mode != WG_MODE_DETECT && mode != WG_MODE_ENFORCE) return WG_ERR_INVALID_ARG;
+  if (n == 0) return WG_OK;
+  if (!h_hdr || !h_val) return WG_ERR_INVALID_ARG;
+  if (op == OP_SIGN && !h_tag_out) return WG_ERR_INVALID_ARG;
+  if (op == OP_VERIFY && !h_tag_in) return WG_ERR_INVALID_ARG;
+  if (op != OP_SIGN && !h_out) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(e->device);
+  if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
+  wg_status s = ensure_staging(e);
+  if (s != WG_OK) return s;
+
+  int buf = 0;
+  for (uint64_t lo = 0; lo < n; lo += kStageEvents, buf ^= 1) {
+    const uint64_t m = (n - lo < kStageEvents) ? (n - lo) : kStageEvents;
+    cudaStream_t st = e->st[buf];
+    StageView v = stage_view(e->d_stage[buf]);
+    // the previous use of this buffer (two chunks ago) finished when its stream's D2H did: same stream, in order
+    WG_CUDA(e, cudaMemcpyAsync(v.hdr, h_hdr + lo, m * 16, cudaMemcpyHostToDevice, st));
+    WG_CUDA(e, cudaMemcpyAsync(v.val, h_val + lo * 32, m * 256, cudaMemcpyHostToDevice, st));
+    if (op == OP_VERIFY)
+      WG_CUDA(e, cudaMemcpyAsync(v.tag, h_tag_in + lo * 32, m * 256, cudaMemcpyHostToDevice, st));
+    if (op == OP_SIGN) {
+      s = sign_common(e, v.hdr, v.val, v.tag, m, st);
+      if (s != WG_OK) return s;
+      WG_CUDA(e, cudaMemcpyAsync(h_tag_out + lo * 32, v.tag, m * 256, cudaMemcpyDeviceToHost, st));
+    } else {
+      s = check_common(e, v.hdr, v.val, v.tag, op == OP_VERIFY, v.out, m, mode, st);
+      if (s != WG_OK) return s;
+      WG_CUDA(e, cudaMemcpyAsync(h_out + lo, v.out, m * 8, cudaMemcpyDeviceToHost, st));
+    }
+  }
+  WG_CUDA(e, cudaStreamSynchronize(e->st[0]));
+  WG_CUDA(e, cudaStreamSynchronize(e->st[1]));
+  return WG_OK;
+}
+
+}  // namespace
+
+namespace wg {
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+}  // namespace wg
+
+extern "C" {
+
+wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc) {
+  if (!eng || !desc) return WG_ERR_INVALID_ARG;
+  if (desc->n_sites && (!desc->kind || !desc->tgt_off)) return WG_ERR_INVALID_ARG;
+  if (!desc->tgt_off) return WG_ERR_INVALID_ARG;
+  if (!policy_ok(desc)) return WG_ERR_BAD_POLICY;  // before any state is touched
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return WG_ERR_CUDA;  // no CPU fallback
+  }
+  if (device < 0 || device >= ndev) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(device);
+  if (!g.ok) return WG_ERR_CUDA;
+
+  const uint32_t n = desc->n_sites;
+  const uint64_t nt = desc->tgt_off[n];
+  // build the new tables completely before replacing the old ones
+  std::vector<wg::SiteRow> rows;
+  try {
+    rows.resize(n);
+  } catch (const std::bad_alloc&) {
+    return WG_ERR_OOM;
+  }
+  for (uint32_t s = 0; s < n; ++s) {
+    rows[s].kind = desc->kind[s];
+    rows[s].off = desc->tgt_off[s];
+    rows[s].cnt = desc->tgt_off[s + 1] - desc->tgt_off[s];
+    rows[s].pad = 0;
+  }
+  wg_engine tmp;
+  tmp.device = device;
+  tmp.n_sites = n;
+  tmp.n_tgts = nt;
+  cudaError_t err = cudaSuccess;
+  auto fail = [&](cudaError_t e2) {
+    free_tables(&tmp);
+    wg_status s = cuda_fail(*eng, e2);
+    return s;
+  };
+  if ((err = cudaDeviceGetAttribute(&tmp.sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess)
+    return fail(err);
+  if ((err = cudaMalloc(&tmp.d_rows, sizeof(wg::SiteRow) * (n ? n : 1))) != cudaSuccess) return fail(err);
+  if ((err = cudaMalloc(&tmp.d_tgts, sizeof(uint64_t) * (nt ? nt : 1))) != cudaSuccess) return fail(err);
+  if ((err = cudaMalloc(&tmp.d_glob, sizeof(unsigned long long) * wg::C_WORDS)) != cudaSuccess) return fail(err);
+  if ((err = cudaMalloc(&tmp.d_site, sizeof(unsigned long long) * 4 * (n ? n : 1))) != cudaSuccess) return fail(err);
+  if (n && (err = cudaMemcpy(tmp.d_rows, rows.data(), sizeof(wg::SiteRow) * n, cudaMemcpyHostToDevice)) != cudaSuccess)
+    return fail(err);
+  if (nt && (err = cudaMemcpy(tmp.d_tgts, desc->tgts, sizeof(uint64_t) * nt, cudaMemcpyHostToDevice)) != cudaSuccess)
+    return fail(err);
+
+  wg_engine* e = *eng;
+  if (!e) {
+    e = new (std::nothrow) wg_engine();
+    if (!e) {
+      free_tables(&tmp);
+      return WG_ERR_OOM;
+    }
+  } else {
+    if (e->device != device) free_staging(e);
+    DeviceGuard g2(e->device);
+    cudaDeviceSynchronize();  // nothing may still be reading the tables we are about to drop
+    free_tables(e);
+  }
+  e->device = device;
+  e->sm_count = tmp.sm_count;
+  e->n_sites = n;
+  e->n_tgts = nt;
+  e->d_rows = tmp.d_rows;
+  e->d_tgts = tmp.d_tgts;
+  e->d_glob = tmp.d_glob;
+  e->d_site = tmp.d_site;
+  // SipHash initialisation: key xor the constant "somepseudorandomlygeneratedbytes" (R1, R20)
+  e->v_init[0] = desc->key[0] ^ 0x736f6d6570736575ull;
+  e->v_init[1] = desc->key[1] ^ 0x646f72616e646f6dull;
+  e->v_init[2] = desc->key[0] ^ 0x6c7967656e657261ull;
+  e->v_init[3] = desc->key[1] ^ 0x7465646279746573ull;
+  e->digest = desc->policy_digest;
+  e->loaded = true;
+  *eng = e;
+  wg_status s = zero_counters(e, nullptr);
+  if (s != WG_OK) return s;
+  WG_CUDA(e, cudaStreamSynchronize(nullptr));
+  return WG_OK;
+}
+
+wg_status wg_sign_continuations(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                                uint64_t* d_tag, uint64_t n, void* cuda_stream) {
+  return sign_common(eng, d_hdr, d_val, d_tag, n, static_cast<cudaStream_t>(cuda_stream));
+}
+
+wg_status wg_verify_continuations(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                                  const uint64_t* d_tag, wg_verdict* d_out, uint64_t n, wg_mode mode,
+                                  void* cuda_stream) {
+  return check_common(eng, d_hdr, d_val, d_tag, true, d_out, n, mode, static_cast<cudaStream_t>(cuda_stream));
+}
+
+wg_status wg_check_forward(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val, wg_verdict* d_out,
+                           uint64_t n, wg_mode mode, void* cuda_stream) {
+  return check_common(eng, d_hdr, d_val, nullptr, false, d_out, n, mode, static_cast<cudaStream_t>(cuda_stream));
+}
+
+wg_status wg_read_counters(wg_engine* eng, wg_counters* h_global, wg_site_counters* h_per_site,
+                           void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (!h_global) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  WG_CUDA(eng, cudaStreamSynchronize(st));
+  static_assert(sizeof(wg_counters) == 26 * 8, "wg_counters layout");
+  WG_CUDA(eng, cudaMemcpy(h_global, eng->d_glob, sizeof(wg_counters), cudaMemcpyDeviceToHost));
+  h_global->policy_digest = eng->digest;
+  h_global->last_mode = eng->last_mode;
+  if (h_per_site && eng->n_sites)
+    WG_CUDA(eng, cudaMemcpy(h_per_site, eng->d_site, sizeof(wg_site_counters) * eng->n_sites,
+                            cudaMemcpyDeviceToHost));
+  return WG_OK;
+}
+
+wg_status wg_reset_counters(wg_engine* eng, void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  return zero_counters(eng, static_cast<cudaStream_t>(cuda_stream));
+}
+
+void wg_destroy(wg_engine* eng) {
+  if (!eng) return;
+  {
+    DeviceGuard g(eng->device);
+    if (g.ok) {
+      cudaDeviceSynchronize();
+      free_staging(eng);
+      free_tables(eng);
+    }
+  }
+  delete eng;
+}
+
+const char* wg_strerror(wg_status s) {
+  switch (s) {
+    case WG_OK: return "ok";
+    case WG_ERR_INVALID_ARG: return "invalid argument";
+    case WG_ERR_BAD_POLICY: return "policy rejected; nothing loaded";
+    case WG_ERR_NO_POLICY: return "no policy loaded";
+    case WG_ERR_CUDA: return "CUDA runtime error (no device or call failed)";
+    case WG_ERR_OOM: return "out of memory";
+  }
+  return "unknown status";
+}
+
+int wg_last_cuda_error(const wg_engine* eng) { return eng ? eng->last_cuda_error : 0; }
+
+wg_status wg_sign_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                                     uint64_t* h_tag, uint64_t n) {
+  return host_common(eng, OP_SIGN, h_hdr, h_val, nullptr, h_tag, nullptr, n, WG_MODE_DETECT);
+}
+wg_status wg_verify_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                                       const uint64_t* h_tag, wg_verdict* h_out, uint64_t n, wg_mode mode) {
+  return host_common(eng, OP_VERIFY, h_hdr, h_val, h_tag, nullptr, h_out, n, mode);
+}
+wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
+                                wg_verdict* h_out, uint64_t n, wg_mode mode) {
+  return host_common(eng, OP_FORWARD, h_hdr, h_val, nullptr, nullptr, h_out, n, mode);
+}
+
+wg_status wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms) {
+  if (!ops_per_s || mix < 0 || mix > 8) return WG_ERR_INVALID_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return WG_ERR_CUDA;
+  }
+  if (device < 0 || device >= ndev) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(device);
+  if (!g.ok) return WG_ERR_CUDA;
+  int sms = 0;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return WG_ERR_CUDA;
+  double t = 0;
+  if (wg::run_int_pipe_probe(mix, sms, ops_per_s, &t) != cudaSuccess) {
+    cudaGetLastError();
+    return WG_ERR_CUDA;
+  }
+  if (ms) *ms = t;
+  return WG_OK;
+}
+
+uint64_t wg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

@@ -1,0 +1,73 @@
+// wg_internal.h — what the C-ABI layer (wg_api.cu) and the kernels (wg_kernels.cu) agree on.
+// Not installed; the public surface is include/warpguard.h only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wg {
+
+// ---- engine-owned device tables (DESIGN.md §5 "data layout") --------------------------------------
+// One 16-byte row per site, gathered once per event.  L2-resident at every config.
+struct __align__(16) SiteRow {
+  uint32_t kind;  // wg_kind
+  uint32_t off;   // first element of this site's set in the device copy of `tgts` (u64 index)
+  uint32_t cnt;   // number of targets (0 unless protected-forward)
+  uint32_t pad;
+};
+
+// Global counter block: the first 26 words have exactly the layout of wg_counters, so a read-out is one
+// copy.  Words 24 (policy_digest) and 25 (last_mode) are kept host-side and patched in at read-out.
+enum CounterWord {
+  C_EVENTS_TOTAL = 0,
+  C_EVENTS_EMPTY = 1,
+  C_EVENTS_UNKNOWN = 2,
+  C_EVENTS_MISROUTED = 3,
+  C_BY_KIND = 4,  // 7 words
+  C_RET_CHECKS = 11,
+  C_FWD_CHECKS = 12,
+  C_RET_LANES = 13,
+  C_FWD_LANES = 14,
+  C_RET_VIOL = 15,
+  C_FWD_VIOL = 16,
+  C_RET_VIOL_EVENTS = 17,
+  C_FWD_VIOL_EVENTS = 18,
+  C_BLOCKED_LANES = 19,
+  C_BLOCKED_EVENTS = 20,
+  C_FIRST_VIOLATION = 21,  // atomicMin, initialised to UINT64_MAX
+  C_SIGNED_LANES = 22,
+  C_SIGN_SKIPPED = 23,
+  C_POLICY_DIGEST = 24,
+  C_LAST_MODE = 25,
+  C_WORDS = 32
+};
+
+// Per-site counters: 4 x u64 per site, layout of wg_site_counters.
+enum SiteWord { S_EVENTS = 0, S_LANES_CHECKED = 1, S_LANES_VIOLATION = 2, S_LANES_BLOCKED = 3 };
+
+// Everything a kernel needs, passed by value (lives in the constant bank: the key never sits in
+// caller-addressable memory).
+struct Params {
+  const uint4* hdr;          // [n] wg_event_hdr as one 16-byte vector
+  const uint64_t* val;       // [n][32]
+  const uint64_t* tag;       // [n][32] or nullptr (forward entry point)
+  uint64_t* tag_out;         // sign only
+  uint2* out;                // [n] wg_verdict
+  uint64_t n;
+  uint64_t seq_base;         // running event index of event 0 of this call (R12)
+  const SiteRow* rows;
+  const uint64_t* tgts;
+  unsigned long long* glob;  // [C_WORDS]
+  unsigned long long* site;  // [n_sites][4]
+  uint32_t n_sites;
+  uint32_t mode;             // 0 detect, 1 enforce
+  uint64_t v0, v1, v2, v3;   // SipHash initial state: key ^ constants (computed host-side at load)
+};
+
+// launchers (wg_kernels.cu); grid sizing from the SM count of the engine's device
+cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st);
+cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st);
+cudaError_t launch_fill_u64(unsigned long long* p, uint64_t n, unsigned long long v, cudaStream_t st);
+cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double* ms);
+void count_launch();
+
+}  // namespace wg

@@ -1,0 +1,113 @@
+// wg_probe.cu — register-only integer micro-benchmark (measurement helper, no part of the check path).
+// It answers "what can the sm_100a integer pipes issue?" so that the ALU roofline of the MAC kernel has a
+// measured denominator beside the one derived from unit counts.  Every chain is a dependent
+// sequence of one instruction kind; 8 independent chains per thread and 16 resident warps per SMSP keep the
+// pipes full.  `asm volatile` pins the instruction selection (checked with cuobjdump -sass).
+#include "wg_internal.h"
+
+namespace wg {
+namespace {
+
+constexpr int kChains = 8;
+constexpr int kInner = 64;    // unrolled steps per chain per loop trip
+constexpr int kTrips = 512;   // loop trips
+constexpr int kThreads = 256;
+
+#define STEP_IADD(x, y) asm volatile("add.u32 %0, %0, %1;" : "+r"(x) : "r"(y))
+#define STEP_LOP(x, y) asm volatile("xor.b32 %0, %0, %1;" : "+r"(x) : "r"(y))
+#define STEP_SHF(x, y) asm volatile("shf.l.wrap.b32 %0, %0, %1, 13;" : "+r"(x) : "r"(y))
+#define STEP_IMAD(x, y) asm volatile("mad.lo.u32 %0, %0, %1, %1;" : "+r"(x) : "r"(y))
+#define STEP_IMADHI(x, y) asm volatile("mad.hi.u32 %0, %0, %1, %1;" : "+r"(x) : "r"(y))
+#define STEP_WIDE(x64, y) asm volatile("{ .reg .b32 lo, hi; mov.b64 {lo, hi}, %0; mad.wide.u32 %0, lo, %1, %0; }" : "+l"(x64) : "r"(y))
+
+template <int MIX>
+__global__ void __launch_bounds__(kThreads) wg_int_probe(uint32_t* sink, uint32_t y) {
+  uint32_t x[kChains];
+  uint64_t w[kChains];
+#pragma unroll
+  for (int i = 0; i < kChains; ++i) {
+    x[i] = threadIdx.x * 2654435761u + i;
+    w[i] = (static_cast<uint64_t>(x[i]) << 32) | blockIdx.x;
+  }
+  for (int t = 0; t < kTrips; ++t) {
+#pragma unroll
+    for (int s = 0; s < kInner; ++s) {
+#pragma unroll
+      for (int i = 0; i < kChains; ++i) {
+        if (MIX == 0) STEP_IADD(x[i], y);
+        if (MIX == 1) STEP_LOP(x[i], y);
+        if (MIX == 2) STEP_SHF(x[i], y);
+        if (MIX == 3) STEP_IMAD(x[i], y);
+        if (MIX == 4) STEP_WIDE(w[i], y);
+        if (MIX == 5) {  // ALU : FMA = 1 : 1
+          if (i & 1) STEP_LOP(x[i], y); else STEP_IMAD(x[i], y);
+        }
+        if (MIX == 6) {  // SipRound-shaped ALU mix 1 : 1 : 1
+          if ((s + i) % 3 == 0) STEP_IADD(x[i], y);
+          if ((s + i) % 3 == 1) STEP_LOP(x[i], y);
+          if ((s + i) % 3 == 2) STEP_SHF(x[i], y);
+        }
+        if (MIX == 7) STEP_IMADHI(x[i], y);
+        if (MIX == 8) {  // ALU : FMA = 2 : 1
+          if ((s + i) % 3 == 0) STEP_IMAD(x[i], y);
+          if ((s + i) % 3 == 1) STEP_LOP(x[i], y);
+          if ((s + i) % 3 == 2) STEP_SHF(x[i], y);
+        }
+      }
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int i = 0; i < kChains; ++i) acc ^= x[i] ^ static_cast<uint32_t>(w[i]) ^ static_cast<uint32_t>(w[i] >> 32);
+  if (acc == 0x12345678u) sink[0] = acc;  // practically never; keeps the chains live
+}
+
+template <int MIX>
+cudaError_t run(int sm_count, uint32_t* sink, double* ops_per_s, double* ms_out) {
+  const int grid = sm_count * 8;  // 8 CTAs x 8 warps = 64 warps per SM
+  cudaEvent_t a, b;
+  cudaError_t err;
+  if ((err = cudaEventCreate(&a)) != cudaSuccess) return err;
+  if ((err = cudaEventCreate(&b)) != cudaSuccess) return err;
+  float best = 1e30f;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(a, nullptr);
+    wg_int_probe<MIX><<<grid, kThreads>>>(sink, 0x9e3779b9u + rep);
+    count_launch();
+    cudaEventRecord(b, nullptr);
+    if ((err = cudaEventSynchronize(b)) != cudaSuccess) return err;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, a, b);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  const double ops = static_cast<double>(grid) * kThreads * kChains * kInner * static_cast<double>(kTrips);
+  *ops_per_s = ops / (best * 1e-3);
+  *ms_out = best;
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double* ms) {
+  uint32_t* sink = nullptr;
+  cudaError_t err = cudaMalloc(&sink, 256);
+  if (err != cudaSuccess) return err;
+  switch (mix) {
+    case 0: err = run<0>(sm_count, sink, ops_per_s, ms); break;
+    case 1: err = run<1>(sm_count, sink, ops_per_s, ms); break;
+    case 2: err = run<2>(sm_count, sink, ops_per_s, ms); break;
+    case 3: err = run<3>(sm_count, sink, ops_per_s, ms); break;
+    case 4: err = run<4>(sm_count, sink, ops_per_s, ms); break;
+    case 5: err = run<5>(sm_count, sink, ops_per_s, ms); break;
+    case 6: err = run<6>(sm_count, sink, ops_per_s, ms); break;
+    case 7: err = run<7>(sm_count, sink, ops_per_s, ms); break;
+    case 8: err = run<8>(sm_count, sink, ops_per_s, ms); break;
+    default: err = cudaErrorInvalidValue;
+  }
+  cudaFree(sink);
+  return err;
+}
+
+}  // namespace wg

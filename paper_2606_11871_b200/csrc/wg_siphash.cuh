@@ -34,9 +34,13 @@ template <int B>
 __device__ __forceinline__ uint64_t rotl(uint64_t x) {
   uint32_t lo, hi;
   unpack64(x, lo, hi);
-  if (B == 32) return pack64(hi, lo);
-  if (B < 32) return pack64(__funnelshift_l(hi, lo, B), __funnelshift_l(lo, hi, B));
-  return pack64(__funnelshift_l(lo, hi, B - 32), __funnelshift_l(hi, lo, B - 32));
+  if constexpr (B == 32) {
+    return pack64(hi, lo);
+  } else if constexpr (B < 32) {
+    return pack64(__funnelshift_l(hi, lo, B), __funnelshift_l(lo, hi, B));
+  } else {
+    return pack64(__funnelshift_l(lo, hi, B - 32), __funnelshift_l(hi, lo, B - 32));
+  }
 }
 
 __device__ __forceinline__ void sipround(Sip& s) {

@@ -1,0 +1,327 @@
+"""Parity proper: the CUDA path (through the C-ABI, via the ctypes binding) against the CPU oracle, element by
+element and bit for bit, on the same seeded inputs (every output is an integer function of
+(policy, key, events, mode, call order) — tolerance 0).  Sizes span many CTAs, several grid strides and a ragged
+tail.  Run with ``-m gpu`` on the B200 box."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_11871_b200 import binding as B
+from paper_2606_11871_b200 import streams as S
+from tests import witness
+from tests.util import mk_hdr, oracle_for
+
+pytestmark = pytest.mark.gpu
+
+DET, ENF = 0, 1
+FULL = 0xFFFFFFFF
+U64MAX = (1 << 64) - 1
+
+
+def dev():
+    return torch.device("cuda", 0)
+
+
+def to_dev(a: np.ndarray) -> torch.Tensor:
+    a = np.ascontiguousarray(a)
+    if a.dtype == np.uint64:
+        a = a.view(np.int64)
+    if a.dtype == np.uint32:
+        a = a.view(np.int32)
+    return torch.from_numpy(a).to(dev())
+
+
+def engine_for(policy) -> B.Engine:
+    return B.Engine(0).load(policy)
+
+
+def assert_counters_equal(eng: B.Engine, orc: "oracle.Oracle"):
+    gg, gs = eng.wg_read_counters()
+    og, os_ = orc.read_counters()
+    diff = {k: (gg[k], og[k]) for k in og if gg[k] != og[k]}
+    assert not diff, f"global counters differ (gpu, oracle): {diff}"
+    assert np.array_equal(gs, os_), f"per-site counters differ at sites {np.nonzero((gs != os_).any(1))[0][:10]}"
+
+
+def run_config(config, n_events, mode=None, **kw):
+    """Oracle and engine on one seeded stream: sign parity, then check parity, then counters."""
+    st = S.make_stream(config, "cpu", n_events=n_events, mode=mode, **kw)
+    pol = st.policy
+    orc, eng = oracle_for(pol), engine_for(pol)
+    hdr_np, val_push = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64).copy()
+    d_hdr = st.hdr.to(dev())
+    # sign: every tag bit-exact, zeros for inactive lanes and non-return sites
+    o_tag = orc.sign(hdr_np, val_push)
+    g_tag = eng.wg_sign_continuations(d_hdr, st.val.to(dev()))
+    assert np.array_equal(g_tag.cpu().numpy().view(np.uint64), o_tag)
+    # corrupt, then check
+    tag_t = torch.from_numpy(o_tag.view(np.int64).copy())
+    st.apply_return_tamper(tag_t)
+    val_np, tag_np = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+    o_out = orc.verify(hdr_np, val_np, tag_np, st.mode)
+    g_out = eng.wg_verify_continuations(d_hdr, st.val.to(dev()), tag_t.to(dev()), st.mode)
+    g_out = g_out.cpu().numpy().view(np.uint32)
+    bad = np.nonzero((g_out != o_out).any(1))[0]
+    assert bad.size == 0, f"{bad.size} verdicts differ, first at event {bad[:5]}: gpu {g_out[bad[:5]]} oracle {o_out[bad[:5]]}"
+    assert_counters_equal(eng, orc)
+    return st, orc, eng, o_out
+
+
+def test_config1_tiny_full_size_both_modes():
+    for mode in (DET, ENF):
+        st, orc, eng, out = run_config(1, None, mode=mode)
+        assert np.array_equal(out[:, 0], witness.expected_viol(st))  # third, independent derivation
+        assert out[:, 0].any()
+        eng.close()
+
+
+def test_config2_backward_only_ragged():
+    st, orc, eng, out = run_config(2, 200_003)
+    g, _ = eng.wg_read_counters()
+    assert g["ret_checks"] > 0 and g["fwd_checks"] == 0 and g["ret_viol_events"] == len(st.ret_tamper)
+    assert g["blocked_lanes"] == g["ret_viol"]
+
+
+def test_config3_forward_only_ragged_detect():
+    st, orc, eng, out = run_config(3, 300_001)
+    g, _ = eng.wg_read_counters()
+    assert g["fwd_checks"] > 0 and g["ret_checks"] == 0 and g["blocked_lanes"] == 0 and g["fwd_viol"] > 0
+    assert (out[:, 1] == (st.hdr.numpy().view(np.uint64)[:, 0] >> np.uint64(32))).all()  # detect never blocks
+
+
+def test_config4_mixed_paper_shaped():
+    st, orc, eng, out = run_config(4, 400_007)
+    assert np.array_equal(out[:, 0], witness.expected_viol(st))
+    g, _ = eng.wg_read_counters()
+    # only protected sites are in the denominator
+    assert g["ret_checks"] + g["fwd_checks"] <= st.meta["n_ret"] + st.meta["n_fwd"]
+    assert sum(g[f"events_by_kind_{k}"] for k in range(2, 7)) == st.meta["n_non"]
+
+
+def test_config5_stress_alternating_modes_accumulate():
+    pol = S.make_policy(5, "cpu", n_sites=20_000, max_set=4096)
+    orc, eng = oracle_for(pol), engine_for(pol)
+    orc.set_binary_search(True)  # proven equal to the linear scan in test_oracle_membership.py
+    for b in range(3):
+        st = S.make_stream(5, "cpu", n_events=60_001, policy=pol, batch_index=b)
+        assert st.mode == (DET if b % 2 == 0 else ENF)
+        hdr_np = st.hdr.numpy().view(np.uint64)
+        o_tag = orc.sign(hdr_np, st.val.numpy().view(np.uint64))
+        d_hdr = st.hdr.to(dev())
+        g_tag = eng.wg_sign_continuations(d_hdr, st.val.to(dev()))
+        assert np.array_equal(g_tag.cpu().numpy().view(np.uint64), o_tag)
+        tag_t = torch.from_numpy(o_tag.view(np.int64).copy())
+        st.apply_return_tamper(tag_t)
+        o_out = orc.verify(hdr_np, st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64), st.mode)
+        g_out = eng.wg_verify_continuations(d_hdr, st.val.to(dev()), tag_t.to(dev()), st.mode)
+        assert np.array_equal(g_out.cpu().numpy().view(np.uint32), o_out)
+        assert np.array_equal(o_out[:, 0], witness.expected_viol(st))
+    assert_counters_equal(eng, orc)  # counters and the event sequence run on across calls and modes
+
+
+def test_forward_entry_point_matches_oracle_and_fails_closed_on_return_sites():
+    st = S.make_stream(1, "cpu", n_events=50_001)
+    orc, eng = oracle_for(st.policy), engine_for(st.policy)
+    hdr_np, val_np = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    for mode in (DET, ENF):
+        o_out = orc.check_forward(hdr_np, val_np, mode)
+        g_out = eng.wg_check_forward(st.hdr.to(dev()), st.val.to(dev()), mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g_out, o_out)
+    assert_counters_equal(eng, orc)
+    g, _ = eng.wg_read_counters()
+    assert g["events_misrouted"] > 0 and g["ret_checks"] == 0
+
+
+def small_policy():
+    kind = np.array([0, 0, 1, 1, 2, 3, 4, 5, 6], dtype=np.uint8)
+    off = np.array([0, 0, 0, 3, 4, 4, 4, 4, 4, 4], dtype=np.uint32)
+    tg = np.array([0x1000, 0x2000, 0x3000, 0x4000], dtype=np.uint64)
+    return kind, off, tg
+
+
+def small_pair(k0=0x1122334455667788, k1=0x99AABBCCDDEEFF00, digest=42):
+    kind, off, tg = small_policy()
+    eng = B.Engine(0)
+    eng.wg_load_policy(kind, off, tg, k0, k1, digest)
+    return oracle.Oracle(kind, off, tg, k0, k1, digest), eng
+
+
+def test_edge_cases_unknown_site_empty_mask_every_kind_single_lanes():
+    rng = np.random.default_rng(7)
+    orc, eng = small_pair()
+    sites = [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 1000, 0xFFFFFFFF, 0, 2, 5, 0, 0, 2, 3, 3]
+    masks = [FULL, 1, FULL, 0x80000000, FULL, 5, 6, 7, 8, FULL, 0xF0, 1, 0, 0, 0, 0x80000001, 2, 0x10, FULL, 1]
+    n = len(sites)
+    hdr = mk_hdr(sites, masks, rng.integers(0, 1 << 64, n, dtype=np.uint64))
+    val = rng.integers(0, 1 << 64, size=(n, 32), dtype=np.uint64)
+    val[2, :] = 0x2000
+    val[2, 5] = 0x2001          # one lane out of set
+    val[3, 31] = 0x4000
+    val[17, 4] = 0x3000
+    val[18, :] = 0x4000
+    val[18, 9] = 0x3000         # legal for site 2, not for site 3 (wrong-site-valid-target)
+    val[19, 0] = 0
+    o_tag = orc.sign(hdr, val)
+    g_tag = eng.wg_sign_continuations(to_dev(hdr), to_dev(val)).cpu().numpy().view(np.uint64)
+    assert np.array_equal(g_tag, o_tag)
+    tag = o_tag.copy()
+    tag[15, 31] ^= np.uint64(1 << 63)  # forged token in the last lane
+    val[16, 1] ^= np.uint64(1)         # hijacked continuation in lane 1
+    for mode in (DET, ENF):
+        o = orc.verify(hdr, val, tag, mode)
+        g = eng.wg_verify_continuations(to_dev(hdr), to_dev(val), to_dev(tag), mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o), (g, o)
+        o = orc.check_forward(hdr, val, mode)
+        g = eng.wg_check_forward(to_dev(hdr), to_dev(val), mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+    assert_counters_equal(eng, orc)
+    g, _ = eng.wg_read_counters()
+    assert g["events_unknown_site"] == 12 and g["events_empty"] == 12 and g["policy_digest"] == 42
+
+
+def test_inactive_lanes_never_influence_any_output():
+    rng = np.random.default_rng(8)
+    orc, eng = small_pair()
+    n = 4099
+    hdr = mk_hdr(rng.integers(0, 9, n), rng.integers(0, 1 << 32, n), rng.integers(0, 1 << 64, n, dtype=np.uint64))
+    val = rng.integers(0, 1 << 64, size=(n, 32), dtype=np.uint64)
+    tag = orc.sign(hdr, val)
+    a = eng.wg_verify_continuations(to_dev(hdr), to_dev(val), to_dev(tag), ENF).cpu()
+    ca, sa = eng.wg_read_counters()
+    inactive = ((hdr[:, 0:1] >> np.uint64(32)) >> np.arange(32, dtype=np.uint64)[None, :]) & np.uint64(1) == 0
+    val2, tag2 = val.copy(), tag.copy()
+    val2[inactive] = rng.integers(0, 1 << 64, size=int(inactive.sum()), dtype=np.uint64)
+    tag2[inactive] = rng.integers(0, 1 << 64, size=int(inactive.sum()), dtype=np.uint64)
+    eng.wg_reset_counters()
+    b = eng.wg_verify_continuations(to_dev(hdr), to_dev(val2), to_dev(tag2), ENF).cpu()
+    cb, sb = eng.wg_read_counters()
+    assert torch.equal(a, b) and ca == cb and np.array_equal(sa, sb)
+
+
+def test_first_violation_key_is_the_smallest_seq_lane_across_calls_and_resets():
+    orc, eng = small_pair()
+    rng = np.random.default_rng(9)
+    n = 70_001
+    hdr = mk_hdr(np.zeros(n, dtype=np.int64), np.full(n, FULL), np.full(n, 0x40))
+    val = rng.integers(0, 1 << 64, size=(n, 32), dtype=np.uint64)
+    tag = orc.sign(hdr, val)
+    d_hdr, d_val = to_dev(hdr), to_dev(val)
+    eng.wg_verify_continuations(d_hdr, d_val, to_dev(tag), DET)       # clean call: seq advances by n
+    assert eng.wg_read_counters()[0]["first_violation_key"] == U64MAX
+    bad = tag.copy()
+    for e, lane in ((69_999, 0), (40_000, 17), (40_000, 30), (55_555, 3)):
+        bad[e, lane] ^= np.uint64(2)
+    eng.wg_verify_continuations(d_hdr, d_val, to_dev(bad), ENF)
+    orc.verify(hdr, val, tag, DET)
+    orc.verify(hdr, val, bad, ENF)
+    g, _ = eng.wg_read_counters()
+    assert g["first_violation_key"] == ((n + 40_000) << 5 | 17) == orc.read_counters()[0]["first_violation_key"]
+    assert g["last_mode"] == ENF
+    eng.wg_reset_counters()
+    eng.wg_verify_continuations(d_hdr, d_val, to_dev(bad), DET)
+    g, _ = eng.wg_read_counters()
+    assert g["first_violation_key"] == (40_000 << 5 | 17) and g["blocked_lanes"] == 0
+
+
+def test_n_zero_is_a_noop_and_errors_are_status_codes():
+    orc, eng = small_pair()
+    z_hdr = torch.zeros((0, 2), dtype=torch.int64, device=dev())
+    z_val = torch.zeros((0, 32), dtype=torch.int64, device=dev())
+    eng.wg_sign_continuations(z_hdr, z_val)
+    eng.wg_verify_continuations(z_hdr, z_val, z_val, ENF)
+    eng.wg_check_forward(z_hdr, z_val, ENF)
+    g, _ = eng.wg_read_counters()
+    assert g["events_total"] == 0 and g["last_mode"] == 0
+    hdr = to_dev(mk_hdr([0], [FULL], [0]))
+    val = torch.zeros((1, 32), dtype=torch.int64, device=dev())
+    with pytest.raises(B.WgError) as ei:
+        eng.wg_verify_continuations(hdr, val, val, 2)
+    assert ei.value.status == B.WG_ERR_INVALID_ARG
+    with pytest.raises(B.WgError) as ei:  # misaligned value pointer
+        eng.wg_check_forward(hdr, torch.zeros(33, dtype=torch.int64, device=dev())[1:].view(1, 32), DET)
+    assert ei.value.status == B.WG_ERR_INVALID_ARG
+    with pytest.raises(B.WgError) as ei:
+        B.Engine(0).wg_check_forward(hdr, val, DET)
+    assert ei.value.status == B.WG_ERR_NO_POLICY
+
+
+@pytest.mark.parametrize("mutate,why", [
+    (lambda k, o, t: k.__setitem__(4, 7), "kind >= 7"),
+    (lambda k, o, t: o.__setitem__(0, 1), "tgt_off[0] != 0"),
+    (lambda k, o, t: o.__setitem__(3, 5), "offsets decrease"),
+    (lambda k, o, t: t.__setitem__(1, 0x1000), "duplicate target"),
+    (lambda k, o, t: t.__setitem__(2, 0x1800), "unsorted set"),
+    (lambda k, o, t: k.__setitem__(0, 1), "forward site with no targets"),
+    (lambda k, o, t: k.__setitem__(3, 0), "return site owning targets"),
+])
+def test_bad_policy_loads_nothing_and_keeps_the_previous_one(mutate, why):
+    orc, eng = small_pair()
+    kind, off, tg = small_policy()
+    mutate(kind, off, tg)
+    assert oracle.validate_policy(kind, off, tg) != 0, why
+    with pytest.raises(B.WgError) as ei:
+        eng.wg_load_policy(kind, off, tg, 1, 2, 3)
+    assert ei.value.status == B.WG_ERR_BAD_POLICY
+    fresh = B.Engine(0)
+    with pytest.raises(B.WgError):
+        fresh.wg_load_policy(kind, off, tg, 1, 2, 3)
+    assert not fresh._h  # nothing was created
+    # the engine still answers with its previous policy and key
+    hdr = mk_hdr([2, 0], [FULL, FULL], [0, 0])
+    val = np.full((2, 32), 0x3000, dtype=np.uint64)
+    tag = orc.sign(hdr, val)
+    g = eng.wg_verify_continuations(to_dev(hdr), to_dev(val), to_dev(tag), ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, orc.verify(hdr, val, tag, ENF)) and (g[:, 0] == 0).all()
+    assert eng.wg_read_counters()[0]["policy_digest"] == 42
+
+
+def test_replacing_the_policy_resets_counters_and_rekeys():
+    orc, eng = small_pair()
+    hdr = mk_hdr([0], [FULL], [0x20])
+    val = np.arange(32, dtype=np.uint64).reshape(1, 32)
+    t1 = eng.wg_sign_continuations(to_dev(hdr), to_dev(val)).cpu().numpy().view(np.uint64)
+    eng.wg_verify_continuations(to_dev(hdr), to_dev(val), to_dev(t1), ENF)
+    kind, off, tg = small_policy()
+    eng.wg_load_policy(kind, off, tg, 5, 6, 7)
+    g, s = eng.wg_read_counters()
+    assert g["events_total"] == 0 and g["signed_lanes"] == 0 and g["policy_digest"] == 7 and not s.any()
+    out = eng.wg_verify_continuations(to_dev(hdr), to_dev(val), to_dev(t1), ENF).cpu().numpy().view(np.uint32)
+    assert out[0, 0] == FULL and out[0, 1] == 0  # tags of the old key no longer verify (wrong key)
+    o2 = oracle.Oracle(kind, off, tg, 5, 6, 7)
+    assert np.array_equal(o2.verify(hdr, val, t1, ENF), out)
+
+
+def test_host_buffer_entry_points_equal_the_device_ones():
+    st = S.make_stream(4, "cpu", n_events=600_011)  # > 2 staging chunks of 256 Ki events, ragged
+    orc, eng = oracle_for(st.policy), engine_for(st.policy)
+    hdr_np = st.hdr.numpy().view(np.uint64)
+    h_hdr, h_val = st.hdr.pin_memory(), st.val.pin_memory()
+    g_tag = eng.wg_sign_continuations_host(h_hdr, h_val)
+    o_tag = orc.sign(hdr_np, st.val.numpy().view(np.uint64))
+    assert np.array_equal(g_tag.numpy().view(np.uint64), o_tag)
+    st.apply_return_tamper(g_tag)
+    h_val = st.val.pin_memory()
+    o_out = orc.verify(hdr_np, st.val.numpy().view(np.uint64), g_tag.numpy().view(np.uint64), ENF)
+    g_out = eng.wg_verify_continuations_host(h_hdr, h_val, g_tag, ENF)
+    assert np.array_equal(g_out.numpy().view(np.uint32), o_out)
+    o_f = orc.check_forward(hdr_np, st.val.numpy().view(np.uint64), DET)
+    g_f = eng.wg_check_forward_host(h_hdr, h_val, DET)  # pageable or pinned both work
+    assert np.array_equal(g_f.numpy().view(np.uint32), o_f)
+    assert_counters_equal(eng, orc)
+
+
+def test_work_runs_on_the_callers_stream():
+    st = S.make_stream(2, "cpu", n_events=100_000)
+    orc, eng = oracle_for(st.policy), engine_for(st.policy)
+    s = torch.cuda.Stream()
+    d_hdr, d_val = st.hdr.to(dev()), st.val.to(dev())
+    torch.cuda.synchronize()
+    before = B.wg_launch_count()
+    with torch.cuda.stream(s):
+        tag = eng.wg_sign_continuations(d_hdr, d_val)
+        out = eng.wg_verify_continuations(d_hdr, d_val, tag, ENF)
+    s.synchronize()
+    assert B.wg_launch_count() - before == 2
+    assert not out[:, 0].any()
+    assert np.array_equal(tag.cpu().numpy().view(np.uint64), orc.sign(st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)))
