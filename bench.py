@@ -1,0 +1,413 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the WarpGuard check path on B200, one JSON line (contract in the task statement).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 4] [--events E]
+
+Workload (N = 1): BASELINE.json config 4, the mixed paper-shaped stream — 51,621 sites, 58.0 M warp events of
+which 52.2 M are checks on protected sites (38.3 M return + 13.9 M forward), 0.05 % violations,
+enforce mode — generated on the GPU by `streams.py` (seeded, synthetic; stands in for the paper's corpus).
+A STEP is one pass of the whole hot path over that stream:
+    wg_sign_continuations   (a1 a2 a3 a7)      backward push of every return event
+    wg_verify_continuations (a1 a2 a4-a8)      check_ret + forward membership + verdicts + counters
+`value` = checks on protected sites per second over the whole step (sign time included), inputs resident in HBM.
+`e2e` = the same step through the *_host C-ABI calls: events in pinned HOST memory, H2D / D2H inside the timed
+region, on a bounded prefix of the same stream.  `cpu_baseline` = the oracle, as it stands, single-threaded, on a
+bounded prefix of the same stream (and its verdicts are compared with the GPU's while we are at it).
+
+Under torchrun (N > 1) every rank runs its own config-4 stream (weak scaling; no data-path collective — the only
+exchange is the counter all-reduce at read-out, outside the hot loop); timing is max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "cfi_checks_per_sec"
+UNIT = "checks/s"
+# algorithmic integer work: 32-bit integer lane-operations
+OPS_PER_MAC_VERIFY = 310   # 12 SipRounds x 24 + 13 injection + 7 finalisation + 2 compare
+OPS_PER_MAC_SIGN = 308
+# bytes per event
+B_RET_VERIFY, B_RET_SIGN, B_FWD, B_NON = 536, 528, 280, 24
+# traffic of the dominant kernel from the committed ncu --set full capture (profiles/); None until captured
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--events", type=int, default=None, help="events per rank (default: the config's full size)")
+    ap.add_argument("--e2e-events", type=int, default=8_000_000)
+    ap.add_argument("--cpu-events", type=int, default=4_000_000)
+    ap.add_argument("--ref-events", type=int, default=1_000_000, help="events per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text())
+        except Exception:
+            pass
+    return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, uuid: str | None):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        cmd = ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"]
+        if uuid:
+            cmd += ["-i", uuid]
+        try:
+            self.p = subprocess.Popen(cmd, stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def forward_search_ops(st, torch) -> int:
+    """(7 ceil(log2(n+1)) + 3) int32 ops per unique active target of every non-empty forward event
+    (SURVEY.md §8(d)); unique targets = 1 for a warp-uniform event, min(popc(active), n) otherwise."""
+    import numpy as np
+    from paper_2606_11871_b200 import streams as S
+    dev = st.hdr.device
+    kind = torch.from_numpy(st.policy.kind.astype(np.int64)).to(dev)
+    cnt = torch.from_numpy(np.diff(st.policy.tgt_off.astype(np.int64))).to(dev)
+    site = st.site_id()
+    sel = kind[site] == S.PROTECTED_FORWARD
+    n = cnt[site[sel]].double()
+    mask = st.active_mask()[sel]
+    pc = torch.zeros_like(mask)
+    for b in range(32):
+        pc += (mask >> b) & 1
+    uniq = torch.where(st.uniform[sel], torch.ones_like(pc), torch.minimum(pc, n.long()))
+    uniq = torch.where(pc > 0, uniq, torch.zeros_like(uniq))
+    per = 7 * torch.ceil(torch.log2(n + 1)) + 3
+    return int((per * uniq.double()).sum().item())
+
+
+# ---------------------------------------------------------------------------------------------------------
+# reference arm: the oracle, as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------------------
+def run_reference(a) -> None:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return  # rank 0 alone runs and prints it
+    import numpy as np
+    import oracle
+    from paper_2606_11871_b200 import streams as S
+
+    st = S.make_stream(a.config, "cpu", n_events=a.ref_events)
+    pol = st.policy
+    orc = oracle.Oracle(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1, pol.policy_digest)
+    hdr = st.hdr.numpy().view(np.uint64)
+    tag_t = __import__("torch").from_numpy(orc.sign(hdr, st.val.numpy().view(np.uint64)).view(np.int64))
+    st.apply_return_tamper(tag_t)
+    val, tag = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+
+    def step():
+        orc.sign(hdr, val)
+        orc.verify(hdr, val, tag, st.mode)
+
+    for _ in range(a.warmup):
+        step()
+    orc.reset_counters()
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        step()
+    dt = time.perf_counter() - t0
+    g, _ = orc.read_counters()
+    checks = (g["ret_checks"] + g["fwd_checks"]) / a.steps
+    lanes = (g["ret_lanes"] + g["fwd_lanes"]) / a.steps
+    v = checks / (dt / a.steps)
+    sample = f"{a.ref_events} events of config {a.config} per step (same recipe and proportions, seed of the config)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+        "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "lane_verdicts_per_sec": lanes / (dt / a.steps),
+        "config": {"workload": f"config{a.config}-{S.NAMES[a.config]}", "events_per_step": a.ref_events,
+                   "step": "oracle sign + oracle verify", "note": "CPU oracle (g++ -O2, 1 thread); bounded sample"},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------------
+def run_ours(a) -> None:
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_11871_b200 import binding as B
+    from paper_2606_11871_b200 import sharding
+    from paper_2606_11871_b200 import streams as S
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the check path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- inputs, resident in HBM before anything is timed ----
+    n_events = S.FULL_EVENTS[a.config] if a.events is None else a.events
+    if a.config == 5 and a.events is None:
+        n_events = S.CONFIG5_BATCH
+    st = S.make_stream(a.config, dev, n_events=n_events, batch_index=rank)
+    eng = B.Engine(local).load(st.policy)
+    tag = eng.wg_sign_continuations(st.hdr, st.val)          # tokens at push time (engine's own signer)
+    st.apply_return_tamper(tag)                               # then the recorded corruption
+    tag_scratch = torch.empty_like(tag)
+    out = torch.empty((n_events, 2), dtype=torch.int32, device=dev)
+    fwd_ops = forward_search_ops(st, torch)
+    torch.cuda.synchronize()
+
+    def step():
+        eng.wg_sign_continuations(st.hdr, st.val, tag_scratch)
+        eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode, out)
+
+    # integer-pipe ceilings of this GPU, measured now (register-only probe)
+    probes = {}
+    for name, mix in (("iadd3", 0), ("lop3", 1), ("shf", 2), ("imad", 3), ("imad_wide", 4),
+                      ("lop3+imad_1:1", 5), ("sipround_alu_mix", 6), ("alu+imad_2:1", 8)):
+        probes[name] = B.wg_probe_int_pipe(local, mix)[0]
+
+    for _ in range(max(a.warmup, 0)):
+        step()
+    eng.wg_reset_counters()
+    barrier()
+    props = torch.cuda.get_device_properties(local)
+    uuid = "GPU-" + str(props.uuid) if hasattr(props, "uuid") else None
+    sampler = ClockSampler(uuid)
+    launches0 = B.wg_launch_count()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(a.steps)]
+    for k in range(a.steps):
+        ev[k][0].record()
+        eng.wg_sign_continuations(st.hdr, st.val, tag_scratch)
+        ev[k][1].record()
+        eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode, out)
+        ev[k][2].record()
+    barrier()
+    clocks = sampler.stop()
+    launches = B.wg_launch_count() - launches0
+    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+    sign_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / a.steps
+    verify_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / a.steps
+    g, _ = eng.wg_read_counters(per_site=False)
+
+    # ---- what one step judged (counters accumulated over K identical steps) ----
+    K = a.steps
+    for k in ("ret_checks", "fwd_checks", "ret_lanes", "fwd_lanes", "ret_viol_events", "fwd_viol_events"):
+        assert g[k] % K == 0, (k, g[k])
+    checks = (g["ret_checks"] + g["fwd_checks"]) // K
+    lanes = (g["ret_lanes"] + g["fwd_lanes"]) // K
+    # properties that hold at any size: every planned corruption is found, nothing else is
+    assert g["ret_viol_events"] // K == len(st.ret_tamper), (g["ret_viol_events"], len(st.ret_tamper))
+    assert g["fwd_viol_events"] // K == len(st.fwd_tamper), (g["fwd_viol_events"], len(st.fwd_tamper))
+    assert g["events_total"] // K == n_events
+    ret_ev, fwd_ev = g["ret_checks"] // K, g["fwd_checks"] // K
+    non_ev = n_events - ret_ev - fwd_ev
+
+    t = torch.tensor([total_ms, sign_ms, verify_ms], dtype=torch.float64, device=dev)
+    tot = torch.tensor([checks, lanes], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    total_ms, sign_ms, verify_ms = t.tolist()
+    all_checks, all_lanes = tot.tolist()
+    ms_per_step = total_ms / K
+    value = all_checks / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (the check kernel of wg_verify_continuations) ----
+    peaks = measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    n_sm = props.multi_processor_count
+    # one warp instruction per cycle per SM sub-partition = 128 int32 lane-ops / SM / clk when the
+    # ALU pipe (64 / SM / clk) and the FMA pipe's IMAD (64 / SM / clk) are both fed; the larger of that derived
+    # figure and every measured probe is the denominator, so a weak probe cannot flatter the fraction.
+    derived_peak = 128.0 * n_sm * sm_max_mhz * 1e6
+    alu_peak = max([derived_peak] + list(probes.values()))
+    verify_ops = OPS_PER_MAC_VERIFY * (g["ret_lanes"] // K) + fwd_ops
+    verify_bytes = B_RET_VERIFY * ret_ev + B_FWD * fwd_ev + B_NON * non_ev
+    sign_ops = OPS_PER_MAC_SIGN * (g["ret_lanes"] // K)
+    t_alu = verify_ops / alu_peak
+    t_hbm = verify_bytes / (hbm_peak * 1e9)
+    achieved = verify_ops / (verify_ms * 1e-3)
+    roofline = {
+        "kernel": "wg_check (wg_verify_continuations)",
+        "bound": "alu" if t_alu >= t_hbm else "hbm",
+        "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tint32op/s", "frac": achieved / alu_peak,
+        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+        "peak_source": ("derived: 128 lanes/SM/clk x %d SMs x %.0f MHz (DESIGN.md §6); max with the measured probes"
+                        % (n_sm, sm_max_mhz)),
+        "ms_per_launch": verify_ms, "algorithmic_ops_per_launch": verify_ops,
+        "algorithmic_bytes_per_launch": verify_bytes,
+        "hbm_achieved_gbs": verify_bytes / (verify_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
+        "hbm_frac": verify_bytes / (verify_ms * 1e-3) / 1e9 / hbm_peak,
+        "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback",
+        "t_roof_ms": 1e3 * max(t_alu, t_hbm), "frac_of_roof_time": max(t_alu, t_hbm) / (verify_ms * 1e-3),
+        "sign_kernel": {"ms_per_launch": sign_ms, "achieved": sign_ops / (sign_ms * 1e-3) / 1e12,
+                        "frac": sign_ops / (sign_ms * 1e-3) / alu_peak,
+                        "hbm_achieved_gbs": (B_RET_SIGN * ret_ev + 16 * (n_events - ret_ev) + 256 * (n_events - ret_ev))
+                        / (sign_ms * 1e-3) / 1e9},
+        "probes_Tops": {k: v / 1e12 for k, v in probes.items()},
+    }
+
+    # ---- end to end: HOST buffers through the *_host C-ABI calls, copies inside the timed region ----
+    e2e = None
+    ne = min(a.e2e_events, n_events)
+    h = {}
+    if not a.no_e2e or not a.no_cpu_baseline:
+        h["hdr"] = st.hdr[:ne].cpu().pin_memory()
+        h["val"] = st.val[:ne].cpu().pin_memory()
+        h["tag"] = tag[:ne].cpu().pin_memory()
+    if not a.no_e2e:
+        h_scratch = torch.empty((ne, 32), dtype=torch.int64).pin_memory()
+        h_out = torch.empty((ne, 2), dtype=torch.int32).pin_memory()
+
+        def e2e_step():
+            eng.wg_sign_continuations_host(h["hdr"], h["val"], h_scratch)
+            eng.wg_verify_continuations_host(h["hdr"], h["val"], h["tag"], st.mode, h_out)
+
+        e2e_step()
+        eng.wg_reset_counters()
+        barrier()
+        reps = 3
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / reps
+        ge, _ = eng.wg_read_counters(per_site=False)
+        e_checks = (ge["ret_checks"] + ge["fwd_checks"]) / reps
+        assert torch.equal(h_out, out[:ne].cpu()), "host-buffer path and device-buffer path disagree"
+        te = torch.tensor([dt], dtype=torch.float64, device=dev)
+        ce = torch.tensor([e_checks], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            dist.all_reduce(ce, op=dist.ReduceOp.SUM)
+        e2e = {"value": ce.item() / te.item(), "unit": UNIT,
+               "h2d_bytes_per_step": ne * ((16 + 256) + (16 + 256 + 256)), "d2h_bytes_per_step": ne * (256 + 8),
+               "events_per_step": ne, "ms_per_step": 1e3 * te.item(),
+               "api": "wg_sign_continuations_host + wg_verify_continuations_host (pinned host buffers)"}
+
+    # ---- the oracle beside it (rank 0, N = 1 only) ----
+    cpu = None
+    if not a.no_cpu_baseline and world == 1:
+        import oracle
+        nc = min(a.cpu_events, ne)
+        pol = st.policy
+        orc = oracle.Oracle(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1, pol.policy_digest)
+        hh, hv, ht = (h[k][:nc].numpy().view(np.uint64) for k in ("hdr", "val", "tag"))
+        t0 = time.perf_counter()
+        orc.sign(hh, hv)
+        o_out = orc.verify(hh, hv, ht, st.mode)
+        dt = time.perf_counter() - t0
+        og, _ = orc.read_counters(per_site=False)
+        same = np.array_equal(o_out, out[:nc].cpu().numpy().view(np.uint32))
+        assert same, "GPU verdicts differ from the oracle on the cpu_baseline sample"
+        cpu = {"value": (og["ret_checks"] + og["fwd_checks"]) / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"first {nc} events of the same stream, oracle sign + verify, {dt:.1f} s; "
+                         f"verdicts equal the GPU's on all {nc} events",
+               "lane_verdicts_per_sec": (og["ret_lanes"] + og["fwd_lanes"]) / dt}
+
+    # ---- read-out exchange (outside the hot loop): counters summed over ranks ----
+    gr, _ = sharding.reduce_counters(g, None, 0, device=dev)
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": a.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u64", "data": "synthetic",
+            "lane_verdicts_per_sec": all_lanes / (ms_per_step * 1e-3),
+            "verify_only_checks_per_sec": all_checks / (verify_ms * 1e-3),
+            "config": {"workload": f"config{a.config}-{S.NAMES[a.config]}", "events_per_gpu": n_events,
+                       "checks_per_step": int(all_checks), "lane_verdicts_per_step": int(all_lanes),
+                       "n_sites": st.policy.n_sites, "mode": "enforce" if st.mode else "detect",
+                       "step": "wg_sign_continuations + wg_verify_continuations over the whole stream",
+                       "l2": "inputs (%.1f GB per step) are far larger than the 126 MB L2; no flush needed"
+                             % ((verify_bytes + B_RET_SIGN * ret_ev) / 1e9),
+                       "parallelism": "1 GPU" if world == 1 else f"{world} ranks x own stream, counters all-reduced at read-out"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            "counters": {k: gr[k] for k in ("events_total", "ret_checks", "fwd_checks", "ret_viol", "fwd_viol",
+                                           "blocked_lanes", "first_violation_key")},
+        }))
+    eng.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
+
+
+if __name__ == "__main__":
+    main()

@@ -432,7 +432,8 @@ def make_stream(config: int, device="cpu", *, n_events: int | None = None, polic
         n = CONFIG5_BATCH
     if policy is None:
         policy = make_policy(config, device, n_sites=n_sites, max_set=max_set)
-    seed = (config - 1) + 1000 + (7919 * (batch_index + 1) if config == 5 else 0)
+    # batch_index > 0 on configs 1-4 gives the independent streams of the other ranks of a weak-scaling run
+    seed = (config - 1) + 1000 + (7919 * (batch_index + 1) if config == 5 else 7919 * batch_index)
     g = _gen(seed, device)
     kind_t = torch.from_numpy(policy.kind.astype(np.int64)).to(device)
     ns = policy.n_sites
