@@ -72,15 +72,14 @@ def measured_peaks() -> dict:
 
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    Q = ("uuid,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, uuid: str | None):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.uuid = (uuid or "").lower()
         cmd = ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"]
-        if uuid:
-            cmd += ["-i", uuid]
         try:
             self.p = subprocess.Popen(cmd, stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
@@ -98,10 +97,11 @@ class ClockSampler:
         self.f.seek(0)
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.f.read().splitlines():
-            c = [x.strip() for x in line.split(",")]
-            if len(c) < 7:
-                continue
+        rows = [[x.strip() for x in line.split(",")] for line in self.f.read().splitlines()]
+        rows = [c for c in rows if len(c) >= 8]
+        mine = [c for c in rows if self.uuid and self.uuid in c[0].lower()]
+        for c in (mine or rows):  # this rank's GPU; every visible GPU if the uuid could not be matched
+            c = c[1:]
             try:
                 sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
             except ValueError:
@@ -233,7 +233,8 @@ def run_ours(a) -> None:
     # integer-pipe ceilings of this GPU, measured now (register-only probe)
     probes = {}
     for name, mix in (("iadd3", 0), ("lop3", 1), ("shf", 2), ("imad", 3), ("imad_wide", 4),
-                      ("lop3+imad_1:1", 5), ("sipround_alu_mix", 6), ("alu+imad_2:1", 8)):
+                      ("lop3+imad_1:1", 5), ("sipround_alu_mix", 6), ("imad_hi", 7), ("alu+imad_2:1", 8),
+                      ("shf+imad_hi_1:1", 9), ("add64_pairs", 10)):
         probes[name] = B.wg_probe_int_pipe(local, mix)[0]
 
     for _ in range(max(a.warmup, 0)):
@@ -241,7 +242,7 @@ def run_ours(a) -> None:
     eng.wg_reset_counters()
     barrier()
     props = torch.cuda.get_device_properties(local)
-    uuid = "GPU-" + str(props.uuid) if hasattr(props, "uuid") else None
+    uuid = str(props.uuid) if hasattr(props, "uuid") else None
     sampler = ClockSampler(uuid)
     launches0 = B.wg_launch_count()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(a.steps)]

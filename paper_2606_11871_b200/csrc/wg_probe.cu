@@ -18,6 +18,7 @@ constexpr int kThreads = 256;
 #define STEP_SHF(x, y) asm volatile("shf.l.wrap.b32 %0, %0, %1, 13;" : "+r"(x) : "r"(y))
 #define STEP_IMAD(x, y) asm volatile("mad.lo.u32 %0, %0, %1, %1;" : "+r"(x) : "r"(y))
 #define STEP_IMADHI(x, y) asm volatile("mad.hi.u32 %0, %0, %1, %1;" : "+r"(x) : "r"(y))
+#define STEP_IMADX(x, y) asm volatile("{ .reg .b32 t; add.cc.u32 t, %0, %1; madc.lo.u32 %0, %0, 1, %1; }" : "+r"(x) : "r"(y))
 #define STEP_WIDE(x64, y) asm volatile("{ .reg .b32 lo, hi; mov.b64 {lo, hi}, %0; mad.wide.u32 %0, lo, %1, %0; }" : "+l"(x64) : "r"(y))
 
 template <int MIX>
@@ -34,25 +35,32 @@ __global__ void __launch_bounds__(kThreads) wg_int_probe(uint32_t* sink, uint32_
     for (int s = 0; s < kInner; ++s) {
 #pragma unroll
       for (int i = 0; i < kChains; ++i) {
-        if (MIX == 0) STEP_IADD(x[i], y);
-        if (MIX == 1) STEP_LOP(x[i], y);
-        if (MIX == 2) STEP_SHF(x[i], y);
-        if (MIX == 3) STEP_IMAD(x[i], y);
-        if (MIX == 4) STEP_WIDE(w[i], y);
+        // the second operand is the NEIGHBOUR chain's current value: no step can be folded algebraically
+        // (x ^ y ^ y, x + y + y -> one IADD3) and every step still has kChains independent instructions in flight
+        uint32_t& o = x[(i + 1) % kChains];
+        if (MIX == 0) STEP_IADD(x[i], o);
+        if (MIX == 1) STEP_LOP(x[i], o);
+        if (MIX == 2) STEP_SHF(x[i], o);
+        if (MIX == 3) STEP_IMAD(x[i], o);
+        if (MIX == 4) STEP_WIDE(w[i], static_cast<uint32_t>(w[(i + 1) % kChains]));
         if (MIX == 5) {  // ALU : FMA = 1 : 1
-          if (i & 1) STEP_LOP(x[i], y); else STEP_IMAD(x[i], y);
+          if (i & 1) STEP_LOP(x[i], o); else STEP_IMAD(x[i], o);
         }
         if (MIX == 6) {  // SipRound-shaped ALU mix 1 : 1 : 1
-          if ((s + i) % 3 == 0) STEP_IADD(x[i], y);
-          if ((s + i) % 3 == 1) STEP_LOP(x[i], y);
-          if ((s + i) % 3 == 2) STEP_SHF(x[i], y);
+          if ((s + i) % 3 == 0) STEP_IADD(x[i], o);
+          if ((s + i) % 3 == 1) STEP_LOP(x[i], o);
+          if ((s + i) % 3 == 2) STEP_SHF(x[i], o);
         }
-        if (MIX == 7) STEP_IMADHI(x[i], y);
+        if (MIX == 7) STEP_IMADHI(x[i], o);
         if (MIX == 8) {  // ALU : FMA = 2 : 1
-          if ((s + i) % 3 == 0) STEP_IMAD(x[i], y);
-          if ((s + i) % 3 == 1) STEP_LOP(x[i], y);
-          if ((s + i) % 3 == 2) STEP_SHF(x[i], y);
+          if ((s + i) % 3 == 0) STEP_IMAD(x[i], o);
+          if ((s + i) % 3 == 1) STEP_LOP(x[i], o);
+          if ((s + i) % 3 == 2) STEP_SHF(x[i], o);
         }
+        if (MIX == 9) {  // ALU : FMA = 1 : 1 with IMAD.HI on the FMA side
+          if (i & 1) STEP_SHF(x[i], o); else STEP_IMADHI(x[i], o);
+        }
+        if (MIX == 10) STEP_IMADX(x[i], o);
       }
     }
   }
@@ -104,6 +112,8 @@ cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double*
     case 6: err = run<6>(sm_count, sink, ops_per_s, ms); break;
     case 7: err = run<7>(sm_count, sink, ops_per_s, ms); break;
     case 8: err = run<8>(sm_count, sink, ops_per_s, ms); break;
+    case 9: err = run<9>(sm_count, sink, ops_per_s, ms); break;
+    case 10: err = run<10>(sm_count, sink, ops_per_s, ms); break;
     default: err = cudaErrorInvalidValue;
   }
   cudaFree(sink);
