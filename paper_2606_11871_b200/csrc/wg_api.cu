@@ -18,6 +18,8 @@ struct wg_engine {
   uint32_t n_sites = 0;
   uint64_t n_tgts = 0;
   wg::SiteRow* d_rows = nullptr;
+  wg::SiteRec* d_recs = nullptr;  // v2 site records (kind, set range, pre-A SipHash mid-state), 64 B each
+  int impl = 2;                   // 2 = tiled kernels (default); 1 = baseline warp-per-event kernels (WG_IMPL=v1)
   uint64_t* d_tgts = nullptr;
   unsigned long long* d_glob = nullptr;  // [C_WORDS]
   unsigned long long* d_site = nullptr;  // [n_sites][4]
@@ -83,6 +85,8 @@ bool policy_ok(const wg_policy_desc* d) {
 
 void free_tables(wg_engine* e) {
   cudaFree(e->d_rows);
+  cudaFree(e->d_recs);
+  e->d_recs = nullptr;
   cudaFree(e->d_tgts);
   cudaFree(e->d_glob);
   cudaFree(e->d_site);
@@ -119,6 +123,8 @@ wg::Params base_params(const wg_engine* e) {
   wg::Params p;
   std::memset(&p, 0, sizeof(p));
   p.rows = e->d_rows;
+  p.recs = e->d_recs;
+  p.n_tgts = e->n_tgts;
   p.tgts = e->d_tgts;
   p.glob = e->d_glob;
   p.site = e->d_site;
@@ -129,6 +135,8 @@ wg::Params base_params(const wg_engine* e) {
   p.v3 = e->v_init[3];
   return p;
 }
+
+constexpr uint64_t kMaxLaunchEvents = 1ull << 30;
 
 wg_status check_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d_val, const uint64_t* d_tag,
                        bool has_tag, wg_verdict* d_out, uint64_t n, wg_mode mode, cudaStream_t st) {
@@ -141,16 +149,20 @@ wg_status check_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* 
   if (n > (1ull << 58)) return WG_ERR_INVALID_ARG;  // (seq << 5) must not wrap
   DeviceGuard g(e->device);
   if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
-  wg::Params p = base_params(e);
-  p.hdr = reinterpret_cast<const uint4*>(d_hdr);
-  p.val = d_val;
-  p.tag = has_tag ? d_tag : nullptr;
-  p.out = reinterpret_cast<uint2*>(d_out);
-  p.n = n;
-  p.seq_base = e->seq;
-  p.mode = static_cast<uint32_t>(mode);
-  WG_CUDA(e, wg::launch_check(p, e->sm_count, st));
-  e->seq += n;
+  // one launch covers at most kMaxLaunchEvents events: the kernels keep per-warp counters in 32-bit registers
+  for (uint64_t lo = 0; lo < n; lo += kMaxLaunchEvents) {
+    const uint64_t m = (n - lo < kMaxLaunchEvents) ? (n - lo) : kMaxLaunchEvents;
+    wg::Params p = base_params(e);
+    p.hdr = reinterpret_cast<const uint4*>(d_hdr + lo);
+    p.val = d_val + lo * 32;
+    p.tag = has_tag ? d_tag + lo * 32 : nullptr;
+    p.out = reinterpret_cast<uint2*>(d_out + lo);
+    p.n = m;
+    p.seq_base = e->seq;
+    p.mode = static_cast<uint32_t>(mode);
+    WG_CUDA(e, e->impl == 1 ? wg::launch_check_v1(p, e->sm_count, st) : wg::launch_check_v2(p, e->sm_count, st));
+    e->seq += m;
+  }
   e->last_mode = static_cast<uint64_t>(mode);
   return WG_OK;
 }
@@ -163,12 +175,15 @@ wg_status sign_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d
   if (!aligned(d_hdr, 16) || !aligned(d_val, 16) || !aligned(d_tag, 16)) return WG_ERR_INVALID_ARG;
   DeviceGuard g(e->device);
   if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
-  wg::Params p = base_params(e);
-  p.hdr = reinterpret_cast<const uint4*>(d_hdr);
-  p.val = d_val;
-  p.tag_out = d_tag;
-  p.n = n;
-  WG_CUDA(e, wg::launch_sign(p, e->sm_count, st));
+  for (uint64_t lo = 0; lo < n; lo += kMaxLaunchEvents) {
+    const uint64_t m = (n - lo < kMaxLaunchEvents) ? (n - lo) : kMaxLaunchEvents;
+    wg::Params p = base_params(e);
+    p.hdr = reinterpret_cast<const uint4*>(d_hdr + lo);
+    p.val = d_val + lo * 32;
+    p.tag_out = d_tag + lo * 32;
+    p.n = m;
+    WG_CUDA(e, e->impl == 1 ? wg::launch_sign_v1(p, e->sm_count, st) : wg::launch_sign_v2(p, e->sm_count, st));
+  }
   return WG_OK;
 }
 
@@ -295,7 +310,13 @@ wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc
   if ((err = cudaDeviceGetAttribute(&tmp.sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess)
     return fail(err);
   if ((err = cudaMalloc(&tmp.d_rows, sizeof(wg::SiteRow) * (n ? n : 1))) != cudaSuccess) return fail(err);
-  if ((err = cudaMalloc(&tmp.d_tgts, sizeof(uint64_t) * (nt ? nt : 1))) != cudaSuccess) return fail(err);
+  // the target table is padded to an even element count so that the TMA bulk copy that stages it moves whole
+  // 16-byte units; the pad element is never addressed by a search
+  const uint64_t nt_pad = (nt + 1) & ~1ull;
+  if ((err = cudaMalloc(&tmp.d_tgts, sizeof(uint64_t) * (nt_pad ? nt_pad : 2))) != cudaSuccess) return fail(err);
+  if ((err = cudaMemset(tmp.d_tgts, 0, sizeof(uint64_t) * (nt_pad ? nt_pad : 2))) != cudaSuccess) return fail(err);
+  if ((err = cudaMalloc(&tmp.d_recs, sizeof(wg::SiteRec) * (n ? n : 1))) != cudaSuccess) return fail(err);
+  if ((err = wg::init_v2()) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_glob, sizeof(unsigned long long) * wg::C_WORDS)) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_site, sizeof(unsigned long long) * 4 * (n ? n : 1))) != cudaSuccess) return fail(err);
   if (n && (err = cudaMemcpy(tmp.d_rows, rows.data(), sizeof(wg::SiteRow) * n, cudaMemcpyHostToDevice)) != cudaSuccess)
@@ -321,6 +342,7 @@ wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc
   e->n_sites = n;
   e->n_tgts = nt;
   e->d_rows = tmp.d_rows;
+  e->d_recs = tmp.d_recs;
   e->d_tgts = tmp.d_tgts;
   e->d_glob = tmp.d_glob;
   e->d_site = tmp.d_site;
@@ -330,6 +352,19 @@ wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc
   e->v_init[2] = desc->key[0] ^ 0x6c7967656e657261ull;
   e->v_init[3] = desc->key[1] ^ 0x7465646279746573ull;
   e->digest = desc->policy_digest;
+  {
+    const char* impl = std::getenv("WG_IMPL");  // measurement knob: the baseline kernels stay selectable
+    e->impl = (impl && impl[0] == 'v' && impl[1] == '1') ? 1 : 2;
+  }
+  // per-site SipHash mid-states, computed on the device from the key-derived initial state
+  {
+    cudaError_t e3 = wg::launch_build_recs(e->d_recs, e->d_rows, n, e->v_init[0], e->v_init[1], e->v_init[2],
+                                           e->v_init[3], nullptr);
+    if (e3 != cudaSuccess) {
+      free_tables(e);
+      return cuda_fail(e, e3);
+    }
+  }
   e->loaded = true;
   *eng = e;
   wg_status s = zero_counters(e, nullptr);

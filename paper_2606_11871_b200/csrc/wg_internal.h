@@ -15,6 +15,19 @@ struct __align__(16) SiteRow {
   uint32_t pad;
 };
 
+// v2 site record: one 64-byte line per site (never straddles a 128-byte cache line), gathered once per event.
+//   words 0-3   kind, off, cnt, 0          (same meaning as SiteRow)
+//   words 4-11  protected-return sites: SipHash state after absorbing LE64(site_id), with quarter-round A of the
+//               next round already applied ("pre-A" mid-state, wg_sip32.cuh), as v0l v0h v1l v1h v2l v2h v3l v3h.
+//               Key-derived, so it lives only in engine-owned memory.  Zero for other kinds.
+//   words 12-15 reserved (0)
+struct __align__(16) SiteRec {
+  uint32_t kind, off, cnt, pad0;
+  uint32_t st[8];
+  uint32_t pad1[4];
+};
+static_assert(sizeof(SiteRec) == 64, "SiteRec is one 64-byte line");
+
 // Global counter block: the first 26 words have exactly the layout of wg_counters, so a read-out is one
 // copy.  Words 24 (policy_digest) and 25 (last_mode) are kept host-side and patched in at read-out.
 enum CounterWord {
@@ -54,8 +67,10 @@ struct Params {
   uint2* out;                // [n] wg_verdict
   uint64_t n;
   uint64_t seq_base;         // running event index of event 0 of this call (R12)
-  const SiteRow* rows;
+  const SiteRow* rows;       // v1 kernels
+  const SiteRec* recs;       // v2 kernels
   const uint64_t* tgts;
+  uint64_t n_tgts;           // elements in tgts (v2 stages the whole table in shared memory when it is small)
   unsigned long long* glob;  // [C_WORDS]
   unsigned long long* site;  // [n_sites][4]
   uint32_t n_sites;
@@ -64,8 +79,14 @@ struct Params {
 };
 
 // launchers (wg_kernels.cu); grid sizing from the SM count of the engine's device
-cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st);
-cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st);
+cudaError_t launch_sign_v1(const Params& p, int sm_count, cudaStream_t st);
+cudaError_t launch_check_v1(const Params& p, int sm_count, cudaStream_t st);
+// v2 (wg_kernels_v2.cu): tiled, cp.async-staged, mid-state-cached kernels
+cudaError_t launch_sign_v2(const Params& p, int sm_count, cudaStream_t st);
+cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st);
+cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sites, uint64_t v0, uint64_t v1,
+                              uint64_t v2, uint64_t v3, cudaStream_t st);
+cudaError_t init_v2();  // one-time function attributes (dynamic shared memory opt-in)
 cudaError_t launch_fill_u64(unsigned long long* p, uint64_t n, unsigned long long v, cudaStream_t st);
 cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double* ms);
 void count_launch();

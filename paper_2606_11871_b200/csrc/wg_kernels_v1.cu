@@ -1,4 +1,5 @@
-// wg_kernels.cu — the check path on sm_100a: sign (a3), verify (a4), forward membership (a5), verdicts (a6),
+// wg_kernels_v1.cu — the FIRST (baseline) mapping of the check path on sm_100a, kept selectable (WG_IMPL=v1) so
+// that the v2 kernels of wg_kernels_v2.cu can be measured against it (profiles/):  sign (a3), verify (a4), forward membership (a5), verdicts (a6),
 // aggregated counters (a7) and the first-violation record (a8) of SURVEY.md §8(a).
 //
 // Mapping (v1, "warp per event"): one warp owns one event at a time, thread l owns lane l of it.  The 16-byte
@@ -227,13 +228,13 @@ int grid_for(uint64_t n_events, int sm_count, int ctas_per_sm) {
 
 }  // namespace
 
-cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st) {
+cudaError_t launch_sign_v1(const Params& p, int sm_count, cudaStream_t st) {
   wg_sign_v1<<<grid_for(p.n, sm_count, 8), kThreads, 0, st>>>(p);
   count_launch();
   return cudaGetLastError();
 }
 
-cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st) {
+cudaError_t launch_check_v1(const Params& p, int sm_count, cudaStream_t st) {
   const int grid = grid_for(p.n, sm_count, 8);
   if (p.tag)
     wg_check_v1<true><<<grid, kThreads, 0, st>>>(p);

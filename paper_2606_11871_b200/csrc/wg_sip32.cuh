@@ -1,0 +1,141 @@
+// wg_sip32.cuh — SipHash-2-4 on 32-bit register halves, for the v2 (tiled) kernels.
+//
+// token = SipHash-2-4_key( LE64(site_id) || LE64(continuation) || LE64(context_id) ), 64-bit output
+// (R1-R4; formula lost at PAPER.md:164-166 / 244-246, "keyed token" over the return state
+// PAPER.md:162, 258).  Three message words + the length word 0x18<<56, c = 2, d = 4: 12 SipRounds.
+//
+// Why halves: sm_100a has no 64-bit integer ALU.  Written on explicit lo/hi registers the round is exactly
+//     4 x (IADD3 + carry IADD3.X / IMAD.X)   8 x LOP3   8 x SHF.L.W   rotate-by-32 = register rename
+// = 24 instructions and no MOV / pack traffic (the 64-bit formulation of v1 cost ~40 per round).  Measured
+// issue costs on B200 (wg_probe_int_pipe): IADD3 / LOP3 128 lanes/SM/clk, SHF / IMAD 64.
+//
+// The round is split in its four quarter-steps so that work which does not depend on the next message word
+// can be hoisted: a word m enters through v3 only, and quarter A touches (v0, v1) only, so A of the first
+// round after an injection can run BEFORE the word is known ("pre-A" states).
+#pragma once
+#include <cstdint>
+
+namespace wg {
+
+struct Sip32 {
+  uint32_t v0l, v0h, v1l, v1h, v2l, v2h, v3l, v3h;
+};
+
+// a += b (64-bit) on halves; ptxas picks IADD3 + IADD3.X or IMAD.X for the carry half
+__device__ __forceinline__ void add64(uint32_t& al, uint32_t& ah, uint32_t bl, uint32_t bh) {
+  asm("add.cc.u32 %0, %0, %2;\n\taddc.u32 %1, %1, %3;" : "+r"(al), "+r"(ah) : "r"(bl), "r"(bh));
+}
+
+// (l, h) = rotl64((l, h), B), 0 < B < 64, B != 32: two funnel shifts
+template <int B>
+__device__ __forceinline__ void rotl64(uint32_t& l, uint32_t& h) {
+  static_assert(B > 0 && B < 64 && B != 32, "rotate amount");
+  const uint32_t ol = l, oh = h;
+  if constexpr (B < 32) {
+    h = __funnelshift_l(ol, oh, B);  // (oh << B) | (ol >> (32 - B))
+    l = __funnelshift_l(oh, ol, B);
+  } else {
+    h = __funnelshift_l(oh, ol, B - 32);
+    l = __funnelshift_l(ol, oh, B - 32);
+  }
+}
+
+__device__ __forceinline__ void swap32(uint32_t& l, uint32_t& h) {
+  const uint32_t t = l;
+  l = h;
+  h = t;
+}
+
+// quarter A: v0 += v1; v1 = rotl(v1,13); v1 ^= v0; v0 = rotl(v0,32)
+__device__ __forceinline__ void sip_qA(Sip32& s) {
+  add64(s.v0l, s.v0h, s.v1l, s.v1h);
+  rotl64<13>(s.v1l, s.v1h);
+  s.v1l ^= s.v0l;
+  s.v1h ^= s.v0h;
+  swap32(s.v0l, s.v0h);
+}
+// quarter B: v2 += v3; v3 = rotl(v3,16); v3 ^= v2
+__device__ __forceinline__ void sip_qB(Sip32& s) {
+  add64(s.v2l, s.v2h, s.v3l, s.v3h);
+  rotl64<16>(s.v3l, s.v3h);
+  s.v3l ^= s.v2l;
+  s.v3h ^= s.v2h;
+}
+// quarter C: v0 += v3; v3 = rotl(v3,21); v3 ^= v0
+__device__ __forceinline__ void sip_qC(Sip32& s) {
+  add64(s.v0l, s.v0h, s.v3l, s.v3h);
+  rotl64<21>(s.v3l, s.v3h);
+  s.v3l ^= s.v0l;
+  s.v3h ^= s.v0h;
+}
+// quarter D: v2 += v1; v1 = rotl(v1,17); v1 ^= v2; v2 = rotl(v2,32)
+__device__ __forceinline__ void sip_qD(Sip32& s) {
+  add64(s.v2l, s.v2h, s.v1l, s.v1h);
+  rotl64<17>(s.v1l, s.v1h);
+  s.v1l ^= s.v2l;
+  s.v1h ^= s.v2h;
+  swap32(s.v2l, s.v2h);
+}
+
+__device__ __forceinline__ void sip_round(Sip32& s) {
+  sip_qA(s);
+  sip_qB(s);
+  sip_qC(s);
+  sip_qD(s);
+}
+
+// one message word, c = 2 rounds
+__device__ __forceinline__ void sip_absorb(Sip32& s, uint32_t ml, uint32_t mh) {
+  s.v3l ^= ml;
+  s.v3h ^= mh;
+  sip_round(s);
+  sip_round(s);
+  s.v0l ^= ml;
+  s.v0h ^= mh;
+}
+// the same when quarter A of the first round was already applied to s (a "pre-A" state)
+__device__ __forceinline__ void sip_absorb_preA(Sip32& s, uint32_t ml, uint32_t mh) {
+  s.v3l ^= ml;
+  s.v3h ^= mh;
+  sip_qB(s);
+  sip_qC(s);
+  sip_qD(s);
+  sip_round(s);
+  s.v0l ^= ml;
+  s.v0h ^= mh;
+}
+
+// length word of the 24-byte message: 0x18 << 56, i.e. lo = 0, hi = 0x18000000
+constexpr uint32_t kLenHi = 0x18000000u;
+
+// absorb the length word, then d = 4 finalisation rounds; the 64-bit output is returned XORed with
+// (xl, xh) — pass the stored tag to get 0 exactly when the token matches, or 0 to get the token itself.
+__device__ __forceinline__ void sip_finish(Sip32& s, uint32_t xl, uint32_t xh, uint32_t& outl, uint32_t& outh) {
+  s.v3h ^= kLenHi;
+  sip_round(s);
+  sip_round(s);
+  s.v0h ^= kLenHi;
+  s.v2l ^= 0xffu;
+  sip_round(s);
+  sip_round(s);
+  sip_round(s);
+  sip_round(s);
+  outl = (s.v0l ^ s.v1l) ^ (s.v2l ^ s.v3l) ^ xl;
+  outh = (s.v0h ^ s.v1h) ^ (s.v2h ^ s.v3h) ^ xh;
+}
+
+// per-lane tail when the event's pre-A state already covers site and continuation (warp-uniform continuation)
+__device__ __forceinline__ void sip_tail_ctx(Sip32 s, uint32_t cl, uint32_t ch, uint32_t xl, uint32_t xh,
+                                             uint32_t& outl, uint32_t& outh) {
+  sip_absorb_preA(s, cl, ch);
+  sip_finish(s, xl, xh, outl, outh);
+}
+// per-lane tail from the site's pre-A state (lane-divergent continuation)
+__device__ __forceinline__ void sip_tail_val_ctx(Sip32 s, uint32_t vl, uint32_t vh, uint32_t cl, uint32_t ch,
+                                                 uint32_t xl, uint32_t xh, uint32_t& outl, uint32_t& outh) {
+  sip_absorb_preA(s, vl, vh);
+  sip_absorb(s, cl, ch);
+  sip_finish(s, xl, xh, outl, outh);
+}
+
+}  // namespace wg
