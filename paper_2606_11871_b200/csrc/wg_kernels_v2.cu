@@ -1,9 +1,14 @@
-// wg_kernels_v2.cu — the check path on sm_100a, second mapping: a warp owns a TILE of T consecutive events.
+// wg_kernels_v2.cu — the check path on sm_100a, second mapping: a warp owns a TILE of 16 consecutive events.
 //
 // Steps: a1 event fetch + guard, a2 policy lookup, a3 MAC sign, a4 MAC verify + compare,
 // a5 forward membership, a6 verdicts, a7 counters, a8 first-violation record.  Paper passages: backward token
 // PAPER.md:162, 248; forward membership PAPER.md:174-178, 250-252; guards PAPER.md:190, 230; detect / enforce
 // PAPER.md:264; accounting PAPER.md:113, 127, 224.  Readings: DESIGN.md §2.  Kernel design: DESIGN.md §6.
+//
+// What bounds it (measured, profiles/): the SipRound is 20 ALU-pipe instructions (4 IADD3 with carry-out,
+// 8 LOP3, 8 SHF) + 4 IMAD.X on the FMA pipe, and every ALU-pipe instruction costs 2 issue cycles per warp on
+// sm_100a, so a round is 40 cycles per warp per SM sub-partition whatever the occupancy or ILP.  The kernel is
+// therefore built to (1) run fewer rounds and (2) spend as few ALU-pipe instructions as possible on anything else.
 //
 // Per tile the warp runs two kinds of phases:
 //   "event-parallel" (lane i <-> event i of the tile): header decode, policy gather (one 64-byte SiteRec),
@@ -13,9 +18,10 @@
 //       warp-uniform forward targets (each unique target is searched once per warp), verdict / counter epilogue;
 //   "lane-parallel" (lane l <-> lane l of one event): the per-lane tail of the MAC (8 of the 12 SipRounds for
 //       a warp-uniform continuation, 10 otherwise) and the compare; per-lane searches of lane-divergent targets.
-// Event rows reach shared memory by cp.async (16-byte chunks, only the rows a tile needs), double-buffered:
-// the rows of tile k+1 are in flight while tile k is computed.  When the policy's whole target table is small
-// (<= kMaxStageTgts entries) every CTA stages it in shared memory once with one TMA bulk copy.
+// Event rows reach shared memory by TMA bulk copies (cp.async.bulk, one 256-byte row per issuing lane, only the
+// rows the tile needs) that complete on the warp's own mbarrier; 20 warps per SM keep the ALU pipe fed while
+// other warps wait for their rows.  When the policy's whole target table is small (<= kMaxStageTgts entries)
+// every CTA stages it in shared memory once with one more bulk copy.
 // Counters: warp-uniform registers + shared-memory atomics, flushed once per CTA; per-site counters are
 // aggregated over equal sites of a tile (__match_any_sync) before the global reduction.
 #include "wg_internal.h"
@@ -31,21 +37,26 @@ enum : uint32_t { K_RET = 0, K_FWD = 1 };
 enum : uint32_t { CLS_NONE = 0, CLS_COUNT = 1, CLS_RET = 2, CLS_FWD = 3, CLS_FAIL = 4 };
 
 constexpr int kT = 16;                 // events per tile
-constexpr int kWarps = 12;             // warps per CTA, one CTA per SM
+constexpr int kWarps = 20;             // warps per CTA, one CTA per SM (5 per sub-partition)
 constexpr int kThreads = kWarps * 32;
 constexpr uint32_t kMaxStageTgts = 2048;  // 16 KB of shared memory for the target table
 constexpr uint32_t kFull = 0xffffffffu;
 
 // ---- shared-memory carve-up ----------------------------------------------------------------------
 // CTA part: [tgts staged: stage_bytes][cnt64: 32 x u64][bykind: 8 x u32][mbar: u64, pad]
-// warp part: hdr[3][T] uint4, st[T][8] u32, val[2][T][32] u64, (verify only) tag[2][T][32] u64
+// warp part: raw headers [2][T] x 16 B (this tile, next tile), decoded headers [T] x 16 B
+//            {8 * first active lane, active mask, context_base & ~31 (lo), context_base (hi)},
+//            per-event SipHash states [T] x 32 B, the warp's mbarrier, value rows [T][32] u64,
+//            (verify only) tag rows [T][32] u64
 template <int MODE>
 struct WarpLayout {
-  static constexpr uint32_t kHdr = 0;
-  static constexpr uint32_t kSt = kHdr + 3 * kT * 16;
-  static constexpr uint32_t kVal = kSt + kT * 32;
-  static constexpr uint32_t kTag = kVal + 2 * kT * 256;
-  static constexpr uint32_t kBytes = kTag + (MODE == MODE_VERIFY ? 2 * kT * 256 : 0);
+  static constexpr uint32_t kRaw = 0;
+  static constexpr uint32_t kDec = kRaw + 2 * kT * 16;
+  static constexpr uint32_t kSt = kDec + kT * 16;
+  static constexpr uint32_t kBar = kSt + kT * 32;
+  static constexpr uint32_t kVal = kBar + 16;
+  static constexpr uint32_t kTag = kVal + kT * 256;
+  static constexpr uint32_t kBytes = kTag + (MODE == MODE_VERIFY ? kT * 256 : 0);
 };
 constexpr uint32_t kCtaFixedBytes = 32 * 8 + 8 * 4 + 16 + 16;  // cnt64, bykind, mbar (+pad to 16)
 
@@ -53,12 +64,6 @@ constexpr uint32_t kCtaFixedBytes = 32 * 8 + 8 * 4 + 16 + 16;  // cnt64, bykind,
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
 __device__ __forceinline__ uint4 ldg_v4(const void* p) {
   uint4 r;
   asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
@@ -140,8 +145,7 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
     return __ldg(set + lo) == v;
   }
 }
-
-// what lane i knows about event i of a tile
+// what lane i knows about event i of the tile
 struct TileEv {
   uint32_t site, active, cls, kind;
   uint32_t off, cnt;  // protected-forward: the site's set
@@ -153,35 +157,11 @@ struct WarpCtr {
   uint32_t total, empty, unknown, misrouted, ret_checks, fwd_checks, ret_lanes, fwd_lanes, signed_lanes, skipped;
 };
 
+// event-parallel: decode header i, gather the SiteRec, classify (a1, a2); leaves the decoded header
+// {8 * first active lane, active, context_base & ~31 (lo), context_base (hi)} in shared memory for the
+// lane-parallel phases
 template <int MODE>
-__device__ __forceinline__ void issue_hdr(const Params& p, uint32_t hdr_s, uint64_t tile, uint32_t buf,
-                                          uint32_t lane) {
-  const uint64_t e = tile * kT + lane;
-  if (lane < kT && e < p.n) cp_async16(hdr_s + (buf * kT + lane) * 16, p.hdr + e);
-}
-
-// rows of the tile: one cp.async instruction moves 16 B per lane = two 256-byte rows per warp instruction
-template <int MODE>
-__device__ __forceinline__ void issue_rows(const Params& p, uint32_t warp_s, uint64_t tile, uint32_t buf,
-                                           uint32_t need_val, uint32_t need_tag, uint32_t lane) {
-  using L = WarpLayout<MODE>;
-  const uint32_t half = lane >> 4, chunk = lane & 15;
-  const uint64_t e0 = tile * kT;
-#pragma unroll
-  for (int j = 0; j < kT / 2; ++j) {
-    const uint32_t e = 2 * j + half;
-    const uint64_t g = (e0 + e) * 32 + chunk * 2;
-    const uint32_t s = ((buf * kT + e) * 32 + chunk * 2) * 8;
-    if ((need_val >> e) & 1u) cp_async16(warp_s + L::kVal + s, p.val + g);
-    if constexpr (MODE == MODE_VERIFY) {
-      if ((need_tag >> e) & 1u) cp_async16(warp_s + L::kTag + s, p.tag + g);
-    }
-  }
-}
-
-// event-parallel: decode header i, gather the SiteRec, classify (a1, a2)
-template <int MODE>
-__device__ __forceinline__ TileEv classify(const Params& p, uint32_t hdr_s, uint64_t tile, uint32_t buf,
+__device__ __forceinline__ TileEv classify(const Params& p, uint32_t raw_s, uint32_t dec_s, uint64_t tile,
                                            uint32_t lane) {
   TileEv ev;
   ev.site = 0;
@@ -192,10 +172,13 @@ __device__ __forceinline__ TileEv classify(const Params& p, uint32_t hdr_s, uint
   ev.cnt = 0;
   ev.st = Sip32{0, 0, 0, 0, 0, 0, 0, 0};
   const uint64_t e = tile * kT + lane;
-  if (lane < kT && e < p.n) {
-    const uint4 h = lds_v4(hdr_s + (buf * kT + lane) * 16);
+  const bool valid = lane < kT && e < p.n;
+  if (lane < kT && !valid) sts_v4(dec_s + lane * 16, 0u, 0u, 0u, 0u);  // ragged tail: a harmless record
+  if (valid) {
+    const uint4 h = lds_v4(raw_s + lane * 16);
     ev.site = h.x;
     ev.active = h.y;
+    sts_v4(dec_s + lane * 16, h.y ? static_cast<uint32_t>(__ffs(h.y) - 1) * 8u : 0u, h.y, h.z & ~31u, h.w);
     if (h.x < p.n_sites) {
       const SiteRec* r = p.recs + h.x;
       const uint4 a = ldg_v4(r);
@@ -239,28 +222,33 @@ template <int MODE, bool STAGED>
 __global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes) {
   using L = WarpLayout<MODE>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t lane = threadIdx.x & 31;
+  const uint32_t lanebit = 1u << lane;
+  // the shuffle tells the compiler that the warp index (and what derives from it) is warp-uniform
+  const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
   const uint32_t smem0 = smem_u32(smem_raw);
   const uint32_t tg_s = smem0;
   unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + stage_bytes);
   uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + stage_bytes + 256);
-  const uint32_t mbar = smem0 + stage_bytes + 256 + 32;
+  const uint32_t mbar_cta = smem0 + stage_bytes + 256 + 32;
   const uint32_t warp_s = smem0 + stage_bytes + kCtaFixedBytes + warp * L::kBytes;
-  const uint32_t hdr_s = warp_s + L::kHdr;
+  const uint32_t dec_s = warp_s + L::kDec;
   const uint32_t st_s = warp_s + L::kSt;
+  const uint32_t mbar = warp_s + L::kBar;
+  const uint32_t val_s = warp_s + L::kVal;
+  const uint32_t tag_s = warp_s + L::kTag;
 
   if (threadIdx.x < 32) cnt64[threadIdx.x] = 0ull;
   if (threadIdx.x < 8) bykind[threadIdx.x] = 0u;
-  if constexpr (STAGED) {
-    if (threadIdx.x == 0) mbar_init(mbar, 1);
-  }
+  if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
+  if (lane == 0) mbar_init(mbar, 1);
   __syncthreads();
   if constexpr (STAGED) {
     if (threadIdx.x == 0) {
-      mbar_expect_tx(mbar, stage_bytes);
-      tma_bulk_g2s(tg_s, p.tgts, stage_bytes, mbar);
+      mbar_expect_tx(mbar_cta, stage_bytes);
+      tma_bulk_g2s(tg_s, p.tgts, stage_bytes, mbar_cta);
     }
-    mbar_wait(mbar, 0);
+    mbar_wait(mbar_cta, 0);
   }
 
   const uint64_t n_tiles = (p.n + kT - 1) / kT;
@@ -268,155 +256,67 @@ __global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, co
   uint64_t t = static_cast<uint64_t>(blockIdx.x) * kWarps + warp;
   const bool enforce = p.mode != 0;
   WarpCtr c = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  uint32_t phase = 0, rb = 0;  // mbarrier phase parity; which raw-header buffer holds this tile
 
-  // ---- prologue: header of the first tile, its classification, its rows + the header of the second ----
-  TileEv nx = classify<MODE>(p, hdr_s, n_tiles, 0, lane);  // an all-NONE tile (tile index past the end)
-  uint32_t hb = 0, hb1 = 1, hb2 = 2, rb = 0;
+  // prologue: raw headers of the first tile
   if (t < n_tiles) {
-    issue_hdr<MODE>(p, hdr_s, t, hb, lane);
-    cp_async_commit();
-    cp_async_wait_all();
-    __syncwarp();
-    nx = classify<MODE>(p, hdr_s, t, hb, lane);
-    const uint32_t nr = __ballot_sync(kFull, nx.cls == CLS_RET);
-    const uint32_t nf = __ballot_sync(kFull, nx.cls == CLS_FWD);
-    issue_rows<MODE>(p, warp_s, t, rb, nr | nf, nr, lane);
-    if (t + stride < n_tiles) issue_hdr<MODE>(p, hdr_s, t + stride, hb1, lane);
-    cp_async_commit();
+    if (lane == 0) {
+      const uint64_t left = p.n - t * kT;
+      const uint32_t bytes = static_cast<uint32_t>(left < kT ? left : kT) * 16u;
+      mbar_expect_tx(mbar, bytes);
+      tma_bulk_g2s(warp_s + L::kRaw, p.hdr + t * kT, bytes, mbar);
+    }
+    mbar_wait(mbar, phase);
+    phase ^= 1u;
   }
 
   while (t < n_tiles) {
-    const TileEv ev = nx;
     const uint64_t tn = t + stride;
-    cp_async_wait_all();  // rows of this tile and the header of the next have landed
-    __syncwarp();
+    const uint64_t e0 = t * kT;
+    // ---- event-parallel: decode, gather, classify (a1, a2) ----
+    const TileEv ev = classify<MODE>(p, warp_s + L::kRaw + rb * kT * 16, dec_s, t, lane);
     const uint32_t m_ret = __ballot_sync(kFull, ev.cls == CLS_RET);
     const uint32_t m_fwd = __ballot_sync(kFull, ev.cls == CLS_FWD);
-    const uint32_t hdr_t = hdr_s + hb * kT * 16;                 // this tile's headers
-    const uint32_t val_t = warp_s + L::kVal + rb * kT * 256;     // this tile's value rows
-    const uint32_t tag_t = warp_s + L::kTag + rb * kT * 256;     // this tile's tag rows (verify)
 
-    // next tile: header decode + SiteRec gather now, so the gather latency hides behind the next phase
-    if (tn < n_tiles) nx = classify<MODE>(p, hdr_s, tn, hb1, lane);
-
-    // ---- which events carry one warp-uniform value?  (a5 dedupe) ----
-    uint32_t uni = 0, ul = 0, uh = 0;
-    for (uint32_t m = m_ret | m_fwd; m; m &= m - 1) {
-      const uint32_t e = __ffs(m) - 1;
-      const uint32_t a = lds_u32(hdr_t + e * 16 + 4);
-      const uint2 v = lds_v2(val_t + e * 256 + lane * 8);
-      const uint2 r = lds_v2(val_t + e * 256 + (__ffs(a) - 1) * 8);  // first active lane's value
-      const bool same = ((v.x == r.x) && (v.y == r.y)) || !((a >> lane) & 1u);
-      if (__all_sync(kFull, same)) {
-        uni |= 1u << e;
-        if (lane == e) {
-          ul = r.x;
-          uh = r.y;
-        }
+    // ---- rows of this tile and raw headers of the next: TMA bulk copies onto the warp's mbarrier ----
+    {
+      uint32_t hdr_bytes = 0;
+      if (tn < n_tiles) {
+        const uint64_t left = p.n - tn * kT;
+        hdr_bytes = static_cast<uint32_t>(left < kT ? left : kT) * 16u;
       }
+      const uint32_t rows = __popc(m_ret | m_fwd) + (MODE == MODE_VERIFY ? __popc(m_ret) : 0);
+      if (lane == 0) mbar_expect_tx(mbar, rows * 256u + hdr_bytes);
+      __syncwarp();
+      if (ev.cls == CLS_RET || ev.cls == CLS_FWD) {
+        tma_bulk_g2s(val_s + lane * 256, p.val + (e0 + lane) * 32, 256u, mbar);
+        if (MODE == MODE_VERIFY && ev.cls == CLS_RET)
+          tma_bulk_g2s(tag_s + lane * 256, p.tag + (e0 + lane) * 32, 256u, mbar);
+      }
+      if (lane == 0 && hdr_bytes)
+        tma_bulk_g2s(warp_s + L::kRaw + (rb ^ 1u) * kT * 16, p.hdr + tn * kT, hdr_bytes, mbar);
     }
 
-    // ---- rows of the next tile + header of the one after go in flight now ----
-    if (tn < n_tiles) {
-      const uint32_t nr = __ballot_sync(kFull, nx.cls == CLS_RET);
-      const uint32_t nf = __ballot_sync(kFull, nx.cls == CLS_FWD);
-      issue_rows<MODE>(p, warp_s, tn, rb ^ 1u, nr | nf, nr, lane);
-      if (tn + stride < n_tiles) issue_hdr<MODE>(p, hdr_s, tn + stride, hb2, lane);
-    }
-    cp_async_commit();
-
-    // ---- event-parallel: per-event part of the MAC; batched search of warp-uniform forward targets ----
-    uint32_t viol = 0;
-    if (ev.cls == CLS_RET) {
-      Sip32 s = ev.st;  // pre-A state after the site word
-      if ((uni >> lane) & 1u) {
-        sip_absorb_preA(s, ul, uh);  // the continuation word, once per event
-        sip_qA(s);                   // and quarter A of the context word's first round
-      }
-      sts_v4(st_s + lane * 32, s.v0l, s.v0h, s.v1l, s.v1h);
-      sts_v4(st_s + lane * 32 + 16, s.v2l, s.v2h, s.v3l, s.v3h);
-    }
-    if constexpr (MODE != MODE_SIGN) {
-      if (ev.cls == CLS_FWD && ((uni >> lane) & 1u))
-        viol = member<STAGED>(p, tg_s, ev.off, ev.cnt, ul, uh) ? 0u : ev.active;
-      if (ev.cls == CLS_FAIL) viol = ev.active;  // fail closed (R13, R14)
-    }
-    __syncwarp();
-
-    // ---- lane-parallel: protected-return events with a warp-uniform continuation (8 rounds per lane) ----
-    for (uint32_t m = m_ret & uni; m; m &= m - 1) {
-      const uint32_t e = __ffs(m) - 1;
-      const uint4 h = lds_v4(hdr_t + e * 16);
-      const Sip32 s = lds_state(st_s + e * 32);
-      const bool on = (h.y >> lane) & 1u;
-      uint32_t dl, dh;
-      if constexpr (MODE == MODE_SIGN) {
-        sip_tail_ctx(s, (h.z & ~31u) | lane, h.w, 0u, 0u, dl, dh);
-        st_stream_v2(p.tag_out + ((t * kT + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
-      } else {
-        const uint2 tg = lds_v2(tag_t + e * 256 + lane * 8);
-        sip_tail_ctx(s, (h.z & ~31u) | lane, h.w, tg.x, tg.y, dl, dh);
-        const uint32_t vb = __ballot_sync(kFull, on && ((dl | dh) != 0u));
-        if (lane == e) viol = vb;
-      }
-    }
-    // ---- lane-parallel: protected-return events with lane-divergent continuations (10 rounds per lane) ----
-    for (uint32_t m = m_ret & ~uni; m; m &= m - 1) {
-      const uint32_t e = __ffs(m) - 1;
-      const uint4 h = lds_v4(hdr_t + e * 16);
-      const Sip32 s = lds_state(st_s + e * 32);
-      const uint2 v = lds_v2(val_t + e * 256 + lane * 8);
-      const bool on = (h.y >> lane) & 1u;
-      uint32_t dl, dh;
-      if constexpr (MODE == MODE_SIGN) {
-        sip_tail_val_ctx(s, v.x, v.y, (h.z & ~31u) | lane, h.w, 0u, 0u, dl, dh);
-        st_stream_v2(p.tag_out + ((t * kT + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
-      } else {
-        const uint2 tg = lds_v2(tag_t + e * 256 + lane * 8);
-        sip_tail_val_ctx(s, v.x, v.y, (h.z & ~31u) | lane, h.w, tg.x, tg.y, dl, dh);
-        const uint32_t vb = __ballot_sync(kFull, on && ((dl | dh) != 0u));
-        if (lane == e) viol = vb;
-      }
-    }
-    // ---- lane-parallel: protected-forward events with lane-divergent targets ----
-    if constexpr (MODE != MODE_SIGN) {
-      for (uint32_t m = m_fwd & ~uni; m; m &= m - 1) {
-        const uint32_t e = __ffs(m) - 1;
-        const uint32_t a = lds_u32(hdr_t + e * 16 + 4);
-        const uint32_t off = __shfl_sync(kFull, ev.off, e), cnt = __shfl_sync(kFull, ev.cnt, e);
-        const uint2 v = lds_v2(val_t + e * 256 + lane * 8);
-        const bool bad = ((a >> lane) & 1u) && !member<STAGED>(p, tg_s, off, cnt, v.x, v.y);
-        const uint32_t vb = __ballot_sync(kFull, bad);
-        if (lane == e) viol = vb;
-      }
-    }
-
-    // ---- event-parallel epilogue: verdicts (a6), counters (a7), first violation (a8) ----
+    // ---- while the rows fly: everything of the epilogue that does not depend on a verdict (a7) ----
     const bool valid = ev.cls != CLS_NONE;
     const bool known = valid && ev.kind < 7u;
     const uint32_t na = __popc(ev.active);
+    const uint32_t judged_na = (ev.cls == CLS_RET || ev.cls == CLS_FWD) ? na : 0u;
+    unsigned long long* sc = p.site + static_cast<uint64_t>(ev.site) * 4;
     if constexpr (MODE == MODE_SIGN) {
-      // every row the loops above did not write is a zero row (R10): non-return sites, empty masks
-      for (uint32_t m = __ballot_sync(kFull, valid && ev.cls != CLS_RET); m; m &= m - 1) {
-        const uint32_t e = __ffs(m) - 1;
-        st_stream_v2(p.tag_out + ((t * kT + e) * 32 + lane), 0u, 0u);
-      }
       const bool is_ret = known && ev.kind == K_RET;
       c.signed_lanes += __reduce_add_sync(kFull, is_ret ? na : 0u);
       c.skipped += __popc(__ballot_sync(kFull, valid && !is_ret));
     } else {
-      if (valid) st_stream_v2(p.out + (t * kT + lane), viol, enforce ? (ev.active & ~viol) : ev.active);
       c.total += __popc(__ballot_sync(kFull, valid));
       c.unknown += __popc(__ballot_sync(kFull, valid && !known));
       c.empty += __popc(__ballot_sync(kFull, known && ev.active == 0u));
       c.misrouted += __popc(__ballot_sync(kFull, known && ev.cls == CLS_FAIL));
       c.ret_checks += __popc(m_ret);
       c.fwd_checks += __popc(m_fwd);
-      const uint32_t judged_na = (ev.cls == CLS_RET || ev.cls == CLS_FWD) ? na : 0u;
       c.ret_lanes += __reduce_add_sync(kFull, ev.cls == CLS_RET ? na : 0u);
       c.fwd_lanes += __reduce_add_sync(kFull, ev.cls == CLS_FWD ? na : 0u);
       if (known) atomicAdd(&bykind[ev.kind], 1u);
-
       // per-site counters: equal sites of the tile are merged first (Zipf: the hottest site is ~1/6 of all events)
       const uint32_t m_known = __ballot_sync(kFull, known);
       uint32_t grp = 0;
@@ -427,12 +327,114 @@ __global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, co
         const uint32_t x = __shfl_sync(kFull, judged_na, j);
         if (((grp >> j) & 1u) && j != lane) sum += x;
       }
-      unsigned long long* sc = p.site + static_cast<uint64_t>(ev.site) * 4;
       if (known && lane == static_cast<uint32_t>(__ffs(grp) - 1)) {
         atomicAdd(sc + S_EVENTS, static_cast<unsigned long long>(__popc(grp)));
         if (sum) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(sum));
       }
+    }
 
+    mbar_wait(mbar, phase);  // rows (and the next raw headers) have landed
+    phase ^= 1u;
+
+    // ---- which events carry one warp-uniform value?  (a5 dedupe)  Unrolled over the tile:
+    //      three independent shared-memory loads and ~6 ALU instructions per event, one REDUX per tile ----
+    uint32_t mism = 0;
+#pragma unroll
+    for (int e = 0; e < kT; ++e) {
+      const uint2 d = lds_v2(dec_s + e * 16);  // {8 * first active lane, active}
+      const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
+      const uint2 r = lds_v2(val_s + e * 256 + d.x);
+      if ((((v.x ^ r.x) | (v.y ^ r.y)) != 0u) && (d.y & lanebit)) mism |= 1u << e;
+    }
+    const uint32_t uni = ~__reduce_or_sync(kFull, mism) & (m_ret | m_fwd);
+
+    // ---- event-parallel: per-event part of the MAC; batched search of warp-uniform forward targets ----
+    uint32_t viol = 0;
+    {
+      const bool is_uni = (uni >> lane) & 1u;
+      uint32_t ul = 0, uh = 0;
+      if (is_uni) {
+        const uint2 d = lds_v2(dec_s + lane * 16);
+        const uint2 r = lds_v2(val_s + lane * 256 + d.x);  // the event's one value
+        ul = r.x;
+        uh = r.y;
+      }
+      if (ev.cls == CLS_RET) {
+        Sip32 s = ev.st;  // pre-A state after the site word
+        if (is_uni) {
+          const uint4 d = lds_v4(dec_s + lane * 16);
+          sip_absorb_preA(s, ul, uh);  // the continuation word, once per event
+          sip_qA(s);                   // quarter A of the context word's first round
+          s.v3l ^= d.z;                // and the lane-independent bits of the context word
+          s.v3h ^= d.w;
+        }
+        sts_v4(st_s + lane * 32, s.v0l, s.v0h, s.v1l, s.v1h);
+        sts_v4(st_s + lane * 32 + 16, s.v2l, s.v2h, s.v3l, s.v3h);
+      }
+      if constexpr (MODE != MODE_SIGN) {
+        if (ev.cls == CLS_FWD && is_uni) viol = member<STAGED>(p, tg_s, ev.off, ev.cnt, ul, uh) ? 0u : ev.active;
+        if (ev.cls == CLS_FAIL) viol = ev.active;  // fail closed (R13, R14)
+      }
+    }
+    __syncwarp();
+
+    // ---- lane-parallel: protected-return events with a warp-uniform continuation (8 rounds per lane) ----
+    for (uint32_t m = m_ret & uni; m; m &= m - 1) {
+      const uint32_t e = __ffs(m) - 1;
+      const uint4 h = lds_v4(dec_s + e * 16);
+      const Sip32 s = lds_state(st_s + e * 32);
+      uint32_t dl, dh;
+      if constexpr (MODE == MODE_SIGN) {
+        sip_tail_lane(s, lane, h.z, h.w, 0u, 0u, dl, dh);
+        const bool on = h.y & lanebit;
+        st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
+      } else {
+        const uint2 tg = lds_v2(tag_s + e * 256 + lane * 8);
+        sip_tail_lane(s, lane, h.z, h.w, tg.x, tg.y, dl, dh);
+        const uint32_t vb = __ballot_sync(kFull, ((dl | dh) != 0u) && (h.y & lanebit));
+        if (lane == e) viol = vb;
+      }
+    }
+    // ---- lane-parallel: protected-return events with lane-divergent continuations (10 rounds per lane) ----
+    for (uint32_t m = m_ret & ~uni; m; m &= m - 1) {
+      const uint32_t e = __ffs(m) - 1;
+      const uint4 h = lds_v4(dec_s + e * 16);
+      const Sip32 s = lds_state(st_s + e * 32);
+      const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
+      uint32_t dl, dh;
+      if constexpr (MODE == MODE_SIGN) {
+        sip_tail_val_lane(s, v.x, v.y, lane, h.z, h.w, 0u, 0u, dl, dh);
+        const bool on = h.y & lanebit;
+        st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
+      } else {
+        const uint2 tg = lds_v2(tag_s + e * 256 + lane * 8);
+        sip_tail_val_lane(s, v.x, v.y, lane, h.z, h.w, tg.x, tg.y, dl, dh);
+        const uint32_t vb = __ballot_sync(kFull, ((dl | dh) != 0u) && (h.y & lanebit));
+        if (lane == e) viol = vb;
+      }
+    }
+    // ---- lane-parallel: protected-forward events with lane-divergent targets ----
+    if constexpr (MODE != MODE_SIGN) {
+      for (uint32_t m = m_fwd & ~uni; m; m &= m - 1) {
+        const uint32_t e = __ffs(m) - 1;
+        const uint32_t a = lds_u32(dec_s + e * 16 + 4);
+        const uint32_t off = __shfl_sync(kFull, ev.off, e), cnt = __shfl_sync(kFull, ev.cnt, e);
+        const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
+        const bool bad = (a & lanebit) && !member<STAGED>(p, tg_s, off, cnt, v.x, v.y);
+        const uint32_t vb = __ballot_sync(kFull, bad);
+        if (lane == e) viol = vb;
+      }
+    }
+
+    // ---- event-parallel epilogue: verdicts (a6), violation counters (a7), first violation (a8) ----
+    if constexpr (MODE == MODE_SIGN) {
+      // every row the loops above did not write is a zero row (R10): non-return sites, empty masks
+      for (uint32_t m = __ballot_sync(kFull, valid && ev.cls != CLS_RET); m; m &= m - 1) {
+        const uint32_t e = __ffs(m) - 1;
+        st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), 0u, 0u);
+      }
+    } else {
+      if (valid) st_stream_v2(p.out + (e0 + lane), viol, enforce ? (ev.active & ~viol) : ev.active);
       // violations are rare (0.05 % of events in the paper-shaped stream): one warp-uniform branch per tile
       if (__ballot_sync(kFull, viol != 0u)) {
         const uint32_t pv = __popc(viol);
@@ -444,7 +446,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, co
         const uint32_t ave = __popc(__ballot_sync(kFull, viol != 0u));
         // first violation: smallest (seq << 5 | lane); seq = running event index (R12)
         unsigned long long key = ~0ull;
-        if (viol) key = ((p.seq_base + t * kT + lane) << 5) | static_cast<uint32_t>(__ffs(viol) - 1);
+        if (viol) key = ((p.seq_base + e0 + lane) << 5) | static_cast<uint32_t>(__ffs(viol) - 1);
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) {
           const unsigned long long o = __shfl_xor_sync(kFull, key, d);
@@ -467,15 +469,10 @@ __global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, co
         }
       }
     }
-
+    __syncwarp();  // every lane is done with this tile's shared memory before the next tile's copies land
     t = tn;
     rb ^= 1u;
-    const uint32_t h0 = hb;
-    hb = hb1;
-    hb1 = hb2;
-    hb2 = h0;
   }
-  cp_async_wait_all();
 
   // ---- flush: warp registers -> CTA shared memory -> one global atomic per counter per CTA ----
   if (lane == 0) {

@@ -120,21 +120,36 @@ __device__ __forceinline__ void sip_finish(Sip32& s, uint32_t xl, uint32_t xh, u
   sip_round(s);
   sip_round(s);
   sip_round(s);
-  outl = (s.v0l ^ s.v1l) ^ (s.v2l ^ s.v3l) ^ xl;
-  outh = (s.v0h ^ s.v1h) ^ (s.v2h ^ s.v3h) ^ xh;
+  outl = s.v0l ^ s.v1l ^ s.v2l ^ s.v3l ^ xl;
+  outh = s.v0h ^ s.v1h ^ s.v2h ^ s.v3h ^ xh;
 }
 
-// per-lane tail when the event's pre-A state already covers site and continuation (warp-uniform continuation)
-__device__ __forceinline__ void sip_tail_ctx(Sip32 s, uint32_t cl, uint32_t ch, uint32_t xl, uint32_t xh,
-                                             uint32_t& outl, uint32_t& outh) {
-  sip_absorb_preA(s, cl, ch);
+// The context word of lane l is (B | l) with B = context_base & ~31 (R2), and B | l == B ^ l.
+// per-lane tail when the event's state already covers site and continuation (warp-uniform continuation), has
+// quarter A of the next round applied, AND has B already folded into v3 (done once per event): the lane only
+// injects its own five bits.
+__device__ __forceinline__ void sip_tail_lane(Sip32 s, uint32_t lane, uint32_t bl, uint32_t bh, uint32_t xl,
+                                              uint32_t xh, uint32_t& outl, uint32_t& outh) {
+  s.v3l ^= lane;
+  sip_qB(s);
+  sip_qC(s);
+  sip_qD(s);
+  sip_round(s);
+  s.v0l ^= bl ^ lane;
+  s.v0h ^= bh;
   sip_finish(s, xl, xh, outl, outh);
 }
 // per-lane tail from the site's pre-A state (lane-divergent continuation)
-__device__ __forceinline__ void sip_tail_val_ctx(Sip32 s, uint32_t vl, uint32_t vh, uint32_t cl, uint32_t ch,
-                                                 uint32_t xl, uint32_t xh, uint32_t& outl, uint32_t& outh) {
+__device__ __forceinline__ void sip_tail_val_lane(Sip32 s, uint32_t vl, uint32_t vh, uint32_t lane, uint32_t bl,
+                                                  uint32_t bh, uint32_t xl, uint32_t xh, uint32_t& outl,
+                                                  uint32_t& outh) {
   sip_absorb_preA(s, vl, vh);
-  sip_absorb(s, cl, ch);
+  s.v3l ^= bl ^ lane;
+  s.v3h ^= bh;
+  sip_round(s);
+  sip_round(s);
+  s.v0l ^= bl ^ lane;
+  s.v0h ^= bh;
   sip_finish(s, xl, xh, outl, outh);
 }
 
