@@ -164,7 +164,9 @@ wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const
  *   mix: 0 = IADD3 only, 1 = LOP3 only, 2 = SHF only, 3 = IMAD only, 4 = IMAD.WIDE.U32 only,
  *        5 = ALU:FMA 1:1 (LOP3 + IMAD), 6 = SipRound-shaped ALU mix (IADD3 / LOP3 / SHF, 8:8:8),
  *        7 = IMAD.HI.U32 only, 8 = ALU:FMA 2:1 (LOP3, SHF + IMAD), 9 = ALU:FMA 1:1 (SHF + IMAD.HI.U32),
- *        10 = 64-bit-add pairs (IADD3 with carry-out + IMAD.X with carry-in; counts PAIRS per second).
+ *        10 = 64-bit-add pairs (IADD3 with carry-out + IMAD.X with carry-in; counts PAIRS per second),
+ *        11 = the SipRound itself (two independent states per thread), counted as 24 int32 operations per round:
+ *             the ceiling of any SipHash kernel on this GPU.
  *   Every step's second operand is a neighbouring chain's live value, so ptxas cannot fold steps away.
  * wg_launch_count: kernels this library has launched since it was loaded (bench.py's gpu_launches). */
 wg_status wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms);

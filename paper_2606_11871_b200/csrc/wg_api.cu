@@ -455,7 +455,7 @@ wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const
 }
 
 wg_status wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms) {
-  if (!ops_per_s || mix < 0 || mix > 10) return WG_ERR_INVALID_ARG;
+  if (!ops_per_s || mix < 0 || mix > 11) return WG_ERR_INVALID_ARG;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
     cudaGetLastError();

@@ -36,10 +36,18 @@ enum : uint32_t { K_RET = 0, K_FWD = 1 };
 // what the tile does with an event
 enum : uint32_t { CLS_NONE = 0, CLS_COUNT = 1, CLS_RET = 2, CLS_FWD = 3, CLS_FAIL = 4 };
 
-constexpr int kT = 16;                 // events per tile
-constexpr int kWarps = 20;             // warps per CTA, one CTA per SM (5 per sub-partition)
-constexpr int kThreads = kWarps * 32;
-constexpr uint32_t kMaxStageTgts = 2048;  // 16 KB of shared memory for the target table
+#ifndef WG_TILE
+#define WG_TILE 16
+#endif
+#ifndef WG_WARPS_CHECK
+#define WG_WARPS_CHECK 20
+#endif
+#ifndef WG_WARPS_SIGN
+#define WG_WARPS_SIGN 20
+#endif
+constexpr int kT = WG_TILE;            // events per tile (<= 32: one lane per event in the event-parallel phases)
+static_assert(kT == 8 || kT == 16 || kT == 32, "tile size");
+constexpr uint32_t kSmemMax = 232448;  // 227 KB opt-in shared memory per CTA on sm_100a
 constexpr uint32_t kFull = 0xffffffffu;
 
 // ---- shared-memory carve-up ----------------------------------------------------------------------
@@ -59,6 +67,15 @@ struct WarpLayout {
   static constexpr uint32_t kBytes = kTag + (MODE == MODE_VERIFY ? kT * 256 : 0);
 };
 constexpr uint32_t kCtaFixedBytes = 32 * 8 + 8 * 4 + 16 + 16;  // cnt64, bykind, mbar (+pad to 16)
+
+// warps per CTA (one CTA per SM) and the largest target table that still fits beside the warps' buffers
+template <int MODE>
+struct Cfg {
+  static constexpr int kWarps = (MODE == MODE_SIGN) ? WG_WARPS_SIGN : WG_WARPS_CHECK;
+  static constexpr int kThreads = kWarps * 32;
+  static constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * WarpLayout<MODE>::kBytes;
+  static constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
+};
 
 // ---- PTX helpers ---------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -219,7 +236,7 @@ __device__ __forceinline__ Sip32 lds_state(uint32_t a) {
 // wg_sign_continuations.  STAGED: the whole target table sits in shared memory.
 // ---------------------------------------------------------------------------------------------------
 template <int MODE, bool STAGED>
-__global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes) {
+__global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes) {
   using L = WarpLayout<MODE>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31;
@@ -252,6 +269,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_tile_kernel(const Params p, co
   }
 
   const uint64_t n_tiles = (p.n + kT - 1) / kT;
+  constexpr int kWarps = Cfg<MODE>::kWarps;
   const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kWarps;
   uint64_t t = static_cast<uint64_t>(blockIdx.x) * kWarps + warp;
   const bool enforce = p.mode != 0;
@@ -527,15 +545,17 @@ __global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sit
 
 template <int MODE>
 uint32_t smem_bytes(uint32_t stage_bytes) {
-  return stage_bytes + kCtaFixedBytes + kWarps * WarpLayout<MODE>::kBytes;
+  return stage_bytes + kCtaFixedBytes + Cfg<MODE>::kWarps * WarpLayout<MODE>::kBytes;
 }
 
 template <int MODE>
 cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
   const uint64_t n_tiles = (p.n + kT - 1) / kT;
+  constexpr int kWarps = Cfg<MODE>::kWarps;
+  constexpr int kThreads = Cfg<MODE>::kThreads;
   const uint64_t want = (n_tiles + kWarps - 1) / kWarps;
   const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) ? want : sm_count);
-  const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= kMaxStageTgts;
+  const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= Cfg<MODE>::kMaxStageTgts;
   const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
   const uint32_t smem = smem_bytes<MODE>(stage_bytes);
   if (staged)
@@ -549,7 +569,7 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
 template <int MODE, bool STAGED>
 cudaError_t opt_in() {
   return cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              static_cast<int>(smem_bytes<MODE>(STAGED ? kMaxStageTgts * 8 : 0)));
+                              static_cast<int>(smem_bytes<MODE>(STAGED ? Cfg<MODE>::kMaxStageTgts * 8 : 0)));
 }
 
 }  // namespace

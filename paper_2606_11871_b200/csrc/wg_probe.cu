@@ -4,6 +4,7 @@
 // sequence of one instruction kind; 8 independent chains per thread and 16 resident warps per SMSP keep the
 // pipes full.  `asm volatile` pins the instruction selection (checked with cuobjdump -sass).
 #include "wg_internal.h"
+#include "wg_sip32.cuh"
 
 namespace wg {
 namespace {
@@ -70,6 +71,57 @@ __global__ void __launch_bounds__(kThreads) wg_int_probe(uint32_t* sink, uint32_
   if (acc == 0x12345678u) sink[0] = acc;  // practically never; keeps the chains live
 }
 
+// mix 11: the SipRound itself (wg_sip32.cuh), two independent states per thread, 16 rounds per loop trip.
+// Reported as 24 int32 lane-operations per round (8 add halves, 8 xor halves, 8 funnel shifts): the ceiling
+// any SipHash kernel on this GPU can reach, whatever its occupancy.
+constexpr int kSipRoundsPerTrip = 16;
+constexpr int kSipTrips = 1024;
+__global__ void __launch_bounds__(kThreads) wg_sip_probe(uint32_t* sink, uint32_t y) {
+  Sip32 s[2];
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const uint32_t x = (blockIdx.x * kThreads + threadIdx.x) * 2654435761u + y + i * 977u;
+    s[i] = Sip32{x, x ^ 0x1234567u, x * 3u, x * 5u, x * 7u, x * 11u, x * 13u, x * 17u};
+  }
+  for (int t = 0; t < kSipTrips; ++t) {
+#pragma unroll
+    for (int r = 0; r < kSipRoundsPerTrip; ++r) {
+      sip_round(s[0]);
+      sip_round(s[1]);
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+    acc ^= s[i].v0l ^ s[i].v0h ^ s[i].v1l ^ s[i].v1h ^ s[i].v2l ^ s[i].v2h ^ s[i].v3l ^ s[i].v3h;
+  if (acc == 0x12345678u) sink[0] = acc;
+}
+
+cudaError_t run_sip(int sm_count, uint32_t* sink, double* ops_per_s, double* ms_out) {
+  const int grid = sm_count * 4;  // 4 CTAs x 8 warps = 8 warps per sub-partition
+  cudaEvent_t a, b;
+  cudaError_t err;
+  if ((err = cudaEventCreate(&a)) != cudaSuccess) return err;
+  if ((err = cudaEventCreate(&b)) != cudaSuccess) return err;
+  float best = 1e30f;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(a, nullptr);
+    wg_sip_probe<<<grid, kThreads>>>(sink, 0x9e3779b9u + rep);
+    count_launch();
+    cudaEventRecord(b, nullptr);
+    if ((err = cudaEventSynchronize(b)) != cudaSuccess) return err;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, a, b);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  const double rounds = static_cast<double>(grid) * kThreads * 2.0 * kSipRoundsPerTrip * kSipTrips;
+  *ops_per_s = rounds * 24.0 / (best * 1e-3);
+  *ms_out = best;
+  return cudaGetLastError();
+}
+
 template <int MIX>
 cudaError_t run(int sm_count, uint32_t* sink, double* ops_per_s, double* ms_out) {
   const int grid = sm_count * 8;  // 8 CTAs x 8 warps = 64 warps per SM
@@ -114,6 +166,7 @@ cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double*
     case 8: err = run<8>(sm_count, sink, ops_per_s, ms); break;
     case 9: err = run<9>(sm_count, sink, ops_per_s, ms); break;
     case 10: err = run<10>(sm_count, sink, ops_per_s, ms); break;
+    case 11: err = run_sip(sm_count, sink, ops_per_s, ms); break;
     default: err = cudaErrorInvalidValue;
   }
   cudaFree(sink);

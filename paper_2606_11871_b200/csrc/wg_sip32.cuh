@@ -7,7 +7,8 @@
 // Why halves: sm_100a has no 64-bit integer ALU.  Written on explicit lo/hi registers the round is exactly
 //     4 x (IADD3 + carry IADD3.X / IMAD.X)   8 x LOP3   8 x SHF.L.W   rotate-by-32 = register rename
 // = 24 instructions and no MOV / pack traffic (the 64-bit formulation of v1 cost ~40 per round).  Measured
-// issue costs on B200 (wg_probe_int_pipe): IADD3 / LOP3 128 lanes/SM/clk, SHF / IMAD 64.
+// issue costs on B200 (wg_probe_int_pipe): every ALU-pipe instruction (IADD3, LOP3, SHF) holds the pipe
+// for 2 cycles per warp, so the round is 40 cycles per warp per sub-partition: 76.8 int32 ops / SM / clk.
 //
 // The round is split in its four quarter-steps so that work which does not depend on the next message word
 // can be hoisted: a word m enters through v3 only, and quarter A touches (v0, v1) only, so A of the first
