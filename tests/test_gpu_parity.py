@@ -325,3 +325,87 @@ def test_work_runs_on_the_callers_stream():
     assert B.wg_launch_count() - before == 2
     assert not out[:, 0].any()
     assert np.array_equal(tag.cpu().numpy().view(np.uint64), orc.sign(st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# tile structure of the v2 kernels: every ragged length around the 16-event tile and the 20-warp CTA
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 2, 15, 16, 17, 31, 32, 33, 319, 320, 321, 16 * 20 * 148 - 1, 16 * 20 * 148 + 17])
+def test_ragged_lengths_around_tile_and_grid_boundaries(n):
+    st = S.make_stream(4, "cpu", n_events=n)
+    run = run_config(4, n)
+    run[2].close()
+    # the forward entry point walks the same tiles without tag rows
+    orc, eng = oracle_for(st.policy), engine_for(st.policy)
+    hdr_np, val_np = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    o = orc.check_forward(hdr_np, val_np, ENF)
+    g = eng.wg_check_forward(st.hdr.to(dev()), st.val.to(dev()), ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    assert_counters_equal(eng, orc)
+    eng.close()
+
+
+def test_every_lane_violates_under_the_wrong_key():
+    """Tags signed under another key: every active lane of every return event must be blocked (the violation
+    path of the kernels is normally rare; here it runs on every tile)."""
+    st = S.make_stream(2, "cpu", n_events=40_003)
+    pol = st.policy
+    orc, eng = oracle_for(pol), engine_for(pol)
+    other = oracle.Oracle(pol.kind, pol.tgt_off, pol.tgts, pol.k0 ^ 1, pol.k1, pol.policy_digest)
+    hdr_np, val_np = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    tag = other.sign(hdr_np, val_np)
+    for mode in (ENF, DET):
+        o = orc.verify(hdr_np, val_np, tag, mode)
+        g = eng.wg_verify_continuations(st.hdr.to(dev()), st.val.to(dev()), to_dev(tag), mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+        assert (o[:, 0] == (hdr_np[:, 0] >> np.uint64(32)).astype(np.uint32)).all()  # viol == active everywhere
+    assert_counters_equal(eng, orc)
+    g, _ = eng.wg_read_counters()
+    first = int(np.nonzero(hdr_np[:, 0] >> np.uint64(32))[0][0])           # first event with an active lane
+    mask = int(hdr_np[first, 0] >> np.uint64(32))
+    assert g["first_violation_key"] == (first << 5) | ((mask & -mask).bit_length() - 1)
+    eng.close()
+
+
+def test_baseline_v1_kernels_stay_bit_exact(monkeypatch):
+    """WG_IMPL=v1 selects the warp-per-event kernels kept as the measured baseline: same outputs."""
+    monkeypatch.setenv("WG_IMPL", "v1")
+    st, orc, eng, out = run_config(4, 100_003)
+    assert np.array_equal(out[:, 0], witness.expected_viol(st))
+    eng.close()
+
+
+def test_config4_full_size_sampled_against_the_oracle():
+    """BASELINE.json's full config 4 (58.0 M events, 52.2 M checks) in the launch configuration bench.py times.
+    The oracle cannot run 1.5 G MACs in a test, so: (1) counters must show exactly the planned corruption and the
+    exact class counts; (2) a random sample of events plus EVERY corrupted event is re-judged by the oracle, tags
+    and verdicts compared bit for bit."""
+    st = S.make_stream(4, dev())
+    n = st.hdr.shape[0]
+    assert n == S.FULL_EVENTS[4]
+    eng = engine_for(st.policy)
+    tag = eng.wg_sign_continuations(st.hdr, st.val)
+    g = torch.Generator(device="cpu").manual_seed(99)
+    idx = torch.randint(0, n, (150_000,), generator=g)
+    idx = torch.unique(torch.cat([idx, st.ret_tamper.ev.cpu(), st.fwd_tamper.ev.cpu(),
+                                  torch.arange(0, 4096), torch.arange(n - 4096, n)])).to(dev())
+    clean_tag = tag[idx].cpu().numpy().view(np.uint64)
+    st.apply_return_tamper(tag)
+    out = eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode)
+    gc, _ = eng.wg_read_counters()
+    assert gc["events_total"] == n and gc["ret_checks"] + gc["fwd_checks"] == 52_200_000
+    assert gc["ret_checks"] == 38_300_000 and gc["fwd_checks"] == 13_900_000
+    assert gc["ret_viol_events"] == len(st.ret_tamper) and gc["fwd_viol_events"] == len(st.fwd_tamper)
+    assert gc["blocked_lanes"] == gc["ret_viol"] + gc["fwd_viol"] and gc["events_unknown_site"] == 0
+    assert int((out[:, 0] != 0).sum().item()) == len(st.ret_tamper) + len(st.fwd_tamper)
+    orc = oracle_for(st.policy)
+    hdr_s = st.hdr[idx].cpu().numpy().view(np.uint64)
+    val_s = st.val[idx].cpu().numpy().view(np.uint64)
+    tag_s = tag[idx].cpu().numpy().view(np.uint64)
+    # the recorded corruption may have touched val of sampled events after signing: sign parity uses clean rows only
+    o_tag = orc.sign(hdr_s, val_s)
+    touched = np.isin(idx.cpu().numpy(), st.ret_tamper.ev.cpu().numpy())
+    assert np.array_equal(o_tag[~touched], clean_tag[~touched])
+    o_out = orc.verify(hdr_s, val_s, tag_s, st.mode)
+    assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), o_out)
+    eng.close()
