@@ -305,7 +305,11 @@ def run_ours(a) -> None:
     roofline = {
         "kernel": "wg_check (wg_verify_continuations)",
         "bound": "alu" if t_alu >= t_hbm else "hbm",
-        "achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tint32op/s", "frac": achieved / alu_peak,
+        **({"achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tint32op/s", "frac": achieved / alu_peak}
+           if t_alu >= t_hbm else
+           {"achieved": verify_bytes / (verify_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+            "frac": verify_bytes / (verify_ms * 1e-3) / 1e9 / hbm_peak}),
+        "alu_achieved_Tops": achieved / 1e12, "alu_frac": achieved / alu_peak,
         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if (a.config == 4 and a.events is None) else None,
         "peak_source": ("derived: 128 lanes/SM/clk x %d SMs x %.0f MHz (DESIGN.md §6); max with the measured probes"
                         % (n_sm, sm_max_mhz)),

@@ -49,9 +49,10 @@ constexpr int kT = WG_TILE;            // events per tile (<= 32: one lane per e
 static_assert(kT == 8 || kT == 16 || kT == 32, "tile size");
 constexpr uint32_t kSmemMax = 232448;  // 227 KB opt-in shared memory per CTA on sm_100a
 constexpr uint32_t kFull = 0xffffffffu;
+constexpr uint32_t kMaxSmemSites = 1024;  // policies up to this size keep their per-site counters in shared memory
 
 // ---- shared-memory carve-up ----------------------------------------------------------------------
-// CTA part: [tgts staged: stage_bytes][cnt64: 32 x u64][bykind: 8 x u32][mbar: u64, pad]
+// CTA part: [tgts staged: stage_bytes][per-site counters: site_bytes][cnt64: 32 x u64][bykind: 8 x u32][mbar: u64, pad]
 // warp part: raw headers [2][T] x 16 B (this tile, next tile), decoded headers [T] x 16 B
 //            {8 * first active lane, active mask, context_base & ~31 (lo), context_base (hi)},
 //            per-event SipHash states [T] x 32 B, the warp's mbarrier, value rows [T][32] u64,
@@ -236,7 +237,8 @@ __device__ __forceinline__ Sip32 lds_state(uint32_t a) {
 // wg_sign_continuations.  STAGED: the whole target table sits in shared memory.
 // ---------------------------------------------------------------------------------------------------
 template <int MODE, bool STAGED>
-__global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes) {
+__global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes,
+                                                                                const uint32_t site_bytes) {
   using L = WarpLayout<MODE>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const uint32_t lane = threadIdx.x & 31;
@@ -245,10 +247,15 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
   const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
   const uint32_t smem0 = smem_u32(smem_raw);
   const uint32_t tg_s = smem0;
-  unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + stage_bytes);
-  uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + stage_bytes + 256);
-  const uint32_t mbar_cta = smem0 + stage_bytes + 256 + 32;
-  const uint32_t warp_s = smem0 + stage_bytes + kCtaFixedBytes + warp * L::kBytes;
+  // small policies (site_bytes != 0): per-site counters are accumulated in shared memory as 4 x u32 per site and
+  // flushed once per CTA.  With few sites the global counter array spans only a few L2 slices and the reductions
+  // of 148 SMs would queue on them (config 3: 40 sites, 7.6 ms -> see DESIGN.md §9).
+  uint32_t* site_s = reinterpret_cast<uint32_t*>(smem_raw + stage_bytes);
+  const uint32_t cta_off = stage_bytes + site_bytes;
+  unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + cta_off);
+  uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + cta_off + 256);
+  const uint32_t mbar_cta = smem0 + cta_off + 256 + 32;
+  const uint32_t warp_s = smem0 + cta_off + kCtaFixedBytes + warp * L::kBytes;
   const uint32_t dec_s = warp_s + L::kDec;
   const uint32_t st_s = warp_s + L::kSt;
   const uint32_t mbar = warp_s + L::kBar;
@@ -256,6 +263,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
   const uint32_t tag_s = warp_s + L::kTag;
 
   if (threadIdx.x < 32) cnt64[threadIdx.x] = 0ull;
+  for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = 0u;
   if (threadIdx.x < 8) bykind[threadIdx.x] = 0u;
   if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
   if (lane == 0) mbar_init(mbar, 1);
@@ -335,19 +343,28 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       c.ret_lanes += __reduce_add_sync(kFull, ev.cls == CLS_RET ? na : 0u);
       c.fwd_lanes += __reduce_add_sync(kFull, ev.cls == CLS_FWD ? na : 0u);
       if (known) atomicAdd(&bykind[ev.kind], 1u);
-      // per-site counters: equal sites of the tile are merged first (Zipf: the hottest site is ~1/6 of all events)
-      const uint32_t m_known = __ballot_sync(kFull, known);
-      uint32_t grp = 0;
-      if (known) grp = __match_any_sync(m_known, ev.site);
-      uint32_t sum = judged_na;
-      for (uint32_t m = __ballot_sync(kFull, __popc(grp) > 1); m; m &= m - 1) {
-        const uint32_t j = __ffs(m) - 1;
-        const uint32_t x = __shfl_sync(kFull, judged_na, j);
-        if (((grp >> j) & 1u) && j != lane) sum += x;
-      }
-      if (known && lane == static_cast<uint32_t>(__ffs(grp) - 1)) {
-        atomicAdd(sc + S_EVENTS, static_cast<unsigned long long>(__popc(grp)));
-        if (sum) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(sum));
+      if (site_bytes) {
+        // per-site counters in shared memory (small policies)
+        if (known) {
+          atomicAdd(&site_s[ev.site * 4 + S_EVENTS], 1u);
+          if (judged_na) atomicAdd(&site_s[ev.site * 4 + S_LANES_CHECKED], judged_na);
+        }
+      } else {
+        // per-site counters in global memory: equal sites of the tile are merged first (Zipf: the hottest site is
+        // ~1/6 of all events)
+        const uint32_t m_known = __ballot_sync(kFull, known);
+        uint32_t grp = 0;
+        if (known) grp = __match_any_sync(m_known, ev.site);
+        uint32_t sum = judged_na;
+        for (uint32_t m = __ballot_sync(kFull, __popc(grp) > 1); m; m &= m - 1) {
+          const uint32_t j = __ffs(m) - 1;
+          const uint32_t x = __shfl_sync(kFull, judged_na, j);
+          if (((grp >> j) & 1u) && j != lane) sum += x;
+        }
+        if (known && lane == static_cast<uint32_t>(__ffs(grp) - 1)) {
+          atomicAdd(sc + S_EVENTS, static_cast<unsigned long long>(__popc(grp)));
+          if (sum) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(sum));
+        }
       }
     }
 
@@ -482,8 +499,13 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
           atomicMin(p.glob + C_FIRST_VIOLATION, key);
         }
         if (viol && known) {
-          if (judged_na) atomicAdd(sc + S_LANES_VIOLATION, static_cast<unsigned long long>(pv));
-          if (enforce) atomicAdd(sc + S_LANES_BLOCKED, static_cast<unsigned long long>(pv));
+          if (site_bytes) {
+            if (judged_na) atomicAdd(&site_s[ev.site * 4 + S_LANES_VIOLATION], pv);
+            if (enforce) atomicAdd(&site_s[ev.site * 4 + S_LANES_BLOCKED], pv);
+          } else {
+            if (judged_na) atomicAdd(sc + S_LANES_VIOLATION, static_cast<unsigned long long>(pv));
+            if (enforce) atomicAdd(sc + S_LANES_BLOCKED, static_cast<unsigned long long>(pv));
+          }
         }
       }
     }
@@ -513,6 +535,10 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     unsigned long long v = cnt64[threadIdx.x];
     if (threadIdx.x >= C_BY_KIND && threadIdx.x < C_BY_KIND + 7) v = bykind[threadIdx.x - C_BY_KIND];
     if (v) atomicAdd(p.glob + threadIdx.x, v);
+  }
+  for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) {
+    const uint32_t v = site_s[i];
+    if (v) atomicAdd(p.site + i, static_cast<unsigned long long>(v));
   }
 }
 
@@ -544,7 +570,7 @@ __global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sit
 }
 
 template <int MODE>
-uint32_t smem_bytes(uint32_t stage_bytes) {
+uint32_t smem_bytes(uint32_t stage_bytes) {  // stage_bytes: staged targets + shared-memory site counters
   return stage_bytes + kCtaFixedBytes + Cfg<MODE>::kWarps * WarpLayout<MODE>::kBytes;
 }
 
@@ -557,11 +583,16 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
   const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) ? want : sm_count);
   const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= Cfg<MODE>::kMaxStageTgts;
   const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
-  const uint32_t smem = smem_bytes<MODE>(stage_bytes);
+  // per-site counters in shared memory when the policy is small and they fit beside the staged targets
+  uint32_t site_bytes = 0;
+  if (MODE != MODE_SIGN && p.n_sites > 0 && p.n_sites <= kMaxSmemSites &&
+      stage_bytes + p.n_sites * 16u <= Cfg<MODE>::kLeft)
+    site_bytes = p.n_sites * 16u;
+  const uint32_t smem = smem_bytes<MODE>(stage_bytes + site_bytes);
   if (staged)
-    wg_tile_kernel<MODE, true><<<grid, kThreads, smem, st>>>(p, stage_bytes);
+    wg_tile_kernel<MODE, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
   else
-    wg_tile_kernel<MODE, false><<<grid, kThreads, smem, st>>>(p, stage_bytes);
+    wg_tile_kernel<MODE, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
   count_launch();
   return cudaGetLastError();
 }
@@ -569,7 +600,7 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
 template <int MODE, bool STAGED>
 cudaError_t opt_in() {
   return cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              static_cast<int>(smem_bytes<MODE>(STAGED ? Cfg<MODE>::kMaxStageTgts * 8 : 0)));
+                              static_cast<int>(kSmemMax));
 }
 
 }  // namespace

@@ -345,6 +345,25 @@ def test_ragged_lengths_around_tile_and_grid_boundaries(n):
     eng.close()
 
 
+def test_wrong_key_on_a_small_policy_counts_in_shared_memory():
+    """Same attack on config 1's 72-site policy: per-site counters (violations and blocked lanes included) take the
+    shared-memory path of the kernel; every counter must still equal the oracle's."""
+    st = S.make_stream(1, "cpu", n_events=30_011)
+    pol = st.policy
+    orc, eng = oracle_for(pol), engine_for(pol)
+    other = oracle.Oracle(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1 ^ (1 << 63), pol.policy_digest)
+    hdr_np, val_np = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    tag = other.sign(hdr_np, val_np)
+    for mode in (ENF, DET, ENF):
+        o = orc.verify(hdr_np, val_np, tag, mode)
+        g = eng.wg_verify_continuations(st.hdr.to(dev()), st.val.to(dev()), to_dev(tag), mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+    assert_counters_equal(eng, orc)
+    _, gs = eng.wg_read_counters()
+    assert gs[:, 3].sum() > 0 and gs[:, 2].sum() > gs[:, 3].sum()  # blocked only in the two enforce passes
+    eng.close()
+
+
 def test_every_lane_violates_under_the_wrong_key():
     """Tags signed under another key: every active lane of every return event must be blocked (the violation
     path of the kernels is normally rare; here it runs on every tile)."""
