@@ -90,6 +90,10 @@ __device__ __forceinline__ uint4 ldg_v4(const void* p) {
 __device__ __forceinline__ void st_stream_v2(void* p, uint32_t a, uint32_t b) {
   asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(p), "r"(a), "r"(b) : "memory");
 }
+__device__ __forceinline__ void st_stream_v4(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d)
+               : "memory");
+}
 __device__ __forceinline__ uint4 lds_v4(uint32_t a) {
   uint4 r;
   asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a));
@@ -121,6 +125,9 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                "l"(src), "r"(bytes), "r"(mbar)
                : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
   asm volatile(
@@ -314,13 +321,29 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       const uint32_t rows = __popc(m_ret | m_fwd) + (MODE == MODE_VERIFY ? __popc(m_ret) : 0);
       if (lane == 0) mbar_expect_tx(mbar, rows * 256u + hdr_bytes);
       __syncwarp();
-      if (ev.cls == CLS_RET || ev.cls == CLS_FWD) {
-        tma_bulk_g2s(val_s + lane * 256, p.val + (e0 + lane) * 32, 256u, mbar);
-        if (MODE == MODE_VERIFY && ev.cls == CLS_RET)
-          tma_bulk_g2s(tag_s + lane * 256, p.tag + (e0 + lane) * 32, 256u, mbar);
+      // one bulk copy per RUN of consecutive needed rows (a bulk copy is issued by one elected lane at a time, so
+      // fewer, longer copies cost fewer issue slots): the first lane of a run copies the whole run
+      {
+        const uint32_t need = m_ret | m_fwd;
+        const uint32_t here = need >> lane;
+        if ((here & 1u) && (lane == 0u || !((need >> (lane - 1u)) & 1u))) {
+          const uint32_t len = static_cast<uint32_t>(__ffs(~here)) - 1u;
+          tma_bulk_g2s(val_s + lane * 256, p.val + (e0 + lane) * 32, len * 256u, mbar);
+        }
+        if constexpr (MODE == MODE_VERIFY) {
+          const uint32_t here_t = m_ret >> lane;
+          if ((here_t & 1u) && (lane == 0u || !((m_ret >> (lane - 1u)) & 1u))) {
+            const uint32_t len = static_cast<uint32_t>(__ffs(~here_t)) - 1u;
+            tma_bulk_g2s(tag_s + lane * 256, p.tag + (e0 + lane) * 32, len * 256u, mbar);
+          }
+        }
       }
-      if (lane == 0 && hdr_bytes)
+      if (lane == 0 && hdr_bytes) {
         tma_bulk_g2s(warp_s + L::kRaw + (rb ^ 1u) * kT * 16, p.hdr + tn * kT, hdr_bytes, mbar);
+        // a tile without return events is HBM-bound work (280 B / event, a few instructions): pull the next
+        // tile's value rows into L2 now, so that its row copies find them there (one more tile of bytes in flight)
+        if (MODE != MODE_SIGN && m_ret == 0u) tma_prefetch_l2(p.val + tn * kT * 32, hdr_bytes * 16u);
+      }
     }
 
     // ---- while the rows fly: everything of the epilogue that does not depend on a verdict (a7) ----
@@ -373,15 +396,18 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
 
     // ---- which events carry one warp-uniform value?  (a5 dedupe)  Unrolled over the tile:
     //      three independent shared-memory loads and ~6 ALU instructions per event, one REDUX per tile ----
-    uint32_t mism = 0;
+    uint32_t uni = 0;
+    if (MODE != MODE_SIGN || m_ret != 0u) {  // (a sign tile without return events has nothing to detect)
+      uint32_t mism = 0;
 #pragma unroll
-    for (int e = 0; e < kT; ++e) {
-      const uint2 d = lds_v2(dec_s + e * 16);  // {8 * first active lane, active}
-      const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
-      const uint2 r = lds_v2(val_s + e * 256 + d.x);
-      if ((((v.x ^ r.x) | (v.y ^ r.y)) != 0u) && (d.y & lanebit)) mism |= 1u << e;
+      for (int e = 0; e < kT; ++e) {
+        const uint2 d = lds_v2(dec_s + e * 16);  // {8 * first active lane, active}
+        const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
+        const uint2 r = lds_v2(val_s + e * 256 + d.x);
+        if ((((v.x ^ r.x) | (v.y ^ r.y)) != 0u) && (d.y & lanebit)) mism |= 1u << e;
+      }
+      uni = ~__reduce_or_sync(kFull, mism) & (m_ret | m_fwd);
     }
-    const uint32_t uni = ~__reduce_or_sync(kFull, mism) & (m_ret | m_fwd);
 
     // ---- event-parallel: per-event part of the MAC; batched search of warp-uniform forward targets ----
     uint32_t viol = 0;
@@ -464,9 +490,15 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     // ---- event-parallel epilogue: verdicts (a6), violation counters (a7), first violation (a8) ----
     if constexpr (MODE == MODE_SIGN) {
       // every row the loops above did not write is a zero row (R10): non-return sites, empty masks
-      for (uint32_t m = __ballot_sync(kFull, valid && ev.cls != CLS_RET); m; m &= m - 1) {
-        const uint32_t e = __ffs(m) - 1;
-        st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), 0u, 0u);
+      // written as 16-byte stores: a half-warp covers one 256-byte row, one instruction covers two events
+      const uint32_t zmask = __ballot_sync(kFull, valid && ev.cls != CLS_RET);
+      if (zmask) {
+        const uint32_t half = lane >> 4, chunk = lane & 15u;
+#pragma unroll
+        for (int j = 0; j < kT / 2; ++j) {
+          const uint32_t e = 2u * j + half;
+          if ((zmask >> e) & 1u) st_stream_v4(p.tag_out + ((e0 + e) * 32 + chunk * 2), 0u, 0u, 0u, 0u);
+        }
       }
     } else {
       if (valid) st_stream_v2(p.out + (e0 + lane), viol, enforce ? (ev.active & ~viol) : ev.active);
