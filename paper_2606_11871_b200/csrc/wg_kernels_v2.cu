@@ -63,7 +63,8 @@ struct WarpLayout {
   static constexpr uint32_t kDec = kRaw + 2 * kT * 16;
   static constexpr uint32_t kSt = kDec + kT * 16;
   static constexpr uint32_t kBar = kSt + kT * 32;
-  static constexpr uint32_t kVal = kBar + 16;
+  static constexpr uint32_t kViol = kBar + 16;  // [T] u32 violation masks of the tile
+  static constexpr uint32_t kVal = kViol + kT * 4;
   static constexpr uint32_t kTag = kVal + kT * 256;
   static constexpr uint32_t kBytes = kTag + (MODE == MODE_VERIFY ? kT * 256 : 0);
 };
@@ -107,6 +108,15 @@ __device__ __forceinline__ uint2 lds_v2(uint32_t a) {
 __device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
   uint32_t r;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ void sts_u32(uint32_t a, uint32_t x) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
+}
+// a * b + c on the FMA pipe (address arithmetic inside the ALU-bound loops)
+__device__ __forceinline__ uint32_t mad32(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
   return r;
 }
 __device__ __forceinline__ void sts_v4(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
@@ -266,8 +276,10 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
   const uint32_t dec_s = warp_s + L::kDec;
   const uint32_t st_s = warp_s + L::kSt;
   const uint32_t mbar = warp_s + L::kBar;
+  const uint32_t viol_s = warp_s + L::kViol;
   const uint32_t val_s = warp_s + L::kVal;
   const uint32_t tag_s = warp_s + L::kTag;
+  const uint32_t val_lane_s = val_s + lane * 8, tag_lane_s = tag_s + lane * 8;  // this lane's column of the rows
 
   if (threadIdx.x < 32) cnt64[threadIdx.x] = 0ull;
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = 0u;
@@ -435,6 +447,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       if constexpr (MODE != MODE_SIGN) {
         if (ev.cls == CLS_FWD && is_uni) viol = member<STAGED>(p, tg_s, ev.off, ev.cnt, ul, uh) ? 0u : ev.active;
         if (ev.cls == CLS_FAIL) viol = ev.active;  // fail closed (R13, R14)
+        if (lane < kT) sts_u32(viol_s + lane * 4, viol);  // the lane-parallel loops below overwrite their events
       }
     }
     __syncwarp();
@@ -442,36 +455,37 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     // ---- lane-parallel: protected-return events with a warp-uniform continuation (8 rounds per lane) ----
     for (uint32_t m = m_ret & uni; m; m &= m - 1) {
       const uint32_t e = __ffs(m) - 1;
-      const uint4 h = lds_v4(dec_s + e * 16);
-      const Sip32 s = lds_state(st_s + e * 32);
+      const uint4 h = lds_v4(mad32(e, 16u, dec_s));
+      const Sip32 s = lds_state(mad32(e, 32u, st_s));
       uint32_t dl, dh;
       if constexpr (MODE == MODE_SIGN) {
         sip_tail_lane(s, lane, h.z, h.w, 0u, 0u, dl, dh);
         const bool on = h.y & lanebit;
         st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
       } else {
-        const uint2 tg = lds_v2(tag_s + e * 256 + lane * 8);
+        const uint2 tg = lds_v2(mad32(e, 256u, tag_lane_s));
         sip_tail_lane(s, lane, h.z, h.w, tg.x, tg.y, dl, dh);
-        const uint32_t vb = __ballot_sync(kFull, ((dl | dh) != 0u) && (h.y & lanebit));
-        if (lane == e) viol = vb;
+        // inactive lanes computed on garbage: masked out after the vote (R10)
+        const uint32_t vb = __ballot_sync(kFull, (dl | dh) != 0u) & h.y;
+        if (lane == 0) sts_u32(mad32(e, 4u, viol_s), vb);
       }
     }
     // ---- lane-parallel: protected-return events with lane-divergent continuations (10 rounds per lane) ----
     for (uint32_t m = m_ret & ~uni; m; m &= m - 1) {
       const uint32_t e = __ffs(m) - 1;
-      const uint4 h = lds_v4(dec_s + e * 16);
-      const Sip32 s = lds_state(st_s + e * 32);
-      const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
+      const uint4 h = lds_v4(mad32(e, 16u, dec_s));
+      const Sip32 s = lds_state(mad32(e, 32u, st_s));
+      const uint2 v = lds_v2(mad32(e, 256u, val_lane_s));
       uint32_t dl, dh;
       if constexpr (MODE == MODE_SIGN) {
         sip_tail_val_lane(s, v.x, v.y, lane, h.z, h.w, 0u, 0u, dl, dh);
         const bool on = h.y & lanebit;
         st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
       } else {
-        const uint2 tg = lds_v2(tag_s + e * 256 + lane * 8);
+        const uint2 tg = lds_v2(mad32(e, 256u, tag_lane_s));
         sip_tail_val_lane(s, v.x, v.y, lane, h.z, h.w, tg.x, tg.y, dl, dh);
-        const uint32_t vb = __ballot_sync(kFull, ((dl | dh) != 0u) && (h.y & lanebit));
-        if (lane == e) viol = vb;
+        const uint32_t vb = __ballot_sync(kFull, (dl | dh) != 0u) & h.y;
+        if (lane == 0) sts_u32(mad32(e, 4u, viol_s), vb);
       }
     }
     // ---- lane-parallel: protected-forward events with lane-divergent targets ----
@@ -483,8 +497,10 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
         const uint2 v = lds_v2(val_s + e * 256 + lane * 8);
         const bool bad = (a & lanebit) && !member<STAGED>(p, tg_s, off, cnt, v.x, v.y);
         const uint32_t vb = __ballot_sync(kFull, bad);
-        if (lane == e) viol = vb;
+        if (lane == 0) sts_u32(viol_s + e * 4, vb);
       }
+      __syncwarp();
+      if (lane < kT) viol = lds_u32(viol_s + lane * 4);  // event-parallel again: lane i <-> event i
     }
 
     // ---- event-parallel epilogue: verdicts (a6), violation counters (a7), first violation (a8) ----
