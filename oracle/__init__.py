@@ -84,6 +84,16 @@ def lib():
         L.wgo_check.argtypes = [vp, vp, vp, vp, vp, u64, C.c_int]
         L.wgo_read_counters.restype = None
         L.wgo_read_counters.argtypes = [vp, vp, vp]
+        L.wgo_set_profile.restype = None
+        L.wgo_set_profile.argtypes = [vp, u32]
+        L.wgo_set_ring_capacity.restype = None
+        L.wgo_set_ring_capacity.argtypes = [vp, u64]
+        L.wgo_read_violations.restype = u64
+        L.wgo_read_violations.argtypes = [vp, vp, u64]
+        L.wgo_read_first_violation.restype = C.c_int
+        L.wgo_read_first_violation.argtypes = [vp, vp]
+        L.wgo_read_telemetry.restype = None
+        L.wgo_read_telemetry.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -185,3 +195,33 @@ class Oracle:
         s = np.zeros((self.n_sites, 4), dtype=np.uint64) if per_site else None
         lib().wgo_read_counters(self._h, _ptr(g), _ptr(s))
         return {k: int(v) for k, v in zip(COUNTER_FIELDS, g)}, s
+
+    # ---- profiles and telemetry (wg_oracle.h; R26-R29) ----
+    def set_profile(self, flags: int):
+        lib().wgo_set_profile(self._h, int(flags))
+
+    def set_ring_capacity(self, capacity: int):
+        lib().wgo_set_ring_capacity(self._h, int(capacity))
+
+    def read_violations(self, cap: int = 1 << 20) -> np.ndarray:
+        out = np.zeros(cap, dtype=VIOLATION_DTYPE)
+        n = lib().wgo_read_violations(self._h, _ptr(out), cap)
+        return out[:n]
+
+    def read_first_violation(self):
+        out = np.zeros(1, dtype=VIOLATION_DTYPE)
+        ok = lib().wgo_read_first_violation(self._h, _ptr(out))
+        return out[0] if ok else None
+
+    def read_telemetry(self) -> dict:
+        t = np.zeros(6, dtype=np.uint64)
+        lib().wgo_read_telemetry(self._h, _ptr(t))
+        return {k: int(v) for k, v in zip(TELEMETRY_FIELDS, t)}
+
+
+PROFILE_SKIP_FORWARD, PROFILE_SKIP_BACKWARD, PROFILE_LOW_TELEMETRY = 1, 2, 4
+VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
+                            ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
+                            ("stored", "<u8")])
+TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
+                    "ring_recorded", "ring_dropped")

@@ -69,6 +69,13 @@ struct wgo_engine {
   int use_binary_search = 0;
   wgo_counters g;
   std::vector<wgo_site_counters> site;
+  // profiles and telemetry (R26-R29)
+  uint32_t profile = 0;
+  uint64_t ring_capacity = 0;
+  std::vector<wgo_violation_rec> ring;
+  wgo_telemetry_counters t = {0, 0, 0, 0, 0, 0};
+  bool have_first = false;
+  wgo_violation_rec first = {};
 };
 
 extern "C" {
@@ -156,6 +163,9 @@ void wgo_reset_counters(wgo_engine* e) {
   e->g.first_violation_key = ~static_cast<uint64_t>(0);
   std::fill(e->site.begin(), e->site.end(), wgo_site_counters{0, 0, 0, 0});
   e->seq = 0;
+  e->ring.clear();  // profile and ring capacity are configuration and stay
+  e->t = wgo_telemetry_counters{0, 0, 0, 0, 0, 0};
+  e->have_first = false;
 }
 
 wgo_engine* wgo_create(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off,
@@ -224,6 +234,8 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
     const uint32_t s = hdr[ev].site_id;
     const uint32_t a = hdr[ev].active_mask;
     uint32_t viol = 0;
+    bool judged_ret = false;  // the stored tag took part in this event's verdict
+    const bool low = (e->profile & WGO_PROFILE_LOW_TELEMETRY) != 0;
     e->g.events_total += 1;
 
     if (s >= e->n_sites) {
@@ -233,11 +245,20 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
     } else {
       const uint8_t k = e->kind[s];
       e->g.events_by_kind[k] += 1;
-      e->site[s].events += 1;
+      if (!low) e->site[s].events += 1;
       if (a == 0) {
         // fully predicated-off instruction: no helper ran (R22)
         e->g.events_empty += 1;
+      } else if (k == WGO_PROTECTED_RETURN && (e->profile & WGO_PROFILE_SKIP_BACKWARD)) {
+        // forward-only profile: outside the protected set, separate denominator (R26)
+        e->t.skipped_ret_events += 1;
+        e->t.skipped_ret_lanes += popcount32(a);
+      } else if (k == WGO_PROTECTED_FORWARD && (e->profile & WGO_PROFILE_SKIP_FORWARD)) {
+        // backward-only profile (R26)
+        e->t.skipped_fwd_events += 1;
+        e->t.skipped_fwd_lanes += popcount32(a);
       } else if (k == WGO_PROTECTED_RETURN && tag != nullptr) {
+        judged_ret = true;
         for (uint32_t lane = 0; lane < 32; ++lane) {
           if (!((a >> lane) & 1u)) continue;  // inactive lanes are never judged
           const uint64_t expect =
@@ -248,8 +269,8 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
         e->g.ret_lanes += popcount32(a);
         e->g.ret_viol += popcount32(viol);
         e->g.ret_viol_events += (viol != 0);
-        e->site[s].lanes_checked += popcount32(a);
-        e->site[s].lanes_violation += popcount32(viol);
+        if (!low) e->site[s].lanes_checked += popcount32(a);
+        if (!low) e->site[s].lanes_violation += popcount32(viol);
       } else if (k == WGO_PROTECTED_RETURN) {
         // handed to the forward entry point: no tag, cannot authenticate (R14)
         viol = a;
@@ -265,8 +286,8 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
         e->g.fwd_lanes += popcount32(a);
         e->g.fwd_viol += popcount32(viol);
         e->g.fwd_viol_events += (viol != 0);
-        e->site[s].lanes_checked += popcount32(a);
-        e->site[s].lanes_violation += popcount32(viol);
+        if (!low) e->site[s].lanes_checked += popcount32(a);
+        if (!low) e->site[s].lanes_violation += popcount32(viol);
       } else {
         // fixed-edge / unsupported / profile-excluded / fallback / no-surface:
         // counted above, never judged (R17)
@@ -277,17 +298,65 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
     if (mode == WGO_ENFORCE && viol != 0) {
       e->g.blocked_lanes += popcount32(viol);
       e->g.blocked_events += 1;
-      if (s < e->n_sites) e->site[s].lanes_blocked += popcount32(viol);
+      if (s < e->n_sites && !low) e->site[s].lanes_blocked += popcount32(viol);
     }
     if (viol != 0) {
       const uint64_t key = (seq << 5) | lowest_set_lane(viol);
-      if (key < e->g.first_violation_key) e->g.first_violation_key = key;
+      // the violation record (R27): diagnostic only, it never feeds a verdict
+      wgo_violation_rec r;
+      r.seq = seq;
+      r.site_id = s;
+      r.kind = (s < e->n_sites) ? e->kind[s] : 7u;
+      r.viol_mask = viol;
+      r.active_mask = a;
+      r.lane = lowest_set_lane(viol);
+      r.mode = static_cast<uint32_t>(mode);
+      r.observed = val[ev * 32 + r.lane];
+      r.stored = judged_ret ? tag[ev * 32 + r.lane] : 0;
+      if (key < e->g.first_violation_key) {  // PAPER.md:266 "records the first violation"
+        e->g.first_violation_key = key;
+        e->first = r;
+        e->have_first = true;
+      }
+      if (!low && e->ring_capacity != 0) {  // bounded ring (R28)
+        if (e->ring.size() < e->ring_capacity) {
+          e->ring.push_back(r);
+          e->t.ring_recorded += 1;
+        } else {
+          e->t.ring_dropped += 1;
+        }
+      }
     }
     out[ev].viol_mask = viol;
     out[ev].allow_mask = allow;
   }
   if (n != 0) e->g.last_mode = static_cast<uint64_t>(mode);
 }
+
+void wgo_set_profile(wgo_engine* e, uint32_t flags) { e->profile = flags; }
+
+void wgo_set_ring_capacity(wgo_engine* e, uint64_t capacity) {
+  e->ring_capacity = capacity;
+  if (e->ring.size() > capacity) {  // shrinking drops the tail, and says so
+    e->t.ring_dropped += e->ring.size() - capacity;
+    e->t.ring_recorded = capacity;
+    e->ring.resize(capacity);
+  }
+}
+
+uint64_t wgo_read_violations(const wgo_engine* e, wgo_violation_rec* out, uint64_t cap) {
+  const uint64_t n = e->ring.size() < cap ? e->ring.size() : cap;
+  for (uint64_t i = 0; i < n; ++i) out[i] = e->ring[i];
+  return n;
+}
+
+int wgo_read_first_violation(const wgo_engine* e, wgo_violation_rec* out) {
+  if (!e->have_first) return 0;
+  *out = e->first;
+  return 1;
+}
+
+void wgo_read_telemetry(const wgo_engine* e, wgo_telemetry_counters* out) { *out = e->t; }
 
 void wgo_read_counters(const wgo_engine* e, wgo_counters* global, wgo_site_counters* per_site) {
   if (global) *global = e->g;

@@ -123,6 +123,42 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
 void wgo_read_counters(const wgo_engine* e, wgo_counters* global,
                        wgo_site_counters* per_site /* [n_sites] or NULL */);
 
+/* ---- profiles and telemetry (§4.8, 264-266 §5.7, Table A2 576-588;
+ *      DESIGN.md readings R26-R29) ------------------------------------------------------------------
+ * Profile flags change the PROTECTED SET, so what they skip is counted under a separate denominator
+ * ("Fast or attribution profiles that skip ... a CFI direction change the protected set and are reported
+ * under separate denominators"):
+ *   WGO_PROFILE_SKIP_FORWARD   "backward-only: authenticated returns only": a non-empty event at a
+ *                              protected-forward site is not judged (viol 0, allow = active); it still counts
+ *                              in events_total / events_by_kind / site.events and in skipped_fwd_*.
+ *   WGO_PROFILE_SKIP_BACKWARD  "forward-only": the same for protected-return sites (in both entry points:
+ *                              such an event is then neither checked nor misrouted).  Signing is not a check
+ *                              and is unaffected.
+ *   WGO_PROFILE_LOW_TELEMETRY  "same checked transfers with less reporting": verdicts, global counters and
+ *                              the first-violation record are unchanged; per-site counters and the violation
+ *                              ring are not updated.
+ * Violation record: one per event with viol != 0 — "counters, telemetry buffers, and first-violation records
+ * are diagnostic": lane = lowest violating lane, observed = val[event][lane], stored =
+ * tag[event][lane] when the event was judged as a return check, else 0; kind = 7 for an unknown site. */
+enum { WGO_PROFILE_SKIP_FORWARD = 1, WGO_PROFILE_SKIP_BACKWARD = 2, WGO_PROFILE_LOW_TELEMETRY = 4 };
+typedef struct {
+  uint64_t seq;
+  uint32_t site_id, kind, viol_mask, active_mask, lane, mode;
+  uint64_t observed, stored;
+} wgo_violation_rec; /* 48 bytes */
+typedef struct {
+  uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
+  uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 (ring enabled) */
+} wgo_telemetry_counters;
+void wgo_set_profile(wgo_engine* e, uint32_t flags);
+/* capacity 0 (default) disables the ring; the oracle keeps the FIRST `capacity` records in event order
+ * (any subset of that size is a valid ring content once it overflows). */
+void wgo_set_ring_capacity(wgo_engine* e, uint64_t capacity);
+uint64_t wgo_read_violations(const wgo_engine* e, wgo_violation_rec* out, uint64_t cap);
+/* returns 1 and fills *out when a violation was seen since the last reset, else 0 */
+int wgo_read_first_violation(const wgo_engine* e, wgo_violation_rec* out);
+void wgo_read_telemetry(const wgo_engine* e, wgo_telemetry_counters* out);
+
 #ifdef __cplusplus
 }
 #endif
