@@ -147,6 +147,55 @@ void wg_destroy(wg_engine* eng);                                /* NULL is allow
 const char* wg_strerror(wg_status s);
 int wg_last_cuda_error(const wg_engine* eng); /* cudaError_t of the last WG_ERR_CUDA, 0 if none */
 
+/* ---- profiles and telemetry (readings R26-R29) ----
+ * PAPER.md:196 (§4.8): "Fast or attribution profiles that skip kernels, sites, counters, or a CFI direction change
+ * the protected set and are reported under separate denominators"; Table A2 names the
+ * profiles; PAPER.md:264-266 (§5.7): counters, telemetry buffers and first-violation records are diagnostic —
+ * nothing below ever changes a verdict of a site that stays in the protected set.
+ *   WG_PROFILE_SKIP_FORWARD   backward-only: non-empty events at protected-forward sites are not judged
+ *                             (viol 0, allow = active); they still count in events_total / events_by_kind /
+ *                             site.events, and in skipped_fwd_events / skipped_fwd_lanes.
+ *   WG_PROFILE_SKIP_BACKWARD  forward-only: the same for protected-return sites, at both check entry points (such
+ *                             an event is then neither verified nor "misrouted").  Signing is unaffected.
+ *   WG_PROFILE_LOW_TELEMETRY  low-telemetry enforcement: same verdicts, global counters and first-violation
+ *                             record; per-site counters and the violation ring are not updated.
+ * The flags are engine configuration: they survive wg_reset_counters and wg_load_policy. */
+typedef enum {
+  WG_PROFILE_FULL = 0,
+  WG_PROFILE_SKIP_FORWARD = 1,
+  WG_PROFILE_SKIP_BACKWARD = 2,
+  WG_PROFILE_LOW_TELEMETRY = 4
+} wg_profile_flags;
+
+/* One record per event with viol_mask != 0: lane = lowest violating lane, observed = d_val[event][lane],
+ * stored = d_tag[event][lane] when the event was judged as a return check (else 0), kind = 7 for an unknown
+ * site, seq = running event index (R12). */
+typedef struct {
+  uint64_t seq;
+  uint32_t site_id, kind, viol_mask, active_mask, lane, mode;
+  uint64_t observed, stored;
+} wg_violation_rec; /* 48 bytes */
+
+typedef struct {
+  uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
+  uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 since the ring was enabled */
+} wg_telemetry_counters;
+
+/* WG_ERR_INVALID_ARG for unknown flag bits.  Applies to the calls made after it returns. */
+wg_status wg_set_profile(wg_engine* eng, uint32_t flags);
+/* Bounded violation ring in engine-owned device memory: `capacity` records (0 = off, the default).  Synchronises
+ * `cuda_stream`, reallocates, and restarts the ring empty.  When the ring is full further records are dropped and
+ * counted; which records a full ring holds is unspecified (any `capacity` of the violating events), their order
+ * in the ring is unspecified too.  Capacity survives wg_reset_counters (which empties the ring). */
+wg_status wg_set_ring_capacity(wg_engine* eng, uint64_t capacity, void* cuda_stream);
+/* Synchronises `cuda_stream`, then copies to HOST memory: the telemetry counters; the first-violation record
+ * (*h_have_first = 0 if none since the last reset; it is the record of first_violation_key and is kept even when
+ * the ring overflowed or telemetry is low); up to ring_cap ring records (*h_n_ring = how many were copied).
+ * h_first / h_ring may be NULL. */
+wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, wg_violation_rec* h_first,
+                            int* h_have_first, wg_violation_rec* h_ring, uint64_t ring_cap, uint64_t* h_n_ring,
+                            void* cuda_stream);
+
 /* ---- HOST-buffer entry points (end-to-end path) ----
  * Same semantics as the calls above but every array is in HOST memory (pinned memory gives full PCIe speed,
  * pageable works).  The engine streams the events through its own double-buffered device staging in chunks,

@@ -26,7 +26,15 @@ EXPORTS = [
     "wg_reset_counters", "wg_destroy", "wg_strerror", "wg_last_cuda_error",
     "wg_sign_continuations_host", "wg_verify_continuations_host", "wg_check_forward_host",
     "wg_probe_int_pipe", "wg_launch_count",
+    "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
 ]
+
+WG_PROFILE_FULL, WG_PROFILE_SKIP_FORWARD, WG_PROFILE_SKIP_BACKWARD, WG_PROFILE_LOW_TELEMETRY = 0, 1, 2, 4
+VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
+                            ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
+                            ("stored", "<u8")])  # wg_violation_rec, 48 bytes
+TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
+                    "ring_recorded", "ring_dropped")
 
 COUNTER_FIELDS = (
     ["events_total", "events_empty", "events_unknown_site", "events_misrouted"]
@@ -76,6 +84,9 @@ def lib() -> C.CDLL:
         L.wg_check_forward_host.argtypes = [vp, vp, vp, vp, u64, i]
         L.wg_probe_int_pipe.argtypes = [i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.wg_launch_count.argtypes = []
+        L.wg_set_profile.argtypes = [vp, C.c_uint32]
+        L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
+        L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
         L.wg_launch_count.restype = u64
         for name in EXPORTS:
             if name not in ("wg_destroy", "wg_strerror", "wg_launch_count"):
@@ -205,6 +216,26 @@ class Engine:
         _chk(lib().wg_read_counters(self._h, g.ctypes.data, None if s is None or s.size == 0 else s.ctypes.data,
                                     _stream_ptr(stream)), "wg_read_counters")
         return {k: int(v) for k, v in zip(COUNTER_FIELDS, g)}, s
+
+    # -- profiles and telemetry (warpguard.h; R26-R29) ----------------------------------
+    def wg_set_profile(self, flags: int) -> None:
+        _chk(lib().wg_set_profile(self._h, int(flags)), "wg_set_profile")
+
+    def wg_set_ring_capacity(self, capacity: int, stream=None) -> None:
+        _chk(lib().wg_set_ring_capacity(self._h, int(capacity), _stream_ptr(stream)), "wg_set_ring_capacity")
+
+    def wg_read_telemetry(self, ring_cap: int = 0, stream=None):
+        """(telemetry counters dict, first-violation record or None, ring records as a structured array)."""
+        t = np.zeros(6, dtype=np.uint64)
+        first = np.zeros(1, dtype=VIOLATION_DTYPE)
+        have = C.c_int(0)
+        ring = np.zeros(max(int(ring_cap), 1), dtype=VIOLATION_DTYPE)
+        n = C.c_uint64(0)
+        _chk(lib().wg_read_telemetry(self._h, t.ctypes.data, first.ctypes.data, C.byref(have),
+                                     ring.ctypes.data if ring_cap else None, int(ring_cap), C.byref(n),
+                                     _stream_ptr(stream)), "wg_read_telemetry")
+        return ({k: int(v) for k, v in zip(TELEMETRY_FIELDS, t)}, first[0] if have.value else None,
+                ring[: n.value] if ring_cap else ring[:0])
 
     def wg_reset_counters(self, stream=None) -> None:
         _chk(lib().wg_reset_counters(self._h, _stream_ptr(stream)), "wg_reset_counters")

@@ -19,6 +19,10 @@ struct wg_engine {
   uint64_t n_tgts = 0;
   wg::SiteRow* d_rows = nullptr;
   wg::SiteRec* d_recs = nullptr;  // v2 site records (kind, set range, pre-A SipHash mid-state), 64 B each
+  uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
+  uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
+  wg::ViolRec* d_ring = nullptr;
+  wg::FirstRec* d_first = nullptr;  // first-violation record + the key it belongs to
   int impl = 2;                   // 2 = tiled kernels (default); 1 = baseline warp-per-event kernels (WG_IMPL=v1)
   uint64_t* d_tgts = nullptr;
   unsigned long long* d_glob = nullptr;  // [C_WORDS]
@@ -114,6 +118,10 @@ wg_status zero_counters(wg_engine* e, cudaStream_t st) {
   WG_CUDA(e, cudaMemsetAsync(e->d_glob + wg::C_FIRST_VIOLATION, 0xff, sizeof(unsigned long long), st));
   if (e->n_sites)
     WG_CUDA(e, cudaMemsetAsync(e->d_site, 0, sizeof(unsigned long long) * 4 * e->n_sites, st));
+  if (e->d_first) {
+    WG_CUDA(e, cudaMemsetAsync(e->d_first, 0, sizeof(wg::FirstRec), st));
+    WG_CUDA(e, cudaMemsetAsync(&e->d_first->key, 0xff, sizeof(unsigned long long), st));
+  }
   e->seq = 0;
   e->last_mode = 0;
   return WG_OK;
@@ -125,6 +133,10 @@ wg::Params base_params(const wg_engine* e) {
   p.rows = e->d_rows;
   p.recs = e->d_recs;
   p.n_tgts = e->n_tgts;
+  p.profile = e->profile;
+  p.ring = e->d_ring;
+  p.ring_cap = e->d_ring ? e->ring_cap : 0;
+  p.first = e->d_first;
   p.tgts = e->d_tgts;
   p.glob = e->d_glob;
   p.site = e->d_site;
@@ -367,6 +379,13 @@ wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc
   }
   e->loaded = true;
   *eng = e;
+  if (!e->d_first) {
+    cudaError_t e4 = cudaMalloc(&e->d_first, sizeof(wg::FirstRec));
+    if (e4 != cudaSuccess) {
+      e->loaded = false;
+      return cuda_fail(e, e4);
+    }
+  }
   wg_status s = zero_counters(e, nullptr);
   if (s != WG_OK) return s;
   WG_CUDA(e, cudaStreamSynchronize(nullptr));
@@ -422,6 +441,8 @@ void wg_destroy(wg_engine* eng) {
       cudaDeviceSynchronize();
       free_staging(eng);
       free_tables(eng);
+      cudaFree(eng->d_ring);
+      cudaFree(eng->d_first);
     }
   }
   delete eng;
@@ -440,6 +461,65 @@ const char* wg_strerror(wg_status s) {
 }
 
 int wg_last_cuda_error(const wg_engine* eng) { return eng ? eng->last_cuda_error : 0; }
+
+wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
+  if (!eng) return WG_ERR_NO_POLICY;
+  if (flags & ~7u) return WG_ERR_INVALID_ARG;
+  eng->profile = flags;  // takes effect with the next check call (kernel parameter)
+  return WG_OK;
+}
+
+wg_status wg_set_ring_capacity(wg_engine* eng, uint64_t capacity, void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (capacity > (1ull << 28)) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  WG_CUDA(eng, cudaStreamSynchronize(st));  // no launch may still be appending to the old ring
+  wg::ViolRec* fresh = nullptr;
+  if (capacity) WG_CUDA(eng, cudaMalloc(&fresh, sizeof(wg::ViolRec) * capacity));
+  cudaFree(eng->d_ring);
+  eng->d_ring = fresh;
+  eng->ring_cap = capacity;
+  // the ring restarts empty; every other counter keeps running
+  WG_CUDA(eng, cudaMemsetAsync(eng->d_glob + wg::C_RING_TOTAL, 0, sizeof(unsigned long long), st));
+  WG_CUDA(eng, cudaStreamSynchronize(st));
+  return WG_OK;
+}
+
+wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, wg_violation_rec* h_first,
+                            int* h_have_first, wg_violation_rec* h_ring, uint64_t ring_cap, uint64_t* h_n_ring,
+                            void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (!h_counters) return WG_ERR_INVALID_ARG;
+  if ((h_first && !h_have_first) || (h_ring && !h_n_ring)) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+  unsigned long long w[5];
+  WG_CUDA(eng, cudaMemcpy(w, eng->d_glob + wg::C_SKIP_RET_EVENTS, sizeof w, cudaMemcpyDeviceToHost));
+  const uint64_t total = w[4];
+  const uint64_t recorded = total < eng->ring_cap ? total : eng->ring_cap;
+  h_counters->skipped_ret_events = w[0];
+  h_counters->skipped_ret_lanes = w[1];
+  h_counters->skipped_fwd_events = w[2];
+  h_counters->skipped_fwd_lanes = w[3];
+  h_counters->ring_recorded = recorded;
+  h_counters->ring_dropped = total - recorded;
+  if (h_first) {
+    wg::FirstRec f;
+    WG_CUDA(eng, cudaMemcpy(&f, eng->d_first, sizeof f, cudaMemcpyDeviceToHost));
+    static_assert(sizeof(wg_violation_rec) == sizeof(wg::ViolRec), "violation record layout");
+    *h_have_first = f.key != ~0ull;
+    if (*h_have_first) std::memcpy(h_first, &f.rec, sizeof(wg_violation_rec));
+  }
+  if (h_ring) {
+    const uint64_t n = recorded < ring_cap ? recorded : ring_cap;
+    if (n) WG_CUDA(eng, cudaMemcpy(h_ring, eng->d_ring, sizeof(wg_violation_rec) * n, cudaMemcpyDeviceToHost));
+    *h_n_ring = n;
+  }
+  return WG_OK;
+}
 
 wg_status wg_sign_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
                                      uint64_t* h_tag, uint64_t n) {

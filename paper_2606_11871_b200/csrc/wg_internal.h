@@ -51,8 +51,29 @@ enum CounterWord {
   C_SIGN_SKIPPED = 23,
   C_POLICY_DIGEST = 24,
   C_LAST_MODE = 25,
+  // telemetry words behind the 26 words of wg_counters (wg_telemetry_counters; R26-R28)
+  C_SKIP_RET_EVENTS = 26,
+  C_SKIP_RET_LANES = 27,
+  C_SKIP_FWD_EVENTS = 28,
+  C_SKIP_FWD_LANES = 29,
+  C_RING_TOTAL = 30,  // violation records offered to the ring (recorded = min(total, capacity))
+  C_TICKET = 31,      // CTAs that finished the current launch: the last one writes the first-violation record
   C_WORDS = 32
 };
+
+// Violation record, layout of wg_violation_rec (48 bytes)
+struct __align__(8) ViolRec {
+  uint64_t seq;
+  uint32_t site_id, kind, viol_mask, active_mask, lane, mode;
+  uint64_t observed, stored;
+};
+static_assert(sizeof(ViolRec) == 48, "ViolRec layout");
+// First-violation record kept on the device: the record and the key it was written for
+struct FirstRec {
+  ViolRec rec;
+  unsigned long long key;  // UINT64_MAX: none
+};
+enum : uint32_t { PROFILE_SKIP_FORWARD = 1, PROFILE_SKIP_BACKWARD = 2, PROFILE_LOW_TELEMETRY = 4 };
 
 // Per-site counters: 4 x u64 per site, layout of wg_site_counters.
 enum SiteWord { S_EVENTS = 0, S_LANES_CHECKED = 1, S_LANES_VIOLATION = 2, S_LANES_BLOCKED = 3 };
@@ -75,6 +96,11 @@ struct Params {
   unsigned long long* site;  // [n_sites][4]
   uint32_t n_sites;
   uint32_t mode;             // 0 detect, 1 enforce
+  uint32_t profile;          // PROFILE_* flags (R26)
+  uint32_t pad0;
+  ViolRec* ring;             // violation ring or nullptr
+  uint64_t ring_cap;         // its capacity in records
+  FirstRec* first;           // first-violation record
   uint64_t v0, v1, v2, v3;   // SipHash initial state: key ^ constants (computed host-side at load)
 };
 

@@ -34,7 +34,7 @@ namespace {
 enum : int { MODE_VERIFY = 0, MODE_FORWARD = 1, MODE_SIGN = 2 };
 enum : uint32_t { K_RET = 0, K_FWD = 1 };
 // what the tile does with an event
-enum : uint32_t { CLS_NONE = 0, CLS_COUNT = 1, CLS_RET = 2, CLS_FWD = 3, CLS_FAIL = 4 };
+enum : uint32_t { CLS_NONE = 0, CLS_COUNT = 1, CLS_RET = 2, CLS_FWD = 3, CLS_FAIL = 4, CLS_SKIP = 5 };
 
 #ifndef WG_TILE
 #define WG_TILE 16
@@ -195,7 +195,7 @@ struct WarpCtr {
 // event-parallel: decode header i, gather the SiteRec, classify (a1, a2); leaves the decoded header
 // {8 * first active lane, active, context_base & ~31 (lo), context_base (hi)} in shared memory for the
 // lane-parallel phases
-template <int MODE>
+template <int MODE, bool TEL>
 __device__ __forceinline__ TileEv classify(const Params& p, uint32_t raw_s, uint32_t dec_s, uint64_t tile,
                                            uint32_t lane) {
   TileEv ev;
@@ -230,6 +230,9 @@ __device__ __forceinline__ TileEv classify(const Params& p, uint32_t raw_s, uint
       } else {
         if (h.y == 0)
           ev.cls = CLS_COUNT;  // fully predicated off: counted, not a check (R22)
+        else if (TEL && ((a.x == K_RET && (p.profile & PROFILE_SKIP_BACKWARD)) ||
+                         (a.x == K_FWD && (p.profile & PROFILE_SKIP_FORWARD))))
+          ev.cls = CLS_SKIP;   // outside this profile's protected set: separate denominator (R26)
         else if (a.x == K_RET)
           ev.cls = (MODE == MODE_VERIFY) ? CLS_RET : CLS_FAIL;  // no tag at the forward entry point (R14)
         else if (a.x == K_FWD)
@@ -253,7 +256,8 @@ __device__ __forceinline__ Sip32 lds_state(uint32_t a) {
 // the tile kernel: MODE_VERIFY = wg_verify_continuations, MODE_FORWARD = wg_check_forward, MODE_SIGN =
 // wg_sign_continuations.  STAGED: the whole target table sits in shared memory.
 // ---------------------------------------------------------------------------------------------------
-template <int MODE, bool STAGED>
+// TEL: a profile flag is set or the violation ring is on (compiled out of the ordinary launch).
+template <int MODE, bool STAGED, bool TEL>
 __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes,
                                                                                 const uint32_t site_bytes) {
   using L = WarpLayout<MODE>;
@@ -319,7 +323,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     const uint64_t tn = t + stride;
     const uint64_t e0 = t * kT;
     // ---- event-parallel: decode, gather, classify (a1, a2) ----
-    const TileEv ev = classify<MODE>(p, warp_s + L::kRaw + rb * kT * 16, dec_s, t, lane);
+    const TileEv ev = classify<MODE, TEL>(p, warp_s + L::kRaw + rb * kT * 16, dec_s, t, lane);
     const uint32_t m_ret = __ballot_sync(kFull, ev.cls == CLS_RET);
     const uint32_t m_fwd = __ballot_sync(kFull, ev.cls == CLS_FWD);
 
@@ -378,7 +382,21 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       c.ret_lanes += __reduce_add_sync(kFull, ev.cls == CLS_RET ? na : 0u);
       c.fwd_lanes += __reduce_add_sync(kFull, ev.cls == CLS_FWD ? na : 0u);
       if (known) atomicAdd(&bykind[ev.kind], 1u);
-      if (site_bytes) {
+      if (TEL && (p.profile & (PROFILE_SKIP_FORWARD | PROFILE_SKIP_BACKWARD))) {
+        const uint32_t sr = __ballot_sync(kFull, ev.cls == CLS_SKIP && ev.kind == K_RET);
+        const uint32_t sf = __ballot_sync(kFull, ev.cls == CLS_SKIP && ev.kind == K_FWD);
+        const uint32_t srl = __reduce_add_sync(kFull, (ev.cls == CLS_SKIP && ev.kind == K_RET) ? na : 0u);
+        const uint32_t sfl = __reduce_add_sync(kFull, (ev.cls == CLS_SKIP && ev.kind == K_FWD) ? na : 0u);
+        if (lane == 0) {
+          if (sr) atomicAdd(cnt64 + C_SKIP_RET_EVENTS, static_cast<unsigned long long>(__popc(sr)));
+          if (srl) atomicAdd(cnt64 + C_SKIP_RET_LANES, static_cast<unsigned long long>(srl));
+          if (sf) atomicAdd(cnt64 + C_SKIP_FWD_EVENTS, static_cast<unsigned long long>(__popc(sf)));
+          if (sfl) atomicAdd(cnt64 + C_SKIP_FWD_LANES, static_cast<unsigned long long>(sfl));
+        }
+      }
+      if (TEL && (p.profile & PROFILE_LOW_TELEMETRY)) {
+        // "same checked transfers with less reporting" (PAPER.md Table A2): no per-site counters
+      } else if (site_bytes) {
         // per-site counters in shared memory (small policies)
         if (known) {
           atomicAdd(&site_s[ev.site * 4 + S_EVENTS], 1u);
@@ -546,7 +564,25 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
           }
           atomicMin(p.glob + C_FIRST_VIOLATION, key);
         }
-        if (viol && known) {
+        if (TEL && viol && !(p.profile & PROFILE_LOW_TELEMETRY) && p.ring_cap != 0) {
+          // violation ring (R27, R28): diagnostic, bounded; a full ring drops and counts
+          const unsigned long long slot = atomicAdd(p.glob + C_RING_TOTAL, 1ull);
+          if (slot < p.ring_cap) {
+            const uint32_t fl = static_cast<uint32_t>(__ffs(viol) - 1);
+            ViolRec r;
+            r.seq = p.seq_base + e0 + lane;
+            r.site_id = ev.site;
+            r.kind = ev.kind;
+            r.viol_mask = viol;
+            r.active_mask = ev.active;
+            r.lane = fl;
+            r.mode = p.mode;
+            r.observed = p.val[(e0 + lane) * 32 + fl];
+            r.stored = (MODE == MODE_VERIFY && ev.cls == CLS_RET) ? p.tag[(e0 + lane) * 32 + fl] : 0ull;
+            p.ring[slot] = r;
+          }
+        }
+        if (viol && known && !(TEL && (p.profile & PROFILE_LOW_TELEMETRY))) {
           if (site_bytes) {
             if (judged_na) atomicAdd(&site_s[ev.site * 4 + S_LANES_VIOLATION], pv);
             if (enforce) atomicAdd(&site_s[ev.site * 4 + S_LANES_BLOCKED], pv);
@@ -579,7 +615,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     }
   }
   __syncthreads();
-  if (threadIdx.x < 24) {
+  if (threadIdx.x < C_RING_TOTAL) {  // words 24, 25 (digest, last mode) are host-side: their slots stay 0 here
     unsigned long long v = cnt64[threadIdx.x];
     if (threadIdx.x >= C_BY_KIND && threadIdx.x < C_BY_KIND + 7) v = bykind[threadIdx.x - C_BY_KIND];
     if (v) atomicAdd(p.glob + threadIdx.x, v);
@@ -587,6 +623,40 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) {
     const uint32_t v = site_s[i];
     if (v) atomicAdd(p.site + i, static_cast<unsigned long long>(v));
+  }
+  if constexpr (MODE != MODE_SIGN) {
+    // first-violation record (R29): the LAST CTA to finish sees the final key of this launch; if
+    // the key moved into this launch's event range it writes the full record of that event.  Deterministic,
+    // and nothing on the hot path: violations only did an atomicMin.
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const unsigned long long ticket = atomicAdd(p.glob + C_TICKET, 1ull);
+      if (ticket == gridDim.x - 1) {
+        p.glob[C_TICKET] = 0ull;
+        const unsigned long long key = atomicMin(p.glob + C_FIRST_VIOLATION, ~0ull);
+        const unsigned long long seq = key >> 5;
+        if (key != ~0ull && key != p.first->key && seq >= p.seq_base && seq - p.seq_base < p.n) {
+          const uint64_t i = seq - p.seq_base;
+          const uint32_t fl = static_cast<uint32_t>(key & 31u);
+          const uint4 hh = p.hdr[i];
+          const uint2 o = __ldcg(p.out + i);  // written by another CTA of this launch: read it from L2
+          ViolRec r;
+          r.seq = seq;
+          r.site_id = hh.x;
+          r.kind = hh.x < p.n_sites ? p.recs[hh.x].kind : 7u;
+          r.viol_mask = o.x;
+          r.active_mask = hh.y;
+          r.lane = fl;
+          r.mode = p.mode;
+          r.observed = p.val[i * 32 + fl];
+          const bool judged_ret = MODE == MODE_VERIFY && r.kind == K_RET && !(p.profile & PROFILE_SKIP_BACKWARD);
+          r.stored = judged_ret ? p.tag[i * 32 + fl] : 0ull;
+          p.first->rec = r;
+          p.first->key = key;
+        }
+      }
+    }
   }
 }
 
@@ -637,17 +707,31 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
       stage_bytes + p.n_sites * 16u <= Cfg<MODE>::kLeft)
     site_bytes = p.n_sites * 16u;
   const uint32_t smem = smem_bytes<MODE>(stage_bytes + site_bytes);
-  if (staged)
-    wg_tile_kernel<MODE, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
-  else
-    wg_tile_kernel<MODE, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+  const bool tel = MODE != MODE_SIGN && (p.profile != 0 || p.ring_cap != 0);
+  if (tel) {
+    if constexpr (MODE != MODE_SIGN) {
+      if (staged)
+        wg_tile_kernel<MODE, true, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+      else
+        wg_tile_kernel<MODE, false, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    }
+  } else if (staged) {
+    wg_tile_kernel<MODE, true, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+  } else {
+    wg_tile_kernel<MODE, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+  }
   count_launch();
   return cudaGetLastError();
 }
 
 template <int MODE, bool STAGED>
 cudaError_t opt_in() {
-  return cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  if constexpr (MODE != MODE_SIGN) {
+    const cudaError_t e = cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, true>,
+                                               cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kSmemMax));
+    if (e != cudaSuccess) return e;
+  }
+  return cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               static_cast<int>(kSmemMax));
 }
 

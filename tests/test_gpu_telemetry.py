@@ -1,0 +1,134 @@
+"""Parity of profiles and telemetry (R26-R29): CUDA path through the C-ABI against the
+oracle.  Verdicts, counters, telemetry counters and the first-violation record are unique and compared bit for
+bit; the ring's ORDER is unspecified, so records are compared sorted by seq, and when the ring overflows only
+what is unique (counts) is compared and the kept records are checked to be valid ones."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_11871_b200 import binding as B
+from paper_2606_11871_b200 import streams as S
+from tests.util import oracle_for
+
+pytestmark = pytest.mark.gpu
+DET, ENF = 0, 1
+
+
+def dev():
+    return torch.device("cuda", 0)
+
+
+def prepared(config, n, mode=None):
+    st = S.make_stream(config, "cpu", n_events=n, mode=mode)
+    orc = oracle_for(st.policy)
+    hdr = st.hdr.numpy().view(np.uint64)
+    tag = orc.sign(hdr, st.val.numpy().view(np.uint64))
+    tag_t = torch.from_numpy(tag.view(np.int64).copy())
+    st.apply_return_tamper(tag_t)
+    orc.reset_counters()
+    eng = B.Engine(0).load(st.policy)
+    return st, orc, eng, hdr, st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64), \
+        (st.hdr.to(dev()), st.val.to(dev()), tag_t.to(dev()))
+
+
+def same_counters(eng, orc):
+    gg, gs = eng.wg_read_counters()
+    og, os_ = orc.read_counters()
+    assert gg == og, {k: (gg[k], og[k]) for k in og if gg[k] != og[k]}
+    assert np.array_equal(gs, os_)
+
+
+def as_tuple(r):
+    return tuple(int(r[f]) for f in B.VIOLATION_DTYPE.names)
+
+
+@pytest.mark.parametrize("config,n", [(4, 250_003), (1, 65_536), (5, 40_001)])
+def test_ring_and_first_record_equal_the_oracle(config, n):
+    if config == 5:
+        pol = S.make_policy(5, "cpu", n_sites=5_000, max_set=512)
+        st = S.make_stream(5, "cpu", n_events=n, policy=pol, batch_index=1)
+        orc = oracle_for(pol)
+        hdr = st.hdr.numpy().view(np.uint64)
+        tag = orc.sign(hdr, st.val.numpy().view(np.uint64))
+        tag_t = torch.from_numpy(tag.view(np.int64).copy())
+        st.apply_return_tamper(tag_t)
+        orc.reset_counters()
+        eng = B.Engine(0).load(pol)
+        val, tagn = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+        d = (st.hdr.to(dev()), st.val.to(dev()), tag_t.to(dev()))
+    else:
+        st, orc, eng, hdr, val, tagn, d = prepared(config, n)
+    cap = 1 << 15
+    orc.set_ring_capacity(cap)
+    eng.wg_set_ring_capacity(cap)
+    for mode in (ENF, DET):  # two calls: seq runs on, the first record stays the first call's
+        o = orc.verify(hdr, val, tagn, mode)
+        g = eng.wg_verify_continuations(*d, mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+    same_counters(eng, orc)
+    t, first, ring = eng.wg_read_telemetry(cap)
+    assert t == orc.read_telemetry() and t["ring_dropped"] == 0 and t["ring_recorded"] > 4
+    o_ring = orc.read_violations(cap)
+    assert sorted(map(as_tuple, ring)) == sorted(map(as_tuple, o_ring))
+    assert first is not None and as_tuple(first) == as_tuple(orc.read_first_violation())
+    # reset empties ring and first record; capacity stays
+    eng.wg_reset_counters()
+    t, first, ring = eng.wg_read_telemetry(cap)
+    assert first is None and len(ring) == 0 and t["ring_recorded"] == 0
+    eng.close()
+
+
+def test_full_ring_drops_and_counts_and_keeps_valid_records():
+    st, orc, eng, hdr, val, tag, d = prepared(4, 300_007)
+    orc.set_ring_capacity(1 << 15)
+    eng.wg_set_ring_capacity(5)
+    o = orc.verify(hdr, val, tag, ENF)
+    g = eng.wg_verify_continuations(*d, ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    valid = set(map(as_tuple, orc.read_violations(1 << 15)))
+    t, first, ring = eng.wg_read_telemetry(16)
+    assert len(ring) == 5 and t["ring_recorded"] == 5 and t["ring_dropped"] == len(valid) - 5
+    kept = list(map(as_tuple, ring))
+    assert len(set(kept)) == 5 and set(kept) <= valid
+    assert as_tuple(first) == as_tuple(orc.read_first_violation())  # survives the overflow
+    eng.close()
+
+
+@pytest.mark.parametrize("flags", [B.WG_PROFILE_SKIP_FORWARD, B.WG_PROFILE_SKIP_BACKWARD, B.WG_PROFILE_LOW_TELEMETRY,
+                                   B.WG_PROFILE_SKIP_FORWARD | B.WG_PROFILE_LOW_TELEMETRY,
+                                   B.WG_PROFILE_SKIP_FORWARD | B.WG_PROFILE_SKIP_BACKWARD])
+@pytest.mark.parametrize("config", [4, 1])
+def test_profiles_match_the_oracle(flags, config):
+    st, orc, eng, hdr, val, tag, d = prepared(config, 120_011)
+    orc.set_profile(flags)
+    eng.wg_set_profile(flags)
+    cap = 1 << 18  # the forward entry point fails closed on every return event: the ring must hold them all
+    orc.set_ring_capacity(cap)
+    eng.wg_set_ring_capacity(cap)
+    o = orc.verify(hdr, val, tag, ENF)
+    g = eng.wg_verify_continuations(*d, ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    o = orc.check_forward(hdr, val, DET)
+    g = eng.wg_check_forward(d[0], d[1], DET).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    same_counters(eng, orc)
+    t, first, ring = eng.wg_read_telemetry(cap)
+    assert t == orc.read_telemetry() and t["ring_dropped"] == 0
+    assert sorted(map(as_tuple, ring)) == sorted(map(as_tuple, orc.read_violations(cap)))
+    of = orc.read_first_violation()
+    assert (first is None) == (of is None) and (first is None or as_tuple(first) == as_tuple(of))
+    # the flags are configuration: they survive a reset; FULL restores the ordinary behaviour
+    eng.wg_reset_counters(); orc.reset_counters()
+    eng.wg_set_profile(B.WG_PROFILE_FULL); orc.set_profile(0)
+    assert np.array_equal(eng.wg_verify_continuations(*d, ENF).cpu().numpy().view(np.uint32), orc.verify(hdr, val, tag, ENF))
+    same_counters(eng, orc)
+    eng.close()
+
+
+def test_bad_profile_flags_are_rejected():
+    st, orc, eng, hdr, val, tag, d = prepared(1, 1000)
+    with pytest.raises(B.WgError) as e:
+        eng.wg_set_profile(8)
+    assert e.value.status == B.WG_ERR_INVALID_ARG
+    eng.close()
