@@ -94,6 +94,18 @@ def lib():
         L.wgo_read_first_violation.argtypes = [vp, vp]
         L.wgo_read_telemetry.restype = None
         L.wgo_read_telemetry.argtypes = [vp, vp]
+        L.wgo_shadow_configure.restype = C.c_int
+        L.wgo_shadow_configure.argtypes = [vp, u32, u32]
+        L.wgo_shadow_push.restype = None
+        L.wgo_shadow_push.argtypes = [vp, vp, vp, vp, u64, C.c_int]
+        L.wgo_shadow_check_ret.restype = None
+        L.wgo_shadow_check_ret.argtypes = [vp, vp, vp, vp, u64, C.c_int]
+        L.wgo_shadow_read_counters.restype = None
+        L.wgo_shadow_read_counters.argtypes = [vp, vp]
+        L.wgo_shadow_poke.restype = C.c_int
+        L.wgo_shadow_poke.argtypes = [vp, u32, u32, u32, C.c_int, u64]
+        L.wgo_shadow_depth.restype = u32
+        L.wgo_shadow_depth.argtypes = [vp, u32, u32]
         _lib = L
     return _lib
 
@@ -219,9 +231,46 @@ class Oracle:
         return {k: int(v) for k, v in zip(TELEMETRY_FIELDS, t)}
 
 
+    # ---- stateful shadow stack (wg_oracle.h; R30-R36) ----
+    def shadow_configure(self, n_warp_slots: int, max_depth: int):
+        if lib().wgo_shadow_configure(self._h, int(n_warp_slots), int(max_depth)) != 0:
+            raise ValueError("max_depth must be in 1..64")
+
+    def _shadow(self, fn, hdr, val, mode):
+        hdr = _hdr_bytes(hdr)
+        val = _c(val, np.uint64)
+        n = hdr.shape[0]
+        out = np.zeros((n, 2), dtype=np.uint32)
+        fn(self._h, _ptr(hdr), _ptr(val), _ptr(out), n, int(mode))
+        return out
+
+    def shadow_push(self, hdr, val, mode):
+        return self._shadow(lib().wgo_shadow_push, hdr, val, mode)
+
+    def shadow_check_ret(self, hdr, val, mode):
+        return self._shadow(lib().wgo_shadow_check_ret, hdr, val, mode)
+
+    def shadow_read_counters(self) -> dict:
+        c = np.zeros(16, dtype=np.uint64)
+        lib().wgo_shadow_read_counters(self._h, _ptr(c))
+        return {k: int(v) for k, v in zip(SHADOW_FIELDS, c)}
+
+    def shadow_poke(self, warp_slot: int, lane: int, entry_depth: int, field: int, xor_value: int):
+        if lib().wgo_shadow_poke(self._h, int(warp_slot), int(lane), int(entry_depth), int(field), int(xor_value)) != 0:
+            raise ValueError("shadow_poke: out of range")
+
+    def shadow_depth(self, warp_slot: int, lane: int) -> int:
+        return int(lib().wgo_shadow_depth(self._h, int(warp_slot), int(lane)))
+
+
 PROFILE_SKIP_FORWARD, PROFILE_SKIP_BACKWARD, PROFILE_LOW_TELEMETRY = 1, 2, 4
 VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
                             ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
                             ("stored", "<u8")])
 TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
                     "ring_recorded", "ring_dropped")
+SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
+                 "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
+                 "non_return_events", "slot_overflow_events", "slot_conflict_events", "viol_lanes", "viol_events",
+                 "blocked_lanes")
+POKE_EXPECTED, POKE_TOKEN, POKE_CALLSITE, POKE_ENTRY_DEPTH, POKE_DEPTH_COUNTER = 0, 1, 2, 3, 4

@@ -76,6 +76,15 @@ struct wgo_engine {
   wgo_telemetry_counters t = {0, 0, 0, 0, 0, 0};
   bool have_first = false;
   wgo_violation_rec first = {};
+  // stateful shadow stack (R30-R36): entry (slot, lane, d) lives at ((slot * 32 + lane) * max_depth + d)
+  struct ShadowEntry {
+    uint64_t expected_return, token;
+    uint32_t callsite_id, depth;
+  };
+  uint32_t sh_slots = 0, sh_max_depth = 0;
+  std::vector<ShadowEntry> sh_entry;
+  std::vector<uint32_t> sh_depth;  // [slot * 32 + lane]
+  wgo_shadow_counters sh = {};
 };
 
 extern "C" {
@@ -362,6 +371,142 @@ void wgo_read_counters(const wgo_engine* e, wgo_counters* global, wgo_site_count
   if (global) *global = e->g;
   if (per_site)
     for (uint32_t s = 0; s < e->n_sites; ++s) per_site[s] = e->site[s];
+}
+
+// ---------------------------------------------------------------------------------------------------
+// stateful shadow stack, PAPER.md:162-166, 242-248, 258 (wg_oracle.h; R30-R36)
+// ---------------------------------------------------------------------------------------------------
+int wgo_shadow_configure(wgo_engine* e, uint32_t n_warp_slots, uint32_t max_depth) {
+  if (max_depth == 0 || max_depth > 64) return -1;
+  e->sh_slots = n_warp_slots;
+  e->sh_max_depth = max_depth;
+  e->sh_entry.assign(static_cast<size_t>(n_warp_slots) * 32 * max_depth, wgo_engine::ShadowEntry{0, 0, 0, 0});
+  e->sh_depth.assign(static_cast<size_t>(n_warp_slots) * 32, 0u);
+  e->sh = wgo_shadow_counters{};
+  return 0;
+}
+
+static uint64_t shadow_ctx(uint64_t context_base, uint32_t depth, uint32_t lane) {
+  const uint64_t epoch = context_base >> 48;
+  const uint64_t slot = (context_base >> 5) & 0xffffffffull;
+  return (epoch << 48) | (static_cast<uint64_t>(depth) << 37) | (slot << 5) | lane;
+}
+
+// 0: process per lane; else every active lane violates and the state is untouched
+static int shadow_event_failure(wgo_engine* e, const std::vector<uint32_t>& uses, const wgo_event_hdr& h) {
+  const uint32_t s = h.site_id;
+  const uint64_t slot = (h.context_base >> 5) & 0xffffffffull;
+  if (s >= e->n_sites || e->kind[s] != WGO_PROTECTED_RETURN) return 1;  // not a return site of the policy
+  if (slot >= e->sh_slots) return 2;                                     // thread-slot overflow
+  if (uses[slot] > 1) return 3;                                          // one call = one step of distinct warps
+  return 0;
+}
+
+static void shadow_run(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, wgo_verdict* out,
+                       uint64_t n, int mode, bool push) {
+  // how often each warp slot occurs in this call (non-empty or not: the header alone decides)
+  std::vector<uint32_t> uses(e->sh_slots, 0u);
+  for (uint64_t ev = 0; ev < n; ++ev) {
+    const uint64_t slot = (hdr[ev].context_base >> 5) & 0xffffffffull;
+    if (slot < e->sh_slots) uses[slot] += 1;
+  }
+  for (uint64_t ev = 0; ev < n; ++ev) {
+    const wgo_event_hdr& h = hdr[ev];
+    const uint32_t a = h.active_mask;
+    uint32_t viol = 0;
+    if (a == 0) {
+      e->sh.empty_events += 1;
+    } else {
+      (push ? e->sh.push_events : e->sh.check_events) += 1;
+      (push ? e->sh.push_lanes : e->sh.check_lanes) += popcount32(a);
+      const int fail = shadow_event_failure(e, uses, h);
+      if (fail) {
+        viol = a;
+        if (fail == 1) e->sh.non_return_events += 1;
+        if (fail == 2) e->sh.slot_overflow_events += 1;
+        if (fail == 3) e->sh.slot_conflict_events += 1;
+      } else {
+        const uint64_t slot = (h.context_base >> 5) & 0xffffffffull;
+        for (uint32_t lane = 0; lane < 32; ++lane) {
+          if (!((a >> lane) & 1u)) continue;  // guard-false lanes made no call / return
+          uint32_t& d = e->sh_depth[slot * 32 + lane];
+          wgo_engine::ShadowEntry* st = &e->sh_entry[(slot * 32 + lane) * e->sh_max_depth];
+          if (push) {
+            if (d >= e->sh_max_depth) {  // overflow fails closed instead of wrapping
+              viol |= 1u << lane;
+              e->sh.overflow_lanes += 1;
+              continue;
+            }
+            st[d].expected_return = val[ev * 32 + lane];
+            st[d].callsite_id = h.site_id;
+            st[d].depth = d;
+            st[d].token = wgo_mac(e->k0, e->k1, h.site_id, val[ev * 32 + lane], shadow_ctx(h.context_base, d, lane));
+            d += 1;
+          } else {
+            if (d == 0) {  // underflow
+              viol |= 1u << lane;
+              e->sh.underflow_lanes += 1;
+              continue;
+            }
+            d -= 1;  // the return consumes the frame whatever the verdict (R33)
+            const wgo_engine::ShadowEntry& r = st[d];
+            if (r.depth != d) {
+              viol |= 1u << lane;
+              e->sh.depth_mismatch_lanes += 1;
+            } else if (r.token != wgo_mac(e->k0, e->k1, r.callsite_id, r.expected_return,
+                                          shadow_ctx(h.context_base, r.depth, lane))) {
+              viol |= 1u << lane;
+              e->sh.token_mismatch_lanes += 1;
+            } else if (r.expected_return != val[ev * 32 + lane] || r.callsite_id != h.site_id) {
+              viol |= 1u << lane;
+              e->sh.target_mismatch_lanes += 1;
+            }
+          }
+        }
+      }
+    }
+    if (viol) {
+      e->sh.viol_lanes += popcount32(viol);
+      e->sh.viol_events += 1;
+      if (mode == WGO_ENFORCE) e->sh.blocked_lanes += popcount32(viol);
+    }
+    out[ev].viol_mask = viol;
+    out[ev].allow_mask = (mode == WGO_ENFORCE) ? (a & ~viol) : a;
+  }
+}
+
+void wgo_shadow_push(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, wgo_verdict* out,
+                     uint64_t n, int mode) {
+  shadow_run(e, hdr, val, out, n, mode, true);
+}
+
+void wgo_shadow_check_ret(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, wgo_verdict* out,
+                          uint64_t n, int mode) {
+  shadow_run(e, hdr, val, out, n, mode, false);
+}
+
+void wgo_shadow_read_counters(const wgo_engine* e, wgo_shadow_counters* out) { *out = e->sh; }
+
+int wgo_shadow_poke(wgo_engine* e, uint32_t warp_slot, uint32_t lane, uint32_t entry_depth, int field,
+                    uint64_t xor_value) {
+  if (warp_slot >= e->sh_slots || lane >= 32) return -1;
+  if (field == 4) {
+    e->sh_depth[static_cast<size_t>(warp_slot) * 32 + lane] ^= static_cast<uint32_t>(xor_value);
+    return 0;
+  }
+  if (entry_depth >= e->sh_max_depth) return -1;
+  wgo_engine::ShadowEntry& r = e->sh_entry[(static_cast<size_t>(warp_slot) * 32 + lane) * e->sh_max_depth + entry_depth];
+  switch (field) {
+    case 0: r.expected_return ^= xor_value; return 0;
+    case 1: r.token ^= xor_value; return 0;
+    case 2: r.callsite_id ^= static_cast<uint32_t>(xor_value); return 0;
+    case 3: r.depth ^= static_cast<uint32_t>(xor_value); return 0;
+  }
+  return -1;
+}
+
+uint32_t wgo_shadow_depth(const wgo_engine* e, uint32_t warp_slot, uint32_t lane) {
+  return e->sh_depth[static_cast<size_t>(warp_slot) * 32 + lane];
 }
 
 }  // extern "C"

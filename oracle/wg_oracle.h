@@ -159,6 +159,45 @@ uint64_t wgo_read_violations(const wgo_engine* e, wgo_violation_rec* out, uint64
 int wgo_read_first_violation(const wgo_engine* e, wgo_violation_rec* out);
 void wgo_read_telemetry(const wgo_engine* e, wgo_telemetry_counters* out);
 
+
+/* ---- stateful shadow stack (§4.4, 242-248 §5.5, 258 §5.6;
+ *      DESIGN.md readings R30-R36) --------------------------------------------------------------------
+ * "one logical shadow stack per CUDA thread slot ... bounded per-thread depth arrays.  Each shadow entry stores
+ * expected_return, callsite_id, depth, and token".  thread slot = (warp_slot, lane) with
+ * warp_slot = bits 36..5 of context_base and epoch = bits 63..48 (the depth field of context_base is ignored:
+ * the engine owns the depth).  Token of an entry at depth d:
+ *     MAC(key, callsite_id, expected_return, (epoch << 48) | (d << 37) | (warp_slot << 5) | lane).
+ * push: per active lane, d = depth: d == max_depth -> overflow, the lane violates and nothing is
+ *   written; else the entry {value, site, d, token} is written at d and depth becomes d + 1.
+ * check_ret: per active lane, d = depth: d == 0 -> underflow, violates; else the entry at d - 1
+ *   is read and the depth becomes d - 1 whatever the verdict (the return consumed the frame); the lane violates
+ *   on, in this order: entry.depth != d - 1 (depth mismatch); token != MAC over the ENTRY's own fields under
+ *   the event's epoch (token mismatch); entry.expected_return != observed value or entry.callsite_id != site
+ *   (target mismatch).  Each violating lane counts under exactly one cause.
+ * Event-level failures, all lanes violate, state untouched ("fail closed instead of aliasing"):
+ *   unknown site or a site that is not protected-return (non_return); warp_slot >= n_warp_slots (slot
+ *   overflow); a warp_slot that occurs more than once in one call (slot conflict: a call is one lock-step step
+ *   of distinct warps).  Empty masks are counted and change nothing. */
+typedef struct {
+  uint64_t push_events, push_lanes, check_events, check_lanes, empty_events;
+  uint64_t overflow_lanes, underflow_lanes, depth_mismatch_lanes, token_mismatch_lanes, target_mismatch_lanes;
+  uint64_t non_return_events, slot_overflow_events, slot_conflict_events;
+  uint64_t viol_lanes, viol_events, blocked_lanes;
+} wgo_shadow_counters; /* 16 x u64 */
+/* (re)allocates and zeroes the shadow state and its counters; max_depth in 1..64 */
+int wgo_shadow_configure(wgo_engine* e, uint32_t n_warp_slots, uint32_t max_depth);
+void wgo_shadow_push(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, wgo_verdict* out,
+                     uint64_t n, int mode);
+void wgo_shadow_check_ret(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, wgo_verdict* out,
+                          uint64_t n, int mode);
+void wgo_shadow_read_counters(const wgo_engine* e, wgo_shadow_counters* out);
+/* the attacker's write into the (ordinary, writable) shadow memory: field 0 expected_return, 1 token,
+ * 2 callsite_id, 3 depth of the entry; 4 = the slot's current depth counter (entry_depth ignored) */
+int wgo_shadow_poke(wgo_engine* e, uint32_t warp_slot, uint32_t lane, uint32_t entry_depth, int field,
+                    uint64_t xor_value);
+/* current depth of a thread slot (test read-back) */
+uint32_t wgo_shadow_depth(const wgo_engine* e, uint32_t warp_slot, uint32_t lane);
+
 #ifdef __cplusplus
 }
 #endif
