@@ -196,6 +196,41 @@ wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, w
                             int* h_have_first, wg_violation_rec* h_ring, uint64_t ring_cap, uint64_t* h_n_ring,
                             void* cuda_stream);
 
+/* ---- stateful shadow stack (readings R30-R36) ----
+ * The steps either side of the MAC in the paper's backward mechanism: "one logical shadow stack per CUDA thread
+ * slot ... bounded per-thread depth arrays.  Each shadow entry stores expected_return, callsite_id, depth, and
+ * token" (§5.5; 162-166 §4.4; 258 §5.6).  thread slot = (warp_slot, lane), warp_slot = bits 36..5 and
+ * epoch = bits 63..48 of context_base (its depth field is ignored: the engine owns the depth).  Entry token:
+ *     MAC(key, callsite_id, expected_return, epoch << 48 | depth << 37 | warp_slot << 5 | lane).
+ * wg_shadow_push: per active lane, depth == max_depth -> overflow: the lane violates, nothing is written; else
+ *   the entry {d_val, site, depth, token} is written and the depth incremented.
+ * wg_shadow_check_ret: per active lane, depth == 0 -> underflow: violates; else the entry at depth - 1 is read
+ *   and the depth decremented whatever the verdict; the lane violates on (first that applies) entry.depth !=
+ *   depth - 1; token != MAC over the entry's own fields under the event's epoch; entry.expected_return != d_val or
+ *   entry.callsite_id != site.
+ * All active lanes violate and no state changes when: the site is unknown or not protected-return; warp_slot >=
+ *   n_warp_slots ("if a launch exceeds the configured capacity, the backward check fails closed instead of
+ *   wrapping"); the warp_slot occurs more than once in the call (one call = one lock-step step of distinct warps).
+ * The shadow arrays are ordinary device memory in the paper's threat model: wg_shadow_poke is the attacker's write
+ * (field 0 expected_return, 1 token, 2 callsite_id, 3 entry depth, 4 the slot's depth counter), used by the tests.
+ * d_out: verdicts as for the check calls (allow = active & ~viol in enforce mode). */
+typedef struct {
+  uint64_t push_events, push_lanes, check_events, check_lanes, empty_events;
+  uint64_t overflow_lanes, underflow_lanes, depth_mismatch_lanes, token_mismatch_lanes, target_mismatch_lanes;
+  uint64_t non_return_events, slot_overflow_events, slot_conflict_events;
+  uint64_t viol_lanes, viol_events, blocked_lanes;
+} wg_shadow_counters; /* 16 x u64 */
+/* (re)allocates and zeroes the shadow state and its counters; max_depth in 1..64; synchronises cuda_stream */
+wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t max_depth, void* cuda_stream);
+wg_status wg_shadow_push(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val, wg_verdict* d_out,
+                         uint64_t n, wg_mode mode, void* cuda_stream);
+wg_status wg_shadow_check_ret(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val, wg_verdict* d_out,
+                              uint64_t n, wg_mode mode, void* cuda_stream);
+wg_status wg_shadow_read_counters(wg_engine* eng, wg_shadow_counters* h_out, void* cuda_stream);
+wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t entry_depth, int field,
+                         uint64_t xor_value, void* cuda_stream);
+wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t* h_depth, void* cuda_stream);
+
 /* ---- HOST-buffer entry points (end-to-end path) ----
  * Same semantics as the calls above but every array is in HOST memory (pinned memory gives full PCIe speed,
  * pageable works).  The engine streams the events through its own double-buffered device staging in chunks,

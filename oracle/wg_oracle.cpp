@@ -449,6 +449,11 @@ static void shadow_run(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* 
               continue;
             }
             d -= 1;  // the return consumes the frame whatever the verdict (R33)
+            if (d >= e->sh_max_depth) {  // a corrupted counter points past the bounded array: no such entry
+              viol |= 1u << lane;
+              e->sh.depth_mismatch_lanes += 1;
+              continue;
+            }
             const wgo_engine::ShadowEntry& r = st[d];
             if (r.depth != d) {
               viol |= 1u << lane;

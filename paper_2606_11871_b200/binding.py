@@ -27,7 +27,13 @@ EXPORTS = [
     "wg_sign_continuations_host", "wg_verify_continuations_host", "wg_check_forward_host",
     "wg_probe_int_pipe", "wg_launch_count",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
+    "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
+    "wg_shadow_depth",
 ]
+SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
+                 "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
+                 "non_return_events", "slot_overflow_events", "slot_conflict_events", "viol_lanes", "viol_events",
+                 "blocked_lanes")
 
 WG_PROFILE_FULL, WG_PROFILE_SKIP_FORWARD, WG_PROFILE_SKIP_BACKWARD, WG_PROFILE_LOW_TELEMETRY = 0, 1, 2, 4
 VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
@@ -84,6 +90,12 @@ def lib() -> C.CDLL:
         L.wg_check_forward_host.argtypes = [vp, vp, vp, vp, u64, i]
         L.wg_probe_int_pipe.argtypes = [i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.wg_launch_count.argtypes = []
+        L.wg_shadow_configure.argtypes = [vp, C.c_uint32, C.c_uint32, vp]
+        L.wg_shadow_push.argtypes = [vp, vp, vp, vp, u64, i, vp]
+        L.wg_shadow_check_ret.argtypes = [vp, vp, vp, vp, u64, i, vp]
+        L.wg_shadow_read_counters.argtypes = [vp, vp, vp]
+        L.wg_shadow_poke.argtypes = [vp, C.c_uint32, C.c_uint32, C.c_uint32, i, u64, vp]
+        L.wg_shadow_depth.argtypes = [vp, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32), vp]
         L.wg_set_profile.argtypes = [vp, C.c_uint32]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
@@ -216,6 +228,40 @@ class Engine:
         _chk(lib().wg_read_counters(self._h, g.ctypes.data, None if s is None or s.size == 0 else s.ctypes.data,
                                     _stream_ptr(stream)), "wg_read_counters")
         return {k: int(v) for k, v in zip(COUNTER_FIELDS, g)}, s
+
+    # -- stateful shadow stack (warpguard.h; R30-R36) -------------------------------------
+    def wg_shadow_configure(self, n_warp_slots: int, max_depth: int, stream=None) -> None:
+        _chk(lib().wg_shadow_configure(self._h, int(n_warp_slots), int(max_depth), _stream_ptr(stream)),
+             "wg_shadow_configure")
+
+    def _shadow(self, fn, what, hdr, val, mode, out, stream):
+        n = hdr.shape[0]
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32, device=hdr.device)
+        _chk(fn(self._h, _dev(hdr, "hdr", 2, 8), _dev(val, "val", 32, 8), _dev(out, "out", 2, 4), n, int(mode),
+                _stream_ptr(stream)), what)
+        return out
+
+    def wg_shadow_push(self, hdr, val, mode: int, out=None, stream=None) -> torch.Tensor:
+        return self._shadow(lib().wg_shadow_push, "wg_shadow_push", hdr, val, mode, out, stream)
+
+    def wg_shadow_check_ret(self, hdr, val, mode: int, out=None, stream=None) -> torch.Tensor:
+        return self._shadow(lib().wg_shadow_check_ret, "wg_shadow_check_ret", hdr, val, mode, out, stream)
+
+    def wg_shadow_read_counters(self, stream=None) -> dict:
+        c = np.zeros(16, dtype=np.uint64)
+        _chk(lib().wg_shadow_read_counters(self._h, c.ctypes.data, _stream_ptr(stream)), "wg_shadow_read_counters")
+        return {k: int(v) for k, v in zip(SHADOW_FIELDS, c)}
+
+    def wg_shadow_poke(self, warp_slot: int, lane: int, entry_depth: int, field: int, xor_value: int, stream=None):
+        _chk(lib().wg_shadow_poke(self._h, int(warp_slot), int(lane), int(entry_depth), int(field), int(xor_value),
+                                  _stream_ptr(stream)), "wg_shadow_poke")
+
+    def wg_shadow_depth(self, warp_slot: int, lane: int, stream=None) -> int:
+        d = C.c_uint32(0)
+        _chk(lib().wg_shadow_depth(self._h, int(warp_slot), int(lane), C.byref(d), _stream_ptr(stream)),
+             "wg_shadow_depth")
+        return int(d.value)
 
     # -- profiles and telemetry (warpguard.h; R26-R29) ----------------------------------
     def wg_set_profile(self, flags: int) -> None:

@@ -14,7 +14,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libwarpguard.so"
-SOURCES = ["wg_api.cu", "wg_kernels_v1.cu", "wg_kernels_v2.cu", "wg_probe.cu"]
+SOURCES = ["wg_api.cu", "wg_kernels_v1.cu", "wg_kernels_v2.cu", "wg_shadow.cu", "wg_probe.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",

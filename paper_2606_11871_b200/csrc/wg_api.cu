@@ -23,6 +23,7 @@ struct wg_engine {
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
   wg::ViolRec* d_ring = nullptr;
   wg::FirstRec* d_first = nullptr;  // first-violation record + the key it belongs to
+  wg::ShadowState sh = {0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // stateful shadow stack
   int impl = 2;                   // 2 = tiled kernels (default); 1 = baseline warp-per-event kernels (WG_IMPL=v1)
   uint64_t* d_tgts = nullptr;
   unsigned long long* d_glob = nullptr;  // [C_WORDS]
@@ -99,6 +100,16 @@ void free_tables(wg_engine* e) {
   e->d_glob = nullptr;
   e->d_site = nullptr;
   e->loaded = false;
+}
+
+void free_shadow(wg_engine* e) {
+  cudaFree(e->sh.depth_ctr);
+  cudaFree(e->sh.expected);
+  cudaFree(e->sh.token);
+  cudaFree(e->sh.meta);
+  cudaFree(e->sh.uses);
+  cudaFree(e->sh.counters);
+  e->sh = wg::ShadowState{0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
 }
 
 void free_staging(wg_engine* e) {
@@ -443,6 +454,7 @@ void wg_destroy(wg_engine* eng) {
       free_tables(eng);
       cudaFree(eng->d_ring);
       cudaFree(eng->d_first);
+      free_shadow(eng);
     }
   }
   delete eng;
@@ -461,6 +473,114 @@ const char* wg_strerror(wg_status s) {
 }
 
 int wg_last_cuda_error(const wg_engine* eng) { return eng ? eng->last_cuda_error : 0; }
+
+// ---- stateful shadow stack (wg_shadow.cu) ----------------------------------------------------------
+wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t max_depth, void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (max_depth == 0 || max_depth > 64) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  WG_CUDA(eng, cudaStreamSynchronize(st));
+  free_shadow(eng);
+  wg::ShadowState sh = {n_warp_slots, max_depth, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  const size_t lanes = static_cast<size_t>(n_warp_slots ? n_warp_slots : 1) * 32;
+  const size_t entries = lanes * max_depth;
+  cudaError_t err;
+  if ((err = cudaMalloc(&sh.depth_ctr, lanes * 4)) != cudaSuccess || (err = cudaMalloc(&sh.expected, entries * 8)) != cudaSuccess ||
+      (err = cudaMalloc(&sh.token, entries * 8)) != cudaSuccess || (err = cudaMalloc(&sh.meta, entries * 8)) != cudaSuccess ||
+      (err = cudaMalloc(&sh.uses, lanes / 32 * 4)) != cudaSuccess || (err = cudaMalloc(&sh.counters, 16 * 8)) != cudaSuccess) {
+    eng->sh = sh;
+    free_shadow(eng);
+    return cuda_fail(eng, err);
+  }
+  eng->sh = sh;
+  WG_CUDA(eng, cudaMemsetAsync(sh.depth_ctr, 0, lanes * 4, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.expected, 0, entries * 8, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.token, 0, entries * 8, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.meta, 0, entries * 8, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.uses, 0, lanes / 32 * 4, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.counters, 0, 16 * 8, st));
+  WG_CUDA(eng, cudaStreamSynchronize(st));
+  return WG_OK;
+}
+
+static wg_status shadow_common(wg_engine* e, bool push, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                               wg_verdict* d_out, uint64_t n, wg_mode mode, void* cuda_stream) {
+  if (!e || !e->loaded || !e->sh.counters) return WG_ERR_NO_POLICY;
+  if (mode != WG_MODE_DETECT && mode != WG_MODE_ENFORCE) return WG_ERR_INVALID_ARG;
+  if (n == 0) return WG_OK;
+  if (!d_hdr || !d_val || !d_out || n > (1ull << 31)) return WG_ERR_INVALID_ARG;
+  if (!aligned(d_hdr, 16) || !aligned(d_val, 16) || !aligned(d_out, 8)) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(e->device);
+  if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
+  wg::Params p = base_params(e);
+  p.hdr = reinterpret_cast<const uint4*>(d_hdr);
+  p.val = d_val;
+  p.out = reinterpret_cast<uint2*>(d_out);
+  p.n = n;
+  p.mode = static_cast<uint32_t>(mode);
+  WG_CUDA(e, wg::launch_shadow(p, e->sh, push, e->sm_count, static_cast<cudaStream_t>(cuda_stream)));
+  return WG_OK;
+}
+
+wg_status wg_shadow_push(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val, wg_verdict* d_out,
+                         uint64_t n, wg_mode mode, void* cuda_stream) {
+  return shadow_common(eng, true, d_hdr, d_val, d_out, n, mode, cuda_stream);
+}
+
+wg_status wg_shadow_check_ret(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val, wg_verdict* d_out,
+                              uint64_t n, wg_mode mode, void* cuda_stream) {
+  return shadow_common(eng, false, d_hdr, d_val, d_out, n, mode, cuda_stream);
+}
+
+wg_status wg_shadow_read_counters(wg_engine* eng, wg_shadow_counters* h_out, void* cuda_stream) {
+  if (!eng || !eng->loaded || !eng->sh.counters) return WG_ERR_NO_POLICY;
+  if (!h_out) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+  static_assert(sizeof(wg_shadow_counters) == 16 * 8, "wg_shadow_counters layout");
+  WG_CUDA(eng, cudaMemcpy(h_out, eng->sh.counters, sizeof(wg_shadow_counters), cudaMemcpyDeviceToHost));
+  return WG_OK;
+}
+
+wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t entry_depth, int field,
+                         uint64_t xor_value, void* cuda_stream) {
+  if (!eng || !eng->loaded || !eng->sh.counters) return WG_ERR_NO_POLICY;
+  if (warp_slot >= eng->sh.n_slots || lane >= 32 || field < 0 || field > 4) return WG_ERR_INVALID_ARG;
+  if (field != 4 && entry_depth >= eng->sh.max_depth) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+  const size_t li = static_cast<size_t>(warp_slot) * 32 + lane;
+  const size_t ei = (static_cast<size_t>(warp_slot) * eng->sh.max_depth + entry_depth) * 32 + lane;
+  void* addr = nullptr;
+  size_t bytes = 8;
+  switch (field) {
+    case 0: addr = eng->sh.expected + ei; break;
+    case 1: addr = eng->sh.token + ei; break;
+    case 2: addr = reinterpret_cast<uint32_t*>(eng->sh.meta + ei); bytes = 4; break;
+    case 3: addr = reinterpret_cast<uint32_t*>(eng->sh.meta + ei) + 1; bytes = 4; break;
+    default: addr = eng->sh.depth_ctr + li; bytes = 4; break;
+  }
+  uint64_t v = 0;
+  WG_CUDA(eng, cudaMemcpy(&v, addr, bytes, cudaMemcpyDeviceToHost));
+  v ^= xor_value;
+  WG_CUDA(eng, cudaMemcpy(addr, &v, bytes, cudaMemcpyHostToDevice));
+  return WG_OK;
+}
+
+wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t* h_depth, void* cuda_stream) {
+  if (!eng || !eng->loaded || !eng->sh.counters) return WG_ERR_NO_POLICY;
+  if (warp_slot >= eng->sh.n_slots || lane >= 32 || !h_depth) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+  WG_CUDA(eng, cudaMemcpy(h_depth, eng->sh.depth_ctr + static_cast<size_t>(warp_slot) * 32 + lane, 4,
+                          cudaMemcpyDeviceToHost));
+  return WG_OK;
+}
 
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;

@@ -104,6 +104,19 @@ struct Params {
   uint64_t v0, v1, v2, v3;   // SipHash initial state: key ^ constants (computed host-side at load)
 };
 
+// Shadow-stack state (wg_shadow.cu; R30-R36): structure of arrays, all engine-allocated but, as in the
+// paper, treated as attacker-writable: nothing read from it is trusted before its token verifies.
+struct ShadowState {
+  uint32_t n_slots, max_depth;
+  uint32_t* depth_ctr;          // [n_slots][32]
+  uint64_t* expected;           // [n_slots][max_depth][32]
+  uint64_t* token;              // [n_slots][max_depth][32]
+  uint2* meta;                  // [n_slots][max_depth][32] {callsite_id, depth}
+  uint32_t* uses;               // [n_slots] occurrences of a warp slot in the current call
+  unsigned long long* counters; // [16] wg_shadow_counters
+};
+cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st);
+
 // launchers (wg_kernels.cu); grid sizing from the SM count of the engine's device
 cudaError_t launch_sign_v1(const Params& p, int sm_count, cudaStream_t st);
 cudaError_t launch_check_v1(const Params& p, int sm_count, cudaStream_t st);

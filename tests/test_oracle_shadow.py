@@ -113,6 +113,14 @@ def test_every_corruption_of_the_writable_shadow_memory_is_caught_on_its_lane_on
     o.shadow_poke(2, 6, 0, oracle.POKE_DEPTH_COUNTER, 1 ^ 3)  # depth 1 -> 3
     out = o.shadow_check_ret(ev(0, FULL, 2), vals(0x40), ENF)
     assert out[0, 0] == 1 << 6 and o.shadow_read_counters()["depth_mismatch_lanes"] == 1
+    # ... or far past the bounded array: no such entry, still a depth mismatch, and a push there overflows
+    o = make(max_depth=4)
+    o.shadow_push(ev(0, FULL, 2), vals(0x40), ENF)
+    o.shadow_poke(2, 6, 0, oracle.POKE_DEPTH_COUNTER, 1 ^ 0x80000000)
+    assert o.shadow_push(ev(0, 1 << 6, 2), vals(0x41), ENF)[0, 0] == 1 << 6
+    out = o.shadow_check_ret(ev(0, FULL, 2), vals(0x40), ENF)
+    c = o.shadow_read_counters()
+    assert out[0, 0] == 1 << 6 and c["depth_mismatch_lanes"] == 1 and c["overflow_lanes"] == 1
 
 
 def test_replay_across_epochs_fails():
