@@ -57,6 +57,8 @@ def parse_args():
     ap.add_argument("--ref-events", type=int, default=1_000_000, help="events per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shadow", action="store_true",
+                    help="also time the stateful shadow stack (SURVEY 8(f-1)): one lock-step push + check_ret over 1 Mi warps")
     return ap.parse_args()
 
 
@@ -389,6 +391,40 @@ def run_ours(a) -> None:
                          f"verdicts equal the GPU's on all {nc} events",
                "lane_verdicts_per_sec": (og["ret_lanes"] + og["fwd_lanes"]) / dt}
 
+    # ---- optional: the stateful shadow stack (wg_shadow_push + wg_shadow_check_ret), one lock-step call each ----
+    shadow = None
+    if a.shadow:
+        ns, depth = 1 << 20, 4
+        eng.wg_shadow_configure(ns, depth)
+        gsh = torch.Generator(device=dev).manual_seed(4242)
+        ret_sites = torch.from_numpy(np.nonzero(st.policy.kind == S.PROTECTED_RETURN)[0]).to(dev)
+        site = ret_sites[torch.randint(0, len(ret_sites), (ns,), generator=gsh, device=dev)]
+        slot = torch.randperm(ns, generator=gsh, device=dev)
+        mask = st.active_mask()[:ns]
+        s_hdr = torch.stack([site | (mask << 32), (1 << 48) | (slot << 5)], dim=1).contiguous()
+        s_val = st.val[:ns].contiguous()
+        s_out = torch.empty((ns, 2), dtype=torch.int32, device=dev)
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        for rep_ in range(4):  # each repetition pushes one frame and pops it again: the state returns to empty
+            evs[0].record()
+            eng.wg_shadow_push(s_hdr, s_val, st.mode, s_out)
+            evs[1].record()
+            eng.wg_shadow_check_ret(s_hdr, s_val, st.mode, s_out)
+            evs[2].record()
+        torch.cuda.synchronize()
+        csh = eng.wg_shadow_read_counters()
+        assert csh["viol_lanes"] == 0 and csh["push_lanes"] == csh["check_lanes"]
+        lanes = csh["push_lanes"] // 4
+        push_ms, chk_ms = evs[0].elapsed_time(evs[1]), evs[1].elapsed_time(evs[2])
+        # bytes: header 16 + value row 256 + verdict 8 + per active lane: depth counter 4 r + 4 w, entry 24 (w or r)
+        byts = ns * 280 + lanes * 32
+        shadow = {"warps_per_call": ns, "max_depth": depth, "lanes_per_call": int(lanes),
+                  "push_ms": push_ms, "check_ret_ms": chk_ms, "launches_per_call": 3,
+                  "push_lanes_per_sec": lanes / (push_ms * 1e-3), "check_lanes_per_sec": lanes / (chk_ms * 1e-3),
+                  "push_alu_frac": OPS_PER_MAC_SIGN * lanes / (push_ms * 1e-3) / alu_peak,
+                  "check_alu_frac": OPS_PER_MAC_VERIFY * lanes / (chk_ms * 1e-3) / alu_peak,
+                  "push_gbs": byts / (push_ms * 1e-3) / 1e9, "check_gbs": byts / (chk_ms * 1e-3) / 1e9}
+
     # ---- read-out exchange (outside the hot loop): counters summed over ranks ----
     gr, _ = sharding.reduce_counters(g, None, 0, device=dev)
     if rank == 0:
@@ -406,6 +442,7 @@ def run_ours(a) -> None:
                              % ((verify_bytes + B_RET_SIGN * ret_ev) / 1e9),
                        "parallelism": "1 GPU" if world == 1 else f"{world} ranks x own stream, counters all-reduced at read-out"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+            **({"shadow": shadow} if shadow else {}),
             "counters": {k: gr[k] for k in ("events_total", "ret_checks", "fwd_checks", "ret_viol", "fwd_viol",
                                            "blocked_lanes", "first_violation_key")},
         }))

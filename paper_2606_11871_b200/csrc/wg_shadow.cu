@@ -137,7 +137,15 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
                   // the token is verified over the ENTRY's own fields under the event's epoch
                   const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
                   uint32_t tl, th;
-                  mac_full(p, m.x, static_cast<uint32_t>(ex), static_cast<uint32_t>(ex >> 32), bl | lane, bh, tl, th);
+                  if (m.x == site) {  // the ordinary case: the site's cached mid-state saves the first word's rounds
+                    const uint4 b = __ldg(reinterpret_cast<const uint4*>(p.recs + site) + 1);
+                    const uint4 cc = __ldg(reinterpret_cast<const uint4*>(p.recs + site) + 2);
+                    const Sip32 s{b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w};
+                    sip_tail_val_lane(s, static_cast<uint32_t>(ex), static_cast<uint32_t>(ex >> 32), lane, bl, bh, 0u,
+                                      0u, tl, th);
+                  } else {
+                    mac_full(p, m.x, static_cast<uint32_t>(ex), static_cast<uint32_t>(ex >> 32), bl | lane, bh, tl, th);
+                  }
                   if (((static_cast<uint64_t>(th) << 32) | tl) != tk)
                     cause = SH_TOKEN_MISMATCH;
                   else if (ex != v || m.x != site)
