@@ -18,8 +18,8 @@
 //       warp-uniform forward targets (each unique target is searched once per warp), verdict / counter epilogue;
 //   "lane-parallel" (lane l <-> lane l of one event): the per-lane tail of the MAC (8 of the 12 SipRounds for
 //       a warp-uniform continuation, 10 otherwise) and the compare; per-lane searches of lane-divergent targets.
-// Event rows reach shared memory by TMA bulk copies (cp.async.bulk, one 256-byte row per issuing lane, only the
-// rows the tile needs) that complete on the warp's own mbarrier; 20 warps per SM keep the ALU pipe fed while
+// Event rows reach shared memory by TMA bulk copies (cp.async.bulk, one copy per run of consecutive needed rows,
+// only the rows the tile needs) that complete on the warp's own mbarrier; 20 warps per SM keep the ALU pipe fed while
 // other warps wait for their rows.  When the policy's whole target table is small (<= kMaxStageTgts entries)
 // every CTA stages it in shared memory once with one more bulk copy.
 // Counters: warp-uniform registers + shared-memory atomics, flushed once per CTA; per-site counters are
