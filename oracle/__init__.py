@@ -94,6 +94,8 @@ def lib():
         L.wgo_read_first_violation.argtypes = [vp, vp]
         L.wgo_read_telemetry.restype = None
         L.wgo_read_telemetry.argtypes = [vp, vp]
+        L.wgo_policy_poke.restype = C.c_int
+        L.wgo_policy_poke.argtypes = [vp, C.c_int, u64, u64]
         L.wgo_shadow_configure.restype = C.c_int
         L.wgo_shadow_configure.argtypes = [vp, u32, u32]
         L.wgo_shadow_push.restype = None
@@ -225,8 +227,12 @@ class Oracle:
         ok = lib().wgo_read_first_violation(self._h, _ptr(out))
         return out[0] if ok else None
 
+    def policy_poke(self, what: int, index: int, xor_value: int):
+        if lib().wgo_policy_poke(self._h, int(what), int(index), int(xor_value)) != 0:
+            raise ValueError("policy_poke: out of range")
+
     def read_telemetry(self) -> dict:
-        t = np.zeros(6, dtype=np.uint64)
+        t = np.zeros(7, dtype=np.uint64)
         lib().wgo_read_telemetry(self._h, _ptr(t))
         return {k: int(v) for k, v in zip(TELEMETRY_FIELDS, t)}
 
@@ -263,12 +269,12 @@ class Oracle:
         return int(lib().wgo_shadow_depth(self._h, int(warp_slot), int(lane)))
 
 
-PROFILE_SKIP_FORWARD, PROFILE_SKIP_BACKWARD, PROFILE_LOW_TELEMETRY = 1, 2, 4
+PROFILE_SKIP_FORWARD, PROFILE_SKIP_BACKWARD, PROFILE_LOW_TELEMETRY, PROFILE_METADATA_INTEGRITY = 1, 2, 4, 8
 VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
                             ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
                             ("stored", "<u8")])
 TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
-                    "ring_recorded", "ring_dropped")
+                    "ring_recorded", "ring_dropped", "fwd_meta_fail_events")
 SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
                  "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
                  "non_return_events", "slot_overflow_events", "slot_conflict_events", "viol_lanes", "viol_events",

@@ -67,13 +67,15 @@ struct wgo_engine {
   uint64_t k0 = 0, k1 = 0;
   uint64_t seq = 0;  // running event index over check calls (R12)
   int use_binary_search = 0;
+  bool poked = false;  // wgo_policy_poke touched the target array: sets may be unsorted
   wgo_counters g;
   std::vector<wgo_site_counters> site;
   // profiles and telemetry (R26-R29)
   uint32_t profile = 0;
   uint64_t ring_capacity = 0;
   std::vector<wgo_violation_rec> ring;
-  wgo_telemetry_counters t = {0, 0, 0, 0, 0, 0};
+  wgo_telemetry_counters t = {0, 0, 0, 0, 0, 0, 0};
+  std::vector<uint64_t> fwd_token;  // per site: token of the forward record at load time (R37)
   bool have_first = false;
   wgo_violation_rec first = {};
   // stateful shadow stack (R30-R36): entry (slot, lane, d) lives at ((slot * 32 + lane) * max_depth + d)
@@ -88,6 +90,9 @@ struct wgo_engine {
 };
 
 extern "C" {
+
+static uint64_t forward_record_token(const wgo_engine* e, uint32_t s);  // defined beside the membership tests
+
 
 // SipHash-c-d with c = 2 compression rounds and d = 4 finalisation rounds,
 // 64-bit output.  Initialisation constants are the ASCII of
@@ -173,7 +178,7 @@ void wgo_reset_counters(wgo_engine* e) {
   std::fill(e->site.begin(), e->site.end(), wgo_site_counters{0, 0, 0, 0});
   e->seq = 0;
   e->ring.clear();  // profile and ring capacity are configuration and stay
-  e->t = wgo_telemetry_counters{0, 0, 0, 0, 0, 0};
+  e->t = wgo_telemetry_counters{0, 0, 0, 0, 0, 0, 0};
   e->have_first = false;
 }
 
@@ -189,6 +194,9 @@ wgo_engine* wgo_create(uint32_t n_sites, const uint8_t* kind, const uint32_t* tg
   e->k0 = k0;
   e->k1 = k1;
   e->site.resize(n_sites);
+  e->fwd_token.assign(n_sites, 0);
+  for (uint32_t s = 0; s < n_sites; ++s)
+    if (kind[s] == WGO_PROTECTED_FORWARD) e->fwd_token[s] = forward_record_token(e, s);
   e->g.policy_digest = policy_digest;
   wgo_reset_counters(e);
   return e;
@@ -220,6 +228,20 @@ void wgo_sign(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, uint
     else
       e->g.sign_skipped_events += 1;
   }
+}
+
+// token of a forward record: SipHash-2-4 over LE64(site_id) || LE64(target_count) || LE64(targets...) as the
+// record stands in memory NOW
+static uint64_t forward_record_token(const wgo_engine* e, uint32_t s) {
+  const uint32_t a = e->tgt_off[s], b = e->tgt_off[s + 1];
+  std::vector<uint8_t> msg;
+  auto put = [&msg](uint64_t w) {
+    for (int i = 0; i < 8; ++i) msg.push_back(static_cast<uint8_t>(w >> (8 * i)));
+  };
+  put(s);
+  put(b - a);
+  for (uint32_t i = a; i < b; ++i) put(e->tgts[i]);
+  return wgo_siphash24(e->k0, e->k1, msg.data(), msg.size());
 }
 
 static bool member_linear(const wgo_engine* e, uint32_t s, uint64_t target) {
@@ -285,10 +307,17 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
         viol = a;
         e->g.events_misrouted += 1;
       } else if (k == WGO_PROTECTED_FORWARD) {
+        bool record_ok = true;
+        if (e->profile & WGO_PROFILE_METADATA_INTEGRITY) {  // authenticate the record before use
+          record_ok = forward_record_token(e, s) == e->fwd_token[s];
+          if (!record_ok) e->t.fwd_meta_fail_events += 1;
+        }
         for (uint32_t lane = 0; lane < 32; ++lane) {
           if (!((a >> lane) & 1u)) continue;
           const uint64_t target = val[ev * 32 + lane];
-          const bool ok = e->use_binary_search ? member_bsearch(e, s, target) : member_linear(e, s, target);
+          // an unauthenticated record authorises nothing; a poked set may be unsorted, so scan it
+          const bool ok = record_ok && ((e->use_binary_search && !e->poked) ? member_bsearch(e, s, target)
+                                                                            : member_linear(e, s, target));
           if (!ok) viol |= (1u << lane);
         }
         e->g.fwd_checks += 1;
@@ -343,6 +372,19 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
 }
 
 void wgo_set_profile(wgo_engine* e, uint32_t flags) { e->profile = flags; }
+
+int wgo_policy_poke(wgo_engine* e, int what, uint64_t index, uint64_t xor_value) {
+  if (what == 0 && index < e->tgts.size()) {
+    e->tgts[index] ^= xor_value;
+    e->poked = true;
+    return 0;
+  }
+  if (what == 1 && index < e->n_sites) {
+    e->fwd_token[index] ^= xor_value;
+    return 0;
+  }
+  return -1;
+}
 
 void wgo_set_ring_capacity(wgo_engine* e, uint64_t capacity) {
   e->ring_capacity = capacity;

@@ -140,7 +140,17 @@ void wgo_read_counters(const wgo_engine* e, wgo_counters* global,
  * Violation record: one per event with viol != 0 — "counters, telemetry buffers, and first-violation records
  * are diagnostic": lane = lowest violating lane, observed = val[event][lane], stored =
  * tag[event][lane] when the event was judged as a return check, else 0; kind = 7 for an unknown site. */
-enum { WGO_PROFILE_SKIP_FORWARD = 1, WGO_PROFILE_SKIP_BACKWARD = 2, WGO_PROFILE_LOW_TELEMETRY = 4 };
+/*   WGO_PROFILE_METADATA_INTEGRITY  ("authenticates the record when metadata
+ *                              integrity is enabled ... The forward metadata token is a MAC over site_id,
+ *                              target_count, and allowed_targets"; 258): before the membership test of a non-empty
+ *                              event at a protected-forward site, the site's record is re-authenticated:
+ *                                  SipHash-2-4_key( LE64(site_id) || LE64(target_count) || LE64(t_0) || ... )
+ *                              over the record AS IT IS NOW in the (writable) metadata memory must equal the token
+ *                              computed when the policy was loaded; else every active lane violates (a forward
+ *                              check with popc(active) violating lanes) and fwd_meta_fail_events counts it.
+ *                              wgo_policy_poke is the attacker's write into that memory. */
+enum { WGO_PROFILE_SKIP_FORWARD = 1, WGO_PROFILE_SKIP_BACKWARD = 2, WGO_PROFILE_LOW_TELEMETRY = 4,
+       WGO_PROFILE_METADATA_INTEGRITY = 8 };
 typedef struct {
   uint64_t seq;
   uint32_t site_id, kind, viol_mask, active_mask, lane, mode;
@@ -149,7 +159,11 @@ typedef struct {
 typedef struct {
   uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
   uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 (ring enabled) */
+  uint64_t fwd_meta_fail_events;        /* forward records that failed their authentication */
 } wgo_telemetry_counters;
+/* what = 0: allowed_targets[index] ^= x (index into the CSR array); what = 1: the stored token of site `index` ^= x.
+ * Returns 0, or -1 when out of range.  The set may become unsorted: membership is the linear scan then. */
+int wgo_policy_poke(wgo_engine* e, int what, uint64_t index, uint64_t xor_value);
 void wgo_set_profile(wgo_engine* e, uint32_t flags);
 /* capacity 0 (default) disables the ring; the oracle keeps the FIRST `capacity` records in event order
  * (any subset of that size is a valid ring content once it overflows). */
