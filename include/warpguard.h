@@ -164,7 +164,14 @@ typedef enum {
   WG_PROFILE_FULL = 0,
   WG_PROFILE_SKIP_FORWARD = 1,
   WG_PROFILE_SKIP_BACKWARD = 2,
-  WG_PROFILE_LOW_TELEMETRY = 4
+  WG_PROFILE_LOW_TELEMETRY = 4,
+  /* SURVEY.md §8(f-2), "authenticates the record when metadata integrity is enabled ... The forward
+   * metadata token is a MAC over site_id, target_count, and allowed_targets", 258; R37-R38: before the
+   * membership test of a non-empty event at a protected-forward site the site's record is re-authenticated —
+   * SipHash-2-4_key(LE64(site_id) || LE64(target_count) || LE64(t_0) || ...) over the record as it is NOW in the
+   * engine's metadata memory must equal the token computed at wg_load_policy; else every active lane violates (a
+   * forward check whose lanes all violate) and fwd_meta_fail_events counts the event. */
+  WG_PROFILE_METADATA_INTEGRITY = 8
 } wg_profile_flags;
 
 /* One record per event with viol_mask != 0: lane = lowest violating lane, observed = d_val[event][lane],
@@ -179,7 +186,12 @@ typedef struct {
 typedef struct {
   uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
   uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 since the ring was enabled */
+  uint64_t fwd_meta_fail_events;        /* forward records that failed their authentication (metadata integrity) */
 } wg_telemetry_counters;
+/* The attacker's write into the policy metadata, for tests (the paper treats forward records as ordinary writable
+ * GPU memory): what = 0: allowed_targets[index] ^= x (index into the CSR array); what = 1: the
+ * stored token of site `index` ^= x.  Synchronises cuda_stream. */
+wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_value, void* cuda_stream);
 
 /* WG_ERR_INVALID_ARG for unknown flag bits.  Applies to the calls made after it returns. */
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags);

@@ -28,7 +28,7 @@ EXPORTS = [
     "wg_probe_int_pipe", "wg_launch_count",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
-    "wg_shadow_depth",
+    "wg_shadow_depth", "wg_policy_poke",
 ]
 SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
                  "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
@@ -36,11 +36,12 @@ SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "em
                  "blocked_lanes")
 
 WG_PROFILE_FULL, WG_PROFILE_SKIP_FORWARD, WG_PROFILE_SKIP_BACKWARD, WG_PROFILE_LOW_TELEMETRY = 0, 1, 2, 4
+WG_PROFILE_METADATA_INTEGRITY = 8
 VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
                             ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
                             ("stored", "<u8")])  # wg_violation_rec, 48 bytes
 TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
-                    "ring_recorded", "ring_dropped")
+                    "ring_recorded", "ring_dropped", "fwd_meta_fail_events")
 
 COUNTER_FIELDS = (
     ["events_total", "events_empty", "events_unknown_site", "events_misrouted"]
@@ -97,6 +98,7 @@ def lib() -> C.CDLL:
         L.wg_shadow_poke.argtypes = [vp, C.c_uint32, C.c_uint32, C.c_uint32, i, u64, vp]
         L.wg_shadow_depth.argtypes = [vp, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32), vp]
         L.wg_set_profile.argtypes = [vp, C.c_uint32]
+        L.wg_policy_poke.argtypes = [vp, i, u64, u64, vp]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
         L.wg_launch_count.restype = u64
@@ -267,12 +269,15 @@ class Engine:
     def wg_set_profile(self, flags: int) -> None:
         _chk(lib().wg_set_profile(self._h, int(flags)), "wg_set_profile")
 
+    def wg_policy_poke(self, what: int, index: int, xor_value: int, stream=None) -> None:
+        _chk(lib().wg_policy_poke(self._h, int(what), int(index), int(xor_value), _stream_ptr(stream)), "wg_policy_poke")
+
     def wg_set_ring_capacity(self, capacity: int, stream=None) -> None:
         _chk(lib().wg_set_ring_capacity(self._h, int(capacity), _stream_ptr(stream)), "wg_set_ring_capacity")
 
     def wg_read_telemetry(self, ring_cap: int = 0, stream=None):
         """(telemetry counters dict, first-violation record or None, ring records as a structured array)."""
-        t = np.zeros(6, dtype=np.uint64)
+        t = np.zeros(7, dtype=np.uint64)
         first = np.zeros(1, dtype=VIOLATION_DTYPE)
         have = C.c_int(0)
         ring = np.zeros(max(int(ring_cap), 1), dtype=VIOLATION_DTYPE)

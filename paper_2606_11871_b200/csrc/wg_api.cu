@@ -381,7 +381,7 @@ wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc
   }
   // per-site SipHash mid-states, computed on the device from the key-derived initial state
   {
-    cudaError_t e3 = wg::launch_build_recs(e->d_recs, e->d_rows, n, e->v_init[0], e->v_init[1], e->v_init[2],
+    cudaError_t e3 = wg::launch_build_recs(e->d_recs, e->d_rows, e->d_tgts, n, e->v_init[0], e->v_init[1], e->v_init[2],
                                            e->v_init[3], nullptr);
     if (e3 != cudaSuccess) {
       free_tables(e);
@@ -584,8 +584,23 @@ wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uin
 
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;
-  if (flags & ~7u) return WG_ERR_INVALID_ARG;
+  if (flags & ~15u) return WG_ERR_INVALID_ARG;
   eng->profile = flags;  // takes effect with the next check call (kernel parameter)
+  return WG_OK;
+}
+
+wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_value, void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (!((what == 0 && index < eng->n_tgts) || (what == 1 && index < eng->n_sites))) return WG_ERR_INVALID_ARG;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+  void* addr = what == 0 ? static_cast<void*>(eng->d_tgts + index)
+                         : static_cast<void*>(reinterpret_cast<char*>(eng->d_recs + index) + 48);
+  uint64_t v = 0;
+  WG_CUDA(eng, cudaMemcpy(&v, addr, 8, cudaMemcpyDeviceToHost));
+  v ^= xor_value;
+  WG_CUDA(eng, cudaMemcpy(addr, &v, 8, cudaMemcpyHostToDevice));
   return WG_OK;
 }
 
@@ -616,8 +631,9 @@ wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, w
   DeviceGuard g(eng->device);
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
-  unsigned long long w[5];
+  unsigned long long w[7];  // words 26 .. 32
   WG_CUDA(eng, cudaMemcpy(w, eng->d_glob + wg::C_SKIP_RET_EVENTS, sizeof w, cudaMemcpyDeviceToHost));
+  h_counters->fwd_meta_fail_events = w[wg::C_META_FAIL - wg::C_SKIP_RET_EVENTS];
   const uint64_t total = w[4];
   const uint64_t recorded = total < eng->ring_cap ? total : eng->ring_cap;
   h_counters->skipped_ret_events = w[0];

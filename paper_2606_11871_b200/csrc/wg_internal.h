@@ -20,7 +20,8 @@ struct __align__(16) SiteRow {
 //   words 4-11  protected-return sites: SipHash state after absorbing LE64(site_id), with quarter-round A of the
 //               next round already applied ("pre-A" mid-state, wg_sip32.cuh), as v0l v0h v1l v1h v2l v2h v3l v3h.
 //               Key-derived, so it lives only in engine-owned memory.  Zero for other kinds.
-//   words 12-15 reserved (0)
+//   words 12-13 protected-forward sites: token of the forward record at load time (SipHash over site_id,
+//               target_count, allowed_targets, R37); words 14-15 reserved (0)
 struct __align__(16) SiteRec {
   uint32_t kind, off, cnt, pad0;
   uint32_t st[8];
@@ -58,7 +59,8 @@ enum CounterWord {
   C_SKIP_FWD_LANES = 29,
   C_RING_TOTAL = 30,  // violation records offered to the ring (recorded = min(total, capacity))
   C_TICKET = 31,      // CTAs that finished the current launch: the last one writes the first-violation record
-  C_WORDS = 32
+  C_META_FAIL = 32,   // forward records that failed their authentication (metadata-integrity profile, R37)
+  C_WORDS = 40
 };
 
 // Violation record, layout of wg_violation_rec (48 bytes)
@@ -73,7 +75,8 @@ struct FirstRec {
   ViolRec rec;
   unsigned long long key;  // UINT64_MAX: none
 };
-enum : uint32_t { PROFILE_SKIP_FORWARD = 1, PROFILE_SKIP_BACKWARD = 2, PROFILE_LOW_TELEMETRY = 4 };
+enum : uint32_t { PROFILE_SKIP_FORWARD = 1, PROFILE_SKIP_BACKWARD = 2, PROFILE_LOW_TELEMETRY = 4,
+                  PROFILE_METADATA_INTEGRITY = 8 };
 
 // Per-site counters: 4 x u64 per site, layout of wg_site_counters.
 enum SiteWord { S_EVENTS = 0, S_LANES_CHECKED = 1, S_LANES_VIOLATION = 2, S_LANES_BLOCKED = 3 };
@@ -123,8 +126,8 @@ cudaError_t launch_check_v1(const Params& p, int sm_count, cudaStream_t st);
 // v2 (wg_kernels_v2.cu): tiled, cp.async-staged, mid-state-cached kernels
 cudaError_t launch_sign_v2(const Params& p, int sm_count, cudaStream_t st);
 cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st);
-cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sites, uint64_t v0, uint64_t v1,
-                              uint64_t v2, uint64_t v3, cudaStream_t st);
+cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                              uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st);
 cudaError_t init_v2();  // one-time function attributes (dynamic shared memory opt-in)
 cudaError_t launch_fill_u64(unsigned long long* p, uint64_t n, unsigned long long v, cudaStream_t st);
 cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double* ms);

@@ -180,10 +180,30 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
     return __ldg(set + lo) == v;
   }
 }
+// token of a forward record ("a MAC over site_id, target_count, and allowed_targets"; R37):
+// SipHash-2-4 over LE64(site_id) || LE64(cnt) || LE64(t_0) ... LE64(t_cnt-1), read through `load(i)`
+template <typename LoadTarget>
+__device__ __forceinline__ uint2 record_token(uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, uint32_t site,
+                                              uint32_t cnt, LoadTarget load) {
+  Sip32 s{static_cast<uint32_t>(v0), static_cast<uint32_t>(v0 >> 32), static_cast<uint32_t>(v1),
+          static_cast<uint32_t>(v1 >> 32), static_cast<uint32_t>(v2), static_cast<uint32_t>(v2 >> 32),
+          static_cast<uint32_t>(v3), static_cast<uint32_t>(v3 >> 32)};
+  sip_absorb(s, site, 0u);
+  sip_absorb(s, cnt, 0u);
+  for (uint32_t i = 0; i < cnt; ++i) {
+    const uint2 t = load(i);
+    sip_absorb(s, t.x, t.y);
+  }
+  uint2 out;
+  sip_finish_len(s, ((8u * (cnt + 2u)) & 0xffu) << 24, 0u, 0u, out.x, out.y);
+  return out;
+}
+
 // what lane i knows about event i of the tile
 struct TileEv {
   uint32_t site, active, cls, kind;
   uint32_t off, cnt;  // protected-forward: the site's set
+  uint32_t tokl, tokh;  // protected-forward: the record's token at load time (metadata-integrity profile)
   Sip32 st;           // protected-return: the site's pre-A mid-state
 };
 
@@ -205,6 +225,8 @@ __device__ __forceinline__ TileEv classify(const Params& p, uint32_t raw_s, uint
   ev.kind = 7;
   ev.off = 0;
   ev.cnt = 0;
+  ev.tokl = 0;
+  ev.tokh = 0;
   ev.st = Sip32{0, 0, 0, 0, 0, 0, 0, 0};
   const uint64_t e = tile * kT + lane;
   const bool valid = lane < kT && e < p.n;
@@ -220,6 +242,11 @@ __device__ __forceinline__ TileEv classify(const Params& p, uint32_t raw_s, uint
       ev.kind = a.x;
       ev.off = a.y;
       ev.cnt = a.z;
+      if (TEL && a.x == K_FWD && (p.profile & PROFILE_METADATA_INTEGRITY)) {
+        const uint4 d = ldg_v4(reinterpret_cast<const char*>(r) + 48);
+        ev.tokl = d.x;
+        ev.tokh = d.y;
+      }
       if (a.x == K_RET && MODE != MODE_FORWARD) {
         const uint4 b = ldg_v4(reinterpret_cast<const char*>(r) + 16);
         const uint4 c = ldg_v4(reinterpret_cast<const char*>(r) + 32);
@@ -441,6 +468,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
 
     // ---- event-parallel: per-event part of the MAC; batched search of warp-uniform forward targets ----
     uint32_t viol = 0;
+    uint32_t m_bad_rec = 0;  // events whose forward record failed its authentication
     {
       const bool is_uni = (uni >> lane) & 1u;
       uint32_t ul = 0, uh = 0;
@@ -463,7 +491,30 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
         sts_v4(st_s + lane * 32 + 16, s.v2l, s.v2h, s.v3l, s.v3h);
       }
       if constexpr (MODE != MODE_SIGN) {
-        if (ev.cls == CLS_FWD && is_uni) viol = member<STAGED>(p, tg_s, ev.off, ev.cnt, ul, uh) ? 0u : ev.active;
+        if constexpr (TEL) {
+          // metadata integrity: the forward record is re-authenticated before it is used, once per
+          // event; a record that fails authorises nothing: every active lane violates
+          if (p.profile & PROFILE_METADATA_INTEGRITY) {
+            bool bad_rec = false;
+            if (ev.cls == CLS_FWD) {
+              uint2 tk;
+              if constexpr (STAGED) {
+                const uint32_t base = tg_s + ev.off * 8;
+                tk = record_token(p.v0, p.v1, p.v2, p.v3, ev.site, ev.cnt, [&](uint32_t i) { return lds_v2(base + i * 8); });
+              } else {
+                const uint2* set = reinterpret_cast<const uint2*>(p.tgts + ev.off);
+                tk = record_token(p.v0, p.v1, p.v2, p.v3, ev.site, ev.cnt, [&](uint32_t i) { return __ldcg(set + i); });
+              }
+              bad_rec = tk.x != ev.tokl || tk.y != ev.tokh;
+            }
+            m_bad_rec = __ballot_sync(kFull, bad_rec);
+            if (m_bad_rec && lane == 0)
+              atomicAdd(p.glob + C_META_FAIL, static_cast<unsigned long long>(__popc(m_bad_rec)));
+            if (bad_rec) viol = ev.active;
+          }
+        }
+        if (ev.cls == CLS_FWD && is_uni && !((m_bad_rec >> lane) & 1u))
+          viol = member<STAGED>(p, tg_s, ev.off, ev.cnt, ul, uh) ? 0u : ev.active;
         if (ev.cls == CLS_FAIL) viol = ev.active;  // fail closed (R13, R14)
         if (lane < kT) sts_u32(viol_s + lane * 4, viol);  // the lane-parallel loops below overwrite their events
       }
@@ -508,7 +559,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     }
     // ---- lane-parallel: protected-forward events with lane-divergent targets ----
     if constexpr (MODE != MODE_SIGN) {
-      for (uint32_t m = m_fwd & ~uni; m; m &= m - 1) {
+      for (uint32_t m = m_fwd & ~uni & ~m_bad_rec; m; m &= m - 1) {
         const uint32_t e = __ffs(m) - 1;
         const uint32_t a = lds_u32(dec_s + e * 16 + 4);
         const uint32_t off = __shfl_sync(kFull, ev.off, e), cnt = __shfl_sync(kFull, ev.cnt, e);
@@ -661,8 +712,8 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
 }
 
 // SiteRec table from the v1 rows: the pre-A mid-state of every protected-return site (runs once per policy load)
-__global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sites, uint64_t v0, uint64_t v1,
-                              uint64_t v2, uint64_t v3) {
+__global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                              uint64_t v1, uint64_t v2, uint64_t v3) {
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n_sites) return;
   const SiteRow r = rows[s];
@@ -683,6 +734,12 @@ __global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sit
     sip_qA(st);             // quarter A of the continuation word's first round
     o.st[0] = st.v0l; o.st[1] = st.v0h; o.st[2] = st.v1l; o.st[3] = st.v1h;
     o.st[4] = st.v2l; o.st[5] = st.v2h; o.st[6] = st.v3l; o.st[7] = st.v3h;
+  }
+  if (r.kind == K_FWD) {  // token of the forward record as loaded (trusted load time)
+    const uint2* set = reinterpret_cast<const uint2*>(tgts + r.off);
+    const uint2 tk = record_token(v0, v1, v2, v3, s, r.cnt, [&](uint32_t i) { return set[i]; });
+    o.pad1[0] = tk.x;
+    o.pad1[1] = tk.y;
   }
   recs[s] = o;
 }
@@ -755,10 +812,10 @@ cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st) {
   return p.tag ? launch_tile<MODE_VERIFY>(p, sm_count, st) : launch_tile<MODE_FORWARD>(p, sm_count, st);
 }
 
-cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, uint32_t n_sites, uint64_t v0, uint64_t v1,
-                              uint64_t v2, uint64_t v3, cudaStream_t st) {
+cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                              uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st) {
   if (n_sites == 0) return cudaSuccess;
-  wg_build_recs<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, rows, n_sites, v0, v1, v2, v3);
+  wg_build_recs<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, rows, tgts, n_sites, v0, v1, v2, v3);
   count_launch();
   return cudaGetLastError();
 }

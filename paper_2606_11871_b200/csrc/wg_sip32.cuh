@@ -111,11 +111,18 @@ constexpr uint32_t kLenHi = 0x18000000u;
 
 // absorb the length word, then d = 4 finalisation rounds; the 64-bit output is returned XORed with
 // (xl, xh) — pass the stored tag to get 0 exactly when the token matches, or 0 to get the token itself.
+// (len_hi: the last message word of a message of whole 8-byte words is its byte length mod 256 in the top byte)
+__device__ __forceinline__ void sip_finish_len(Sip32& s, uint32_t len_hi, uint32_t xl, uint32_t xh, uint32_t& outl,
+                                               uint32_t& outh);
 __device__ __forceinline__ void sip_finish(Sip32& s, uint32_t xl, uint32_t xh, uint32_t& outl, uint32_t& outh) {
-  s.v3h ^= kLenHi;
+  sip_finish_len(s, kLenHi, xl, xh, outl, outh);
+}
+__device__ __forceinline__ void sip_finish_len(Sip32& s, uint32_t len_hi, uint32_t xl, uint32_t xh, uint32_t& outl,
+                                               uint32_t& outh) {
+  s.v3h ^= len_hi;
   sip_round(s);
   sip_round(s);
-  s.v0h ^= kLenHi;
+  s.v0h ^= len_hi;
   s.v2l ^= 0xffu;
   sip_round(s);
   sip_round(s);

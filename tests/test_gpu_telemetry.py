@@ -129,6 +129,61 @@ def test_profiles_match_the_oracle(flags, config):
 def test_bad_profile_flags_are_rejected():
     st, orc, eng, hdr, val, tag, d = prepared(1, 1000)
     with pytest.raises(B.WgError) as e:
-        eng.wg_set_profile(8)
+        eng.wg_set_profile(16)
     assert e.value.status == B.WG_ERR_INVALID_ARG
+    eng.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# metadata-integrity profile (R37-R38)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,n", [(4, 150_003), (3, 90_001), (5, 30_011)])
+def test_metadata_integrity_matches_the_oracle_with_and_without_corruption(config, n):
+    rng = np.random.default_rng(config)
+    if config == 5:
+        pol = S.make_policy(5, "cpu", n_sites=4_000, max_set=300)   # > 2,048 targets: the global-memory search path
+        st = S.make_stream(5, "cpu", n_events=n, policy=pol, batch_index=0)
+    else:
+        st = S.make_stream(config, "cpu", n_events=n)
+        pol = st.policy
+    orc = oracle_for(pol)
+    hdr = st.hdr.numpy().view(np.uint64)
+    tag = orc.sign(hdr, st.val.numpy().view(np.uint64))
+    tag_t = torch.from_numpy(tag.view(np.int64).copy())
+    st.apply_return_tamper(tag_t)
+    orc.reset_counters()
+    val, tagn = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+    eng = B.Engine(0).load(pol)
+    d = (st.hdr.to(dev()), st.val.to(dev()), tag_t.to(dev()))
+    flags = B.WG_PROFILE_METADATA_INTEGRITY
+    orc.set_profile(flags)
+    eng.wg_set_profile(flags)
+    # intact records: same verdicts as the ordinary profile
+    o = orc.verify(hdr, val, tagn, ENF)
+    g = eng.wg_verify_continuations(*d, ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    assert eng.wg_read_telemetry()[0]["fwd_meta_fail_events"] == 0
+    # corrupt a few forward records (targets and tokens), the same way on both sides
+    fwd_sites = np.nonzero(pol.kind == 1)[0]
+    site_of_event = (hdr[:, 0] & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    hot = [int(s) for s in fwd_sites if (site_of_event == s).any()][:6]
+    for k, s in enumerate(hot):
+        if k % 2 == 0:
+            idx = int(pol.tgt_off[s]) + int(rng.integers(0, pol.tgt_off[s + 1] - pol.tgt_off[s]))
+            x = 1 << int(rng.integers(4, 28))
+            orc.policy_poke(0, idx, x)
+            eng.wg_policy_poke(0, idx, x)
+        else:
+            x = int(rng.integers(1, 1 << 63))
+            orc.policy_poke(1, s, x)
+            eng.wg_policy_poke(1, s, x)
+    o = orc.verify(hdr, val, tagn, DET)
+    g = eng.wg_verify_continuations(*d, DET).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    o = orc.check_forward(hdr, val, ENF)
+    g = eng.wg_check_forward(d[0], d[1], ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    same_counters(eng, orc)
+    t = eng.wg_read_telemetry()[0]
+    assert t == orc.read_telemetry() and t["fwd_meta_fail_events"] > 0
     eng.close()
