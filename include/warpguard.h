@@ -243,6 +243,18 @@ wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint
                          uint64_t xor_value, void* cuda_stream);
 wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t* h_depth, void* cuda_stream);
 
+/* ---- inline device form (include/warpguard_device.cuh) ----
+ * What a kernel needs to run the checks at its own sites: pointers into the engine's device tables.  Pass the view
+ * to the kernel BY VALUE; it stays valid until the next wg_load_policy or wg_destroy.  site_recs: 64 bytes per site
+ * {kind, set offset, set size, 0; key-derived SipHash mid-state (8 words); forward-record token; 0 0}. */
+typedef struct {
+  const void* site_recs;
+  const uint64_t* targets;
+  uint32_t n_sites;
+  uint32_t reserved;
+} wg_device_view;
+wg_status wg_get_device_view(wg_engine* eng, wg_device_view* h_view);
+
 /* ---- HOST-buffer entry points (end-to-end path) ----
  * Same semantics as the calls above but every array is in HOST memory (pinned memory gives full PCIe speed,
  * pageable works).  The engine streams the events through its own double-buffered device staging in chunks,

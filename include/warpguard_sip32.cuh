@@ -1,4 +1,5 @@
-// wg_sip32.cuh — SipHash-2-4 on 32-bit register halves, for the v2 (tiled) kernels.
+// warpguard_sip32.cuh — SipHash-2-4 on 32-bit register halves: the device-side MAC of the engine kernels
+// (paper_2606_11871_b200/csrc) and of the inline device API (warpguard_device.cuh).
 //
 // token = SipHash-2-4_key( LE64(site_id) || LE64(continuation) || LE64(context_id) ), 64-bit output
 // (R1-R4; formula lost at PAPER.md:164-166 / 244-246, "keyed token" over the return state

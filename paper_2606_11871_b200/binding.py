@@ -28,8 +28,13 @@ EXPORTS = [
     "wg_probe_int_pipe", "wg_launch_count",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
-    "wg_shadow_depth", "wg_policy_poke",
+    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view",
 ]
+
+
+class DeviceView(C.Structure):
+    """wg_device_view: pass it by value to a kernel that uses include/warpguard_device.cuh"""
+    _fields_ = [("site_recs", C.c_void_p), ("targets", C.c_void_p), ("n_sites", C.c_uint32), ("reserved", C.c_uint32)]
 SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
                  "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
                  "non_return_events", "slot_overflow_events", "slot_conflict_events", "viol_lanes", "viol_events",
@@ -99,6 +104,7 @@ def lib() -> C.CDLL:
         L.wg_shadow_depth.argtypes = [vp, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32), vp]
         L.wg_set_profile.argtypes = [vp, C.c_uint32]
         L.wg_policy_poke.argtypes = [vp, i, u64, u64, vp]
+        L.wg_get_device_view.argtypes = [vp, C.POINTER(DeviceView)]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
         L.wg_launch_count.restype = u64
@@ -268,6 +274,11 @@ class Engine:
     # -- profiles and telemetry (warpguard.h; R26-R29) ----------------------------------
     def wg_set_profile(self, flags: int) -> None:
         _chk(lib().wg_set_profile(self._h, int(flags)), "wg_set_profile")
+
+    def wg_get_device_view(self) -> DeviceView:
+        v = DeviceView()
+        _chk(lib().wg_get_device_view(self._h, C.byref(v)), "wg_get_device_view")
+        return v
 
     def wg_policy_poke(self, what: int, index: int, xor_value: int, stream=None) -> None:
         _chk(lib().wg_policy_poke(self._h, int(what), int(index), int(xor_value), _stream_ptr(stream)), "wg_policy_poke")

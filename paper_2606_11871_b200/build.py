@@ -32,7 +32,7 @@ def nvcc() -> str:
 
 
 def _newest_source() -> float:
-    files = list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + [ROOT / "include" / "warpguard.h"]
+    files = list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + list((ROOT / "include").glob("*"))
     return max(f.stat().st_mtime for f in files)
 
 

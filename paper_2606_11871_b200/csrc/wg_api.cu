@@ -589,6 +589,16 @@ wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   return WG_OK;
 }
 
+wg_status wg_get_device_view(wg_engine* eng, wg_device_view* h_view) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (!h_view) return WG_ERR_INVALID_ARG;
+  h_view->site_recs = eng->d_recs;
+  h_view->targets = eng->d_tgts;
+  h_view->n_sites = eng->n_sites;
+  h_view->reserved = 0;
+  return WG_OK;
+}
+
 wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_value, void* cuda_stream) {
   if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
   if (!((what == 0 && index < eng->n_tgts) || (what == 1 && index < eng->n_sites))) return WG_ERR_INVALID_ARG;

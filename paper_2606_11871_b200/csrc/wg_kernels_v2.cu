@@ -25,7 +25,7 @@
 // Counters: warp-uniform registers + shared-memory atomics, flushed once per CTA; per-site counters are
 // aggregated over equal sites of a tile (__match_any_sync) before the global reduction.
 #include "wg_internal.h"
-#include "wg_sip32.cuh"
+#include "../../include/warpguard_sip32.cuh"
 
 namespace wg {
 

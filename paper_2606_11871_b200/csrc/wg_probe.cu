@@ -4,7 +4,7 @@
 // sequence of one instruction kind; 8 independent chains per thread and 16 resident warps per SMSP keep the
 // pipes full.  `asm volatile` pins the instruction selection (checked with cuobjdump -sass).
 #include "wg_internal.h"
-#include "wg_sip32.cuh"
+#include "../../include/warpguard_sip32.cuh"
 
 namespace wg {
 namespace {

@@ -13,7 +13,7 @@
 // A call is one lock-step step of DISTINCT warps: a counting pass marks warp slots that occur twice in the call
 // and those events fail closed; a clearing pass resets the marks.
 #include "wg_internal.h"
-#include "wg_sip32.cuh"
+#include "../../include/warpguard_sip32.cuh"
 
 namespace wg {
 
