@@ -60,6 +60,7 @@ def parse_args():
     ap.add_argument("--profile", type=int, default=0,
                     help="wg_set_profile flags for the timed calls (1 backward-only, 2 forward-only, 4 low-telemetry, "
                          "8 metadata integrity); the headline run uses 0")
+    ap.add_argument("--sparse", action="store_true", help="wg_set_tuning(WG_TUNE_SPARSE_LANES) for the timed calls")
     ap.add_argument("--shadow", action="store_true",
                     help="also time the stateful shadow stack (SURVEY 8(f-1)): one lock-step push + check_ret over 1 Mi warps")
     return ap.parse_args()
@@ -228,6 +229,8 @@ def run_ours(a) -> None:
     st.apply_return_tamper(tag)                               # then the recorded corruption
     if a.profile:
         eng.wg_set_profile(a.profile)
+    if a.sparse:
+        eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
     tag_scratch = torch.empty_like(tag)
     out = torch.empty((n_events, 2), dtype=torch.int32, device=dev)
     fwd_ops = forward_search_ops(st, torch)

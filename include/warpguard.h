@@ -243,6 +243,13 @@ wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint
                          uint64_t xor_value, void* cuda_stream);
 wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t* h_depth, void* cuda_stream);
 
+/* ---- tuning (never changes a result) ----
+ * WG_TUNE_SPARSE_LANES: for streams whose active masks are far from full (BASELINE config 5: 1 to 32 active lanes)
+ * the per-lane MAC passes of sign / verify run over a compacted list of the ACTIVE (event, lane) pairs of a tile
+ * instead of one 32-lane pass per event.  It costs a little on dense masks (p = 0.9), hence a switch. */
+typedef enum { WG_TUNE_DEFAULT = 0, WG_TUNE_SPARSE_LANES = 1 } wg_tuning_flags;
+wg_status wg_set_tuning(wg_engine* eng, uint32_t flags);
+
 /* ---- inline device form (include/warpguard_device.cuh) ----
  * What a kernel needs to run the checks at its own sites: pointers into the engine's device tables.  Pass the view
  * to the kernel BY VALUE; it stays valid until the next wg_load_policy or wg_destroy.  site_recs: 64 bytes per site

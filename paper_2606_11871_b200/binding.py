@@ -28,8 +28,9 @@ EXPORTS = [
     "wg_probe_int_pipe", "wg_launch_count",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
-    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view",
+    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_set_tuning",
 ]
+WG_TUNE_DEFAULT, WG_TUNE_SPARSE_LANES = 0, 1
 
 
 class DeviceView(C.Structure):
@@ -105,6 +106,7 @@ def lib() -> C.CDLL:
         L.wg_set_profile.argtypes = [vp, C.c_uint32]
         L.wg_policy_poke.argtypes = [vp, i, u64, u64, vp]
         L.wg_get_device_view.argtypes = [vp, C.POINTER(DeviceView)]
+        L.wg_set_tuning.argtypes = [vp, C.c_uint32]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
         L.wg_launch_count.restype = u64
@@ -274,6 +276,9 @@ class Engine:
     # -- profiles and telemetry (warpguard.h; R26-R29) ----------------------------------
     def wg_set_profile(self, flags: int) -> None:
         _chk(lib().wg_set_profile(self._h, int(flags)), "wg_set_profile")
+
+    def wg_set_tuning(self, flags: int) -> None:
+        _chk(lib().wg_set_tuning(self._h, int(flags)), "wg_set_tuning")
 
     def wg_get_device_view(self) -> DeviceView:
         v = DeviceView()

@@ -19,6 +19,7 @@ struct wg_engine {
   uint64_t n_tgts = 0;
   wg::SiteRow* d_rows = nullptr;
   wg::SiteRec* d_recs = nullptr;  // v2 site records (kind, set range, pre-A SipHash mid-state), 64 B each
+  uint32_t tuning = 0;             // WG_TUNE_* flags
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
   wg::ViolRec* d_ring = nullptr;
@@ -145,6 +146,7 @@ wg::Params base_params(const wg_engine* e) {
   p.recs = e->d_recs;
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
+  p.sparse = (e->tuning & WG_TUNE_SPARSE_LANES) ? 1u : 0u;
   p.ring = e->d_ring;
   p.ring_cap = e->d_ring ? e->ring_cap : 0;
   p.first = e->d_first;
@@ -586,6 +588,13 @@ wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;
   if (flags & ~15u) return WG_ERR_INVALID_ARG;
   eng->profile = flags;  // takes effect with the next check call (kernel parameter)
+  return WG_OK;
+}
+
+wg_status wg_set_tuning(wg_engine* eng, uint32_t flags) {
+  if (!eng) return WG_ERR_NO_POLICY;
+  if (flags & ~static_cast<uint32_t>(WG_TUNE_SPARSE_LANES)) return WG_ERR_INVALID_ARG;
+  eng->tuning = flags;
   return WG_OK;
 }
 

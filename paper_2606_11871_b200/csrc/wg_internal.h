@@ -100,7 +100,7 @@ struct Params {
   uint32_t n_sites;
   uint32_t mode;             // 0 detect, 1 enforce
   uint32_t profile;          // PROFILE_* flags (R26)
-  uint32_t pad0;
+  uint32_t sparse;           // tuning: compacted-lane MAC passes (wg_set_tuning)
   ViolRec* ring;             // violation ring or nullptr
   uint64_t ring_cap;         // its capacity in records
   FirstRec* first;           // first-violation record

@@ -64,7 +64,8 @@ struct WarpLayout {
   static constexpr uint32_t kSt = kDec + kT * 16;
   static constexpr uint32_t kBar = kSt + kT * 32;
   static constexpr uint32_t kViol = kBar + 16;  // [T] u32 violation masks of the tile
-  static constexpr uint32_t kVal = kViol + kT * 4;
+  static constexpr uint32_t kList = kViol + kT * 4;  // [T * 32] u16 work items (event * 32 + lane) of the sparse path
+  static constexpr uint32_t kVal = kList + (MODE == MODE_FORWARD ? 0 : kT * 64);
   static constexpr uint32_t kTag = kVal + kT * 256;
   static constexpr uint32_t kBytes = kTag + (MODE == MODE_VERIFY ? kT * 256 : 0);
 };
@@ -109,6 +110,17 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
   uint32_t r;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(a));
   return r;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
+  uint32_t r;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(r) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ void sts_u16(uint32_t a, uint32_t x) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "r"(x) : "memory");
+}
+__device__ __forceinline__ void atoms_or(uint32_t a, uint32_t x) {
+  asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
 }
 __device__ __forceinline__ void sts_u32(uint32_t a, uint32_t x) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
@@ -284,7 +296,9 @@ __device__ __forceinline__ Sip32 lds_state(uint32_t a) {
 // wg_sign_continuations.  STAGED: the whole target table sits in shared memory.
 // ---------------------------------------------------------------------------------------------------
 // TEL: a profile flag is set or the violation ring is on (compiled out of the ordinary launch).
-template <int MODE, bool STAGED, bool TEL>
+// SPARSE: the lane-parallel MAC passes run over a compacted list of ACTIVE (event, lane) items instead of one pass
+// per event — for streams whose active masks are far from full (config 5: 1-32 lanes, half of a pass would idle).
+template <int MODE, bool STAGED, bool TEL, bool SPARSE>
 __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const Params p, const uint32_t stage_bytes,
                                                                                 const uint32_t site_bytes) {
   using L = WarpLayout<MODE>;
@@ -308,6 +322,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
   const uint32_t st_s = warp_s + L::kSt;
   const uint32_t mbar = warp_s + L::kBar;
   const uint32_t viol_s = warp_s + L::kViol;
+  const uint32_t list_s = warp_s + L::kList;
   const uint32_t val_s = warp_s + L::kVal;
   const uint32_t tag_s = warp_s + L::kTag;
   const uint32_t val_lane_s = val_s + lane * 8, tag_lane_s = tag_s + lane * 8;  // this lane's column of the rows
@@ -521,6 +536,58 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     }
     __syncwarp();
 
+    if constexpr (SPARSE && MODE != MODE_FORWARD) {
+      // ---- sparse path: work items = the ACTIVE lanes of the tile's return events, uniform events from the front
+      //      of the list, divergent ones from the back; 32 items per pass whatever event they belong to ----
+      uint32_t n_u = 0, n_d = 0;
+      for (uint32_t m = m_ret; m; m &= m - 1) {
+        const uint32_t e = __ffs(m) - 1;
+        const uint32_t a = lds_u32(dec_s + e * 16 + 4);
+        const bool is_u = (uni >> e) & 1u;
+        const uint32_t pos = __popc(a & (lanebit - 1u));
+        if (a & lanebit) {
+          sts_u16(list_s + 2u * (is_u ? n_u + pos : (kT * 32u - 1u) - (n_d + pos)), e * 32u + lane);
+        } else if (MODE == MODE_SIGN) {
+          st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), 0u, 0u);  // inactive lanes sign nothing (R10)
+        }
+        const uint32_t na_e = __popc(a);
+        if (is_u) n_u += na_e; else n_d += na_e;
+      }
+      __syncwarp();
+      for (uint32_t k0 = 0; k0 < n_u; k0 += 32) {
+        const bool on = k0 + lane < n_u;
+        const uint32_t item = lds_u16(list_s + 2u * (on ? k0 + lane : 0u));
+        const uint32_t e = item >> 5, l = item & 31u;
+        const uint4 h = lds_v4(dec_s + e * 16);
+        const Sip32 st = lds_state(st_s + e * 32);
+        uint32_t dl, dh;
+        if constexpr (MODE == MODE_SIGN) {
+          sip_tail_lane(st, l, h.z, h.w, 0u, 0u, dl, dh);
+          if (on) st_stream_v2(p.tag_out + (e0 * 32 + item), dl, dh);
+        } else {
+          const uint2 tg = lds_v2(tag_s + item * 8);
+          sip_tail_lane(st, l, h.z, h.w, tg.x, tg.y, dl, dh);
+          if (on && (dl | dh) != 0u) atoms_or(viol_s + e * 4, 1u << l);
+        }
+      }
+      for (uint32_t k0 = 0; k0 < n_d; k0 += 32) {
+        const bool on = k0 + lane < n_d;
+        const uint32_t item = lds_u16(list_s + 2u * ((kT * 32u - 1u) - (on ? k0 + lane : 0u)));
+        const uint32_t e = item >> 5, l = item & 31u;
+        const uint4 h = lds_v4(dec_s + e * 16);
+        const Sip32 st = lds_state(st_s + e * 32);
+        const uint2 v = lds_v2(val_s + item * 8);
+        uint32_t dl, dh;
+        if constexpr (MODE == MODE_SIGN) {
+          sip_tail_val_lane(st, v.x, v.y, l, h.z, h.w, 0u, 0u, dl, dh);
+          if (on) st_stream_v2(p.tag_out + (e0 * 32 + item), dl, dh);
+        } else {
+          const uint2 tg = lds_v2(tag_s + item * 8);
+          sip_tail_val_lane(st, v.x, v.y, l, h.z, h.w, tg.x, tg.y, dl, dh);
+          if (on && (dl | dh) != 0u) atoms_or(viol_s + e * 4, 1u << l);
+        }
+      }
+    } else {
     // ---- lane-parallel: protected-return events with a warp-uniform continuation (8 rounds per lane) ----
     for (uint32_t m = m_ret & uni; m; m &= m - 1) {
       const uint32_t e = __ffs(m) - 1;
@@ -557,6 +624,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
         if (lane == 0) sts_u32(mad32(e, 4u, viol_s), vb);
       }
     }
+    }  // dense path
     // ---- lane-parallel: protected-forward events with lane-divergent targets ----
     if constexpr (MODE != MODE_SIGN) {
       for (uint32_t m = m_fwd & ~uni & ~m_bad_rec; m; m &= m - 1) {
@@ -768,14 +836,21 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
   if (tel) {
     if constexpr (MODE != MODE_SIGN) {
       if (staged)
-        wg_tile_kernel<MODE, true, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+        wg_tile_kernel<MODE, true, true, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
       else
-        wg_tile_kernel<MODE, false, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+        wg_tile_kernel<MODE, false, true, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    }
+  } else if (MODE != MODE_FORWARD && p.sparse) {
+    if constexpr (MODE != MODE_FORWARD) {
+      if (staged)
+        wg_tile_kernel<MODE, true, false, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+      else
+        wg_tile_kernel<MODE, false, false, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
     }
   } else if (staged) {
-    wg_tile_kernel<MODE, true, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    wg_tile_kernel<MODE, true, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
   } else {
-    wg_tile_kernel<MODE, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    wg_tile_kernel<MODE, false, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
   }
   count_launch();
   return cudaGetLastError();
@@ -784,11 +859,16 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
 template <int MODE, bool STAGED>
 cudaError_t opt_in() {
   if constexpr (MODE != MODE_SIGN) {
-    const cudaError_t e = cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, true>,
+    const cudaError_t e = cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, true, false>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kSmemMax));
     if (e != cudaSuccess) return e;
   }
-  return cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  if constexpr (MODE != MODE_FORWARD) {
+    const cudaError_t e = cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, false, true>,
+                                               cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kSmemMax));
+    if (e != cudaSuccess) return e;
+  }
+  return cudaFuncSetAttribute(wg_tile_kernel<MODE, STAGED, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               static_cast<int>(kSmemMax));
 }
 

@@ -463,3 +463,22 @@ def test_config5_full_size_policy_one_batch_sampled_against_the_oracle():
     assert np.array_equal(o_tag[~touched], clean_tag[~touched])
     assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), orc.verify(hdr_s, val_s, tag_s, st.mode))
     eng.close()
+
+
+@pytest.mark.parametrize("config,n", [(5, 70_001), (4, 100_003), (1, 65_536), (2, 33)])
+def test_sparse_lane_tuning_changes_no_result(config, n, monkeypatch):
+    """WG_TUNE_SPARSE_LANES (compacted (event, lane) work items) must give the oracle's tags, verdicts and counters."""
+    orig_load = B.Engine.load
+
+    def load_sparse(self, policy):
+        eng = orig_load(self, policy)
+        eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
+        return eng
+
+    monkeypatch.setattr(B.Engine, "load", load_sparse)
+    if config == 5:
+        test_config5_stress_alternating_modes_accumulate()
+    else:
+        st, orc, eng, out = run_config(config, n)
+        assert out[:, 0].any() or config == 2
+        eng.close()
