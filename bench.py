@@ -78,7 +78,7 @@ def measured_peaks() -> dict:
 
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
-    Q = ("uuid,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    Q = ("timestamp,uuid,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -90,6 +90,10 @@ class ClockSampler:
             self.p = subprocess.Popen(cmd, stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
+
+    def window(self, t0, t1) -> None:
+        """Only samples stamped inside [t0, t1] (datetime, local time) are kept: the timed region."""
+        self.t0, self.t1 = t0, t1
 
     def stop(self) -> dict:
         if self.p is None:
@@ -104,7 +108,20 @@ class ClockSampler:
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         rows = [[x.strip() for x in line.split(",")] for line in self.f.read().splitlines()]
-        rows = [c for c in rows if len(c) >= 8]
+        rows = [c for c in rows if len(c) >= 9]
+        t0, t1 = getattr(self, "t0", None), getattr(self, "t1", None)
+        if t0 is not None:
+            import datetime as _dt
+            kept = []
+            for c in rows:
+                try:
+                    ts = _dt.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f")
+                except ValueError:
+                    continue
+                if t0 <= ts <= t1:
+                    kept.append(c)
+            rows = kept or rows  # (a region shorter than one sampling period keeps the whole run's samples)
+        rows = [c[1:] for c in rows]
         mine = [c for c in rows if self.uuid and self.uuid in c[0].lower()]
         for c in (mine or rows):  # this rank's GPU; every visible GPU if the uuid could not be matched
             c = c[1:]
@@ -247,13 +264,15 @@ def run_ours(a) -> None:
                       ("shf+imad_hi_1:1", 9), ("add64_pairs", 10), ("sipround_x24", 11)):
         probes[name] = B.wg_probe_int_pipe(local, mix)[0]
 
+    props = torch.cuda.get_device_properties(local)
+    uuid = str(props.uuid) if hasattr(props, "uuid") else None
+    sampler = ClockSampler(uuid)  # started before the warm-up so that it is sampling when the timed region begins
     for _ in range(max(a.warmup, 0)):
         step()
     eng.wg_reset_counters()
     barrier()
-    props = torch.cuda.get_device_properties(local)
-    uuid = str(props.uuid) if hasattr(props, "uuid") else None
-    sampler = ClockSampler(uuid)
+    import datetime as _dt
+    t_region0 = _dt.datetime.now()
     launches0 = B.wg_launch_count()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(a.steps)]
     for k in range(a.steps):
@@ -263,6 +282,7 @@ def run_ours(a) -> None:
         eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode, out)
         ev[k][2].record()
     barrier()
+    sampler.window(t_region0, _dt.datetime.now())
     clocks = sampler.stop()
     launches = B.wg_launch_count() - launches0
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
