@@ -60,6 +60,9 @@ def parse_args():
     ap.add_argument("--profile", type=int, default=0,
                     help="wg_set_profile flags for the timed calls (1 backward-only, 2 forward-only, 4 low-telemetry, "
                          "8 metadata integrity); the headline run uses 0")
+    ap.add_argument("--batches", type=int, default=0,
+                    help="config 5 only: stream that many 8 M-event batches (BASELINE.json: 64 = 512 M events), "
+                         "alternating detect / enforce, and report the summed kernel time")
     ap.add_argument("--sparse", action="store_true", help="wg_set_tuning(WG_TUNE_SPARSE_LANES) for the timed calls")
     ap.add_argument("--shadow", action="store_true",
                     help="also time the stateful shadow stack (SURVEY 8(f-1)): one lock-step push + check_ret over 1 Mi warps")
@@ -481,10 +484,70 @@ def run_ours(a) -> None:
         dist.destroy_process_group()
 
 
+def run_config5_stream(a) -> None:
+    """BASELINE.json config 5 as a stream: `--batches` batches of 8 M events over the 1 M-site policy (sets up to 4,096
+    entries), detect on even and enforce on odd batches, each batch generated on the GPU, signed, corrupted and
+    verified; kernel time summed over the batches (generation excluded).  A parity-test case measured, not the
+    headline line: prints one JSON object."""
+    import torch
+
+    from paper_2606_11871_b200 import binding as B
+    from paper_2606_11871_b200 import streams as S
+
+    dev = torch.device("cuda", 0)
+    pol = S.make_policy(5, dev)
+    eng = B.Engine(0).load(pol)
+    if a.sparse:
+        eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
+    sign_ms = verify_ms = 0.0
+    planned_ret = planned_fwd = events = 0
+    out = tag = None
+    for b in range(-1, a.batches):  # batch -1 is the warm-up
+        st = S.make_stream(5, dev, policy=pol, batch_index=max(b, 0))
+        n = st.hdr.shape[0]
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32, device=dev)
+            tag = torch.empty((n, 32), dtype=torch.int64, device=dev)
+        e0, e1, e2, e3 = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+        e0.record()
+        eng.wg_sign_continuations(st.hdr, st.val, tag)
+        e1.record()
+        st.apply_return_tamper(tag)
+        e2.record()
+        eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode, out)
+        e3.record()
+        torch.cuda.synchronize()
+        if b < 0:
+            eng.wg_reset_counters()
+            continue
+        sign_ms += e0.elapsed_time(e1)
+        verify_ms += e2.elapsed_time(e3)
+        planned_ret += len(st.ret_tamper)
+        planned_fwd += len(st.fwd_tamper)
+        events += n
+        del st
+    g, _ = eng.wg_read_counters(per_site=False)
+    assert g["events_total"] == events and g["ret_viol_events"] == planned_ret
+    assert planned_fwd - 20 * a.batches <= g["fwd_viol_events"] <= planned_fwd
+    checks, lanes = g["ret_checks"] + g["fwd_checks"], g["ret_lanes"] + g["fwd_lanes"]
+    print(json.dumps({
+        "workload": "config5-stress stream", "batches": a.batches, "events": events, "checks": checks,
+        "lane_verdicts": lanes, "sign_ms_total": sign_ms, "verify_ms_total": verify_ms,
+        "checks_per_sec_verify": checks / (verify_ms * 1e-3), "lane_verdicts_per_sec_verify": lanes / (verify_ms * 1e-3),
+        "checks_per_sec_sign_plus_verify": checks / ((sign_ms + verify_ms) * 1e-3),
+        "violations_found": {"ret_events": g["ret_viol_events"], "fwd_events": g["fwd_viol_events"],
+                             "planned_ret": planned_ret, "planned_fwd": planned_fwd},
+        "blocked_lanes": g["blocked_lanes"], "sparse_lanes": bool(a.sparse), "n_sites": pol.n_sites,
+        "n_targets": int(pol.tgt_off[-1])}))
+    eng.close()
+
+
 def main():
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.config == 5 and a.batches > 0:
+        run_config5_stream(a)
     else:
         run_ours(a)
 
