@@ -183,6 +183,20 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
     return m.x == vl && m.y == vh;
   } else {
     const uint64_t* set = p.tgts + off;
+    // large sets live in L2 / HBM and every probe is a dependent ~1 us load: quaternary steps issue three
+    // independent probes at once and halve the number of dependent rounds (config 5: sets up to 4,096 entries;
+    // measured 2.55 -> 2.38 ms per batch; 8-ary steps were slower again, 2.49 ms: more traffic than latency saved)
+    while (len > 8) {
+      const uint32_t q = len >> 2;
+      const uint64_t m1 = __ldg(set + lo + q), m2 = __ldg(set + lo + 2 * q), m3 = __ldg(set + lo + 3 * q);
+      if (m3 <= v) {
+        lo += 3 * q;
+        len -= 3 * q;
+      } else {
+        lo += (m2 <= v) ? 2 * q : (m1 <= v) ? q : 0u;
+        len = q;
+      }
+    }
     while (len > 1) {
       const uint32_t half = len >> 1;
       const uint64_t mid = __ldg(set + lo + half);
