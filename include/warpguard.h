@@ -193,7 +193,8 @@ typedef struct {
  * stored token of site `index` ^= x.  Synchronises cuda_stream. */
 wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_value, void* cuda_stream);
 
-/* WG_ERR_INVALID_ARG for unknown flag bits.  Applies to the calls made after it returns. */
+/* WG_ERR_INVALID_ARG for unknown flag bits (and for any flag / ring when the measurement baseline kernels were
+ * selected with WG_IMPL=v1: they implement the five calls only).  Applies to the calls made after it returns. */
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags);
 /* Bounded violation ring in engine-owned device memory: `capacity` records (0 = off, the default).  Synchronises
  * `cuda_stream`, reallocates, and restarts the ring empty.  When the ring is full further records are dropped and

@@ -587,6 +587,7 @@ wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uin
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;
   if (flags & ~15u) return WG_ERR_INVALID_ARG;
+  if (flags && eng->impl == 1) return WG_ERR_INVALID_ARG;  // the baseline kernels (WG_IMPL=v1) know no profiles
   eng->profile = flags;  // takes effect with the next check call (kernel parameter)
   return WG_OK;
 }
@@ -626,6 +627,7 @@ wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_
 wg_status wg_set_ring_capacity(wg_engine* eng, uint64_t capacity, void* cuda_stream) {
   if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
   if (capacity > (1ull << 28)) return WG_ERR_INVALID_ARG;
+  if (capacity && eng->impl == 1) return WG_ERR_INVALID_ARG;  // no telemetry in the baseline kernels
   DeviceGuard g(eng->device);
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
