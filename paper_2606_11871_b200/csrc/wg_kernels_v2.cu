@@ -22,8 +22,8 @@
 // only the rows the tile needs) that complete on the warp's own mbarrier; 20 warps per SM keep the ALU pipe fed while
 // other warps wait for their rows.  When the policy's whole target table is small (<= kMaxStageTgts entries)
 // every CTA stages it in shared memory once with one more bulk copy.
-// Counters: warp-uniform registers + shared-memory atomics, flushed once per CTA; per-site counters are
-// aggregated over equal sites of a tile (__match_any_sync) before the global reduction.
+// Counters: warp-uniform registers + shared-memory atomics, flushed once per CTA; per-site counters live in shared
+// memory for small policies, else one L2 reduction per event and counter.
 #include "wg_internal.h"
 #include "../../include/warpguard_sip32.cuh"
 
@@ -459,20 +459,13 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
           if (judged_na) atomicAdd(&site_s[ev.site * 4 + S_LANES_CHECKED], judged_na);
         }
       } else {
-        // per-site counters in global memory: equal sites of the tile are merged first (Zipf: the hottest site is
-        // ~1/6 of all events)
-        const uint32_t m_known = __ballot_sync(kFull, known);
-        uint32_t grp = 0;
-        if (known) grp = __match_any_sync(m_known, ev.site);
-        uint32_t sum = judged_na;
-        for (uint32_t m = __ballot_sync(kFull, __popc(grp) > 1); m; m &= m - 1) {
-          const uint32_t j = __ffs(m) - 1;
-          const uint32_t x = __shfl_sync(kFull, judged_na, j);
-          if (((grp >> j) & 1u) && j != lane) sum += x;
-        }
-        if (known && lane == static_cast<uint32_t>(__ffs(grp) - 1)) {
-          atomicAdd(sc + S_EVENTS, static_cast<unsigned long long>(__popc(grp)));
-          if (sum) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(sum));
+        // per-site counters in global memory
+// one reduction per event straight to L2: measured faster than merging equal sites of the tile first
+        // (__match_any_sync + shuffles cost more ALU-pipe slots than the hot site's reductions cost in L2:
+        // config 4 verify 14.90 -> 14.64 ms, config 2 1.457 -> 1.449 ms)
+        if (known) {
+          atomicAdd(sc + S_EVENTS, 1ull);
+          if (judged_na) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(judged_na));
         }
       }
     }
