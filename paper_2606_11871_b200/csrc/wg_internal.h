@@ -58,7 +58,7 @@ enum CounterWord {
   C_SKIP_FWD_EVENTS = 28,
   C_SKIP_FWD_LANES = 29,
   C_RING_TOTAL = 30,  // violation records offered to the ring (recorded = min(total, capacity))
-  C_TICKET = 31,      // CTAs that finished the current launch: the last one writes the first-violation record
+  C_SPARE31 = 31,
   C_META_FAIL = 32,   // forward records that failed their authentication (metadata-integrity profile, R37)
   C_WORDS = 40
 };

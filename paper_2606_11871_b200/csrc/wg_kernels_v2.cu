@@ -750,40 +750,33 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     const uint32_t v = site_s[i];
     if (v) atomicAdd(p.site + i, static_cast<unsigned long long>(v));
   }
-  if constexpr (MODE != MODE_SIGN) {
-    // first-violation record (R29): the LAST CTA to finish sees the final key of this launch; if
-    // the key moved into this launch's event range it writes the full record of that event.  Deterministic,
-    // and nothing on the hot path: violations only did an atomicMin.
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      const unsigned long long ticket = atomicAdd(p.glob + C_TICKET, 1ull);
-      if (ticket == gridDim.x - 1) {
-        p.glob[C_TICKET] = 0ull;
-        const unsigned long long key = atomicMin(p.glob + C_FIRST_VIOLATION, ~0ull);
-        const unsigned long long seq = key >> 5;
-        if (key != ~0ull && key != p.first->key && seq >= p.seq_base && seq - p.seq_base < p.n) {
-          const uint64_t i = seq - p.seq_base;
-          const uint32_t fl = static_cast<uint32_t>(key & 31u);
-          const uint4 hh = p.hdr[i];
-          const uint2 o = __ldcg(p.out + i);  // written by another CTA of this launch: read it from L2
-          ViolRec r;
-          r.seq = seq;
-          r.site_id = hh.x;
-          r.kind = hh.x < p.n_sites ? p.recs[hh.x].kind : 7u;
-          r.viol_mask = o.x;
-          r.active_mask = hh.y;
-          r.lane = fl;
-          r.mode = p.mode;
-          r.observed = p.val[i * 32 + fl];
-          const bool judged_ret = MODE == MODE_VERIFY && r.kind == K_RET && !(p.profile & PROFILE_SKIP_BACKWARD);
-          r.stored = judged_ret ? p.tag[i * 32 + fl] : 0ull;
-          p.first->rec = r;
-          p.first->key = key;
-        }
-      }
-    }
-  }
+}
+
+// first-violation record (R29), one thread, enqueued behind every check launch: the launch is over, so
+// the key is final for it; if the key moved into that launch's event range the full record of that event is written.
+// Deterministic, and nothing on the hot path: violations only did the atomicMin they always did.  (An earlier version
+// let the last CTA of the tile kernel do this behind a ticket counter; it cost config 3 five per cent.)
+__global__ void wg_first_record(const Params p, const int has_tag) {
+  const unsigned long long key = p.glob[C_FIRST_VIOLATION];
+  const unsigned long long seq = key >> 5;
+  if (key == ~0ull || key == p.first->key || seq < p.seq_base || seq - p.seq_base >= p.n) return;
+  const uint64_t i = seq - p.seq_base;
+  const uint32_t fl = static_cast<uint32_t>(key & 31u);
+  const uint4 hh = p.hdr[i];
+  const uint2 o = p.out[i];
+  ViolRec r;
+  r.seq = seq;
+  r.site_id = hh.x;
+  r.kind = hh.x < p.n_sites ? p.recs[hh.x].kind : 7u;
+  r.viol_mask = o.x;
+  r.active_mask = hh.y;
+  r.lane = fl;
+  r.mode = p.mode;
+  r.observed = p.val[i * 32 + fl];
+  const bool judged_ret = has_tag && r.kind == K_RET && !(p.profile & PROFILE_SKIP_BACKWARD);
+  r.stored = judged_ret ? p.tag[i * 32 + fl] : 0ull;
+  p.first->rec = r;
+  p.first->key = key;
 }
 
 // SiteRec table from the v1 rows: the pre-A mid-state of every protected-return site (runs once per policy load)
@@ -896,7 +889,11 @@ cudaError_t launch_sign_v2(const Params& p, int sm_count, cudaStream_t st) {
 }
 
 cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st) {
-  return p.tag ? launch_tile<MODE_VERIFY>(p, sm_count, st) : launch_tile<MODE_FORWARD>(p, sm_count, st);
+  const cudaError_t e = p.tag ? launch_tile<MODE_VERIFY>(p, sm_count, st) : launch_tile<MODE_FORWARD>(p, sm_count, st);
+  if (e != cudaSuccess) return e;
+  wg_first_record<<<1, 1, 0, st>>>(p, p.tag != nullptr);
+  count_launch();
+  return cudaGetLastError();
 }
 
 cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,

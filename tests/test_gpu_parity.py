@@ -322,7 +322,7 @@ def test_work_runs_on_the_callers_stream():
         tag = eng.wg_sign_continuations(d_hdr, d_val)
         out = eng.wg_verify_continuations(d_hdr, d_val, tag, ENF)
     s.synchronize()
-    assert B.wg_launch_count() - before == 2
+    assert B.wg_launch_count() - before == 3  # sign; check + its one-thread first-violation-record kernel
     assert not out[:, 0].any()
     assert np.array_equal(tag.cpu().numpy().view(np.uint64), orc.sign(st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)))
 
