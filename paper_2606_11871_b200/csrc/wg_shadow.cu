@@ -156,8 +156,10 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
           }
         }
         viol = __ballot_sync(kFull, cause != 0);
+        if (viol) {  // rare: one cause per violating lane
 #pragma unroll
-        for (int k = SH_OVERFLOW; k <= SH_TARGET_MISMATCH; ++k) c[k] += __popc(__ballot_sync(kFull, cause == k));
+          for (int k = SH_OVERFLOW; k <= SH_TARGET_MISMATCH; ++k) c[k] += __popc(__ballot_sync(kFull, cause == k));
+        }
       }
     }
     if (viol) {
