@@ -373,9 +373,14 @@ def _apply_forward_bitflip(hdr, val, fwd_events, m, g, device, *, addr_bits_only
 # the five configs (BASELINE.json "configs")
 # ----------------------------------------------------------------------------------------------
 
-FULL_EVENTS = {1: 65_536, 2: 4_000_000, 3: 16_000_000, 4: 58_000_000, 5: 512_000_000}
-NAMES = {1: "tiny", 2: "backward-only", 3: "forward-only", 4: "mixed-paper-shaped", 5: "stress"}
-DEFAULT_MODE = {1: ENFORCE, 2: ENFORCE, 3: DETECT, 4: ENFORCE, 5: DETECT}
+# configs 6 and 7 are extra, public-code-SHAPED streams: only the shapes the paper reports —
+# a recovered 38-target family at one indirect site and a sealed callback whose wrong-callback run
+# records 64 forward-violation checks (Table A10) — no item of any third-party code.
+FULL_EVENTS = {1: 65_536, 2: 4_000_000, 3: 16_000_000, 4: 58_000_000, 5: 512_000_000, 6: 50_000, 7: 4_160}
+NAMES = {1: "tiny", 2: "backward-only", 3: "forward-only", 4: "mixed-paper-shaped", 5: "stress",
+         6: "38-target-family", 7: "wrong-callback-burst"}
+DEFAULT_MODE = {1: ENFORCE, 2: ENFORCE, 3: DETECT, 4: ENFORCE, 5: DETECT, 6: ENFORCE, 7: ENFORCE}
+BURST_CHECKS = 64
 CONFIG5_BATCH = 8_000_000
 
 
@@ -416,6 +421,14 @@ def make_policy(config: int, device="cpu", *, n_sites: int | None = None, max_se
         fs = torch.floor(torch.pow(2.0, u * float(np.log2(max_set)))).long().clamp_(1, max_set)
         sizes = _place_sizes(kind, fs, g, device)
         return _finish_policy(kind, sizes, 1 << 24, g, device, k0, k1, dig, disjoint=False)
+    if config == 6:  # one indirect site with a 38-target family, 32 return sites, 8 fixed-edge sites
+        kind = _shuffled_kinds({PROTECTED_FORWARD: 1, PROTECTED_RETURN: 32, FIXED_EDGE: 8}, g, device)
+        sizes = _place_sizes(kind, torch.tensor([38], dtype=torch.int64, device=device), g, device)
+        return _finish_policy(kind, sizes, 1 << 16, g, device, k0, k1, dig)
+    if config == 7:  # four sealed callback sites (one legal target each), 8 return sites
+        kind = _shuffled_kinds({PROTECTED_FORWARD: 4, PROTECTED_RETURN: 8}, g, device)
+        sizes = _place_sizes(kind, torch.ones(4, dtype=torch.int64, device=device), g, device)
+        return _finish_policy(kind, sizes, 1 << 16, g, device, k0, k1, dig)
     raise ValueError(f"config {config}")
 
 
@@ -466,6 +479,19 @@ def make_stream(config: int, device="cpu", *, n_events: int | None = None, polic
     elif config == 5:
         site = torch.randint(0, ns, (n,), generator=g, device=device, dtype=torch.int64)
         mask_mode, ru, fu = "k-uniform", 0.7, 0.9
+    elif config == 6:  # 40 % of the events go through the one gate site
+        site = torch.randint(0, ns, (n,), generator=g, device=device, dtype=torch.int64)
+        gate = torch.nonzero(kind_t == PROTECTED_FORWARD).flatten()[0]
+        site[torch.rand(n, generator=g, device=device) < 0.4] = gate
+        mask_mode, ru, fu = "p0.9", 0.7, 0.5
+    elif config == 7:  # benign traffic, then one contiguous run of BURST_CHECKS events at one callback site
+        site = torch.randint(0, ns, (n,), generator=g, device=device, dtype=torch.int64)
+        cb = torch.nonzero(kind_t == PROTECTED_FORWARD).flatten()
+        burst_site = cb[int(torch.randint(0, cb.numel(), (1,), generator=g, device=device))]
+        b0 = n - BURST_CHECKS - 17
+        site[b0:b0 + BURST_CHECKS] = burst_site
+        mask_mode, ru, fu = "p0.9", 0.7, 1.0
+        meta.update(burst_start=b0, burst_site=int(burst_site))
     else:
         raise ValueError(config)
 
@@ -487,6 +513,15 @@ def make_stream(config: int, device="cpu", *, n_events: int | None = None, polic
     elif config == 4:  # 0.05 % violations on protected events
         rt = _plan_return_bitflips(hdr, ret_ev, round(0.0005 * ret_ev.numel()), g, device)
         ft = _apply_forward_outofset(policy, hdr, val, uni, fwd_ev, round(0.0005 * fwd_ev.numel()), g, device)
+    elif config == 6:  # 0.5 % wrong targets at the gate site
+        rt = TamperPlan.empty(device)
+        ft = _apply_forward_outofset(policy, hdr, val, uni, fwd_ev, round(0.005 * fwd_ev.numel()), g, device)
+    elif config == 7:  # every check of the burst carries the wrong callback; nothing else is corrupted
+        rt = TamperPlan.empty(device)
+        b0 = meta["burst_start"]
+        burst = torch.arange(b0, b0 + BURST_CHECKS, device=device)
+        burst = burst[(hdr[burst, 0] >> 32) & 0xFFFFFFFF != 0]  # (an empty mask is not a check)
+        ft = _apply_forward_outofset(policy, hdr, val, uni, burst, burst.numel(), g, device)
     else:  # config 5: forged tags with 1-8 bit flips; targets one bit away from a legal target
         rt = _plan_return_bitflips(hdr, ret_ev, round(0.01 * ret_ev.numel()), g, device, max_bits=8, tag_only=True)
         ft = _apply_forward_bitflip(hdr, val, fwd_ev, round(0.01 * fwd_ev.numel()), g, device, addr_bits_only=True)

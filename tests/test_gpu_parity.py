@@ -482,3 +482,22 @@ def test_sparse_lane_tuning_changes_no_result(config, n, monkeypatch):
         st, orc, eng, out = run_config(config, n)
         assert out[:, 0].any() or config == 2
         eng.close()
+
+
+@pytest.mark.parametrize("config", [6, 7])
+def test_public_code_shaped_streams(config):
+    """a 38-target family at one indirect site and a wrong-callback burst that
+    records 64 forward-violation checks — shapes only."""
+    st, orc, eng, out = run_config(config, None)
+    assert np.array_equal(out[:, 0], witness.expected_viol(st))
+    g, _ = eng.wg_read_counters()
+    if config == 6:
+        sizes = np.diff(st.policy.tgt_off.astype(np.int64))
+        assert sizes.max() == 38 and (sizes > 0).sum() == 1 and g["fwd_viol_events"] == len(st.fwd_tamper) > 50
+    else:
+        b0 = st.meta["burst_start"]
+        assert g["fwd_viol_events"] == S.BURST_CHECKS == 64 and g["ret_viol"] == 0
+        assert out[b0:b0 + 64, 0].all() and not out[:b0, 0].any() and not out[b0 + 64:, 0].any()
+        assert (out[b0:b0 + 64, 1] == 0).all()                      # enforce: the whole burst is blocked
+        assert g["first_violation_key"] >> 5 == b0
+    eng.close()

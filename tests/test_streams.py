@@ -64,3 +64,24 @@ def test_config5_masks_span_single_lane_to_full():
     pc = popc(st.active_mask().numpy())
     assert pc.min() == 1 and pc.max() == 32 and 15.5 < pc.mean() < 17.5
     assert st.mode == S.DETECT and S.make_stream(5, n_events=10, n_sites=2000, max_set=64, batch_index=1).mode == S.ENFORCE
+
+
+def test_public_code_shaped_configs_have_the_reported_shapes():
+    """Configs 6 and 7: one 38-target site; a contiguous 64-check wrong-callback burst."""
+    import numpy as np
+    from paper_2606_11871_b200 import streams as S
+    from tests import witness
+    from tests.util import oracle_for
+
+    st = S.make_stream(6, "cpu")
+    sizes = np.diff(st.policy.tgt_off.astype(np.int64))
+    assert sorted(sizes[sizes > 0].tolist()) == [38] and st.hdr.shape[0] == 50_000
+    st = S.make_stream(7, "cpu")
+    orc = oracle_for(st.policy)
+    hdr, val = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    out = orc.verify(hdr, val, orc.sign(hdr, val), st.mode)
+    b0 = st.meta["burst_start"]
+    assert np.array_equal(out[:, 0], witness.expected_viol(st))
+    assert int((out[:, 0] != 0).sum()) == 64 and out[b0:b0 + 64, 0].all()
+    g, _ = orc.read_counters()
+    assert g["fwd_viol_events"] == 64 and g["blocked_events"] == 64
