@@ -430,9 +430,11 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       c.skipped += __popc(__ballot_sync(kFull, valid && !is_ret));
     } else {
       c.total += __popc(__ballot_sync(kFull, valid));
-      c.unknown += __popc(__ballot_sync(kFull, valid && !known));
-      c.empty += __popc(__ballot_sync(kFull, known && ev.active == 0u));
-      c.misrouted += __popc(__ballot_sync(kFull, known && ev.cls == CLS_FAIL));
+      if (__ballot_sync(kFull, valid && (!known || ev.active == 0u || ev.cls == CLS_FAIL))) {  // uncommon events
+        c.unknown += __popc(__ballot_sync(kFull, valid && !known));
+        c.empty += __popc(__ballot_sync(kFull, known && ev.active == 0u));
+        c.misrouted += __popc(__ballot_sync(kFull, known && ev.cls == CLS_FAIL));
+      }
       c.ret_checks += __popc(m_ret);
       c.fwd_checks += __popc(m_fwd);
       c.ret_lanes += __reduce_add_sync(kFull, ev.cls == CLS_RET ? na : 0u);
@@ -459,8 +461,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
           if (judged_na) atomicAdd(&site_s[ev.site * 4 + S_LANES_CHECKED], judged_na);
         }
       } else {
-        // per-site counters in global memory
-// one reduction per event straight to L2: measured faster than merging equal sites of the tile first
+        // per-site counters in global memory, one reduction per event straight to L2: measured faster than merging equal sites of the tile first
         // (__match_any_sync + shuffles cost more ALU-pipe slots than the hot site's reductions cost in L2:
         // config 4 verify 14.90 -> 14.64 ms, config 2 1.457 -> 1.449 ms)
         if (known) {
