@@ -94,6 +94,10 @@ def lib():
         L.wgo_read_first_violation.argtypes = [vp, vp]
         L.wgo_read_telemetry.restype = None
         L.wgo_read_telemetry.argtypes = [vp, vp]
+        L.wgo_policy_digest.restype = u64
+        L.wgo_policy_digest.argtypes = [u32, vp, vp, vp, u64, u64]
+        L.wgo_create_bound.restype = vp
+        L.wgo_create_bound.argtypes = [u32, vp, vp, vp, u64, u64, u64]
         L.wgo_policy_poke.restype = C.c_int
         L.wgo_policy_poke.argtypes = [vp, C.c_int, u64, u64]
         L.wgo_shadow_configure.restype = C.c_int
@@ -140,6 +144,11 @@ def validate_policy(kind, tgt_off, tgts) -> int:
     return int(lib().wgo_validate_policy(kind.size, _ptr(kind), _ptr(tgt_off), _ptr(tgts)))
 
 
+def policy_digest(kind, tgt_off, tgts, k0: int, k1: int) -> int:
+    kind, tgt_off, tgts = _c(kind, np.uint8), _c(tgt_off, np.uint32), _c(tgts, np.uint64)
+    return int(lib().wgo_policy_digest(kind.size, _ptr(kind), _ptr(tgt_off), _ptr(tgts), k0, k1))
+
+
 def _hdr_bytes(hdr: np.ndarray) -> np.ndarray:
     """Accept [n,2] (u)int64 rows (site | mask<<32, context_base) and return them as raw rows."""
     h = np.ascontiguousarray(hdr)
@@ -150,17 +159,19 @@ def _hdr_bytes(hdr: np.ndarray) -> np.ndarray:
 class Oracle:
     """One loaded policy + key + counters (the oracle's analogue of wg_engine)."""
 
-    def __init__(self, kind, tgt_off, tgts, k0: int, k1: int, policy_digest: int = 0):
+    def __init__(self, kind, tgt_off, tgts, k0: int, k1: int, policy_digest: int = 0, bound: bool = False):
+        """bound=True: wgo_create_bound — the image's digest must equal policy_digest and is folded into the tokens."""
         self.kind = _c(kind, np.uint8)
         self.tgt_off = _c(tgt_off, np.uint32)
         self.tgts = _c(tgts, np.uint64)
         assert self.tgt_off.size == self.kind.size + 1
         self.n_sites = int(self.kind.size)
-        self._h = lib().wgo_create(self.n_sites, _ptr(self.kind), _ptr(self.tgt_off), _ptr(self.tgts),
-                                   k0, k1, policy_digest)
+        create = lib().wgo_create_bound if bound else lib().wgo_create
+        self._h = create(self.n_sites, _ptr(self.kind), _ptr(self.tgt_off), _ptr(self.tgts), k0, k1, policy_digest)
         if not self._h:
-            raise ValueError("oracle rejected the policy (wgo_validate_policy = %d)"
-                             % validate_policy(self.kind, self.tgt_off, self.tgts))
+            raise ValueError("oracle rejected the policy (wgo_validate_policy = %d%s)"
+                             % (validate_policy(self.kind, self.tgt_off, self.tgts),
+                                ", or its digest is not the expected one" if bound else ""))
 
     def close(self):
         if getattr(self, "_h", None):

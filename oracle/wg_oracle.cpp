@@ -67,7 +67,8 @@ struct wgo_engine {
   uint64_t k0 = 0, k1 = 0;
   uint64_t seq = 0;  // running event index over check calls (R12)
   int use_binary_search = 0;
-  bool poked = false;  // wgo_policy_poke touched the target array: sets may be unsorted
+  bool poked = false;
+  bool bind_digest = false;  // R39: fold the policy digest into the token's first word  // wgo_policy_poke touched the target array: sets may be unsorted
   wgo_counters g;
   std::vector<wgo_site_counters> site;
   // profiles and telemetry (R26-R29)
@@ -138,6 +139,19 @@ uint64_t wgo_mac(uint64_t k0, uint64_t k1, uint32_t site_id, uint64_t value, uin
   store_le64(msg + 8, value);
   store_le64(msg + 16, context_id);
   return wgo_siphash24(k0, k1, msg, sizeof msg);
+}
+
+// Token as the ENGINE computes it: with digest binding on (R39, "policy binding is checked before
+// use") the low 32 bits of the policy digest ride in the upper half of the first message word, so
+// a token minted under one policy image does not verify under another.
+static uint64_t engine_token(const wgo_engine* e, uint32_t site_id, uint64_t value, uint64_t context_id) {
+  uint8_t msg[24];
+  const uint64_t w0 = static_cast<uint64_t>(site_id) |
+                      (e->bind_digest ? (e->g.policy_digest & 0xffffffffull) << 32 : 0ull);
+  store_le64(msg + 0, w0);
+  store_le64(msg + 8, value);
+  store_le64(msg + 16, context_id);
+  return wgo_siphash24(e->k0, e->k1, msg, sizeof msg);
 }
 
 // DESIGN.md R2: the caller's context_base has its low five bits reserved for
@@ -220,7 +234,7 @@ void wgo_sign(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, uint
       const bool active = (a >> lane) & 1u;
       uint64_t t = 0;
       if (protected_return && active)
-        t = wgo_mac(e->k0, e->k1, s, val[ev * 32 + lane], wgo_lane_ctx(hdr[ev].context_base, lane));
+        t = engine_token(e, s, val[ev * 32 + lane], wgo_lane_ctx(hdr[ev].context_base, lane));
       tag[ev * 32 + lane] = t;
     }
     if (protected_return)
@@ -293,7 +307,7 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
         for (uint32_t lane = 0; lane < 32; ++lane) {
           if (!((a >> lane) & 1u)) continue;  // inactive lanes are never judged
           const uint64_t expect =
-              wgo_mac(e->k0, e->k1, s, val[ev * 32 + lane], wgo_lane_ctx(hdr[ev].context_base, lane));
+              engine_token(e, s, val[ev * 32 + lane], wgo_lane_ctx(hdr[ev].context_base, lane));
           if (expect != tag[ev * 32 + lane]) viol |= (1u << lane);
         }
         e->g.ret_checks += 1;
@@ -369,6 +383,40 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
     out[ev].allow_mask = allow;
   }
   if (n != 0) e->g.last_mode = static_cast<uint64_t>(mode);
+}
+
+// Digest of a policy image (R39): SipHash-2-4 under the policy's key over
+//   LE64(n_sites) || LE64(n_targets) || kind[n_sites] (zero-padded to 8 bytes) || tgt_off[n_sites + 1] as LE32
+//   (zero-padded to 8 bytes) || tgts as LE64.
+uint64_t wgo_policy_digest(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off, const uint64_t* tgts,
+                           uint64_t k0, uint64_t k1) {
+  std::vector<uint8_t> msg;
+  auto put64 = [&msg](uint64_t w) {
+    for (int i = 0; i < 8; ++i) msg.push_back(static_cast<uint8_t>(w >> (8 * i)));
+  };
+  auto pad8 = [&msg]() {
+    while (msg.size() % 8) msg.push_back(0);
+  };
+  const uint64_t nt = tgt_off[n_sites];
+  put64(n_sites);
+  put64(nt);
+  for (uint32_t s = 0; s < n_sites; ++s) msg.push_back(kind[s]);
+  pad8();
+  for (uint32_t s = 0; s <= n_sites; ++s)
+    for (int i = 0; i < 4; ++i) msg.push_back(static_cast<uint8_t>(tgt_off[s] >> (8 * i)));
+  pad8();
+  for (uint64_t i = 0; i < nt; ++i) put64(tgts[i]);
+  return wgo_siphash24(k0, k1, msg.data(), msg.size());
+}
+
+// "When an enforcement profile requires a policy digest, a mismatch aborts before the policy is used"
+wgo_engine* wgo_create_bound(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off, const uint64_t* tgts,
+                             uint64_t k0, uint64_t k1, uint64_t expected_digest) {
+  if (wgo_validate_policy(n_sites, kind, tgt_off, tgts) != WGO_POLICY_OK) return nullptr;
+  if (wgo_policy_digest(n_sites, kind, tgt_off, tgts, k0, k1) != expected_digest) return nullptr;
+  wgo_engine* e = wgo_create(n_sites, kind, tgt_off, tgts, k0, k1, expected_digest);
+  if (e) e->bind_digest = true;
+  return e;
 }
 
 void wgo_set_profile(wgo_engine* e, uint32_t flags) { e->profile = flags; }
@@ -482,7 +530,7 @@ static void shadow_run(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* 
             st[d].expected_return = val[ev * 32 + lane];
             st[d].callsite_id = h.site_id;
             st[d].depth = d;
-            st[d].token = wgo_mac(e->k0, e->k1, h.site_id, val[ev * 32 + lane], shadow_ctx(h.context_base, d, lane));
+            st[d].token = engine_token(e, h.site_id, val[ev * 32 + lane], shadow_ctx(h.context_base, d, lane));
             d += 1;
           } else {
             if (d == 0) {  // underflow
@@ -500,7 +548,7 @@ static void shadow_run(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* 
             if (r.depth != d) {
               viol |= 1u << lane;
               e->sh.depth_mismatch_lanes += 1;
-            } else if (r.token != wgo_mac(e->k0, e->k1, r.callsite_id, r.expected_return,
+            } else if (r.token != engine_token(e, r.callsite_id, r.expected_return,
                                           shadow_ctx(h.context_base, r.depth, lane))) {
               viol |= 1u << lane;
               e->sh.token_mismatch_lanes += 1;

@@ -164,6 +164,16 @@ typedef struct {
 /* what = 0: allowed_targets[index] ^= x (index into the CSR array); what = 1: the stored token of site `index` ^= x.
  * Returns 0, or -1 when out of range.  The set may become unsorted: membership is the linear scan then. */
 int wgo_policy_poke(wgo_engine* e, int what, uint64_t index, uint64_t xor_value);
+/* ---- policy-digest binding (second half; R39) ----
+ * wgo_policy_digest: SipHash-2-4 under the policy's key over LE64(n_sites) || LE64(n_targets) || kind bytes
+ * (zero-padded to 8) || tgt_off as LE32 (zero-padded to 8) || tgts as LE64.
+ * wgo_create_bound: NULL unless the image's digest equals expected_digest ("a mismatch aborts before the policy is
+ * used"); the engine then folds the digest's low 32 bits into the upper half of every backward token's first
+ * message word (LE64(site_id | digest32 << 32)), so tokens do not carry over to another policy image. */
+uint64_t wgo_policy_digest(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off, const uint64_t* tgts,
+                           uint64_t k0, uint64_t k1);
+wgo_engine* wgo_create_bound(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off, const uint64_t* tgts,
+                             uint64_t k0, uint64_t k1, uint64_t expected_digest);
 void wgo_set_profile(wgo_engine* e, uint32_t flags);
 /* capacity 0 (default) disables the ring; the oracle keeps the FIRST `capacity` records in event order
  * (any subset of that size is a valid ring content once it overflows). */

@@ -103,3 +103,38 @@ def test_record_token_format_against_libcrypto():
         o2.policy_poke(1, 4, ossl(KEY, record_msg(4, old)) ^ ossl(KEY, msg))
         o2.check_forward(hdr, val, ENF)
         assert o2.read_telemetry()["fwd_meta_fail_events"] == 1
+
+
+# ---------------------------------------------------------------------------------------------------------
+# policy-digest binding (second half; R39)
+# ---------------------------------------------------------------------------------------------------------
+def test_policy_digest_format_and_bound_load_against_libcrypto():
+    ossl = openssl_mac.get()
+    if ossl is None:
+        pytest.skip("libcrypto without SIPHASH")
+    o, kind, off, tg = make()
+    msg = struct.pack("<QQ", len(kind), len(tg)) + bytes(kind) + b"\0" * (-len(kind) % 8)
+    msg += b"".join(struct.pack("<I", int(x)) for x in off) + b"\0" * (-4 * len(off) % 8)
+    msg += b"".join(struct.pack("<Q", int(t)) for t in tg)
+    d = oracle.policy_digest(kind, off, tg, K0, K1)
+    assert d == ossl(KEY, msg)
+    # a bound load refuses any other digest, and any other image under the right digest
+    with pytest.raises(ValueError):
+        oracle.Oracle(kind, off, tg, K0, K1, d ^ 1, bound=True)
+    tg2 = tg.copy(); tg2[3] += np.uint64(16)
+    with pytest.raises(ValueError):
+        oracle.Oracle(kind, off, tg2, K0, K1, d, bound=True)
+    ob = oracle.Oracle(kind, off, tg, K0, K1, d, bound=True)
+    # tokens of the bound engine: first message word = site | digest32 << 32 (libcrypto over struct.pack)
+    hdr = mk_hdr([0], [FULL], [0x0001000000000040])
+    val = np.full((1, 32), 0x7F5A40000010, dtype=np.uint64)
+    tag = ob.sign(hdr, val)
+    for lane in (0, 5, 31):
+        w0 = 0 | ((d & 0xFFFFFFFF) << 32)
+        assert int(tag[0, lane]) == ossl(KEY, struct.pack("<QQQ", w0, 0x7F5A40000010, 0x0001000000000040 | lane))
+    # ... verify under the same binding, and do not carry over to the unbound engine nor to another image
+    assert ob.verify(hdr, val, tag, ENF)[0, 0] == 0
+    assert o.verify(hdr, val, tag, ENF)[0, 0] == FULL
+    d2 = oracle.policy_digest(kind, off, tg2, K0, K1)
+    other = oracle.Oracle(kind, off, tg2, K0, K1, d2, bound=True)
+    assert d2 != d and other.verify(hdr, val, tag, ENF)[0, 0] == FULL
