@@ -117,6 +117,17 @@ typedef struct {
  * A successful load zeroes all counters and the event sequence number. */
 wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc);
 
+/* Policy-digest binding ("When an enforcement profile requires a policy digest, a
+ * mismatch aborts before the policy is used"; R39).
+ * wg_policy_digest: SipHash-2-4 under desc->key over LE64(n_sites) || LE64(n_targets) || kind bytes (zero-padded to
+ *   8) || tgt_off as LE32 (zero-padded to 8) || tgts as LE64 — computed on the host, at load time only.
+ * wg_load_policy_bound: as wg_load_policy, but desc->policy_digest must equal that digest (else WG_ERR_BAD_POLICY,
+ *   nothing loaded), and its low 32 bits are folded into the upper half of every backward token's first message word
+ *   (LE64(site_id | digest32 << 32)): tokens signed under one policy image do not verify under another.  The
+ *   binding holds until the next load. */
+wg_status wg_policy_digest(const wg_policy_desc* desc, uint64_t* h_digest);
+wg_status wg_load_policy_bound(wg_engine** eng, int device, const wg_policy_desc* desc);
+
 /* Backward push: d_tag[e][l] = token(site, d_val[e][l], lane context) for every active
  * lane of every event whose site is protected-return, 0 for every other lane (R10).
  *   d_hdr [n] wg_event_hdr, d_val [n][32] u64 in, d_tag [n][32] u64 out.  n == 0 is a no-op. */

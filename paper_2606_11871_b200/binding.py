@@ -28,7 +28,8 @@ EXPORTS = [
     "wg_probe_int_pipe", "wg_launch_count",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
-    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_set_tuning",
+    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_set_tuning", "wg_policy_digest",
+    "wg_load_policy_bound",
 ]
 WG_TUNE_DEFAULT, WG_TUNE_SPARSE_LANES = 0, 1
 
@@ -82,6 +83,8 @@ def lib() -> C.CDLL:
         L = C.CDLL(str(LIB_PATH))
         vp, u64, i = C.c_void_p, C.c_uint64, C.c_int
         L.wg_load_policy.argtypes = [C.POINTER(vp), i, C.POINTER(_PolicyDesc)]
+        L.wg_load_policy_bound.argtypes = [C.POINTER(vp), i, C.POINTER(_PolicyDesc)]
+        L.wg_policy_digest.argtypes = [C.POINTER(_PolicyDesc), C.POINTER(u64)]
         L.wg_sign_continuations.argtypes = [vp, vp, vp, vp, u64, vp]
         L.wg_verify_continuations.argtypes = [vp, vp, vp, vp, vp, u64, i, vp]
         L.wg_check_forward.argtypes = [vp, vp, vp, vp, u64, i, vp]
@@ -158,7 +161,8 @@ class Engine:
         self.n_sites = 0
 
     # -- wg_load_policy ---------------------------------------------------------------------------
-    def wg_load_policy(self, kind, tgt_off, tgts, k0: int, k1: int, policy_digest: int = 0) -> None:
+    def wg_load_policy(self, kind, tgt_off, tgts, k0: int, k1: int, policy_digest: int = 0, bound: bool = False) -> None:
+        """bound=True calls wg_load_policy_bound: policy_digest must be the image's digest (wg_policy_digest)."""
         kind = np.ascontiguousarray(kind, dtype=np.uint8)
         tgt_off = np.ascontiguousarray(tgt_off, dtype=np.uint32)
         tgts = np.ascontiguousarray(tgts, dtype=np.uint64)
@@ -172,7 +176,10 @@ class Engine:
         d.key[0] = k0 & (2**64 - 1)
         d.key[1] = k1 & (2**64 - 1)
         d.policy_digest = policy_digest & (2**64 - 1)
-        _chk(lib().wg_load_policy(C.byref(self._h), self.device, C.byref(d)), "wg_load_policy")
+        if bound:
+            _chk(lib().wg_load_policy_bound(C.byref(self._h), self.device, C.byref(d)), "wg_load_policy_bound")
+        else:
+            _chk(lib().wg_load_policy(C.byref(self._h), self.device, C.byref(d)), "wg_load_policy")
         self.n_sites = int(kind.size)
 
     def load(self, policy) -> "Engine":
@@ -319,6 +326,23 @@ class Engine:
             self.wg_destroy()
         except Exception:  # interpreter shutdown
             pass
+
+
+def wg_policy_digest(kind, tgt_off, tgts, k0: int, k1: int) -> int:
+    """Digest of a policy image (warpguard.h): host-side, no GPU needed."""
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    tgt_off = np.ascontiguousarray(tgt_off, dtype=np.uint32)
+    tgts = np.ascontiguousarray(tgts, dtype=np.uint64)
+    d = _PolicyDesc()
+    d.n_sites = kind.size
+    d.kind = kind.ctypes.data if kind.size else None
+    d.tgt_off = tgt_off.ctypes.data
+    d.tgts = tgts.ctypes.data if tgts.size else None
+    d.key[0] = k0 & (2**64 - 1)
+    d.key[1] = k1 & (2**64 - 1)
+    out = C.c_uint64(0)
+    _chk(lib().wg_policy_digest(C.byref(d), C.byref(out)), "wg_policy_digest")
+    return int(out.value)
 
 
 def wg_probe_int_pipe(device: int, mix: int) -> tuple[float, float]:

@@ -19,6 +19,7 @@ struct wg_engine {
   uint64_t n_tgts = 0;
   wg::SiteRow* d_rows = nullptr;
   wg::SiteRec* d_recs = nullptr;  // v2 site records (kind, set range, pre-A SipHash mid-state), 64 B each
+  uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
   uint32_t tuning = 0;             // WG_TUNE_* flags
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
@@ -146,6 +147,7 @@ wg::Params base_params(const wg_engine* e) {
   p.recs = e->d_recs;
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
+  p.bind_hi = e->bind_hi;
   p.sparse = (e->tuning & WG_TUNE_SPARSE_LANES) ? 1u : 0u;
   p.ring = e->d_ring;
   p.ring_cap = e->d_ring ? e->ring_cap : 0;
@@ -292,7 +294,72 @@ void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 extern "C" {
 
+// SipHash-2-4 on the host, for the load-time digest of a policy image only (no check runs on the host)
+static uint64_t host_siphash24(uint64_t k0, uint64_t k1, const std::vector<uint8_t>& m) {
+  auto rotl = [](uint64_t x, int b) { return (x << b) | (x >> (64 - b)); };
+  uint64_t v0 = k0 ^ 0x736f6d6570736575ull, v1 = k1 ^ 0x646f72616e646f6dull;
+  uint64_t v2 = k0 ^ 0x6c7967656e657261ull, v3 = k1 ^ 0x7465646279746573ull;
+  auto round = [&]() {
+    v0 += v1; v1 = rotl(v1, 13); v1 ^= v0; v0 = rotl(v0, 32);
+    v2 += v3; v3 = rotl(v3, 16); v3 ^= v2;
+    v0 += v3; v3 = rotl(v3, 21); v3 ^= v0;
+    v2 += v1; v1 = rotl(v1, 17); v1 ^= v2; v2 = rotl(v2, 32);
+  };
+  const size_t n = m.size(), full = n / 8;
+  for (size_t i = 0; i < full; ++i) {
+    uint64_t w = 0;
+    for (int j = 0; j < 8; ++j) w |= static_cast<uint64_t>(m[8 * i + j]) << (8 * j);
+    v3 ^= w; round(); round(); v0 ^= w;
+  }
+  uint64_t last = static_cast<uint64_t>(n & 0xff) << 56;
+  for (size_t j = 0; j < n % 8; ++j) last |= static_cast<uint64_t>(m[8 * full + j]) << (8 * j);
+  v3 ^= last; round(); round(); v0 ^= last;
+  v2 ^= 0xff; round(); round(); round(); round();
+  return v0 ^ v1 ^ v2 ^ v3;
+}
+
+static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* desc, uint32_t bind_hi);
+
+wg_status wg_policy_digest(const wg_policy_desc* desc, uint64_t* h_digest) {
+  if (!desc || !h_digest || !desc->tgt_off || (desc->n_sites && !desc->kind)) return WG_ERR_INVALID_ARG;
+  if (!policy_ok(desc)) return WG_ERR_BAD_POLICY;
+  const uint32_t n = desc->n_sites;
+  const uint64_t nt = desc->tgt_off[n];
+  std::vector<uint8_t> m;
+  try {
+    m.reserve(16 + n + 8 + 4 * (static_cast<size_t>(n) + 1) + 8 + 8 * nt);
+  } catch (const std::bad_alloc&) {
+    return WG_ERR_OOM;
+  }
+  auto put64 = [&m](uint64_t w) {
+    for (int i = 0; i < 8; ++i) m.push_back(static_cast<uint8_t>(w >> (8 * i)));
+  };
+  put64(n);
+  put64(nt);
+  for (uint32_t s = 0; s < n; ++s) m.push_back(desc->kind[s]);
+  while (m.size() % 8) m.push_back(0);
+  for (uint32_t s = 0; s <= n; ++s)
+    for (int i = 0; i < 4; ++i) m.push_back(static_cast<uint8_t>(desc->tgt_off[s] >> (8 * i)));
+  while (m.size() % 8) m.push_back(0);
+  for (uint64_t i = 0; i < nt; ++i) put64(desc->tgts[i]);
+  *h_digest = host_siphash24(desc->key[0], desc->key[1], m);
+  return WG_OK;
+}
+
 wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc) {
+  return load_common(eng, device, desc, 0u);
+}
+
+wg_status wg_load_policy_bound(wg_engine** eng, int device, const wg_policy_desc* desc) {
+  uint64_t d = 0;
+  const wg_status s = wg_policy_digest(desc, &d);
+  if (s != WG_OK) return s;
+  if (d != desc->policy_digest) return WG_ERR_BAD_POLICY;  // "a mismatch aborts before the policy is used"
+  { const char* impl = std::getenv("WG_IMPL"); if (impl && impl[0] == 'v' && impl[1] == '1') return WG_ERR_INVALID_ARG; }
+  return load_common(eng, device, desc, static_cast<uint32_t>(d));
+}
+
+static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* desc, uint32_t bind_hi) {
   if (!eng || !desc) return WG_ERR_INVALID_ARG;
   if (desc->n_sites && (!desc->kind || !desc->tgt_off)) return WG_ERR_INVALID_ARG;
   if (!desc->tgt_off) return WG_ERR_INVALID_ARG;
@@ -377,13 +444,14 @@ wg_status wg_load_policy(wg_engine** eng, int device, const wg_policy_desc* desc
   e->v_init[2] = desc->key[0] ^ 0x6c7967656e657261ull;
   e->v_init[3] = desc->key[1] ^ 0x7465646279746573ull;
   e->digest = desc->policy_digest;
+  e->bind_hi = bind_hi;
   {
     const char* impl = std::getenv("WG_IMPL");  // measurement knob: the baseline kernels stay selectable
     e->impl = (impl && impl[0] == 'v' && impl[1] == '1') ? 1 : 2;
   }
   // per-site SipHash mid-states, computed on the device from the key-derived initial state
   {
-    cudaError_t e3 = wg::launch_build_recs(e->d_recs, e->d_rows, e->d_tgts, n, e->v_init[0], e->v_init[1], e->v_init[2],
+    cudaError_t e3 = wg::launch_build_recs(e->d_recs, e->d_rows, e->d_tgts, n, bind_hi, e->v_init[0], e->v_init[1], e->v_init[2],
                                            e->v_init[3], nullptr);
     if (e3 != cudaSuccess) {
       free_tables(e);

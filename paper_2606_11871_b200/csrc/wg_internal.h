@@ -101,6 +101,9 @@ struct Params {
   uint32_t mode;             // 0 detect, 1 enforce
   uint32_t profile;          // PROFILE_* flags (R26)
   uint32_t sparse;           // tuning: compacted-lane MAC passes (wg_set_tuning)
+  uint32_t bind_hi;          // upper half of the token's first message word: low 32 bits of the policy digest when
+                             // the policy was loaded with wg_load_policy_bound (R39), else 0
+  uint32_t pad1;
   ViolRec* ring;             // violation ring or nullptr
   uint64_t ring_cap;         // its capacity in records
   FirstRec* first;           // first-violation record
@@ -126,8 +129,8 @@ cudaError_t launch_check_v1(const Params& p, int sm_count, cudaStream_t st);
 // v2 (wg_kernels_v2.cu): tiled, cp.async-staged, mid-state-cached kernels
 cudaError_t launch_sign_v2(const Params& p, int sm_count, cudaStream_t st);
 cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st);
-cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
-                              uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st);
+cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint32_t bind_hi,
+                              uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st);
 cudaError_t init_v2();  // one-time function attributes (dynamic shared memory opt-in)
 cudaError_t launch_fill_u64(unsigned long long* p, uint64_t n, unsigned long long v, cudaStream_t st);
 cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double* ms);

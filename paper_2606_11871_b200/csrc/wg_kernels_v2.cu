@@ -781,8 +781,8 @@ __global__ void wg_first_record(const Params p, const int has_tag) {
 }
 
 // SiteRec table from the v1 rows: the pre-A mid-state of every protected-return site (runs once per policy load)
-__global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
-                              uint64_t v1, uint64_t v2, uint64_t v3) {
+__global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites,
+                              uint32_t bind_hi, uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3) {
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n_sites) return;
   const SiteRow r = rows[s];
@@ -799,7 +799,7 @@ __global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t
     Sip32 st{static_cast<uint32_t>(v0), static_cast<uint32_t>(v0 >> 32), static_cast<uint32_t>(v1),
              static_cast<uint32_t>(v1 >> 32), static_cast<uint32_t>(v2), static_cast<uint32_t>(v2 >> 32),
              static_cast<uint32_t>(v3), static_cast<uint32_t>(v3 >> 32)};
-    sip_absorb(st, s, 0u);  // LE64(zero-extended site_id) (R3, R5)
+    sip_absorb(st, s, bind_hi);  // LE64(site_id | digest32 << 32): zero-extended site id unless bound (R3, R5, R39)
     sip_qA(st);             // quarter A of the continuation word's first round
     o.st[0] = st.v0l; o.st[1] = st.v0h; o.st[2] = st.v1l; o.st[3] = st.v1h;
     o.st[4] = st.v2l; o.st[5] = st.v2h; o.st[6] = st.v3l; o.st[7] = st.v3h;
@@ -897,10 +897,10 @@ cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
-                              uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st) {
+cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint32_t bind_hi,
+                              uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st) {
   if (n_sites == 0) return cudaSuccess;
-  wg_build_recs<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, rows, tgts, n_sites, v0, v1, v2, v3);
+  wg_build_recs<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, rows, tgts, n_sites, bind_hi, v0, v1, v2, v3);
   count_launch();
   return cudaGetLastError();
 }

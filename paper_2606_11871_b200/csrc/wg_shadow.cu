@@ -49,7 +49,7 @@ __device__ __forceinline__ void mac_full(const Params& p, uint32_t site, uint32_
   Sip32 s{static_cast<uint32_t>(p.v0), static_cast<uint32_t>(p.v0 >> 32), static_cast<uint32_t>(p.v1),
           static_cast<uint32_t>(p.v1 >> 32), static_cast<uint32_t>(p.v2), static_cast<uint32_t>(p.v2 >> 32),
           static_cast<uint32_t>(p.v3), static_cast<uint32_t>(p.v3 >> 32)};
-  sip_absorb(s, site, 0u);
+  sip_absorb(s, site, p.bind_hi);
   sip_absorb(s, vl, vh);
   sip_absorb(s, cl, ch);
   sip_finish(s, 0u, 0u, outl, outh);

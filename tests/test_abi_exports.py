@@ -51,3 +51,23 @@ def test_product_package_never_touches_the_oracle():
         if f.suffix in (".py", ".cu", ".cuh", ".h"):
             text = f.read_text()
             assert not re.search(r"^\s*(import|from)\s+oracle\b|wg_oracle|wgo_|#include\s+\"[^\"]*oracle", text, re.M), f
+
+
+def test_policy_digest_runs_on_the_host_and_equals_the_oracle():
+    """wg_policy_digest needs no GPU (load-time host code): it must equal the oracle's digest, itself pinned against
+    libcrypto in tests/test_oracle_metadata.py."""
+    import numpy as np
+
+    import oracle
+    from paper_2606_11871_b200 import binding as B
+    from paper_2606_11871_b200 import streams as S
+
+    for config in (1, 3):
+        pol = S.make_policy(config, "cpu")
+        assert B.wg_policy_digest(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1) == \
+            oracle.policy_digest(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1)
+    kind = np.array([0, 1, 2], dtype=np.uint8)
+    off = np.array([0, 0, 2, 2], dtype=np.uint32)
+    tg = np.array([16, 32], dtype=np.uint64)
+    a = B.wg_policy_digest(kind, off, tg, 1, 2)
+    assert a == oracle.policy_digest(kind, off, tg, 1, 2) and a != B.wg_policy_digest(kind, off, tg, 1, 3)

@@ -187,3 +187,55 @@ def test_metadata_integrity_matches_the_oracle_with_and_without_corruption(confi
     t = eng.wg_read_telemetry()[0]
     assert t == orc.read_telemetry() and t["fwd_meta_fail_events"] > 0
     eng.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# policy-digest binding (second half; R39)
+# ---------------------------------------------------------------------------------------------------------
+def test_bound_load_refuses_a_mismatch_and_binds_the_tokens():
+    st = S.make_stream(4, "cpu", n_events=60_007)
+    pol = st.policy
+    d = B.wg_policy_digest(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1)
+    assert d == oracle.policy_digest(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1)
+    eng = B.Engine(0).load(pol)                       # an ordinary engine first
+    with pytest.raises(B.WgError) as e:               # wrong digest: refused, the previous policy stays
+        eng.wg_load_policy(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1, d ^ 4, bound=True)
+    assert e.value.status == B.WG_ERR_BAD_POLICY
+    hdr, val = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    d_hdr, d_val = st.hdr.to(dev()), st.val.to(dev())
+    plain_orc = oracle_for(pol)
+    plain_tag = plain_orc.sign(hdr, val)
+    assert np.array_equal(eng.wg_sign_continuations(d_hdr, d_val).cpu().numpy().view(np.uint64), plain_tag)
+    # bound load: tokens, verdicts and counters equal the bound oracle's; plain tokens no longer verify
+    eng.wg_load_policy(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1, d, bound=True)
+    orc = oracle.Oracle(pol.kind, pol.tgt_off, pol.tgts, pol.k0, pol.k1, d, bound=True)
+    o_tag = orc.sign(hdr, val)
+    g_tag = eng.wg_sign_continuations(d_hdr, d_val)
+    assert np.array_equal(g_tag.cpu().numpy().view(np.uint64), o_tag) and not np.array_equal(o_tag, plain_tag)
+    tag_t = torch.from_numpy(o_tag.view(np.int64).copy())
+    st.apply_return_tamper(tag_t)
+    tagn = tag_t.numpy().view(np.uint64)
+    val = st.val.numpy().view(np.uint64)
+    for tags in (tagn, plain_tag):
+        o = orc.verify(hdr, val, tags, ENF)
+        g = eng.wg_verify_continuations(d_hdr, st.val.to(dev()), torch.from_numpy(tags.view(np.int64).copy()).to(dev()), ENF)
+        assert np.array_equal(g.cpu().numpy().view(np.uint32), o)
+    same_counters(eng, orc)
+    g, _ = eng.wg_read_counters()
+    assert g["ret_viol_events"] > g["ret_checks"] // 2          # the whole plain-token pass violated
+    # the shadow stack and the inline form use the same bound token
+    orc.shadow_configure(64, 2)
+    eng.wg_shadow_configure(64, 2)
+    sh = np.zeros((8, 2), dtype=np.uint64)
+    ret_site = int(np.nonzero(pol.kind == 0)[0][0])
+    sh[:, 0] = np.uint64(ret_site) | (np.uint64(0xFFFF) << np.uint64(32))
+    sh[:, 1] = (np.uint64(1) << np.uint64(48)) | (np.arange(8, dtype=np.uint64) << np.uint64(5))
+    sv = np.full((8, 32), 0x7F5A40000040, dtype=np.uint64)
+    to = lambda a: torch.from_numpy(a.view(np.int64)).to(dev())
+    assert np.array_equal(eng.wg_shadow_push(to(sh), to(sv), ENF).cpu().numpy().view(np.uint32), orc.shadow_push(sh, sv, ENF))
+    assert np.array_equal(eng.wg_shadow_check_ret(to(sh), to(sv), ENF).cpu().numpy().view(np.uint32), orc.shadow_check_ret(sh, sv, ENF))
+    assert eng.wg_shadow_read_counters() == orc.shadow_read_counters() and orc.shadow_read_counters()["viol_lanes"] == 0
+    # an ordinary load drops the binding again
+    eng.load(pol)
+    assert np.array_equal(eng.wg_sign_continuations(d_hdr, d_val).cpu().numpy().view(np.uint64), plain_tag)
+    eng.close()
