@@ -501,3 +501,34 @@ def test_public_code_shaped_streams(config):
         assert (out[b0:b0 + 64, 1] == 0).all()                      # enforce: the whole burst is blocked
         assert g["first_violation_key"] >> 5 == b0
     eng.close()
+
+
+@pytest.mark.parametrize("config", [2, 3])
+def test_configs_2_and_3_full_size_sampled_against_the_oracle(config):
+    """BASELINE.json configs 2 (4 M backward-only events) and 3 (16 M forward-only events) at full size: counters show
+    exactly the planned corruption; a random sample plus every corrupted event is re-judged by the oracle."""
+    st = S.make_stream(config, dev())
+    n = st.hdr.shape[0]
+    assert n == S.FULL_EVENTS[config]
+    eng = engine_for(st.policy)
+    tag = eng.wg_sign_continuations(st.hdr, st.val)
+    g = torch.Generator(device="cpu").manual_seed(config)
+    idx = torch.unique(torch.cat([torch.randint(0, n, (80_000,), generator=g), st.ret_tamper.ev.cpu(),
+                                  st.fwd_tamper.ev.cpu(), torch.arange(n - 50, n)])).to(dev())
+    clean_tag = tag[idx].cpu().numpy().view(np.uint64)
+    st.apply_return_tamper(tag)
+    out = eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode)
+    gc, gs = eng.wg_read_counters()
+    assert gc["events_total"] == n and gc["ret_checks"] + gc["fwd_checks"] + gc["events_empty"] == n
+    assert gc["ret_viol_events"] == len(st.ret_tamper) and gc["fwd_viol_events"] == len(st.fwd_tamper)
+    assert int(gs[:, 0].sum()) == n and int(gs[:, 1].sum()) == gc["ret_lanes"] + gc["fwd_lanes"]
+    if config == 3:
+        assert gc["blocked_lanes"] == 0 and bool((out[:, 1] == (st.hdr[:, 0] >> 32).to(torch.int32)).all())  # detect
+    orc = oracle_for(st.policy)
+    hdr_s = st.hdr[idx].cpu().numpy().view(np.uint64)
+    val_s = st.val[idx].cpu().numpy().view(np.uint64)
+    tag_s = tag[idx].cpu().numpy().view(np.uint64)
+    touched = np.isin(idx.cpu().numpy(), st.ret_tamper.ev.cpu().numpy())
+    assert np.array_equal(orc.sign(hdr_s, val_s)[~touched], clean_tag[~touched])
+    assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), orc.verify(hdr_s, val_s, tag_s, st.mode))
+    eng.close()
