@@ -92,6 +92,17 @@ __device__ __forceinline__ uint4 ldg_v4(const void* p) {
 __device__ __forceinline__ void st_stream_v2(void* p, uint32_t a, uint32_t b) {
   asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(p), "r"(a), "r"(b) : "memory");
 }
+// tag row store of the sign kernels: the token for an active lane, zero for an inactive one (R10), as two
+// predicated stores (one ALU-pipe instruction for the predicate instead of two selects)
+__device__ __forceinline__ void st_tag_or_zero(void* p, uint32_t on, uint32_t lo, uint32_t hi) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\t"
+      "setp.ne.u32 q, %3, 0;\n\t"
+      "@q st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};\n\t"
+      "@!q st.global.L1::no_allocate.v2.u32 [%0], {%4,%4};\n\t}" ::"l"(p),
+      "r"(lo), "r"(hi), "r"(on), "r"(0u)
+      : "memory");
+}
 __device__ __forceinline__ void st_stream_v4(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d)
                : "memory");
@@ -378,6 +389,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
   while (t < n_tiles) {
     const uint64_t tn = t + stride;
     const uint64_t e0 = t * kT;
+    uint64_t* const tag_out_lane = (MODE == MODE_SIGN) ? p.tag_out + (e0 * 32 + lane) : nullptr;  // this lane's column
     // ---- event-parallel: decode, gather, classify (a1, a2) ----
     const TileEv ev = classify<MODE, TEL>(p, warp_s + L::kRaw + rb * kT * 16, dec_s, t, lane);
     const uint32_t m_ret = __ballot_sync(kFull, ev.cls == CLS_RET);
@@ -604,8 +616,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       uint32_t dl, dh;
       if constexpr (MODE == MODE_SIGN) {
         sip_tail_lane(s, lane, h.z, h.w, 0u, 0u, dl, dh);
-        const bool on = h.y & lanebit;
-        st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
+        st_tag_or_zero(tag_out_lane + e * 32, h.y & lanebit, dl, dh);
       } else {
         const uint2 tg = lds_v2(mad32(e, 256u, tag_lane_s));
         sip_tail_lane(s, lane, h.z, h.w, tg.x, tg.y, dl, dh);
@@ -623,8 +634,7 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       uint32_t dl, dh;
       if constexpr (MODE == MODE_SIGN) {
         sip_tail_val_lane(s, v.x, v.y, lane, h.z, h.w, 0u, 0u, dl, dh);
-        const bool on = h.y & lanebit;
-        st_stream_v2(p.tag_out + ((e0 + e) * 32 + lane), on ? dl : 0u, on ? dh : 0u);
+        st_tag_or_zero(tag_out_lane + e * 32, h.y & lanebit, dl, dh);
       } else {
         const uint2 tg = lds_v2(mad32(e, 256u, tag_lane_s));
         sip_tail_val_lane(s, v.x, v.y, lane, h.z, h.w, tg.x, tg.y, dl, dh);
