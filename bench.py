@@ -63,7 +63,8 @@ def parse_args():
     ap.add_argument("--batches", type=int, default=0,
                     help="config 5 only: stream that many 8 M-event batches (BASELINE.json: 64 = 512 M events), "
                          "alternating detect / enforce, and report the summed kernel time")
-    ap.add_argument("--sparse", action="store_true", help="wg_set_tuning(WG_TUNE_SPARSE_LANES) for the timed calls")
+    ap.add_argument("--dense", action="store_true", help="wg_set_tuning(WG_TUNE_DENSE_LANES) for the timed calls")
+    ap.add_argument("--sparse", action="store_true", help="accepted for compatibility: per-tile lane compaction is the default")
     ap.add_argument("--shadow", action="store_true",
                     help="also time the stateful shadow stack (SURVEY 8(f-1)): one lock-step push + check_ret over 1 Mi warps")
     return ap.parse_args()
@@ -249,8 +250,8 @@ def run_ours(a) -> None:
     st.apply_return_tamper(tag)                               # then the recorded corruption
     if a.profile:
         eng.wg_set_profile(a.profile)
-    if a.sparse:
-        eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
+    if a.dense:
+        eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
     tag_scratch = torch.empty_like(tag)
     out = torch.empty((n_events, 2), dtype=torch.int32, device=dev)
     fwd_ops = forward_search_ops(st, torch)
@@ -497,8 +498,8 @@ def run_config5_stream(a) -> None:
     dev = torch.device("cuda", 0)
     pol = S.make_policy(5, dev)
     eng = B.Engine(0).load(pol)
-    if a.sparse:
-        eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
+    if a.dense:
+        eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
     sign_ms = verify_ms = 0.0
     planned_ret = planned_fwd = events = 0
     out = tag = None
@@ -537,7 +538,7 @@ def run_config5_stream(a) -> None:
         "checks_per_sec_sign_plus_verify": checks / ((sign_ms + verify_ms) * 1e-3),
         "violations_found": {"ret_events": g["ret_viol_events"], "fwd_events": g["fwd_viol_events"],
                              "planned_ret": planned_ret, "planned_fwd": planned_fwd},
-        "blocked_lanes": g["blocked_lanes"], "sparse_lanes": bool(a.sparse), "n_sites": pol.n_sites,
+        "blocked_lanes": g["blocked_lanes"], "dense_lanes_only": bool(a.dense), "n_sites": pol.n_sites,
         "n_targets": int(pol.tgt_off[-1])}))
     eng.close()
 

@@ -31,7 +31,7 @@ EXPORTS = [
     "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_set_tuning", "wg_policy_digest",
     "wg_load_policy_bound",
 ]
-WG_TUNE_DEFAULT, WG_TUNE_SPARSE_LANES = 0, 1
+WG_TUNE_DEFAULT, WG_TUNE_SPARSE_LANES, WG_TUNE_DENSE_LANES = 0, 1, 2
 
 
 class DeviceView(C.Structure):

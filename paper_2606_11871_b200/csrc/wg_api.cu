@@ -148,7 +148,7 @@ wg::Params base_params(const wg_engine* e) {
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
   p.bind_hi = e->bind_hi;
-  p.sparse = (e->tuning & WG_TUNE_SPARSE_LANES) ? 1u : 0u;
+  p.sparse = (e->tuning & WG_TUNE_DENSE_LANES) ? 0u : 1u;
   p.ring = e->d_ring;
   p.ring_cap = e->d_ring ? e->ring_cap : 0;
   p.first = e->d_first;
@@ -662,7 +662,7 @@ wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
 
 wg_status wg_set_tuning(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;
-  if (flags & ~static_cast<uint32_t>(WG_TUNE_SPARSE_LANES)) return WG_ERR_INVALID_ARG;
+  if (flags & ~static_cast<uint32_t>(WG_TUNE_SPARSE_LANES | WG_TUNE_DENSE_LANES)) return WG_ERR_INVALID_ARG;
   eng->tuning = flags;
   return WG_OK;
 }

@@ -436,9 +436,11 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     const uint32_t na = __popc(ev.active);
     const uint32_t judged_na = (ev.cls == CLS_RET || ev.cls == CLS_FWD) ? na : 0u;
     unsigned long long* sc = p.site + static_cast<uint64_t>(ev.site) * 4;
+    uint32_t tile_ret_lanes = 0;  // active lanes over the tile's return events
     if constexpr (MODE == MODE_SIGN) {
       const bool is_ret = known && ev.kind == K_RET;
-      c.signed_lanes += __reduce_add_sync(kFull, is_ret ? na : 0u);
+      tile_ret_lanes = __reduce_add_sync(kFull, is_ret ? na : 0u);
+      c.signed_lanes += tile_ret_lanes;
       c.skipped += __popc(__ballot_sync(kFull, valid && !is_ret));
     } else {
       c.total += __popc(__ballot_sync(kFull, valid));
@@ -449,7 +451,8 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       }
       c.ret_checks += __popc(m_ret);
       c.fwd_checks += __popc(m_fwd);
-      c.ret_lanes += __reduce_add_sync(kFull, ev.cls == CLS_RET ? na : 0u);
+      tile_ret_lanes = __reduce_add_sync(kFull, ev.cls == CLS_RET ? na : 0u);
+      c.ret_lanes += tile_ret_lanes;
       c.fwd_lanes += __reduce_add_sync(kFull, ev.cls == CLS_FWD ? na : 0u);
       if (known) atomicAdd(&bykind[ev.kind], 1u);
       if (TEL && (p.profile & (PROFILE_SKIP_FORWARD | PROFILE_SKIP_BACKWARD))) {
@@ -556,7 +559,9 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     }
     __syncwarp();
 
-    if constexpr (SPARSE && MODE != MODE_FORWARD) {
+    // the sparse instantiation decides per tile: compaction pays when at least a quarter of the lanes of the
+    // tile's return events are idle (the list costs ~8 instructions per event, a saved pass ~200)
+    if (SPARSE && MODE != MODE_FORWARD && tile_ret_lanes * 4u <= 96u * static_cast<uint32_t>(__popc(m_ret))) {
       // ---- sparse path: work items = the ACTIVE lanes of the tile's return events, uniform events from the front
       //      of the list, divergent ones from the back; 32 items per pass whatever event they belong to ----
       uint32_t n_u = 0, n_d = 0;

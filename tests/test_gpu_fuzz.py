@@ -84,7 +84,7 @@ def test_random_policies_and_streams(seed, n_sites, n_tgts, n):
         orc.set_profile(flags)
         eng.wg_set_profile(flags)
         if trial == 1:
-            eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
+            eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
         if trial >= 2:
             orc.set_ring_capacity(64)
             eng.wg_set_ring_capacity(64)

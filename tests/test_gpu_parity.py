@@ -466,13 +466,14 @@ def test_config5_full_size_policy_one_batch_sampled_against_the_oracle():
 
 
 @pytest.mark.parametrize("config,n", [(5, 70_001), (4, 100_003), (1, 65_536), (2, 33)])
-def test_sparse_lane_tuning_changes_no_result(config, n, monkeypatch):
-    """WG_TUNE_SPARSE_LANES (compacted (event, lane) work items) must give the oracle's tags, verdicts and counters."""
+def test_dense_lane_tuning_changes_no_result(config, n, monkeypatch):
+    """WG_TUNE_DENSE_LANES (the kernels without the per-tile lane compaction, which is the default and is what every
+    other test runs) must give the oracle's tags, verdicts and counters too."""
     orig_load = B.Engine.load
 
     def load_sparse(self, policy):
         eng = orig_load(self, policy)
-        eng.wg_set_tuning(B.WG_TUNE_SPARSE_LANES)
+        eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
         return eng
 
     monkeypatch.setattr(B.Engine, "load", load_sparse)
