@@ -41,7 +41,7 @@ OPS_PER_MAC_SIGN = 308
 # bytes per event
 B_RET_VERIFY, B_RET_SIGN, B_FWD, B_NON = 536, 528, 280, 24
 # traffic of the dominant kernel from the committed ncu --set full capture (profiles/); None until captured
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 24_772_144_000  # profiles/r01_v2_tile_ncu.md: 24.2774 GB read + 0.4948 GB written, 58 M-event launch
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 24_772_875_000  # profiles/r01_v2_tile_ncu.md: 24.2775 GB read + 0.4954 GB written, 58 M-event launch
 
 
 def parse_args():
