@@ -162,9 +162,6 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint
 __device__ __forceinline__ void tma_prefetch_l2(const void* src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
 __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
   asm volatile(
       "{\n\t.reg .pred p;\n"
@@ -433,22 +430,6 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
       }
     }
 
-    // a target table too large for shared memory is searched from L2 / HBM, every probe a dependent ~1 us load:
-    // the probes of the first search step depend on the site only, so they are pulled into L2 while the rows fly
-    if constexpr (!STAGED && MODE != MODE_SIGN) {
-      if (ev.cls == CLS_FWD) {
-        const uint64_t* set = p.tgts + ev.off;
-        if (ev.cnt > 8u) {
-          const uint32_t q = ev.cnt >> 2;
-          prefetch_l2(set + q);
-          prefetch_l2(set + 2u * q);
-          prefetch_l2(set + 3u * q);
-        } else {
-          prefetch_l2(set + (ev.cnt >> 1));
-        }
-      }
-    }
-
     // ---- while the rows fly: everything of the epilogue that does not depend on a verdict (a7) ----
     const bool valid = ev.cls != CLS_NONE;
     const bool known = valid && ev.kind < 7u;
@@ -507,18 +488,6 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
 
     mbar_wait(mbar, phase);  // rows (and the next raw headers) have landed
     phase ^= 1u;
-    // large policies (the same instantiation): the next tile's site records are pulled into L2 now, so that its
-    // gather does not start with a DRAM round trip
-    if constexpr (!STAGED) {
-      if (tn < n_tiles && lane < kT && tn * kT + lane < p.n) {
-        const uint32_t site = lds_u32(warp_s + L::kRaw + (rb ^ 1u) * kT * 16 + lane * 16);
-        if (site < p.n_sites) {
-          const char* r = reinterpret_cast<const char*>(p.recs + site);
-          prefetch_l2(r);
-          prefetch_l2(r + 32);
-        }
-      }
-    }
 
     // ---- which events carry one warp-uniform value?  (a5 dedupe)  Unrolled over the tile:
     //      three independent shared-memory loads and ~6 ALU instructions per event, one REDUX per tile ----
