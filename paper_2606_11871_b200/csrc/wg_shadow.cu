@@ -61,6 +61,18 @@ enum ShWord {  // wg_shadow_counters
   SH_NON_RETURN, SH_SLOT_OVERFLOW, SH_SLOT_CONFLICT, SH_VIOL_LANES, SH_VIOL_EVENTS, SH_BLOCKED_LANES, SH_WORDS
 };
 
+// what an event needs from memory, in the order it can be asked for: the header; then what the header addresses
+// (site record, use count of the warp slot, the lane's value and depth counter); then (check) the entry the depth
+// counter addresses.  Every load is a dependent HBM / L2 round trip, so the kernel keeps three events in flight per
+// warp: while event k is computed, the entry of k+1, the header-addressed words of k+2 and the header of k+3 fly.
+struct StageB {
+  uint4 rec0, sb, sc;  // SiteRec: {kind, off, cnt, -}; pre-A mid-state after the site word
+  uint32_t uses, d, vl, vh;
+};
+struct StageE {
+  uint32_t exl, exh, tkl, tkh, callsite, depth;
+};
+
 template <bool PUSH>
 __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, const ShadowState sh) {
   __shared__ unsigned long long sm[SH_WORDS];
@@ -72,8 +84,60 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
 #pragma unroll
   for (int i = 0; i < SH_WORDS; ++i) c[i] = 0;
 
+  auto load_h = [&](uint64_t e) -> uint4 { return e < p.n ? __ldg(reinterpret_cast<const uint4*>(p.hdr) + e) : make_uint4(0u, 0u, 0u, 0u); };
+  auto load_b = [&](const uint4& h, uint64_t e) -> StageB {
+    StageB b;
+    b.rec0 = make_uint4(7u, 0u, 0u, 0u);
+    b.sb = b.sc = make_uint4(0u, 0u, 0u, 0u);
+    b.uses = b.d = b.vl = b.vh = 0u;
+    if (e < p.n && h.y != 0u) {
+      const uint32_t slot = slot_of(h.z, h.w);
+      const bool on = (h.y >> lane) & 1u;
+      if (h.x < p.n_sites) {
+        const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
+        b.rec0 = __ldg(r);
+        b.sb = __ldg(r + 1);
+        b.sc = __ldg(r + 2);
+      }
+      if (slot < sh.n_slots) {
+        b.uses = sh.uses[slot];
+        if (on) b.d = sh.depth_ctr[static_cast<uint64_t>(slot) * 32 + lane];
+      }
+      if (on) {
+        const uint2 v = *reinterpret_cast<const uint2*>(p.val + e * 32 + lane);
+        b.vl = v.x;
+        b.vh = v.y;
+      }
+    }
+    return b;
+  };
+  auto load_e = [&](const uint4& h, const StageB& b) -> StageE {
+    StageE x{0u, 0u, 0u, 0u, 0u, 0u};
+    if constexpr (!PUSH) {
+      const uint32_t slot = slot_of(h.z, h.w);
+      if (((h.y >> lane) & 1u) && slot < sh.n_slots && b.d != 0u && b.d - 1u < sh.max_depth) {
+        const uint64_t idx = (static_cast<uint64_t>(slot) * sh.max_depth + (b.d - 1u)) * 32 + lane;
+        const uint2 ex = *reinterpret_cast<const uint2*>(sh.expected + idx);
+        const uint2 tk = *reinterpret_cast<const uint2*>(sh.token + idx);
+        const uint2 m = sh.meta[idx];
+        x = StageE{ex.x, ex.y, tk.x, tk.y, m.x, m.y};
+      }
+    }
+    return x;
+  };
+
+  // prologue: fill the pipeline
+  uint4 h0 = load_h(warp0), h1 = load_h(warp0 + nwarps), h2 = load_h(warp0 + 2 * nwarps);
+  StageB b0 = load_b(h0, warp0), b1 = load_b(h1, warp0 + nwarps);
+  StageE x0 = load_e(h0, b0);
+
   for (uint64_t e = warp0; e < p.n; e += nwarps) {
-    const uint4 h = p.hdr[e];
+    // loads of the events behind this one
+    const uint4 h3 = load_h(e + 3 * nwarps);
+    const StageB b2 = load_b(h2, e + 2 * nwarps);
+    const StageE x1 = load_e(h1, b1);
+
+    const uint4 h = h0;
     const uint32_t site = h.x, a = h.y;
     const uint32_t slot = slot_of(h.z, h.w);
     uint32_t viol = 0;
@@ -82,39 +146,34 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
     } else {
       c[PUSH ? SH_PUSH_EVENTS : SH_CHECK_EVENTS] += 1;
       c[PUSH ? SH_PUSH_LANES : SH_CHECK_LANES] += __popc(a);
-      uint4 rec0 = make_uint4(7u, 0u, 0u, 0u);
-      if (site < p.n_sites) rec0 = __ldg(reinterpret_cast<const uint4*>(p.recs + site));
-      if (rec0.x != K_RET) {  // unknown site, or not a return site of the policy: fail closed, state untouched
+      if (b0.rec0.x != K_RET) {  // unknown site, or not a return site of the policy: fail closed, state untouched
         viol = a;
         c[SH_NON_RETURN] += 1;
       } else if (slot >= sh.n_slots) {  // thread-slot overflow fails closed instead of wrapping
         viol = a;
         c[SH_SLOT_OVERFLOW] += 1;
-      } else if (sh.uses[slot] > 1u) {  // the same warp twice in one lock-step call
+      } else if (b0.uses > 1u) {  // the same warp twice in one lock-step call
         viol = a;
         c[SH_SLOT_CONFLICT] += 1;
       } else {
         const bool on = (a >> lane) & 1u;
-        const uint64_t v = on ? p.val[e * 32 + lane] : 0ull;
-        const uint32_t vl = static_cast<uint32_t>(v), vh = static_cast<uint32_t>(v >> 32);
+        const uint32_t vl = b0.vl, vh = b0.vh;
         uint32_t* dctr = sh.depth_ctr + static_cast<uint64_t>(slot) * 32 + lane;
-        uint32_t d = on ? *dctr : 0u;
+        uint32_t d = b0.d;
         uint32_t cause = 0;  // 0 ok, else SH_* word of the lane's one cause
+        const Sip32 s_site{b0.sb.x, b0.sb.y, b0.sb.z, b0.sb.w, b0.sc.x, b0.sc.y, b0.sc.z, b0.sc.w};  // pre-A state after the site word
         if (on) {
           if (PUSH) {
             if (d >= sh.max_depth) {
               cause = SH_OVERFLOW;
             } else {
-              const uint4 b = __ldg(reinterpret_cast<const uint4*>(p.recs + site) + 1);
-              const uint4 cc = __ldg(reinterpret_cast<const uint4*>(p.recs + site) + 2);
-              const Sip32 s{b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w};  // pre-A state after the site word
               // context: epoch<<48 | d<<37 | slot<<5 | lane (lane is injected by the tail)
               const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
               uint32_t tl, th;
-              sip_tail_val_lane(s, vl, vh, lane, bl, bh, 0u, 0u, tl, th);
+              sip_tail_val_lane(s_site, vl, vh, lane, bl, bh, 0u, 0u, tl, th);
               const uint64_t idx = (static_cast<uint64_t>(slot) * sh.max_depth + d) * 32 + lane;
-              sh.expected[idx] = v;
-              sh.token[idx] = (static_cast<uint64_t>(th) << 32) | tl;
+              *reinterpret_cast<uint2*>(sh.expected + idx) = make_uint2(vl, vh);
+              *reinterpret_cast<uint2*>(sh.token + idx) = make_uint2(tl, th);
               sh.meta[idx] = make_uint2(site, d);
               *dctr = d + 1;
             }
@@ -127,30 +186,21 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
               // a corrupted counter may point past the arrays' depth: such an entry does not exist -> depth mismatch
               if (d >= sh.max_depth) {
                 cause = SH_DEPTH_MISMATCH;
+              } else if (x0.depth != d) {
+                cause = SH_DEPTH_MISMATCH;
               } else {
-                const uint64_t idx = (static_cast<uint64_t>(slot) * sh.max_depth + d) * 32 + lane;
-                const uint64_t ex = sh.expected[idx], tk = sh.token[idx];
-                const uint2 m = sh.meta[idx];
-                if (m.y != d) {
-                  cause = SH_DEPTH_MISMATCH;
+                // the token is verified over the ENTRY's own fields under the event's epoch
+                const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
+                uint32_t tl, th;
+                if (x0.callsite == site) {  // the ordinary case: the site's cached mid-state saves the first word's rounds
+                  sip_tail_val_lane(s_site, x0.exl, x0.exh, lane, bl, bh, 0u, 0u, tl, th);
                 } else {
-                  // the token is verified over the ENTRY's own fields under the event's epoch
-                  const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
-                  uint32_t tl, th;
-                  if (m.x == site) {  // the ordinary case: the site's cached mid-state saves the first word's rounds
-                    const uint4 b = __ldg(reinterpret_cast<const uint4*>(p.recs + site) + 1);
-                    const uint4 cc = __ldg(reinterpret_cast<const uint4*>(p.recs + site) + 2);
-                    const Sip32 s{b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w};
-                    sip_tail_val_lane(s, static_cast<uint32_t>(ex), static_cast<uint32_t>(ex >> 32), lane, bl, bh, 0u,
-                                      0u, tl, th);
-                  } else {
-                    mac_full(p, m.x, static_cast<uint32_t>(ex), static_cast<uint32_t>(ex >> 32), bl | lane, bh, tl, th);
-                  }
-                  if (((static_cast<uint64_t>(th) << 32) | tl) != tk)
-                    cause = SH_TOKEN_MISMATCH;
-                  else if (ex != v || m.x != site)
-                    cause = SH_TARGET_MISMATCH;
+                  mac_full(p, x0.callsite, x0.exl, x0.exh, bl | lane, bh, tl, th);
                 }
+                if (tl != x0.tkl || th != x0.tkh)
+                  cause = SH_TOKEN_MISMATCH;
+                else if (x0.exl != vl || x0.exh != vh || x0.callsite != site)
+                  cause = SH_TARGET_MISMATCH;
               }
             }
           }
@@ -168,6 +218,13 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
       if (enforce) c[SH_BLOCKED_LANES] += __popc(viol);
     }
     if (lane == 0) p.out[e] = make_uint2(viol, enforce ? (a & ~viol) : a);
+
+    h0 = h1;
+    h1 = h2;
+    h2 = h3;
+    b0 = b1;
+    b1 = b2;
+    x0 = x1;
   }
 
   if (threadIdx.x < SH_WORDS) sm[threadIdx.x] = 0ull;
@@ -188,8 +245,18 @@ cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int
   const int grid_m = static_cast<int>(want_m < static_cast<uint64_t>(sm_count) * 8 ? want_m : sm_count * 8);
   wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, 0);
   count_launch();
+  // persistent warps, three events in flight each: exactly the blocks that are resident at once
+  static int per_sm[2] = {0, 0};
+  if (per_sm[push] == 0) {
+    int nb = 0;
+    const cudaError_t err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<true>, kThreads, 0)
+                                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<false>, kThreads, 0);
+    if (err != cudaSuccess) return err;
+    per_sm[push] = nb > 0 ? nb : 1;
+  }
   const uint64_t want = (p.n + kWarps - 1) / kWarps;
-  const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) * 8 ? want : sm_count * 8);
+  const uint64_t resident = static_cast<uint64_t>(sm_count) * per_sm[push];
+  const int grid = static_cast<int>(want < resident ? want : resident);
   if (push)
     wg_shadow_kernel<true><<<grid, kThreads, 0, st>>>(p, sh);
   else
