@@ -95,6 +95,24 @@ def test_random_call_return_sequences(n_slots, max_depth, n):
     eng.close()
 
 
+@pytest.mark.parametrize("n", [1, 2, 3, 7, 33])
+def test_calls_shorter_than_the_kernels_pipeline(n):
+    """The shadow kernels keep three events in flight per warp: calls with fewer events than that (and than one
+    block's warps) must still match the oracle, push then return, twice over."""
+    rng = np.random.default_rng(100 + n)
+    pol, orc, eng = pair(64, 2)
+    for rnd in range(3):  # the third push overflows the depth-2 stacks
+        hdr, _ = random_call(rng, pol, 64, n, slot_span=64, bad_site=0.0)
+        val = rng.integers(0, 1 << 16, size=(n, 32)).astype(np.uint64) * np.uint64(16) + np.uint64(0x7F5A40000000)
+        step(orc, eng, True, hdr, val, ENF)
+        if rnd == 1:
+            val = val.copy()
+            val[0, 5] ^= np.uint64(0x10)
+            step(orc, eng, False, hdr, val, DET)
+    same_state(orc, eng, rng, 64)
+    eng.close()
+
+
 def test_attacker_writes_and_replay_are_caught_like_the_oracle_says():
     rng = np.random.default_rng(5)
     n_slots, max_depth, n = 1024, 4, 900
