@@ -12,6 +12,8 @@
 // Mapping: one warp per event (the state access is a gather by warp slot; each lane owns its own stack).
 // A call is one lock-step step of DISTINCT warps: a counting pass marks warp slots that occur twice in the call
 // and those events fail closed; a clearing pass resets the marks.
+#include <cstdlib>
+
 #include "wg_internal.h"
 #include "../../include/warpguard_sip32.cuh"
 
@@ -238,6 +240,232 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
   if (threadIdx.x < SH_WORDS && sm[threadIdx.x]) atomicAdd(sh.counters + threadIdx.x, sm[threadIdx.x]);
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// Tile mapping (the default): a warp owns 16 consecutive events.  What the warp-per-event kernel above does once per
+// EVENT with all 32 lanes doing the same thing — header decode, SiteRec gather, use count, the fail-closed
+// classification, the event counters, the verdict store — is done here once per TILE with lane i <-> event i
+// ("event-parallel", as in wg_kernels_v2.cu); only the part that really is per thread slot (depth counter, value,
+// entry, MAC, compare) runs lane-parallel, one pass per ordinary event, fed from shared memory.  The per-lane loads
+// of a pass are dependent round trips (depth counter -> entry), so they are issued two passes (counter, value) and
+// one pass (entry) ahead; only those 9 registers rotate.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kST = 16;  // events per tile
+enum : uint32_t { ST_NONE = 0, ST_EMPTY, ST_NON_RETURN, ST_SLOT_OVERFLOW, ST_SLOT_CONFLICT, ST_NORMAL };
+
+struct TileSmem {
+  uint4 rec[kST];        // {active, slot, site, context hi without the depth: epoch<<16 | slot>>27}
+  uint4 st[kST][2];      // the site's pre-A mid-state
+};
+
+__device__ __forceinline__ uint32_t sm_addr(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ uint4 lds4(uint32_t a) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a));
+  return r;
+}
+
+template <bool PUSH>
+__global__ void __launch_bounds__(kThreads) wg_shadow_tile_kernel(const Params p, const ShadowState sh) {
+  __shared__ unsigned long long sm[SH_WORDS];
+  __shared__ __align__(16) TileSmem tiles[kWarps];
+  const uint32_t lane = threadIdx.x & 31;
+  const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
+  TileSmem& ts = tiles[warp];
+  const uint32_t rec_s = sm_addr(ts.rec), st_s = sm_addr(ts.st);
+  const uint64_t n_tiles = (p.n + kST - 1) / kST;
+  const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kWarps;
+  const bool enforce = p.mode != 0;
+  const uint32_t max_depth = sh.max_depth;
+  uint32_t c[SH_WORDS];
+#pragma unroll
+  for (int i = 0; i < SH_WORDS; ++i) c[i] = 0;
+
+  // lane-parallel loads of one pass.  S1: the lane's depth counter and value; S2 (check): the entry under the counter.
+  struct S1 { uint32_t d, vl, vh; };
+  auto load1 = [&](uint32_t i, uint64_t e0) -> S1 {
+    S1 r{0u, 0u, 0u};
+    if (i < static_cast<uint32_t>(kST)) {
+      const uint4 a = lds4(rec_s + i * 16);
+      if ((a.x >> lane) & 1u) {
+        r.d = sh.depth_ctr[static_cast<uint64_t>(a.y) * 32 + lane];
+        const uint2 v = *reinterpret_cast<const uint2*>(p.val + (e0 + i) * 32 + lane);
+        r.vl = v.x;
+        r.vh = v.y;
+      }
+    }
+    return r;
+  };
+  auto load2 = [&](uint32_t i, const S1& b) -> StageE {
+    StageE x{0u, 0u, 0u, 0u, 0u, 0u};
+    if constexpr (!PUSH) {
+      if (i < static_cast<uint32_t>(kST)) {
+        const uint4 a = lds4(rec_s + i * 16);
+        if (((a.x >> lane) & 1u) && b.d != 0u && b.d - 1u < max_depth) {
+          const uint64_t idx = (static_cast<uint64_t>(a.y) * max_depth + (b.d - 1u)) * 32 + lane;
+          const uint2 ex = *reinterpret_cast<const uint2*>(sh.expected + idx);
+          const uint2 tk = *reinterpret_cast<const uint2*>(sh.token + idx);
+          const uint2 m = sh.meta[idx];
+          x = StageE{ex.x, ex.y, tk.x, tk.y, m.x, m.y};
+        }
+      }
+    }
+    return x;
+  };
+  // index of the lowest set bit of m, or kST ("no pass") when m is empty
+  auto first = [](uint32_t m) -> uint32_t { return m ? static_cast<uint32_t>(__ffs(m)) - 1u : static_cast<uint32_t>(kST); };
+
+  for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * kWarps + warp; t < n_tiles; t += stride) {
+    const uint64_t e0 = t * kST;
+    // ---- event-parallel: header, site record, use count, classification, event counters ----
+    const uint64_t e = e0 + lane;
+    const bool valid = lane < static_cast<uint32_t>(kST) && e < p.n;
+    uint4 h = make_uint4(0u, 0u, 0u, 0u);
+    if (valid) h = __ldg(reinterpret_cast<const uint4*>(p.hdr) + e);
+    const uint32_t a = h.y, slot = slot_of(h.z, h.w);
+    uint32_t status = ST_NONE;
+    if (valid) {
+      status = ST_EMPTY;  // no lane executed the call / return
+      if (a != 0u) {
+        uint32_t kind = 7u;
+        const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
+        if (h.x < p.n_sites) kind = __ldg(r).x;
+        const uint32_t uses = slot < sh.n_slots ? sh.uses[slot] : 0u;
+        if (kind != K_RET) {
+          status = ST_NON_RETURN;  // unknown site, or not a return site of the policy: fail closed, state untouched
+        } else if (slot >= sh.n_slots) {
+          status = ST_SLOT_OVERFLOW;  // thread-slot overflow fails closed instead of wrapping
+        } else if (uses > 1u) {
+          status = ST_SLOT_CONFLICT;  // the same warp twice in one lock-step call
+        } else {
+          status = ST_NORMAL;
+          const uint4 sb = __ldg(r + 1), sc = __ldg(r + 2);
+          ts.rec[lane] = make_uint4(a, slot, h.x, (slot >> 27) | (h.w & 0xffff0000u));
+          ts.st[lane][0] = sb;
+          ts.st[lane][1] = sc;
+        }
+      }
+    }
+    uint32_t viol = (status >= ST_NON_RETURN && status <= ST_SLOT_CONFLICT) ? a : 0u;
+    const uint32_t m_norm = __ballot_sync(kFull, status == ST_NORMAL);
+    {
+      const uint32_t m_live = __ballot_sync(kFull, status >= ST_NON_RETURN);
+      c[PUSH ? SH_PUSH_EVENTS : SH_CHECK_EVENTS] += __popc(m_live);
+      c[PUSH ? SH_PUSH_LANES : SH_CHECK_LANES] += __reduce_add_sync(kFull, status >= ST_NON_RETURN ? __popc(a) : 0u);
+      if (__ballot_sync(kFull, status != ST_NORMAL && status != ST_NONE)) {  // uncommon events
+        c[SH_EMPTY_EVENTS] += __popc(__ballot_sync(kFull, status == ST_EMPTY));
+        c[SH_NON_RETURN] += __popc(__ballot_sync(kFull, status == ST_NON_RETURN));
+        c[SH_SLOT_OVERFLOW] += __popc(__ballot_sync(kFull, status == ST_SLOT_OVERFLOW));
+        c[SH_SLOT_CONFLICT] += __popc(__ballot_sync(kFull, status == ST_SLOT_CONFLICT));
+      }
+    }
+    __syncwarp();
+
+    // ---- lane-parallel: one pass per ordinary event (distinct warp slots, so the passes touch disjoint state) ----
+    uint32_t m = m_norm;
+    uint32_t i0 = first(m);
+    m &= m - 1u;
+    uint32_t i1 = first(m);
+    m = m ? (m & (m - 1u)) : 0u;
+    S1 b0 = load1(i0, e0), b1 = load1(i1, e0);
+    StageE x0 = load2(i0, b0);
+    while (i0 < static_cast<uint32_t>(kST)) {
+      const uint32_t i2 = first(m);
+      m = m ? (m & (m - 1u)) : 0u;
+      const S1 b2 = load1(i2, e0);
+      const StageE x1 = load2(i1, b1);
+
+      const uint4 ra = lds4(rec_s + i0 * 16);
+      const uint32_t act = ra.x, sl = ra.y, site = ra.z;
+      const bool on = (act >> lane) & 1u;
+      const uint32_t vl = b0.vl, vh = b0.vh;
+      uint32_t d = b0.d;
+      uint32_t cause = 0;  // 0 ok, else SH_* word of the lane's one cause
+      if (on) {
+        uint32_t* dctr = sh.depth_ctr + static_cast<uint64_t>(sl) * 32 + lane;
+        if (PUSH) {
+          if (d >= max_depth) {
+            cause = SH_OVERFLOW;
+          } else {
+            const uint4 s0 = lds4(st_s + i0 * 32), s1 = lds4(st_s + i0 * 32 + 16);
+            const Sip32 s_site{s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+            // context: epoch<<48 | d<<37 | slot<<5 | lane (lane is injected by the tail)
+            const uint32_t bl = sl << 5, bh = ra.w | (d << 5);
+            uint32_t tl, th;
+            sip_tail_val_lane(s_site, vl, vh, lane, bl, bh, 0u, 0u, tl, th);
+            const uint64_t idx = (static_cast<uint64_t>(sl) * max_depth + d) * 32 + lane;
+            *reinterpret_cast<uint2*>(sh.expected + idx) = make_uint2(vl, vh);
+            *reinterpret_cast<uint2*>(sh.token + idx) = make_uint2(tl, th);
+            sh.meta[idx] = make_uint2(site, d);
+            *dctr = d + 1;
+          }
+        } else {
+          if (d == 0) {
+            cause = SH_UNDERFLOW;
+          } else {
+            d -= 1;
+            *dctr = d;  // the return consumes the frame whatever the verdict (R33)
+            // a corrupted counter may point past the arrays' depth: such an entry does not exist -> depth mismatch
+            if (d >= max_depth) {
+              cause = SH_DEPTH_MISMATCH;
+            } else if (x0.depth != d) {
+              cause = SH_DEPTH_MISMATCH;
+            } else {
+              // the token is verified over the ENTRY's own fields under the event's epoch
+              const uint32_t bl = sl << 5, bh = ra.w | (d << 5);
+              uint32_t tl, th;
+              if (x0.callsite == site) {  // the ordinary case: the site's cached mid-state saves the first word's rounds
+                const uint4 s0 = lds4(st_s + i0 * 32), s1 = lds4(st_s + i0 * 32 + 16);
+                const Sip32 s_site{s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+                sip_tail_val_lane(s_site, x0.exl, x0.exh, lane, bl, bh, 0u, 0u, tl, th);
+              } else {
+                mac_full(p, x0.callsite, x0.exl, x0.exh, bl | lane, bh, tl, th);
+              }
+              if (tl != x0.tkl || th != x0.tkh)
+                cause = SH_TOKEN_MISMATCH;
+              else if (x0.exl != vl || x0.exh != vh || x0.callsite != site)
+                cause = SH_TARGET_MISMATCH;
+            }
+          }
+        }
+      }
+      const uint32_t vb = __ballot_sync(kFull, cause != 0);
+      if (vb) {  // rare: one cause per violating lane
+#pragma unroll
+        for (int k = SH_OVERFLOW; k <= SH_TARGET_MISMATCH; ++k) c[k] += __popc(__ballot_sync(kFull, cause == k));
+      }
+      if (lane == i0) viol = vb;  // event-parallel again below: lane i <-> event i
+
+      i0 = i1;
+      i1 = i2;
+      b0 = b1;
+      b1 = b2;
+      x0 = x1;
+    }
+
+    // ---- event-parallel: verdicts and violation counters ----
+    if (valid) p.out[e] = make_uint2(viol, enforce ? (a & ~viol) : a);
+    const uint32_t m_viol = __ballot_sync(kFull, viol != 0u);
+    if (m_viol) {
+      const uint32_t lanes = __reduce_add_sync(kFull, __popc(viol));
+      c[SH_VIOL_LANES] += lanes;
+      c[SH_VIOL_EVENTS] += __popc(m_viol);
+      if (enforce) c[SH_BLOCKED_LANES] += lanes;
+    }
+    __syncwarp();  // every lane is done with this tile's records before the next tile overwrites them
+  }
+
+  if (threadIdx.x < SH_WORDS) sm[threadIdx.x] = 0ull;
+  __syncthreads();
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < SH_WORDS; ++i)
+      if (c[i]) atomicAdd(sm + i, static_cast<unsigned long long>(c[i]));
+  }
+  __syncthreads();
+  if (threadIdx.x < SH_WORDS && sm[threadIdx.x]) atomicAdd(sh.counters + threadIdx.x, sm[threadIdx.x]);
+}
+
 }  // namespace
 
 cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st) {
@@ -245,22 +473,37 @@ cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int
   const int grid_m = static_cast<int>(want_m < static_cast<uint64_t>(sm_count) * 8 ? want_m : sm_count * 8);
   wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, 0);
   count_launch();
-  // persistent warps, three events in flight each: exactly the blocks that are resident at once
+  // persistent warps: exactly the blocks that are resident at once.  WG_SHADOW=v1 selects the warp-per-event
+  // kernel (measurement knob, like WG_IMPL=v1 for the check kernels).
+  static const bool v1 = [] { const char* s = std::getenv("WG_SHADOW"); return s && s[0] == 'v' && s[1] == '1'; }();
   static int per_sm[2] = {0, 0};
   if (per_sm[push] == 0) {
     int nb = 0;
-    const cudaError_t err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<true>, kThreads, 0)
-                                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<false>, kThreads, 0);
+    cudaError_t err;
+    if (v1)
+      err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<true>, kThreads, 0)
+                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<false>, kThreads, 0);
+    else
+      err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<true>, kThreads, 0)
+                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<false>, kThreads, 0);
     if (err != cudaSuccess) return err;
     per_sm[push] = nb > 0 ? nb : 1;
   }
-  const uint64_t want = (p.n + kWarps - 1) / kWarps;
+  const uint64_t units = v1 ? p.n : (p.n + kST - 1) / kST;  // a warp's unit of work: an event / a tile
+  const uint64_t want = (units + kWarps - 1) / kWarps;
   const uint64_t resident = static_cast<uint64_t>(sm_count) * per_sm[push];
   const int grid = static_cast<int>(want < resident ? want : resident);
-  if (push)
-    wg_shadow_kernel<true><<<grid, kThreads, 0, st>>>(p, sh);
-  else
-    wg_shadow_kernel<false><<<grid, kThreads, 0, st>>>(p, sh);
+  if (v1) {
+    if (push)
+      wg_shadow_kernel<true><<<grid, kThreads, 0, st>>>(p, sh);
+    else
+      wg_shadow_kernel<false><<<grid, kThreads, 0, st>>>(p, sh);
+  } else {
+    if (push)
+      wg_shadow_tile_kernel<true><<<grid, kThreads, 0, st>>>(p, sh);
+    else
+      wg_shadow_tile_kernel<false><<<grid, kThreads, 0, st>>>(p, sh);
+  }
   count_launch();
   wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, 1);
   count_launch();
