@@ -250,7 +250,18 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
 // of a pass are dependent round trips (depth counter -> entry), so they are issued two passes (counter, value) and
 // one pass (entry) ahead; only those 9 registers rotate.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kST = 16;  // events per tile
+// Tile size / block size sweep on B200 (1 Mi warps, depth 4; push / check_ret ms per call): 8 x 256 threads 0.55 / 0.60,
+// 16 x 128 0.55 / 0.58, 16 x 256 0.55 / 0.58, 32 x 128 0.58 / 0.58, 32 x 256 0.55 / 0.57, 32 x 512 0.54 / 0.55.
+#ifndef WG_SH_THREADS
+#define WG_SH_THREADS 512
+#endif
+#ifndef WG_SH_TILE
+#define WG_SH_TILE 32
+#endif
+constexpr int kST = WG_SH_TILE;  // events per tile (<= 32: one lane per event in the event-parallel phase)
+static_assert(kST == 8 || kST == 16 || kST == 32, "tile size");
+constexpr int kTileThreads = WG_SH_THREADS;
+constexpr int kTileWarps = kTileThreads / 32;
 enum : uint32_t { ST_NONE = 0, ST_EMPTY, ST_NON_RETURN, ST_SLOT_OVERFLOW, ST_SLOT_CONFLICT, ST_NORMAL };
 
 struct TileSmem {
@@ -266,15 +277,15 @@ __device__ __forceinline__ uint4 lds4(uint32_t a) {
 }
 
 template <bool PUSH>
-__global__ void __launch_bounds__(kThreads) wg_shadow_tile_kernel(const Params p, const ShadowState sh) {
+__global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Params p, const ShadowState sh) {
   __shared__ unsigned long long sm[SH_WORDS];
-  __shared__ __align__(16) TileSmem tiles[kWarps];
+  __shared__ __align__(16) TileSmem tiles[kTileWarps];
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
   TileSmem& ts = tiles[warp];
   const uint32_t rec_s = sm_addr(ts.rec), st_s = sm_addr(ts.st);
   const uint64_t n_tiles = (p.n + kST - 1) / kST;
-  const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kWarps;
+  const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kTileWarps;
   const bool enforce = p.mode != 0;
   const uint32_t max_depth = sh.max_depth;
   uint32_t c[SH_WORDS];
@@ -315,34 +326,59 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_tile_kernel(const Params p
   // index of the lowest set bit of m, or kST ("no pass") when m is empty
   auto first = [](uint32_t m) -> uint32_t { return m ? static_cast<uint32_t>(__ffs(m)) - 1u : static_cast<uint32_t>(kST); };
 
-  for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * kWarps + warp; t < n_tiles; t += stride) {
+  // event-parallel loads of a tile, in the order they can be asked for: the header; then what it addresses (site
+  // record, use count of the warp slot).  Two tiles ahead / one tile ahead, so a tile starts with both in registers.
+  struct TB { uint4 rec0, sb, sc; uint32_t uses; };
+  auto load_th = [&](uint64_t t) -> uint4 {
+    const uint64_t e = t * kST + lane;
+    return (t < n_tiles && lane < static_cast<uint32_t>(kST) && e < p.n) ? __ldg(reinterpret_cast<const uint4*>(p.hdr) + e)
+                                                                         : make_uint4(0u, 0u, 0u, 0u);
+  };
+  auto load_tb = [&](const uint4& h) -> TB {
+    TB b;
+    b.rec0 = make_uint4(7u, 0u, 0u, 0u);
+    b.sb = b.sc = make_uint4(0u, 0u, 0u, 0u);
+    b.uses = 0u;
+    if (h.y != 0u) {  // (a lane without an event holds a zero header)
+      if (h.x < p.n_sites) {
+        const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
+        b.rec0 = __ldg(r);
+        b.sb = __ldg(r + 1);
+        b.sc = __ldg(r + 2);
+      }
+      const uint32_t slot = slot_of(h.z, h.w);
+      if (slot < sh.n_slots) b.uses = sh.uses[slot];
+    }
+    return b;
+  };
+  const uint64_t t_first = static_cast<uint64_t>(blockIdx.x) * kTileWarps + warp;
+  uint4 h_cur = load_th(t_first), h_nxt = load_th(t_first + stride);
+  TB b_cur = load_tb(h_cur);
+
+  for (uint64_t t = t_first; t < n_tiles; t += stride) {
     const uint64_t e0 = t * kST;
+    const uint4 h_nn = load_th(t + 2 * stride);
+    const TB b_nxt = load_tb(h_nxt);
     // ---- event-parallel: header, site record, use count, classification, event counters ----
     const uint64_t e = e0 + lane;
     const bool valid = lane < static_cast<uint32_t>(kST) && e < p.n;
-    uint4 h = make_uint4(0u, 0u, 0u, 0u);
-    if (valid) h = __ldg(reinterpret_cast<const uint4*>(p.hdr) + e);
+    const uint4 h = h_cur;
     const uint32_t a = h.y, slot = slot_of(h.z, h.w);
     uint32_t status = ST_NONE;
     if (valid) {
       status = ST_EMPTY;  // no lane executed the call / return
       if (a != 0u) {
-        uint32_t kind = 7u;
-        const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
-        if (h.x < p.n_sites) kind = __ldg(r).x;
-        const uint32_t uses = slot < sh.n_slots ? sh.uses[slot] : 0u;
-        if (kind != K_RET) {
+        if (b_cur.rec0.x != K_RET) {
           status = ST_NON_RETURN;  // unknown site, or not a return site of the policy: fail closed, state untouched
         } else if (slot >= sh.n_slots) {
           status = ST_SLOT_OVERFLOW;  // thread-slot overflow fails closed instead of wrapping
-        } else if (uses > 1u) {
+        } else if (b_cur.uses > 1u) {
           status = ST_SLOT_CONFLICT;  // the same warp twice in one lock-step call
         } else {
           status = ST_NORMAL;
-          const uint4 sb = __ldg(r + 1), sc = __ldg(r + 2);
           ts.rec[lane] = make_uint4(a, slot, h.x, (slot >> 27) | (h.w & 0xffff0000u));
-          ts.st[lane][0] = sb;
-          ts.st[lane][1] = sc;
+          ts.st[lane][0] = b_cur.sb;
+          ts.st[lane][1] = b_cur.sc;
         }
       }
     }
@@ -453,6 +489,9 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_tile_kernel(const Params p
       if (enforce) c[SH_BLOCKED_LANES] += lanes;
     }
     __syncwarp();  // every lane is done with this tile's records before the next tile overwrites them
+    h_cur = h_nxt;
+    h_nxt = h_nn;
+    b_cur = b_nxt;
   }
 
   if (threadIdx.x < SH_WORDS) sm[threadIdx.x] = 0ull;
@@ -484,13 +523,14 @@ cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int
       err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<true>, kThreads, 0)
                  : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<false>, kThreads, 0);
     else
-      err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<true>, kThreads, 0)
-                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<false>, kThreads, 0);
+      err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<true>, kTileThreads, 0)
+                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<false>, kTileThreads, 0);
     if (err != cudaSuccess) return err;
     per_sm[push] = nb > 0 ? nb : 1;
   }
   const uint64_t units = v1 ? p.n : (p.n + kST - 1) / kST;  // a warp's unit of work: an event / a tile
-  const uint64_t want = (units + kWarps - 1) / kWarps;
+  const uint64_t wpb = v1 ? kWarps : kTileWarps;  // warps per block
+  const uint64_t want = (units + wpb - 1) / wpb;
   const uint64_t resident = static_cast<uint64_t>(sm_count) * per_sm[push];
   const int grid = static_cast<int>(want < resident ? want : resident);
   if (v1) {
@@ -500,9 +540,9 @@ cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int
       wg_shadow_kernel<false><<<grid, kThreads, 0, st>>>(p, sh);
   } else {
     if (push)
-      wg_shadow_tile_kernel<true><<<grid, kThreads, 0, st>>>(p, sh);
+      wg_shadow_tile_kernel<true><<<grid, kTileThreads, 0, st>>>(p, sh);
     else
-      wg_shadow_tile_kernel<false><<<grid, kThreads, 0, st>>>(p, sh);
+      wg_shadow_tile_kernel<false><<<grid, kTileThreads, 0, st>>>(p, sh);
   }
   count_launch();
   wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, 1);
