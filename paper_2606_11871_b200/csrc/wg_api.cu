@@ -25,7 +25,7 @@ struct wg_engine {
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
   wg::ViolRec* d_ring = nullptr;
   wg::FirstRec* d_first = nullptr;  // first-violation record + the key it belongs to
-  wg::ShadowState sh = {0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // stateful shadow stack
+  wg::ShadowState sh = {0, 0, nullptr, nullptr, nullptr, nullptr};  // stateful shadow stack
   int impl = 2;                   // 2 = tiled kernels (default); 1 = baseline warp-per-event kernels (WG_IMPL=v1)
   uint64_t* d_tgts = nullptr;
   unsigned long long* d_glob = nullptr;  // [C_WORDS]
@@ -106,12 +106,10 @@ void free_tables(wg_engine* e) {
 
 void free_shadow(wg_engine* e) {
   cudaFree(e->sh.depth_ctr);
-  cudaFree(e->sh.expected);
-  cudaFree(e->sh.token);
-  cudaFree(e->sh.meta);
+  cudaFree(e->sh.entry);
   cudaFree(e->sh.uses);
   cudaFree(e->sh.counters);
-  e->sh = wg::ShadowState{0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  e->sh = wg::ShadowState{0, 0, nullptr, nullptr, nullptr, nullptr};
 }
 
 void free_staging(wg_engine* e) {
@@ -553,12 +551,11 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   WG_CUDA(eng, cudaStreamSynchronize(st));
   free_shadow(eng);
-  wg::ShadowState sh = {n_warp_slots, max_depth, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  wg::ShadowState sh = {n_warp_slots, max_depth, nullptr, nullptr, nullptr, nullptr};
   const size_t lanes = static_cast<size_t>(n_warp_slots ? n_warp_slots : 1) * 32;
   const size_t entries = lanes * max_depth;
   cudaError_t err;
-  if ((err = cudaMalloc(&sh.depth_ctr, lanes * 4)) != cudaSuccess || (err = cudaMalloc(&sh.expected, entries * 8)) != cudaSuccess ||
-      (err = cudaMalloc(&sh.token, entries * 8)) != cudaSuccess || (err = cudaMalloc(&sh.meta, entries * 8)) != cudaSuccess ||
+  if ((err = cudaMalloc(&sh.depth_ctr, lanes * 4)) != cudaSuccess || (err = cudaMalloc(&sh.entry, entries * 24)) != cudaSuccess ||
       (err = cudaMalloc(&sh.uses, lanes / 32 * 4)) != cudaSuccess || (err = cudaMalloc(&sh.counters, 16 * 8)) != cudaSuccess) {
     eng->sh = sh;
     free_shadow(eng);
@@ -566,9 +563,7 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   }
   eng->sh = sh;
   WG_CUDA(eng, cudaMemsetAsync(sh.depth_ctr, 0, lanes * 4, st));
-  WG_CUDA(eng, cudaMemsetAsync(sh.expected, 0, entries * 8, st));
-  WG_CUDA(eng, cudaMemsetAsync(sh.token, 0, entries * 8, st));
-  WG_CUDA(eng, cudaMemsetAsync(sh.meta, 0, entries * 8, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.entry, 0, entries * 24, st));
   WG_CUDA(eng, cudaMemsetAsync(sh.uses, 0, lanes / 32 * 4, st));
   WG_CUDA(eng, cudaMemsetAsync(sh.counters, 0, 16 * 8, st));
   WG_CUDA(eng, cudaStreamSynchronize(st));
@@ -624,14 +619,14 @@ wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
   const size_t li = static_cast<size_t>(warp_slot) * 32 + lane;
-  const size_t ei = (static_cast<size_t>(warp_slot) * eng->sh.max_depth + entry_depth) * 32 + lane;
+  const size_t ei = (static_cast<size_t>(warp_slot) * eng->sh.max_depth + entry_depth) * 96 + lane;  // field rows at +0 / +32 / +64
   void* addr = nullptr;
   size_t bytes = 8;
   switch (field) {
-    case 0: addr = eng->sh.expected + ei; break;
-    case 1: addr = eng->sh.token + ei; break;
-    case 2: addr = reinterpret_cast<uint32_t*>(eng->sh.meta + ei); bytes = 4; break;
-    case 3: addr = reinterpret_cast<uint32_t*>(eng->sh.meta + ei) + 1; bytes = 4; break;
+    case 0: addr = eng->sh.entry + ei; break;
+    case 1: addr = eng->sh.entry + ei + 32; break;
+    case 2: addr = reinterpret_cast<uint32_t*>(eng->sh.entry + ei + 64); bytes = 4; break;
+    case 3: addr = reinterpret_cast<uint32_t*>(eng->sh.entry + ei + 64) + 1; bytes = 4; break;
     default: addr = eng->sh.depth_ctr + li; bytes = 4; break;
   }
   uint64_t v = 0;

@@ -115,9 +115,9 @@ struct Params {
 struct ShadowState {
   uint32_t n_slots, max_depth;
   uint32_t* depth_ctr;          // [n_slots][32]
-  uint64_t* expected;           // [n_slots][max_depth][32]
-  uint64_t* token;              // [n_slots][max_depth][32]
-  uint2* meta;                  // [n_slots][max_depth][32] {callsite_id, depth}
+  uint64_t* entry;              // [n_slots][max_depth][3][32]: expected_return, token, {callsite_id, depth} — the three
+                                // 256-byte field rows of one (slot, depth) are adjacent, so a lane reaches all three
+                                // from ONE 64-bit address with immediate offsets 0 / 256 / 512
   uint32_t* uses;               // [n_slots] occurrences of a warp slot in the current call
   unsigned long long* counters; // [16] wg_shadow_counters
 };
