@@ -162,4 +162,12 @@ __device__ __forceinline__ void sip_tail_val_lane(Sip32 s, uint32_t vl, uint32_t
   sip_finish(s, xl, xh, outl, outh);
 }
 
+// per-lane tail when the event's state already covers site and continuation and has quarter A of the next round
+// applied, but the context word (cl, ch) is the lane's own in every bit (shadow stack: the depth is part of it)
+__device__ __forceinline__ void sip_tail_ctx(Sip32 s, uint32_t cl, uint32_t ch, uint32_t xl, uint32_t xh,
+                                             uint32_t& outl, uint32_t& outh) {
+  sip_absorb_preA(s, cl, ch);
+  sip_finish(s, xl, xh, outl, outh);
+}
+
 }  // namespace wg

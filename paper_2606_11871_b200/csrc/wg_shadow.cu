@@ -266,12 +266,20 @@ enum : uint32_t { ST_NONE = 0, ST_EMPTY, ST_NON_RETURN, ST_SLOT_OVERFLOW, ST_SLO
 struct TileSmem {
   uint4 rec[kST];        // {active, slot, site, context hi without the depth: epoch<<16 | slot>>27}
   uint4 st[kST][2];      // the site's pre-A mid-state
+  uint4 ust[kST][2];     // the state after the site word AND the value of the event's first active lane (+ quarter A)
+  uint2 vf[kST];         // that value
 };
 
 __device__ __forceinline__ uint32_t sm_addr(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ uint4 lds4(uint32_t a) {
   uint4 r;
   asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a));
+  return r;
+}
+
+__device__ __forceinline__ uint2 lds2(uint32_t a) {
+  uint2 r;
+  asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(a));
   return r;
 }
 
@@ -282,9 +290,13 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
   const uint32_t lane = threadIdx.x & 31;
   const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
   TileSmem& ts = tiles[warp];
-  const uint32_t rec_s = sm_addr(ts.rec), st_s = sm_addr(ts.st);
+  const uint32_t rec_s = sm_addr(ts.rec), st_s = sm_addr(ts.st), ust_s = sm_addr(ts.ust), vf_s = sm_addr(ts.vf);
   const uint64_t n_tiles = (p.n + kST - 1) / kST;
   const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kTileWarps;
+  // the warp-uniform-value prefix (8 of 12 rounds per lane) is compiled into check_ret only: push waits on memory
+  // (its entry writes are partial sectors that DRAM read-fills), and the extra gather and shared memory made it
+  // slower there (0.539 -> 0.559 ms) while check_ret gained (0.544 -> 0.514 ms)
+  constexpr bool kFast = !PUSH;
   const bool enforce = p.mode != 0;
   const uint32_t max_depth = sh.max_depth;
   uint32_t c[SH_WORDS];
@@ -325,18 +337,25 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
 
   // event-parallel loads of a tile, in the order they can be asked for: the header; then what it addresses (site
   // record, use count of the warp slot).  Two tiles ahead / one tile ahead, so a tile starts with both in registers.
-  struct TB { uint4 rec0, sb, sc; uint32_t uses; };
+  struct TB { uint4 rec0, sb, sc; uint32_t uses, vfl, vfh; };
   auto load_th = [&](uint64_t t) -> uint4 {
     const uint64_t e = t * kST + lane;
     return (t < n_tiles && lane < static_cast<uint32_t>(kST) && e < p.n) ? __ldg(reinterpret_cast<const uint4*>(p.hdr) + e)
                                                                          : make_uint4(0u, 0u, 0u, 0u);
   };
-  auto load_tb = [&](const uint4& h) -> TB {
+  auto load_tb = [&](const uint4& h, uint64_t t) -> TB {
     TB b;
     b.rec0 = make_uint4(7u, 0u, 0u, 0u);
     b.sb = b.sc = make_uint4(0u, 0u, 0u, 0u);
-    b.uses = 0u;
+    b.uses = b.vfl = b.vfh = 0u;
     if (h.y != 0u) {  // (a lane without an event holds a zero header)
+      // the value of the event's first active lane: when every active lane carries it (a warp-uniform return
+      // address) its two SipRounds are done once per event, 32 events at a time, instead of once per lane
+      if constexpr (kFast) {
+        const uint2 vf = *reinterpret_cast<const uint2*>(p.val + (t * kST + lane) * 32 + (__ffs(h.y) - 1));
+        b.vfl = vf.x;
+        b.vfh = vf.y;
+      }
       if (h.x < p.n_sites) {
         const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
         b.rec0 = __ldg(r);
@@ -350,12 +369,12 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
   };
   const uint64_t t_first = static_cast<uint64_t>(blockIdx.x) * kTileWarps + warp;
   uint4 h_cur = load_th(t_first), h_nxt = load_th(t_first + stride);
-  TB b_cur = load_tb(h_cur);
+  TB b_cur = load_tb(h_cur, t_first);
 
   for (uint64_t t = t_first; t < n_tiles; t += stride) {
     const uint64_t e0 = t * kST;
     const uint4 h_nn = load_th(t + 2 * stride);
-    const TB b_nxt = load_tb(h_nxt);
+    const TB b_nxt = load_tb(h_nxt, t + stride);
     // ---- event-parallel: header, site record, use count, classification, event counters ----
     const uint64_t e = e0 + lane;
     const bool valid = lane < static_cast<uint32_t>(kST) && e < p.n;
@@ -376,7 +395,18 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
           ts.rec[lane] = make_uint4(a, slot, h.x, (slot >> 27) | (h.w & 0xffff0000u));
           ts.st[lane][0] = b_cur.sb;
           ts.st[lane][1] = b_cur.sc;
+          if constexpr (kFast) ts.vf[lane] = make_uint2(b_cur.vfl, b_cur.vfh);
         }
+      }
+    }
+    if constexpr (kFast) {  // the MAC prefix of a warp-uniform value, for all events of the tile at once (used by the passes that find
+       // every MAC-computing lane on that value; harmless garbage for the others)
+      Sip32 u{b_cur.sb.x, b_cur.sb.y, b_cur.sb.z, b_cur.sb.w, b_cur.sc.x, b_cur.sc.y, b_cur.sc.z, b_cur.sc.w};
+      sip_absorb_preA(u, b_cur.vfl, b_cur.vfh);
+      sip_qA(u);
+      if (status == ST_NORMAL) {
+        ts.ust[lane][0] = make_uint4(u.v0l, u.v0h, u.v1l, u.v1h);
+        ts.ust[lane][1] = make_uint4(u.v2l, u.v2h, u.v3l, u.v3h);
       }
     }
     uint32_t viol = (status >= ST_NON_RETURN && status <= ST_SLOT_CONFLICT) ? a : 0u;
@@ -395,6 +425,9 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
     __syncwarp();
 
     // ---- lane-parallel: one pass per ordinary event (distinct warp slots, so the passes touch disjoint state) ----
+    // (Unrolling this loop three times over three named register sets, so that no loaded register is ever copied
+    // before its pass, was measured: push 0.56 ms, check_ret 0.56 ms — no gain for push, whose loads wait on a
+    // DRAM that partial-sector entry writes keep busy, and a loss for check_ret through its register count.)
     uint32_t m = m_norm;
     uint32_t i0 = first(m);
     m &= m - 1u;
@@ -409,29 +442,23 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
       const StageE x1 = load2(i1, b1);
 
       const uint4 ra = lds4(rec_s + i0 * 16);
+      uint2 vf = make_uint2(0u, 0u);
+      if constexpr (kFast) vf = lds2(vf_s + i0 * 8);
       const uint32_t act = ra.x, sl = ra.y, site = ra.z;
       const bool on = (act >> lane) & 1u;
       const uint32_t vl = b0.vl, vh = b0.vh;
       uint32_t d = b0.d;
       uint32_t cause = 0;  // 0 ok, else SH_* word of the lane's one cause
+      // which lanes reach the MAC, and over which (callsite, value)
+      bool mac = false;
+      uint32_t ml = vl, mh = vh, msite = site;
+      uint32_t* dctr = sh.depth_ctr + static_cast<uint64_t>(sl) * 32 + lane;
       if (on) {
-        uint32_t* dctr = sh.depth_ctr + static_cast<uint64_t>(sl) * 32 + lane;
         if (PUSH) {
-          if (d >= max_depth) {
+          if (d >= max_depth)
             cause = SH_OVERFLOW;
-          } else {
-            const uint4 s0 = lds4(st_s + i0 * 32), s1 = lds4(st_s + i0 * 32 + 16);
-            const Sip32 s_site{s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
-            // context: epoch<<48 | d<<37 | slot<<5 | lane (lane is injected by the tail)
-            const uint32_t bl = sl << 5, bh = ra.w | (d << 5);
-            uint32_t tl, th;
-            sip_tail_val_lane(s_site, vl, vh, lane, bl, bh, 0u, 0u, tl, th);
-            uint2* en = reinterpret_cast<uint2*>(sh.entry + (static_cast<uint64_t>(sl) * max_depth + d) * 96 + lane);
-            en[0] = make_uint2(vl, vh);
-            en[32] = make_uint2(tl, th);
-            en[64] = make_uint2(site, d);
-            *dctr = d + 1;
-          }
+          else
+            mac = true;
         } else {
           if (d == 0) {
             cause = SH_UNDERFLOW;
@@ -439,27 +466,46 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
             d -= 1;
             *dctr = d;  // the return consumes the frame whatever the verdict (R33)
             // a corrupted counter may point past the arrays' depth: such an entry does not exist -> depth mismatch
-            if (d >= max_depth) {
-              cause = SH_DEPTH_MISMATCH;
-            } else if (x0.depth != d) {
+            if (d >= max_depth || x0.depth != d) {
               cause = SH_DEPTH_MISMATCH;
             } else {
-              // the token is verified over the ENTRY's own fields under the event's epoch
-              const uint32_t bl = sl << 5, bh = ra.w | (d << 5);
-              uint32_t tl, th;
-              if (x0.callsite == site) {  // the ordinary case: the site's cached mid-state saves the first word's rounds
-                const uint4 s0 = lds4(st_s + i0 * 32), s1 = lds4(st_s + i0 * 32 + 16);
-                const Sip32 s_site{s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
-                sip_tail_val_lane(s_site, x0.exl, x0.exh, lane, bl, bh, 0u, 0u, tl, th);
-              } else {
-                mac_full(p, x0.callsite, x0.exl, x0.exh, bl | lane, bh, tl, th);
-              }
-              if (tl != x0.tkl || th != x0.tkh)
-                cause = SH_TOKEN_MISMATCH;
-              else if (x0.exl != vl || x0.exh != vh || x0.callsite != site)
-                cause = SH_TARGET_MISMATCH;
+              mac = true;  // the token is verified over the ENTRY's own fields under the event's epoch
+              ml = x0.exl;
+              mh = x0.exh;
+              msite = x0.callsite;
             }
           }
+        }
+      }
+      // context: epoch<<48 | d<<37 | slot<<5 | lane
+      const uint32_t bl = sl << 5, bh = ra.w | (d << 5);
+      uint32_t tl = 0, th = 0;
+      if (kFast && __all_sync(kFull, !mac || (ml == vf.x && mh == vf.y && msite == site))) {
+        // the ordinary case: one return address for the whole warp — 8 of the 12 rounds per lane
+        if (mac) {
+          const uint4 s0 = lds4(ust_s + i0 * 32), s1 = lds4(ust_s + i0 * 32 + 16);
+          sip_tail_ctx(Sip32{s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w}, bl | lane, bh, 0u, 0u, tl, th);
+        }
+      } else if (mac) {
+        if (msite == site) {  // the site's cached mid-state saves the first word's rounds
+          const uint4 s0 = lds4(st_s + i0 * 32), s1 = lds4(st_s + i0 * 32 + 16);
+          sip_tail_val_lane(Sip32{s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w}, ml, mh, lane, bl, bh, 0u, 0u, tl, th);
+        } else {
+          mac_full(p, msite, ml, mh, bl | lane, bh, tl, th);
+        }
+      }
+      if (mac) {
+        if (PUSH) {
+          uint2* en = reinterpret_cast<uint2*>(sh.entry + (static_cast<uint64_t>(sl) * max_depth + d) * 96 + lane);
+          en[0] = make_uint2(vl, vh);
+          en[32] = make_uint2(tl, th);
+          en[64] = make_uint2(site, d);
+          *dctr = d + 1;
+        } else {
+          if (tl != x0.tkl || th != x0.tkh)
+            cause = SH_TOKEN_MISMATCH;
+          else if (x0.exl != vl || x0.exh != vh || x0.callsite != site)
+            cause = SH_TARGET_MISMATCH;
         }
       }
       const uint32_t vb = __ballot_sync(kFull, cause != 0);
