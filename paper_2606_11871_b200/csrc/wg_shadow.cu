@@ -557,8 +557,10 @@ cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int
   count_launch();
   // persistent warps: exactly the blocks that are resident at once.  WG_SHADOW=v1 selects the warp-per-event
   // kernel (measurement knob, like WG_IMPL=v1 for the check kernels).
-  static const bool v1 = [] { const char* s = std::getenv("WG_SHADOW"); return s && s[0] == 'v' && s[1] == '1'; }();
-  static int per_sm[2] = {0, 0};
+  const char* knob = std::getenv("WG_SHADOW");
+  const bool v1 = knob && knob[0] == 'v' && knob[1] == '1';
+  static int per_sm_tab[2][2] = {{0, 0}, {0, 0}};
+  int* per_sm = per_sm_tab[v1];
   if (per_sm[push] == 0) {
     int nb = 0;
     cudaError_t err;

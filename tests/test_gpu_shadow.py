@@ -95,6 +95,12 @@ def test_random_call_return_sequences(n_slots, max_depth, n):
     eng.close()
 
 
+def test_warp_per_event_shadow_kernels_stay_bit_exact(monkeypatch):
+    """WG_SHADOW=v1 selects the warp-per-event shadow kernels kept as the measured baseline: same results."""
+    monkeypatch.setenv("WG_SHADOW", "v1")
+    test_random_call_return_sequences(4096, 4, 3000)
+
+
 @pytest.mark.parametrize("n", [1, 2, 3, 7, 33])
 def test_calls_shorter_than_the_kernels_pipeline(n):
     """The shadow kernels keep three events in flight per warp: calls with fewer events than that (and than one
@@ -139,6 +145,45 @@ def test_attacker_writes_and_replay_are_caught_like_the_oracle_says():
     c = orc.shadow_read_counters()
     assert o1[:, 0].any() and c["token_mismatch_lanes"] > 0 and c["depth_mismatch_lanes"] > 0
     assert (o2[:, 1] == 0xFFFFFFFF).all()  # detect mode releases
+    eng.close()
+
+
+def test_warp_uniform_returns_with_attacker_writes():
+    """check_ret computes the MAC prefix of a warp-uniform return address once per event and falls
+    back to the per-lane prefix when any MAC-computing lane's entry disagrees with the first active lane's observed
+    value or with the event's site.  Uniform pushes, then every way of breaking that agreement — a hijacked first
+    active lane, a hijacked other lane, poked expected_return / token / callsite / depth / depth counter, a replay
+    under another epoch — against the oracle."""
+    rng = np.random.default_rng(77)
+    n_slots, max_depth, n = 2048, 3, 1500
+    pol, orc, eng = pair(n_slots, max_depth)
+    hdr, slots = random_call(rng, pol, n_slots, n, slot_span=n_slots, bad_site=0.0)
+    val = np.repeat(rng.integers(0, 1 << 20, size=(n, 1)).astype(np.uint64) * np.uint64(16) + np.uint64(0x7F5A40000000), 32, 1)
+    step(orc, eng, True, hdr, val, ENF)
+    step(orc, eng, True, hdr, val + np.uint64(32), ENF)
+    for i in range(200):
+        s, l, d = int(slots[rng.integers(0, n)]), int(rng.integers(0, 32)), int(rng.integers(0, 2))
+        field = int(rng.integers(0, 5))
+        x = int(rng.integers(1, 1 << 31)) if field >= 2 else int(rng.integers(1, 1 << 63))
+        if field == 4:
+            x = int(rng.integers(1, 4))
+        orc.shadow_poke(s, l, d, field, x)
+        eng.wg_shadow_poke(s, l, d, field, x)
+    obs = val + np.uint64(32)
+    masks = (hdr[:, 0] >> np.uint64(32)).astype(np.uint64)
+    first = np.array([(int(m) & -int(m)).bit_length() - 1 if m else 0 for m in masks])
+    hij = rng.random(n) < 0.05
+    obs[hij, first[hij]] ^= np.uint64(0x100)           # the first active lane returns somewhere else
+    hij2 = rng.random(n) < 0.05
+    obs[hij2, rng.integers(0, 32, int(hij2.sum()))] ^= np.uint64(0x80)  # some other lane does
+    o1 = step(orc, eng, False, hdr, obs, ENF)
+    hdr2 = hdr.copy()
+    hdr2[:, 1] += np.uint64(1) << np.uint64(48)       # the older frames replayed under another epoch
+    step(orc, eng, False, hdr2, val, DET)
+    same_state(orc, eng, rng, n_slots)
+    c = orc.shadow_read_counters()
+    assert o1[:, 0].any() and c["token_mismatch_lanes"] > 0 and c["target_mismatch_lanes"] > 0
+    assert c["depth_mismatch_lanes"] > 0
     eng.close()
 
 
