@@ -555,7 +555,7 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   const size_t lanes = static_cast<size_t>(n_warp_slots ? n_warp_slots : 1) * 32;
   const size_t entries = lanes * max_depth;
   cudaError_t err;
-  if ((err = cudaMalloc(&sh.depth_ctr, lanes * 4)) != cudaSuccess || (err = cudaMalloc(&sh.entry, entries * 24)) != cudaSuccess ||
+  if ((err = cudaMalloc(&sh.depth_ctr, lanes * 4)) != cudaSuccess || (err = cudaMalloc(&sh.entry, entries * 32)) != cudaSuccess ||
       (err = cudaMalloc(&sh.uses, lanes / 32 * 4)) != cudaSuccess || (err = cudaMalloc(&sh.counters, 16 * 8)) != cudaSuccess) {
     eng->sh = sh;
     free_shadow(eng);
@@ -563,7 +563,7 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   }
   eng->sh = sh;
   WG_CUDA(eng, cudaMemsetAsync(sh.depth_ctr, 0, lanes * 4, st));
-  WG_CUDA(eng, cudaMemsetAsync(sh.entry, 0, entries * 24, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.entry, 0, entries * 32, st));
   WG_CUDA(eng, cudaMemsetAsync(sh.uses, 0, lanes / 32 * 4, st));
   WG_CUDA(eng, cudaMemsetAsync(sh.counters, 0, 16 * 8, st));
   WG_CUDA(eng, cudaStreamSynchronize(st));
@@ -619,14 +619,14 @@ wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
   const size_t li = static_cast<size_t>(warp_slot) * 32 + lane;
-  const size_t ei = (static_cast<size_t>(warp_slot) * eng->sh.max_depth + entry_depth) * 96 + lane;  // field rows at +0 / +32 / +64
+  const size_t ei = ((static_cast<size_t>(warp_slot) * eng->sh.max_depth + entry_depth) * 32 + lane) * 4;  // the entry's sector
   void* addr = nullptr;
   size_t bytes = 8;
   switch (field) {
     case 0: addr = eng->sh.entry + ei; break;
-    case 1: addr = eng->sh.entry + ei + 32; break;
-    case 2: addr = reinterpret_cast<uint32_t*>(eng->sh.entry + ei + 64); bytes = 4; break;
-    case 3: addr = reinterpret_cast<uint32_t*>(eng->sh.entry + ei + 64) + 1; bytes = 4; break;
+    case 1: addr = eng->sh.entry + ei + 1; break;
+    case 2: addr = reinterpret_cast<uint32_t*>(eng->sh.entry + ei + 2); bytes = 4; break;
+    case 3: addr = reinterpret_cast<uint32_t*>(eng->sh.entry + ei + 2) + 1; bytes = 4; break;
     default: addr = eng->sh.depth_ctr + li; bytes = 4; break;
   }
   uint64_t v = 0;

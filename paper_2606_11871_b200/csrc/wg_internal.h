@@ -115,9 +115,10 @@ struct Params {
 struct ShadowState {
   uint32_t n_slots, max_depth;
   uint32_t* depth_ctr;          // [n_slots][32]
-  uint64_t* entry;              // [n_slots][max_depth][3][32]: expected_return, token, {callsite_id, depth} — the three
-                                // 256-byte field rows of one (slot, depth) are adjacent, so a lane reaches all three
-                                // from ONE 64-bit address with immediate offsets 0 / 256 / 512
+  uint64_t* entry;              // [n_slots][max_depth][32][4]: one 32-byte sector per thread slot and depth,
+                                // {expected_return, token, callsite_id | depth << 32, 0}: an active lane writes
+                                // its whole sector (two 16-byte stores the L2 merges), so DRAM never has to
+                                // read-fill a partially written one; inactive lanes' sectors are not touched
   uint32_t* uses;               // [n_slots] occurrences of a warp slot in the current call
   unsigned long long* counters; // [16] wg_shadow_counters
 };

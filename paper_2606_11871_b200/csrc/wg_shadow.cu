@@ -8,8 +8,8 @@
 // read from it is trusted before the token verifies.
 //
 // Layout (structure of arrays, so that the 32 lanes of a warp touch 256 contiguous bytes per field):
-//   depth_ctr[slot][32] u32;  entry[slot][d][field][32] u64, field = expected, token, {callsite, depth}: the three
-//   field rows of one (slot, depth) are adjacent (one 64-bit address per lane, immediate offsets 0 / 256 / 512).
+//   depth_ctr[slot][32] u32;  entry[slot][d][32][4] u64 = {expected, token, callsite | depth << 32, 0}: one 32-byte
+//   sector per thread slot and depth, written whole by its (active) lane.
 // Mapping: one warp per event (the state access is a gather by warp slot; each lane owns its own stack).
 // A call is one lock-step step of DISTINCT warps: a counting pass marks warp slots that occur twice in the call
 // and those events fail closed; a clearing pass resets the marks.
@@ -119,9 +119,9 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
     if constexpr (!PUSH) {
       const uint32_t slot = slot_of(h.z, h.w);
       if (((h.y >> lane) & 1u) && slot < sh.n_slots && b.d != 0u && b.d - 1u < sh.max_depth) {
-        const uint2* en = reinterpret_cast<const uint2*>(sh.entry + (static_cast<uint64_t>(slot) * sh.max_depth + (b.d - 1u)) * 96 + lane);
-        const uint2 ex = en[0], tk = en[32], m = en[64];
-        x = StageE{ex.x, ex.y, tk.x, tk.y, m.x, m.y};
+        const uint4* en = reinterpret_cast<const uint4*>(sh.entry) + ((static_cast<uint64_t>(slot) * sh.max_depth + (b.d - 1u)) * 32 + lane) * 2;
+        const uint4 et = en[0], m = en[1];
+        x = StageE{et.x, et.y, et.z, et.w, m.x, m.y};
       }
     }
     return x;
@@ -172,10 +172,9 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
               const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
               uint32_t tl, th;
               sip_tail_val_lane(s_site, vl, vh, lane, bl, bh, 0u, 0u, tl, th);
-              uint2* en = reinterpret_cast<uint2*>(sh.entry + (static_cast<uint64_t>(slot) * sh.max_depth + d) * 96 + lane);
-              en[0] = make_uint2(vl, vh);
-              en[32] = make_uint2(tl, th);
-              en[64] = make_uint2(site, d);
+              uint4* en = reinterpret_cast<uint4*>(sh.entry) + ((static_cast<uint64_t>(slot) * sh.max_depth + d) * 32 + lane) * 2;
+              en[0] = make_uint4(vl, vh, tl, th);
+              en[1] = make_uint4(site, d, 0u, 0u);
               *dctr = d + 1;
             }
           } else {
@@ -324,9 +323,9 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
       if (i < static_cast<uint32_t>(kST)) {
         const uint4 a = lds4(rec_s + i * 16);
         if (((a.x >> lane) & 1u) && b.d != 0u && b.d - 1u < max_depth) {
-          const uint2* en = reinterpret_cast<const uint2*>(sh.entry + (static_cast<uint64_t>(a.y) * max_depth + (b.d - 1u)) * 96 + lane);
-          const uint2 ex = en[0], tk = en[32], m = en[64];
-          x = StageE{ex.x, ex.y, tk.x, tk.y, m.x, m.y};
+          const uint4* en = reinterpret_cast<const uint4*>(sh.entry) + ((static_cast<uint64_t>(a.y) * max_depth + (b.d - 1u)) * 32 + lane) * 2;
+          const uint4 et = en[0], m = en[1];
+          x = StageE{et.x, et.y, et.z, et.w, m.x, m.y};
         }
       }
     }
@@ -496,10 +495,9 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
       }
       if (mac) {
         if (PUSH) {
-          uint2* en = reinterpret_cast<uint2*>(sh.entry + (static_cast<uint64_t>(sl) * max_depth + d) * 96 + lane);
-          en[0] = make_uint2(vl, vh);
-          en[32] = make_uint2(tl, th);
-          en[64] = make_uint2(site, d);
+          uint4* en = reinterpret_cast<uint4*>(sh.entry) + ((static_cast<uint64_t>(sl) * max_depth + d) * 32 + lane) * 2;
+          en[0] = make_uint4(vl, vh, tl, th);
+          en[1] = make_uint4(site, d, 0u, 0u);
           *dctr = d + 1;
         } else {
           if (tl != x0.tkl || th != x0.tkh)
