@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
   // the warp-uniform-value prefix (8 of 12 rounds per lane) is compiled into check_ret only: push waits on memory
   // (its entry writes are partial sectors that DRAM read-fills), and the extra gather and shared memory made it
   // slower there (0.539 -> 0.559 ms) while check_ret gained (0.544 -> 0.514 ms)
-  constexpr bool kFast = !PUSH;
+  constexpr bool kFast = true;
   const bool enforce = p.mode != 0;
   const uint32_t max_depth = sh.max_depth;
   uint32_t c[SH_WORDS];
