@@ -292,9 +292,9 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
   const uint32_t rec_s = sm_addr(ts.rec), st_s = sm_addr(ts.st), ust_s = sm_addr(ts.ust), vf_s = sm_addr(ts.vf);
   const uint64_t n_tiles = (p.n + kST - 1) / kST;
   const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kTileWarps;
-  // the warp-uniform-value prefix (8 of 12 rounds per lane) is compiled into check_ret only: push waits on memory
-  // (its entry writes are partial sectors that DRAM read-fills), and the extra gather and shared memory made it
-  // slower there (0.539 -> 0.559 ms) while check_ret gained (0.544 -> 0.514 ms)
+  // the warp-uniform-value prefix (8 of 12 rounds per lane): check_ret 0.544 -> 0.514 ms, push 0.500 -> 0.474 ms.
+  // (While the entry fields lived in three separate rows, push waited on DRAM read-filling its partially written
+  // sectors and the prefix made it slower, 0.539 -> 0.559 ms; the switch is kept for such measurements.)
   constexpr bool kFast = true;
   const bool enforce = p.mode != 0;
   const uint32_t max_depth = sh.max_depth;
@@ -425,8 +425,8 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
 
     // ---- lane-parallel: one pass per ordinary event (distinct warp slots, so the passes touch disjoint state) ----
     // (Unrolling this loop three times over three named register sets, so that no loaded register is ever copied
-    // before its pass, was measured: push 0.56 ms, check_ret 0.56 ms — no gain for push, whose loads wait on a
-    // DRAM that partial-sector entry writes keep busy, and a loss for check_ret through its register count.)
+    // before its pass, was measured with the earlier three-row entry layout: push 0.56 ms, check_ret 0.56 ms — no
+    // gain for push and a loss for check_ret through its register count.)
     uint32_t m = m_norm;
     uint32_t i0 = first(m);
     m &= m - 1u;
