@@ -450,8 +450,8 @@ def run_ours(a) -> None:
         assert csh["viol_lanes"] == 0 and csh["push_lanes"] == csh["check_lanes"]
         lanes = csh["push_lanes"] // 4
         push_ms, chk_ms = evs[0].elapsed_time(evs[1]), evs[1].elapsed_time(evs[2])
-        # bytes: header 16 + value row 256 + verdict 8 + per active lane: depth counter 4 r + 4 w, entry 24 (w or r)
-        byts = ns * 280 + lanes * 32
+        # bytes: header 16 + value row 256 + verdict 8 + per active lane: depth counter 4 r + 4 w, entry sector 32 (w or r)
+        byts = ns * 280 + lanes * 40
         shadow = {"warps_per_call": ns, "max_depth": depth, "lanes_per_call": int(lanes),
                   "push_ms": push_ms, "check_ret_ms": chk_ms, "launches_per_call": 3,
                   "push_lanes_per_sec": lanes / (push_ms * 1e-3), "check_lanes_per_sec": lanes / (chk_ms * 1e-3),
