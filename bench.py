@@ -453,7 +453,7 @@ def run_ours(a) -> None:
         # bytes: header 16 + value row 256 + verdict 8 + per active lane: depth counter 4 r + 4 w, entry sector 32 (w or r)
         byts = ns * 280 + lanes * 40
         shadow = {"warps_per_call": ns, "max_depth": depth, "lanes_per_call": int(lanes),
-                  "push_ms": push_ms, "check_ret_ms": chk_ms, "launches_per_call": 3,
+                  "push_ms": push_ms, "check_ret_ms": chk_ms, "launches_per_call": 2,
                   "push_lanes_per_sec": lanes / (push_ms * 1e-3), "check_lanes_per_sec": lanes / (chk_ms * 1e-3),
                   "push_alu_frac": OPS_PER_MAC_SIGN * lanes / (push_ms * 1e-3) / alu_peak,
                   "check_alu_frac": OPS_PER_MAC_VERIFY * lanes / (chk_ms * 1e-3) / alu_peak,

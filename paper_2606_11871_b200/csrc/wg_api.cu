@@ -556,7 +556,7 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   const size_t entries = lanes * max_depth;
   cudaError_t err;
   if ((err = cudaMalloc(&sh.depth_ctr, lanes * 4)) != cudaSuccess || (err = cudaMalloc(&sh.entry, entries * 32)) != cudaSuccess ||
-      (err = cudaMalloc(&sh.uses, lanes / 32 * 4)) != cudaSuccess || (err = cudaMalloc(&sh.counters, 16 * 8)) != cudaSuccess) {
+      (err = cudaMalloc(&sh.uses, lanes / 32 * 8)) != cudaSuccess || (err = cudaMalloc(&sh.counters, 16 * 8)) != cudaSuccess) {
     eng->sh = sh;
     free_shadow(eng);
     return cuda_fail(eng, err);
@@ -564,7 +564,7 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   eng->sh = sh;
   WG_CUDA(eng, cudaMemsetAsync(sh.depth_ctr, 0, lanes * 4, st));
   WG_CUDA(eng, cudaMemsetAsync(sh.entry, 0, entries * 32, st));
-  WG_CUDA(eng, cudaMemsetAsync(sh.uses, 0, lanes / 32 * 4, st));
+  WG_CUDA(eng, cudaMemsetAsync(sh.uses, 0, lanes / 32 * 8, st));
   WG_CUDA(eng, cudaMemsetAsync(sh.counters, 0, 16 * 8, st));
   WG_CUDA(eng, cudaStreamSynchronize(st));
   return WG_OK;
@@ -585,6 +585,11 @@ static wg_status shadow_common(wg_engine* e, bool push, const wg_event_hdr* d_hd
   p.out = reinterpret_cast<uint2*>(d_out);
   p.n = n;
   p.mode = static_cast<uint32_t>(mode);
+  if (++e->sh.stamp == 0) {  // 2^32 calls later the stamps start over
+    WG_CUDA(e, cudaMemsetAsync(e->sh.uses, 0, static_cast<size_t>(e->sh.n_slots ? e->sh.n_slots : 1) * 8,
+                               static_cast<cudaStream_t>(cuda_stream)));
+    e->sh.stamp = 1;
+  }
   WG_CUDA(e, wg::launch_shadow(p, e->sh, push, e->sm_count, static_cast<cudaStream_t>(cuda_stream)));
   return WG_OK;
 }

@@ -119,8 +119,9 @@ struct ShadowState {
                                 // {expected_return, token, callsite_id | depth << 32, 0}: an active lane writes
                                 // its whole sector (two 16-byte stores the L2 merges), so DRAM never has to
                                 // read-fill a partially written one; inactive lanes' sectors are not touched
-  uint32_t* uses;               // [n_slots] occurrences of a warp slot in the current call
+  unsigned long long* uses;     // [n_slots] {stamp of the call that last used the slot << 32 | its occurrences in that call}
   unsigned long long* counters; // [16] wg_shadow_counters
+  uint32_t stamp;               // the current call (1, 2, ...): a use count under an older stamp counts as zero, so nothing is cleared
 };
 cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st);
 

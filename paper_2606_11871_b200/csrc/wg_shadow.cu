@@ -12,7 +12,7 @@
 //   sector per thread slot and depth, written whole by its (active) lane.
 // Mapping: one warp per event (the state access is a gather by warp slot; each lane owns its own stack).
 // A call is one lock-step step of DISTINCT warps: a counting pass marks warp slots that occur twice in the call
-// and those events fail closed; a clearing pass resets the marks.
+// and those events fail closed; the marks carry the call's stamp, so no clearing pass is needed.
 #include <cstdlib>
 
 #include "wg_internal.h"
@@ -31,17 +31,18 @@ __device__ __forceinline__ uint32_t slot_of(uint32_t ctx_lo, uint32_t ctx_hi) {
   return (ctx_lo >> 5) | (ctx_hi << 27);  // bits 36..5 of context_base
 }
 
-__global__ void wg_shadow_mark(const uint4* __restrict__ hdr, uint64_t n, uint32_t* uses, uint32_t n_slots, int clear) {
+// counting pass: {stamp << 32 | occurrences} per warp slot.  The max installs this call's stamp with a zero count
+// over whatever an earlier call left (older stamps are smaller), the add counts; nothing has to be cleared afterwards.
+__global__ void wg_shadow_mark(const uint4* __restrict__ hdr, uint64_t n, unsigned long long* uses, uint32_t n_slots,
+                               uint32_t stamp) {
   uint64_t i = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   const uint64_t stride = static_cast<uint64_t>(gridDim.x) * blockDim.x;
   for (; i < n; i += stride) {
     const uint4 h = hdr[i];
     const uint32_t slot = slot_of(h.z, h.w);
     if (slot < n_slots) {
-      if (clear)
-        uses[slot] = 0u;
-      else
-        atomicAdd(uses + slot, 1u);
+      atomicMax(uses + slot, static_cast<unsigned long long>(stamp) << 32);
+      atomicAdd(uses + slot, 1ull);
     }
   }
 }
@@ -103,7 +104,7 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
         b.sc = __ldg(r + 2);
       }
       if (slot < sh.n_slots) {
-        b.uses = sh.uses[slot];
+        b.uses = static_cast<uint32_t>(sh.uses[slot]);  // (every slot of this call carries this call's stamp)
         if (on) b.d = sh.depth_ctr[static_cast<uint64_t>(slot) * 32 + lane];
       }
       if (on) {
@@ -362,7 +363,7 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
         b.sc = __ldg(r + 2);
       }
       const uint32_t slot = slot_of(h.z, h.w);
-      if (slot < sh.n_slots) b.uses = sh.uses[slot];
+      if (slot < sh.n_slots) b.uses = static_cast<uint32_t>(sh.uses[slot]);  // (the slot carries this call's stamp)
     }
     return b;
   };
@@ -551,7 +552,7 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
 cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st) {
   const uint64_t want_m = (p.n + 255) / 256;
   const int grid_m = static_cast<int>(want_m < static_cast<uint64_t>(sm_count) * 8 ? want_m : sm_count * 8);
-  wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, 0);
+  wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, sh.stamp);
   count_launch();
   // persistent warps: exactly the blocks that are resident at once.  WG_SHADOW=v1 selects the warp-per-event
   // kernel (measurement knob, like WG_IMPL=v1 for the check kernels).
@@ -587,8 +588,6 @@ cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int
     else
       wg_shadow_tile_kernel<false><<<grid, kTileThreads, 0, st>>>(p, sh);
   }
-  count_launch();
-  wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, 1);
   count_launch();
   return cudaGetLastError();
 }
