@@ -244,7 +244,9 @@ typedef struct {
   uint64_t non_return_events, slot_overflow_events, slot_conflict_events;
   uint64_t viol_lanes, viol_events, blocked_lanes;
 } wg_shadow_counters; /* 16 x u64 */
-/* (re)allocates and zeroes the shadow state and its counters; max_depth in 1..64; synchronises cuda_stream */
+/* (re)allocates and zeroes the shadow state and its counters; max_depth in 1..64; synchronises cuda_stream.
+ * Engine-owned device memory: n_warp_slots x (32 x (4 + 32 x max_depth) + 8) bytes — one 32-byte entry per thread
+ * slot and depth, a 4-byte depth counter per thread slot, an 8-byte use count per warp slot. */
 wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t max_depth, void* cuda_stream);
 wg_status wg_shadow_push(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val, wg_verdict* d_out,
                          uint64_t n, wg_mode mode, void* cuda_stream);
