@@ -251,6 +251,8 @@ __global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, con
 // ---------------------------------------------------------------------------------------------------
 // Tile size / block size sweep on B200 (1 Mi warps, depth 4; push / check_ret ms per call): 8 x 256 threads 0.55 / 0.60,
 // 16 x 128 0.55 / 0.58, 16 x 256 0.55 / 0.58, 32 x 128 0.58 / 0.58, 32 x 256 0.55 / 0.57, 32 x 512 0.54 / 0.55.
+// Again on the final kernels (whole-sector entries, warp-uniform prefix): 16 x 512 0.474 / 0.526, 32 x 256 0.490 / 0.562,
+// 32 x 384 0.480 / 0.537, 32 x 512 0.467 / 0.517 — 32 resident warps at 64 registers beat 24 at 71 - 73.
 #ifndef WG_SH_THREADS
 #define WG_SH_THREADS 512
 #endif
