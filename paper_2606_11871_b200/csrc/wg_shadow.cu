@@ -286,10 +286,13 @@ __device__ __forceinline__ uint2 lds2(uint32_t a) {
 }
 
 template <bool PUSH>
-__global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Params p, const ShadowState sh) {
+__global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_tile_kernel(const Params p, const ShadowState sh) {
   __shared__ unsigned long long sm[SH_WORDS];
   __shared__ __align__(16) TileSmem tiles[kTileWarps];
-  const uint32_t lane = threadIdx.x & 31;
+  // (volatile: ptxas otherwise re-derives the lane from SR_TID at every guard, an S2R round trip each time)
+  uint32_t lane, lanebit;
+  asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
+  asm volatile("shl.b32 %0, 1, %1;" : "=r"(lanebit) : "r"(lane));
   const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
   TileSmem& ts = tiles[warp];
   const uint32_t rec_s = sm_addr(ts.rec), st_s = sm_addr(ts.st), ust_s = sm_addr(ts.ust), vf_s = sm_addr(ts.vf);
@@ -311,7 +314,7 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
     S1 r{0u, 0u, 0u};
     if (i < static_cast<uint32_t>(kST)) {
       const uint4 a = lds4(rec_s + i * 16);
-      if ((a.x >> lane) & 1u) {
+      if (a.x & lanebit) {
         r.d = sh.depth_ctr[static_cast<uint64_t>(a.y) * 32 + lane];
         const uint2 v = *reinterpret_cast<const uint2*>(p.val + (e0 + i) * 32 + lane);
         r.vl = v.x;
@@ -325,7 +328,7 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
     if constexpr (!PUSH) {
       if (i < static_cast<uint32_t>(kST)) {
         const uint4 a = lds4(rec_s + i * 16);
-        if (((a.x >> lane) & 1u) && b.d != 0u && b.d - 1u < max_depth) {
+        if ((a.x & lanebit) && b.d != 0u && b.d - 1u < max_depth) {
           const uint4* en = reinterpret_cast<const uint4*>(sh.entry) + ((static_cast<uint64_t>(a.y) * max_depth + (b.d - 1u)) * 32 + lane) * 2;
           const uint4 et = en[0], m = en[1];
           x = StageE{et.x, et.y, et.z, et.w, m.x, m.y};
@@ -447,7 +450,7 @@ __global__ void __launch_bounds__(kTileThreads) wg_shadow_tile_kernel(const Para
       uint2 vf = make_uint2(0u, 0u);
       if constexpr (kFast) vf = lds2(vf_s + i0 * 8);
       const uint32_t act = ra.x, sl = ra.y, site = ra.z;
-      const bool on = (act >> lane) & 1u;
+      const bool on = (act & lanebit) != 0u;
       const uint32_t vl = b0.vl, vh = b0.vh;
       uint32_t d = b0.d;
       uint32_t cause = 0;  // 0 ok, else SH_* word of the lane's one cause
