@@ -533,3 +533,34 @@ def test_configs_2_and_3_full_size_sampled_against_the_oracle(config):
     assert np.array_equal(orc.sign(hdr_s, val_s)[~touched], clean_tag[~touched])
     assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), orc.verify(hdr_s, val_s, tag_s, st.mode))
     eng.close()
+
+
+def test_two_engines_on_two_streams_share_no_state():
+    """Two engines (different policies, keys, modes) fed from two streams with no synchronisation in between: each
+    one's verdicts and accumulated counters are the oracle's, i.e. nothing in the library is process-global."""
+    st_a, st_b = S.make_stream(2, "cpu", n_events=200_003), S.make_stream(3, "cpu", n_events=150_001)
+    orc_a, eng_a = oracle_for(st_a.policy), engine_for(st_a.policy)
+    orc_b, eng_b = oracle_for(st_b.policy), engine_for(st_b.policy)
+    hdr_a, val_a = st_a.hdr.numpy().view(np.uint64), st_a.val.numpy().view(np.uint64)
+    hdr_b, val_b = st_b.hdr.numpy().view(np.uint64), st_b.val.numpy().view(np.uint64)
+    tag_a = oracle_for(st_a.policy).sign(hdr_a, val_a)  # a second oracle: signing counts, and eng_a signs nothing
+    tag_t = torch.from_numpy(tag_a.view(np.int64).copy())
+    st_a.apply_return_tamper(tag_t)
+    tag_a = tag_t.numpy().view(np.uint64)
+    d = [t.to(dev()) for t in (st_a.hdr, st_a.val, tag_t, st_b.hdr, st_b.val)]
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for it in range(4):
+        outs.append((eng_a.wg_verify_continuations(d[0], d[1], d[2], ENF if it % 2 else DET, stream=s1),
+                     eng_b.wg_check_forward(d[3], d[4], DET if it % 2 else ENF, stream=s2)))
+    torch.cuda.synchronize()
+    for it, (ga, gb) in enumerate(outs):
+        oa = orc_a.verify(hdr_a, val_a, tag_a, ENF if it % 2 else DET)
+        ob = orc_b.check_forward(hdr_b, val_b, DET if it % 2 else ENF)
+        assert np.array_equal(ga.cpu().numpy().view(np.uint32), oa)
+        assert np.array_equal(gb.cpu().numpy().view(np.uint32), ob)
+    assert_counters_equal(eng_a, orc_a)
+    assert_counters_equal(eng_b, orc_b)
+    eng_a.close()
+    eng_b.close()
