@@ -80,6 +80,19 @@ def measured_peaks() -> dict:
     return {}
 
 
+def probe_int_pipe(device: int, mix: int) -> float:
+    """int32 lane-ops per second of the register-only integer probe (csrc/wg_probe.cu -> libwg_probe.so, a
+    measurement helper that is not part of libwarpguard.so)."""
+    import ctypes as C
+    lib = C.CDLL(str(ROOT / "paper_2606_11871_b200" / "libwg_probe.so"))
+    lib.wg_probe_int_pipe.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    ops, ms = C.c_double(0), C.c_double(0)
+    err = lib.wg_probe_int_pipe(int(device), int(mix), C.byref(ops), C.byref(ms))
+    if err != 0:
+        raise RuntimeError(f"wg_probe_int_pipe: cudaError {err}")
+    return ops.value
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
     Q = ("timestamp,uuid,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -266,7 +279,7 @@ def run_ours(a) -> None:
     for name, mix in (("iadd3", 0), ("lop3", 1), ("shf", 2), ("imad", 3), ("imad_wide", 4),
                       ("lop3+imad_1:1", 5), ("sipround_alu_mix", 6), ("imad_hi", 7), ("alu+imad_2:1", 8),
                       ("shf+imad_hi_1:1", 9), ("add64_pairs", 10), ("sipround_x24", 11)):
-        probes[name] = B.wg_probe_int_pipe(local, mix)[0]
+        probes[name] = probe_int_pipe(local, mix)
 
     props = torch.cuda.get_device_properties(local)
     uuid = str(props.uuid) if hasattr(props, "uuid") else None
@@ -277,7 +290,7 @@ def run_ours(a) -> None:
     barrier()
     import datetime as _dt
     t_region0 = _dt.datetime.now()
-    launches0 = B.wg_launch_count()
+    launches0 = eng.wg_kernel_launches()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(a.steps)]
     for k in range(a.steps):
         ev[k][0].record()
@@ -288,7 +301,7 @@ def run_ours(a) -> None:
     barrier()
     sampler.window(t_region0, _dt.datetime.now())
     clocks = sampler.stop()
-    launches = B.wg_launch_count() - launches0
+    launches = eng.wg_kernel_launches() - launches0
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     sign_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / a.steps
     verify_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / a.steps

@@ -21,10 +21,17 @@
  *  - `d_*` arguments are caller-owned DEVICE pointers on the engine's device, 16-byte aligned, valid until
  *    `cuda_stream` has executed the call's work; the engine neither frees nor keeps them.  `h_*` / `desc`
  *    arguments are HOST pointers.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
- *  - Policy tables, the key and all counters live in engine-owned device memory ("backend-private state",
- *    PAPER.md:256 §5.6; Table A3): the caller never gets their addresses.
+ *  - Policy tables and counters live in engine-owned device memory ("backend-private state", §5.6;
+ *    Table A3).  The key, and everything derived from it, is NOT in device global memory at all: the engine keeps it
+ *    host-side and hands it to its kernels as launch parameters (constant bank) — "keys are passed to injected helpers
+ *    as instrumentation arguments and are not exposed as ordinary target-writable CUDA objects" — so a
+ *    device-side read / write primitive (in scope) finds no key material to read through any pointer
+ *    this library hands out or keeps.  The policy tables themselves are, as in the paper, ordinary device memory:
+ *    the metadata-integrity profile below authenticates them per check.
  *  - Sign / verify / check enqueue work on `cuda_stream` and return without waiting.  Counters accumulate across
- *    calls until wg_reset_counters or the next successful wg_load_policy.
+ *    calls until wg_reset_counters (synchronous) or the next successful wg_load_policy.  The *_host calls are
+ *    synchronous and run on the engine's own streams: they are not ordered after work still pending on a caller
+ *    stream, so synchronise that stream first when both forms are mixed.
  *  - There is no CPU fallback: without a CUDA device every call that needs one returns WG_ERR_CUDA.
  */
 #ifndef WARPGUARD_H
@@ -44,7 +51,8 @@ typedef enum {
   WG_ERR_BAD_POLICY = 2,  /* policy rejected at load; nothing was loaded                             */
   WG_ERR_NO_POLICY = 3,   /* engine handle is NULL or holds no policy                                */
   WG_ERR_CUDA = 4,        /* a CUDA runtime call failed (wg_last_cuda_error gives the code)          */
-  WG_ERR_OOM = 5          /* host or device allocation failed                                        */
+  WG_ERR_OOM = 5,         /* host or device allocation failed                                        */
+  WG_ERR_INTERNAL = 6     /* an engine invariant does not hold (a bug): nothing returned may be trusted      */
 } wg_status;
 
 /* Site outcome kinds: PAPER.md:145-154 (Table 2), "protected" split by edge direction. */
@@ -70,7 +78,8 @@ typedef struct {
   const uint32_t* tgt_off; /* [n_sites + 1] CSR offsets, tgt_off[0] == 0, non-decreasing             */
   const uint64_t* tgts;    /* [tgt_off[n_sites]] per site strictly ascending; may be NULL if empty   */
   uint64_t key[2];         /* k0, k1 = little-endian 64-bit halves of the 128-bit backend key (R20)  */
-  uint64_t policy_digest;  /* stored and echoed by wg_read_counters; not checked (R25)               */
+  uint64_t policy_digest;  /* stored and echoed by wg_read_counters; wg_load_policy does not check it (R25),  */
+                           /* wg_load_policy_bound refuses the policy unless it is the image's digest (R39)   */
 } wg_policy_desc;
 
 /* One per-warp check event (16 bytes, little-endian).  context_base packs the caller's epoch / depth /
@@ -198,6 +207,7 @@ typedef struct {
   uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
   uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 since the ring was enabled */
   uint64_t fwd_meta_fail_events;        /* forward records that failed their authentication (metadata integrity) */
+  uint64_t kernel_launches;             /* CUDA kernels this engine has enqueued since it was created (diagnostic)  */
 } wg_telemetry_counters;
 /* The attacker's write into the policy metadata, for tests (the paper treats forward records as ordinary writable
  * GPU memory): what = 0: allowed_targets[index] ^= x (index into the CSR array); what = 1: the
@@ -267,14 +277,17 @@ typedef enum { WG_TUNE_DEFAULT = 0, WG_TUNE_SPARSE_LANES = 1, WG_TUNE_DENSE_LANE
 wg_status wg_set_tuning(wg_engine* eng, uint32_t flags);
 
 /* ---- inline device form (include/warpguard_device.cuh) ----
- * What a kernel needs to run the checks at its own sites: pointers into the engine's device tables.  Pass the view
- * to the kernel BY VALUE; it stays valid until the next wg_load_policy or wg_destroy.  site_recs: 64 bytes per site
- * {kind, set offset, set size, 0; key-derived SipHash mid-state (8 words); forward-record token; 0 0}. */
+ * What a kernel needs to run the checks at its own sites: the engine's policy tables and the key-derived SipHash
+ * initial state.  Pass the view to the kernel BY VALUE — kernel parameter space is where the paper puts the key
+ * ("passed to injected helpers as instrumentation arguments"); never copy it into device global memory.
+ * It stays valid until the next wg_load_policy or wg_destroy.  site_recs: 16 bytes per site {kind, set offset, set
+ * size, flags}; nothing in device memory is key-derived. */
 typedef struct {
   const void* site_recs;
   const uint64_t* targets;
   uint32_t n_sites;
-  uint32_t reserved;
+  uint32_t bind_hi;    /* low 32 bits of the policy digest when loaded with wg_load_policy_bound (R39), else 0 */
+  uint64_t v_init[4];  /* key xor the SipHash constants: key-equivalent, host / parameter space only           */
 } wg_device_view;
 wg_status wg_get_device_view(wg_engine* eng, wg_device_view* h_view);
 
@@ -288,20 +301,6 @@ wg_status wg_verify_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr
                                        const uint64_t* h_tag, wg_verdict* h_out, uint64_t n, wg_mode mode);
 wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
                                 wg_verdict* h_out, uint64_t n, wg_mode mode);
-
-/* ---- measurement helpers (no part of the check path) ----
- * wg_probe_int_pipe: runs a register-only integer micro-benchmark on `device` and returns, in *ops_per_s, the
- * achieved 32-bit integer lane-operations per second (DESIGN.md §6 "integer-pipe peak").
- *   mix: 0 = IADD3 only, 1 = LOP3 only, 2 = SHF only, 3 = IMAD only, 4 = IMAD.WIDE.U32 only,
- *        5 = ALU:FMA 1:1 (LOP3 + IMAD), 6 = SipRound-shaped ALU mix (IADD3 / LOP3 / SHF, 8:8:8),
- *        7 = IMAD.HI.U32 only, 8 = ALU:FMA 2:1 (LOP3, SHF + IMAD), 9 = ALU:FMA 1:1 (SHF + IMAD.HI.U32),
- *        10 = 64-bit-add pairs (IADD3 with carry-out + IMAD.X with carry-in; counts PAIRS per second),
- *        11 = the SipRound itself (two independent states per thread), counted as 24 int32 operations per round:
- *             the ceiling of any SipHash kernel on this GPU.
- *   Every step's second operand is a neighbouring chain's live value, so ptxas cannot fold steps away.
- * wg_launch_count: kernels this library has launched since it was loaded (bench.py's gpu_launches). */
-wg_status wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms);
-uint64_t wg_launch_count(void);
 
 #ifdef __cplusplus
 }

@@ -18,16 +18,20 @@
 
 // sign / verify: `context_id` is the full 64-bit context word of THIS thread (the batched API's
 // (context_base & ~31) | lane).  Unknown or non-return sites: sign returns 0, verify returns false (fail closed).
+// The key-derived SipHash initial state comes from the view, i.e. from kernel parameter space; nothing key-derived
+// is read from device memory.
 __device__ __forceinline__ uint64_t wg_dev_sign(const wg_device_view& v, uint32_t site_id, uint64_t continuation,
                                                 uint64_t context_id) {
   if (site_id >= v.n_sites) return 0;
-  const uint4* rec = reinterpret_cast<const uint4*>(v.site_recs) + static_cast<uint64_t>(site_id) * 4;
-  const uint4 a = __ldg(rec);
+  const uint4 a = __ldg(reinterpret_cast<const uint4*>(v.site_recs) + site_id);
   if (a.x != WG_KIND_PROTECTED_RETURN) return 0;
-  const uint4 b = __ldg(rec + 1), c = __ldg(rec + 2);
-  wg::Sip32 s{b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w};  // pre-A state after the site word
+  wg::Sip32 s{static_cast<uint32_t>(v.v_init[0]), static_cast<uint32_t>(v.v_init[0] >> 32),
+              static_cast<uint32_t>(v.v_init[1]), static_cast<uint32_t>(v.v_init[1] >> 32),
+              static_cast<uint32_t>(v.v_init[2]), static_cast<uint32_t>(v.v_init[2] >> 32),
+              static_cast<uint32_t>(v.v_init[3]), static_cast<uint32_t>(v.v_init[3] >> 32)};
   uint32_t tl, th;
-  wg::sip_absorb_preA(s, static_cast<uint32_t>(continuation), static_cast<uint32_t>(continuation >> 32));
+  wg::sip_absorb(s, site_id, v.bind_hi);  // LE64(site_id | digest32 << 32) (R3, R39)
+  wg::sip_absorb(s, static_cast<uint32_t>(continuation), static_cast<uint32_t>(continuation >> 32));
   wg::sip_absorb(s, static_cast<uint32_t>(context_id), static_cast<uint32_t>(context_id >> 32));
   wg::sip_finish(s, 0u, 0u, tl, th);
   return (static_cast<uint64_t>(th) << 32) | tl;
@@ -36,15 +40,14 @@ __device__ __forceinline__ uint64_t wg_dev_sign(const wg_device_view& v, uint32_
 __device__ __forceinline__ bool wg_dev_verify(const wg_device_view& v, uint32_t site_id, uint64_t observed,
                                               uint64_t context_id, uint64_t stored_tag) {
   if (site_id >= v.n_sites) return false;
-  const uint4* rec = reinterpret_cast<const uint4*>(v.site_recs) + static_cast<uint64_t>(site_id) * 4;
-  if (__ldg(rec).x != WG_KIND_PROTECTED_RETURN) return false;
+  if (__ldg(reinterpret_cast<const uint4*>(v.site_recs) + site_id).x != WG_KIND_PROTECTED_RETURN) return false;
   return wg_dev_sign(v, site_id, observed, context_id) == stored_tag;
 }
 
 // forward check: true iff `target` is a member of the site's set (branch-free lower-bound walk)
 __device__ __forceinline__ bool wg_dev_check_forward(const wg_device_view& v, uint32_t site_id, uint64_t target) {
   if (site_id >= v.n_sites) return false;
-  const uint4 a = __ldg(reinterpret_cast<const uint4*>(v.site_recs) + static_cast<uint64_t>(site_id) * 4);
+  const uint4 a = __ldg(reinterpret_cast<const uint4*>(v.site_recs) + site_id);
   if (a.x != WG_KIND_PROTECTED_FORWARD) return false;
   const uint64_t* set = v.targets + a.y;
   uint32_t lo = 0, len = a.z;

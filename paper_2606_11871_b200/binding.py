@@ -18,14 +18,13 @@ import torch
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libwarpguard.so"
 
-WG_OK, WG_ERR_INVALID_ARG, WG_ERR_BAD_POLICY, WG_ERR_NO_POLICY, WG_ERR_CUDA, WG_ERR_OOM = range(6)
+WG_OK, WG_ERR_INVALID_ARG, WG_ERR_BAD_POLICY, WG_ERR_NO_POLICY, WG_ERR_CUDA, WG_ERR_OOM, WG_ERR_INTERNAL = range(7)
 WG_MODE_DETECT, WG_MODE_ENFORCE = 0, 1
 
 EXPORTS = [
     "wg_load_policy", "wg_sign_continuations", "wg_verify_continuations", "wg_check_forward", "wg_read_counters",
     "wg_reset_counters", "wg_destroy", "wg_strerror", "wg_last_cuda_error",
     "wg_sign_continuations_host", "wg_verify_continuations_host", "wg_check_forward_host",
-    "wg_probe_int_pipe", "wg_launch_count",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
     "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_set_tuning", "wg_policy_digest",
@@ -36,7 +35,8 @@ WG_TUNE_DEFAULT, WG_TUNE_SPARSE_LANES, WG_TUNE_DENSE_LANES = 0, 1, 2
 
 class DeviceView(C.Structure):
     """wg_device_view: pass it by value to a kernel that uses include/warpguard_device.cuh"""
-    _fields_ = [("site_recs", C.c_void_p), ("targets", C.c_void_p), ("n_sites", C.c_uint32), ("reserved", C.c_uint32)]
+    _fields_ = [("site_recs", C.c_void_p), ("targets", C.c_void_p), ("n_sites", C.c_uint32), ("bind_hi", C.c_uint32),
+                ("v_init", C.c_uint64 * 4)]
 SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
                  "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
                  "non_return_events", "slot_overflow_events", "slot_conflict_events", "viol_lanes", "viol_events",
@@ -49,6 +49,8 @@ VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"),
                             ("stored", "<u8")])  # wg_violation_rec, 48 bytes
 TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
                     "ring_recorded", "ring_dropped", "fwd_meta_fail_events")
+# words of wg_telemetry_counters behind TELEMETRY_FIELDS that have no counterpart in the method (engine diagnostics)
+TELEMETRY_ENGINE_FIELDS = ("kernel_launches",)
 
 COUNTER_FIELDS = (
     ["events_total", "events_empty", "events_unknown_site", "events_misrouted"]
@@ -98,8 +100,6 @@ def lib() -> C.CDLL:
         L.wg_sign_continuations_host.argtypes = [vp, vp, vp, vp, u64]
         L.wg_verify_continuations_host.argtypes = [vp, vp, vp, vp, vp, u64, i]
         L.wg_check_forward_host.argtypes = [vp, vp, vp, vp, u64, i]
-        L.wg_probe_int_pipe.argtypes = [i, i, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-        L.wg_launch_count.argtypes = []
         L.wg_shadow_configure.argtypes = [vp, C.c_uint32, C.c_uint32, vp]
         L.wg_shadow_push.argtypes = [vp, vp, vp, vp, u64, i, vp]
         L.wg_shadow_check_ret.argtypes = [vp, vp, vp, vp, u64, i, vp]
@@ -112,9 +112,8 @@ def lib() -> C.CDLL:
         L.wg_set_tuning.argtypes = [vp, C.c_uint32]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
-        L.wg_launch_count.restype = u64
         for name in EXPORTS:
-            if name not in ("wg_destroy", "wg_strerror", "wg_launch_count"):
+            if name not in ("wg_destroy", "wg_strerror"):
                 getattr(L, name).restype = i
         _lib = L
     return _lib
@@ -300,7 +299,7 @@ class Engine:
 
     def wg_read_telemetry(self, ring_cap: int = 0, stream=None):
         """(telemetry counters dict, first-violation record or None, ring records as a structured array)."""
-        t = np.zeros(7, dtype=np.uint64)
+        t = np.zeros(len(TELEMETRY_FIELDS) + len(TELEMETRY_ENGINE_FIELDS), dtype=np.uint64)
         first = np.zeros(1, dtype=VIOLATION_DTYPE)
         have = C.c_int(0)
         ring = np.zeros(max(int(ring_cap), 1), dtype=VIOLATION_DTYPE)
@@ -308,8 +307,16 @@ class Engine:
         _chk(lib().wg_read_telemetry(self._h, t.ctypes.data, first.ctypes.data, C.byref(have),
                                      ring.ctypes.data if ring_cap else None, int(ring_cap), C.byref(n),
                                      _stream_ptr(stream)), "wg_read_telemetry")
+        self.kernel_launches = int(t[len(TELEMETRY_FIELDS)])
         return ({k: int(v) for k, v in zip(TELEMETRY_FIELDS, t)}, first[0] if have.value else None,
                 ring[: n.value] if ring_cap else ring[:0])
+
+    def wg_kernel_launches(self) -> int:
+        """wg_telemetry_counters.kernel_launches: CUDA kernels this engine has enqueued since it was created."""
+        t = np.zeros(len(TELEMETRY_FIELDS) + len(TELEMETRY_ENGINE_FIELDS), dtype=np.uint64)
+        _chk(lib().wg_read_telemetry(self._h, t.ctypes.data, None, None, None, 0, None, _stream_ptr(None)),
+             "wg_read_telemetry")
+        return int(t[len(TELEMETRY_FIELDS)])
 
     def wg_reset_counters(self, stream=None) -> None:
         _chk(lib().wg_reset_counters(self._h, _stream_ptr(stream)), "wg_reset_counters")
@@ -343,14 +350,3 @@ def wg_policy_digest(kind, tgt_off, tgts, k0: int, k1: int) -> int:
     out = C.c_uint64(0)
     _chk(lib().wg_policy_digest(C.byref(d), C.byref(out)), "wg_policy_digest")
     return int(out.value)
-
-
-def wg_probe_int_pipe(device: int, mix: int) -> tuple[float, float]:
-    """(int32 lane-ops per second, milliseconds) of the register-only integer probe; see warpguard.h."""
-    ops, ms = C.c_double(0), C.c_double(0)
-    _chk(lib().wg_probe_int_pipe(int(device), int(mix), C.byref(ops), C.byref(ms)), "wg_probe_int_pipe")
-    return ops.value, ms.value
-
-
-def wg_launch_count() -> int:
-    return int(lib().wg_launch_count())

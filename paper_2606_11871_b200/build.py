@@ -1,4 +1,5 @@
-"""Builds libwarpguard.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo).
+"""Builds libwarpguard.so (the product) and libwg_probe.so (bench.py's integer-pipe micro-benchmark, not part of the
+product) in-tree with nvcc for sm_100a (no JIT cache: the .so files travel with the repo).
 
     python -m paper_2606_11871_b200.build [--force]
 """
@@ -14,7 +15,9 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libwarpguard.so"
-SOURCES = ["wg_api.cu", "wg_kernels_v1.cu", "wg_kernels_v2.cu", "wg_shadow.cu", "wg_probe.cu"]
+PROBE_LIB = PKG / "libwg_probe.so"
+SOURCES = ["wg_api.cu", "wg_kernels_v2.cu", "wg_shadow.cu"]
+PROBE_SOURCES = ["wg_probe.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
@@ -36,24 +39,31 @@ def _newest_source() -> float:
     return max(f.stat().st_mtime for f in files)
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and LIB.exists() and LIB.stat().st_mtime >= _newest_source():
-        return LIB
-    tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [nvcc(), *NVCC_FLAGS, "-shared", "-I", str(ROOT / "include"), "-o", str(tmp)]
-    cmd += [str(CSRC / s) for s in SOURCES]
+def _link(lib: Path, sources: list[str], log: str | None, verbose: bool, extra: list[str] | None = None) -> None:
+    tmp = lib.with_suffix(f".so.tmp{os.getpid()}")
+    cmd = [nvcc(), *NVCC_FLAGS, *(extra or []), "-shared", "-I", str(ROOT / "include"), "-o", str(tmp)]
+    cmd += [str(CSRC / s) for s in sources]
     cmd += ["-lcudart_static", "-lpthread", "-ldl", "-lrt"]
     r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
-        raise RuntimeError("nvcc failed building libwarpguard.so")
+        raise RuntimeError(f"nvcc failed building {lib.name}")
     if verbose:
         sys.stderr.write(r.stderr)
-    (PKG / "build_ptxas.log").write_text(r.stderr)
-    os.replace(tmp, LIB)
+    if log:
+        (PKG / log).write_text(r.stderr)
+    os.replace(tmp, lib)
+
+
+def build(force: bool = False, verbose: bool = False, extra: list[str] | None = None) -> Path:
+    newest = _newest_source()
+    if force or not LIB.exists() or LIB.stat().st_mtime < newest:
+        _link(LIB, SOURCES, "build_ptxas.log", verbose, extra)
+    if force or not PROBE_LIB.exists() or PROBE_LIB.stat().st_mtime < newest:
+        _link(PROBE_LIB, PROBE_SOURCES, None, False)
     return LIB
 
 
 if __name__ == "__main__":
-    p = build(force="--force" in sys.argv, verbose=True)
+    p = build(force="--force" in sys.argv, verbose=True, extra=[a for a in sys.argv[1:] if a.startswith("-D")])
     print(p)

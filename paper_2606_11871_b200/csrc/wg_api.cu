@@ -2,8 +2,6 @@
 // policy loads nothing), engine-owned device tables, launches, counter read-out, and the HOST-buffer entry
 // points that stream events through a double-buffered device staging area.  No verdict, MAC or membership
 // arithmetic happens on the host: every step of the path runs in the kernels of wg_kernels.cu.
-#include <atomic>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -17,16 +15,16 @@ struct wg_engine {
   bool loaded = false;
   uint32_t n_sites = 0;
   uint64_t n_tgts = 0;
-  wg::SiteRow* d_rows = nullptr;
-  wg::SiteRec* d_recs = nullptr;  // v2 site records (kind, set range, pre-A SipHash mid-state), 64 B each
+  wg::SiteRec* d_recs = nullptr;  // site records {kind, set range, flags}, 16 B each; nothing key-derived
+  uint64_t* d_tok = nullptr;       // [n_sites] forward-record tokens at load time (metadata-integrity profile, R37)
   uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
   uint32_t tuning = 0;             // WG_TUNE_* flags
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
   wg::ViolRec* d_ring = nullptr;
   wg::FirstRec* d_first = nullptr;  // first-violation record + the key it belongs to
-  wg::ShadowState sh = {0, 0, nullptr, nullptr, nullptr, nullptr};  // stateful shadow stack
-  int impl = 2;                   // 2 = tiled kernels (default); 1 = baseline warp-per-event kernels (WG_IMPL=v1)
+  wg::ShadowState sh = {0, 0, nullptr, nullptr, nullptr, nullptr, 0, {0, 0}};  // stateful shadow stack
+  uint64_t launches = 0;          // kernels this engine has enqueued (wg_telemetry_counters.kernel_launches)
   uint64_t* d_tgts = nullptr;
   unsigned long long* d_glob = nullptr;  // [C_WORDS]
   unsigned long long* d_site = nullptr;  // [n_sites][4]
@@ -40,11 +38,10 @@ struct wg_engine {
   void* d_stage[2] = {nullptr, nullptr};
   cudaStream_t st[2] = {nullptr, nullptr};
   cudaEvent_t ev_done[2] = {nullptr, nullptr};
+  cudaEvent_t ev_rec = nullptr;  // orders the first-violation-record kernels of consecutive chunks across the two streams
 };
 
 namespace {
-
-std::atomic<uint64_t> g_launches{0};
 
 struct DeviceGuard {
   int prev = -1;
@@ -91,13 +88,13 @@ bool policy_ok(const wg_policy_desc* d) {
 }
 
 void free_tables(wg_engine* e) {
-  cudaFree(e->d_rows);
   cudaFree(e->d_recs);
   e->d_recs = nullptr;
+  cudaFree(e->d_tok);
+  e->d_tok = nullptr;
   cudaFree(e->d_tgts);
   cudaFree(e->d_glob);
   cudaFree(e->d_site);
-  e->d_rows = nullptr;
   e->d_tgts = nullptr;
   e->d_glob = nullptr;
   e->d_site = nullptr;
@@ -109,7 +106,7 @@ void free_shadow(wg_engine* e) {
   cudaFree(e->sh.entry);
   cudaFree(e->sh.uses);
   cudaFree(e->sh.counters);
-  e->sh = wg::ShadowState{0, 0, nullptr, nullptr, nullptr, nullptr};
+  e->sh = wg::ShadowState{0, 0, nullptr, nullptr, nullptr, nullptr, 0, {0, 0}};
 }
 
 void free_staging(wg_engine* e) {
@@ -121,6 +118,8 @@ void free_staging(wg_engine* e) {
     e->st[i] = nullptr;
     e->ev_done[i] = nullptr;
   }
+  if (e->ev_rec) cudaEventDestroy(e->ev_rec);
+  e->ev_rec = nullptr;
   e->stage_cap = 0;
 }
 
@@ -141,8 +140,8 @@ wg_status zero_counters(wg_engine* e, cudaStream_t st) {
 wg::Params base_params(const wg_engine* e) {
   wg::Params p;
   std::memset(&p, 0, sizeof(p));
-  p.rows = e->d_rows;
   p.recs = e->d_recs;
+  p.tok = e->d_tok;
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
   p.bind_hi = e->bind_hi;
@@ -163,8 +162,11 @@ wg::Params base_params(const wg_engine* e) {
 
 constexpr uint64_t kMaxLaunchEvents = 1ull << 30;
 
+// rec_after: an event the first-violation-record kernel waits for (host path: the record kernel of the previous chunk,
+// which ran on the other staging stream), or nullptr
 wg_status check_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d_val, const uint64_t* d_tag,
-                       bool has_tag, wg_verdict* d_out, uint64_t n, wg_mode mode, cudaStream_t st) {
+                       bool has_tag, wg_verdict* d_out, uint64_t n, wg_mode mode, cudaStream_t st,
+                       cudaEvent_t rec_after = nullptr) {
   if (!e || !e->loaded) return WG_ERR_NO_POLICY;
   if (mode != WG_MODE_DETECT && mode != WG_MODE_ENFORCE) return WG_ERR_INVALID_ARG;
   if (n == 0) return WG_OK;  // R24: nothing changes
@@ -185,7 +187,10 @@ wg_status check_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* 
     p.n = m;
     p.seq_base = e->seq;
     p.mode = static_cast<uint32_t>(mode);
-    WG_CUDA(e, e->impl == 1 ? wg::launch_check_v1(p, e->sm_count, st) : wg::launch_check_v2(p, e->sm_count, st));
+    WG_CUDA(e, wg::launch_check(p, e->sm_count, st, &e->launches));
+    // first-violation record (R29): one thread behind the check launch; the launch is over, so the key is final for it
+    if (rec_after) WG_CUDA(e, cudaStreamWaitEvent(st, rec_after, 0));
+    WG_CUDA(e, wg::launch_first_record(p, st, &e->launches));
     e->seq += m;
   }
   e->last_mode = static_cast<uint64_t>(mode);
@@ -207,7 +212,7 @@ wg_status sign_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d
     p.val = d_val + lo * 32;
     p.tag_out = d_tag + lo * 32;
     p.n = m;
-    WG_CUDA(e, e->impl == 1 ? wg::launch_sign_v1(p, e->sm_count, st) : wg::launch_sign_v2(p, e->sm_count, st));
+    WG_CUDA(e, wg::launch_sign(p, e->sm_count, st, &e->launches));
   }
   return WG_OK;
 }
@@ -223,6 +228,7 @@ wg_status ensure_staging(wg_engine* e) {
     WG_CUDA(e, cudaStreamCreateWithFlags(&e->st[i], cudaStreamNonBlocking));
     WG_CUDA(e, cudaEventCreateWithFlags(&e->ev_done[i], cudaEventDisableTiming));
   }
+  WG_CUDA(e, cudaEventCreateWithFlags(&e->ev_rec, cudaEventDisableTiming));
   e->stage_cap = kStageEvents;
   return WG_OK;
 }
@@ -259,7 +265,11 @@ wg_status host_common(wg_engine* e, HostOp op, const wg_event_hdr* h_hdr, const 
   wg_status s = ensure_staging(e);
   if (s != WG_OK) return s;
 
+  // The chunks alternate between two staging streams, so two check kernels may overlap.  Their first-violation-record
+  // kernels must not: each one waits (ev_rec) for the record kernel of the chunk before it, so the records are written
+  // in chunk order by one kernel at a time, and the last writer is the chunk that holds the final minimum key.
   int buf = 0;
+  bool rec_pending = false;
   for (uint64_t lo = 0; lo < n; lo += kStageEvents, buf ^= 1) {
     const uint64_t m = (n - lo < kStageEvents) ? (n - lo) : kStageEvents;
     cudaStream_t st = e->st[buf];
@@ -274,8 +284,10 @@ wg_status host_common(wg_engine* e, HostOp op, const wg_event_hdr* h_hdr, const 
       if (s != WG_OK) return s;
       WG_CUDA(e, cudaMemcpyAsync(h_tag_out + lo * 32, v.tag, m * 256, cudaMemcpyDeviceToHost, st));
     } else {
-      s = check_common(e, v.hdr, v.val, v.tag, op == OP_VERIFY, v.out, m, mode, st);
+      s = check_common(e, v.hdr, v.val, v.tag, op == OP_VERIFY, v.out, m, mode, st, rec_pending ? e->ev_rec : nullptr);
       if (s != WG_OK) return s;
+      WG_CUDA(e, cudaEventRecord(e->ev_rec, st));
+      rec_pending = true;
       WG_CUDA(e, cudaMemcpyAsync(h_out + lo, v.out, m * 8, cudaMemcpyDeviceToHost, st));
     }
   }
@@ -285,10 +297,6 @@ wg_status host_common(wg_engine* e, HostOp op, const wg_event_hdr* h_hdr, const 
 }
 
 }  // namespace
-
-namespace wg {
-void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
-}  // namespace wg
 
 extern "C" {
 
@@ -353,7 +361,6 @@ wg_status wg_load_policy_bound(wg_engine** eng, int device, const wg_policy_desc
   const wg_status s = wg_policy_digest(desc, &d);
   if (s != WG_OK) return s;
   if (d != desc->policy_digest) return WG_ERR_BAD_POLICY;  // "a mismatch aborts before the policy is used"
-  { const char* impl = std::getenv("WG_IMPL"); if (impl && impl[0] == 'v' && impl[1] == '1') return WG_ERR_INVALID_ARG; }
   return load_common(eng, device, desc, static_cast<uint32_t>(d));
 }
 
@@ -374,95 +381,107 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
 
   const uint32_t n = desc->n_sites;
   const uint64_t nt = desc->tgt_off[n];
-  // build the new tables completely before replacing the old ones
-  std::vector<wg::SiteRow> rows;
+  // build the new tables completely (in `tmp`, on the new device) before anything of an existing engine is replaced:
+  // whatever fails below leaves *eng exactly as it was, and leaks nothing
+  std::vector<wg::SiteRec> recs;
   try {
-    rows.resize(n);
+    recs.resize(n);
   } catch (const std::bad_alloc&) {
     return WG_ERR_OOM;
   }
   for (uint32_t s = 0; s < n; ++s) {
-    rows[s].kind = desc->kind[s];
-    rows[s].off = desc->tgt_off[s];
-    rows[s].cnt = desc->tgt_off[s + 1] - desc->tgt_off[s];
-    rows[s].pad = 0;
+    recs[s].kind = desc->kind[s];
+    recs[s].off = desc->tgt_off[s];
+    recs[s].cnt = desc->tgt_off[s + 1] - desc->tgt_off[s];
+    recs[s].flags = 0;
   }
   wg_engine tmp;
   tmp.device = device;
   tmp.n_sites = n;
   tmp.n_tgts = nt;
+  // SipHash initialisation: key xor the constant "somepseudorandomlygeneratedbytes" (R1, R20).  Kept host-side and
+  // handed to the kernels as parameters (constant bank): the key never sits in device global memory.
+  tmp.v_init[0] = desc->key[0] ^ 0x736f6d6570736575ull;
+  tmp.v_init[1] = desc->key[1] ^ 0x646f72616e646f6dull;
+  tmp.v_init[2] = desc->key[0] ^ 0x6c7967656e657261ull;
+  tmp.v_init[3] = desc->key[1] ^ 0x7465646279746573ull;
+  wg::FirstRec* new_first = nullptr;
   cudaError_t err = cudaSuccess;
   auto fail = [&](cudaError_t e2) {
     free_tables(&tmp);
-    wg_status s = cuda_fail(*eng, e2);
-    return s;
+    cudaFree(new_first);
+    return cuda_fail(*eng, e2);  // (records the code in an existing engine; a first load has nowhere to record it)
   };
   if ((err = cudaDeviceGetAttribute(&tmp.sm_count, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess)
     return fail(err);
-  if ((err = cudaMalloc(&tmp.d_rows, sizeof(wg::SiteRow) * (n ? n : 1))) != cudaSuccess) return fail(err);
   // the target table is padded to an even element count so that the TMA bulk copy that stages it moves whole
   // 16-byte units; the pad element is never addressed by a search
   const uint64_t nt_pad = (nt + 1) & ~1ull;
   if ((err = cudaMalloc(&tmp.d_tgts, sizeof(uint64_t) * (nt_pad ? nt_pad : 2))) != cudaSuccess) return fail(err);
   if ((err = cudaMemset(tmp.d_tgts, 0, sizeof(uint64_t) * (nt_pad ? nt_pad : 2))) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_recs, sizeof(wg::SiteRec) * (n ? n : 1))) != cudaSuccess) return fail(err);
-  if ((err = wg::init_v2()) != cudaSuccess) return fail(err);
+  if ((err = cudaMalloc(&tmp.d_tok, sizeof(uint64_t) * (n ? n : 1))) != cudaSuccess) return fail(err);
+  if ((err = wg::init_kernels()) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_glob, sizeof(unsigned long long) * wg::C_WORDS)) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_site, sizeof(unsigned long long) * 4 * (n ? n : 1))) != cudaSuccess) return fail(err);
-  if (n && (err = cudaMemcpy(tmp.d_rows, rows.data(), sizeof(wg::SiteRow) * n, cudaMemcpyHostToDevice)) != cudaSuccess)
+  if (n && (err = cudaMemcpy(tmp.d_recs, recs.data(), sizeof(wg::SiteRec) * n, cudaMemcpyHostToDevice)) != cudaSuccess)
     return fail(err);
   if (nt && (err = cudaMemcpy(tmp.d_tgts, desc->tgts, sizeof(uint64_t) * nt, cudaMemcpyHostToDevice)) != cudaSuccess)
     return fail(err);
-
+  // tokens of the forward records, computed on the device at (trusted) load time (R37)
+  if ((err = wg::launch_build_tokens(tmp.d_tok, tmp.d_recs, tmp.d_tgts, n, tmp.v_init[0], tmp.v_init[1], tmp.v_init[2],
+                                     tmp.v_init[3], nullptr, &tmp.launches)) != cudaSuccess)
+    return fail(err);
+  if ((err = cudaStreamSynchronize(nullptr)) != cudaSuccess) return fail(err);
   wg_engine* e = *eng;
+  const bool moved = e && e->device != device;
+  if (!e || moved || !e->d_first) {
+    if ((err = cudaMalloc(&new_first, sizeof(wg::FirstRec))) != cudaSuccess) return fail(err);
+  }
   if (!e) {
     e = new (std::nothrow) wg_engine();
     if (!e) {
       free_tables(&tmp);
+      cudaFree(new_first);
       return WG_ERR_OOM;
     }
   } else {
-    if (e->device != device) free_staging(e);
     DeviceGuard g2(e->device);
     cudaDeviceSynchronize();  // nothing may still be reading the tables we are about to drop
     free_tables(e);
+    if (moved) {
+      // everything else the engine owns lives on the OLD device: staging, first-violation record, ring (its capacity is
+      // configuration and is re-created empty on the new device below), shadow state (dropped: wg_shadow_configure again)
+      free_staging(e);
+      cudaFree(e->d_first);
+      e->d_first = nullptr;
+      cudaFree(e->d_ring);
+      e->d_ring = nullptr;
+      free_shadow(e);
+    }
   }
   e->device = device;
   e->sm_count = tmp.sm_count;
   e->n_sites = n;
   e->n_tgts = nt;
-  e->d_rows = tmp.d_rows;
   e->d_recs = tmp.d_recs;
+  e->d_tok = tmp.d_tok;
   e->d_tgts = tmp.d_tgts;
   e->d_glob = tmp.d_glob;
   e->d_site = tmp.d_site;
-  // SipHash initialisation: key xor the constant "somepseudorandomlygeneratedbytes" (R1, R20)
-  e->v_init[0] = desc->key[0] ^ 0x736f6d6570736575ull;
-  e->v_init[1] = desc->key[1] ^ 0x646f72616e646f6dull;
-  e->v_init[2] = desc->key[0] ^ 0x6c7967656e657261ull;
-  e->v_init[3] = desc->key[1] ^ 0x7465646279746573ull;
+  e->launches += tmp.launches;
+  for (int i = 0; i < 4; ++i) e->v_init[i] = tmp.v_init[i];
   e->digest = desc->policy_digest;
   e->bind_hi = bind_hi;
-  {
-    const char* impl = std::getenv("WG_IMPL");  // measurement knob: the baseline kernels stay selectable
-    e->impl = (impl && impl[0] == 'v' && impl[1] == '1') ? 1 : 2;
-  }
-  // per-site SipHash mid-states, computed on the device from the key-derived initial state
-  {
-    cudaError_t e3 = wg::launch_build_recs(e->d_recs, e->d_rows, e->d_tgts, n, bind_hi, e->v_init[0], e->v_init[1], e->v_init[2],
-                                           e->v_init[3], nullptr);
-    if (e3 != cudaSuccess) {
-      free_tables(e);
-      return cuda_fail(e, e3);
-    }
-  }
+  if (new_first) e->d_first = new_first;
   e->loaded = true;
   *eng = e;
-  if (!e->d_first) {
-    cudaError_t e4 = cudaMalloc(&e->d_first, sizeof(wg::FirstRec));
-    if (e4 != cudaSuccess) {
-      e->loaded = false;
-      return cuda_fail(e, e4);
+  if (moved && e->ring_cap) {
+    cudaError_t e5 = cudaMalloc(&e->d_ring, sizeof(wg::ViolRec) * e->ring_cap);
+    if (e5 != cudaSuccess) {
+      e->ring_cap = 0;  // the ring is diagnostic: the policy is loaded, the ring is off
+      e->d_ring = nullptr;
+      cuda_fail(e, e5);
     }
   }
   wg_status s = zero_counters(e, nullptr);
@@ -509,7 +528,12 @@ wg_status wg_reset_counters(wg_engine* eng, void* cuda_stream) {
   if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
   DeviceGuard g(eng->device);
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
-  return zero_counters(eng, static_cast<cudaStream_t>(cuda_stream));
+  // synchronous: the *_host calls run on the engine's own staging streams, which are not ordered after work the
+  // caller enqueued on `cuda_stream`; when this returns the counters are zero for every later call, whatever its stream
+  const wg_status s = zero_counters(eng, static_cast<cudaStream_t>(cuda_stream));
+  if (s != WG_OK) return s;
+  WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
+  return WG_OK;
 }
 
 void wg_destroy(wg_engine* eng) {
@@ -536,6 +560,7 @@ const char* wg_strerror(wg_status s) {
     case WG_ERR_NO_POLICY: return "no policy loaded";
     case WG_ERR_CUDA: return "CUDA runtime error (no device or call failed)";
     case WG_ERR_OOM: return "out of memory";
+    case WG_ERR_INTERNAL: return "engine invariant violated";
   }
   return "unknown status";
 }
@@ -551,7 +576,8 @@ wg_status wg_shadow_configure(wg_engine* eng, uint32_t n_warp_slots, uint32_t ma
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   WG_CUDA(eng, cudaStreamSynchronize(st));
   free_shadow(eng);
-  wg::ShadowState sh = {n_warp_slots, max_depth, nullptr, nullptr, nullptr, nullptr};
+  wg::ShadowState sh = {n_warp_slots, max_depth, nullptr, nullptr, nullptr, nullptr, 0, {0, 0}};
+  WG_CUDA(eng, wg::shadow_occupancy(&sh.per_sm[1], &sh.per_sm[0]));  // resolved once per configuration, on this device
   const size_t lanes = static_cast<size_t>(n_warp_slots ? n_warp_slots : 1) * 32;
   const size_t entries = lanes * max_depth;
   cudaError_t err;
@@ -590,7 +616,7 @@ static wg_status shadow_common(wg_engine* e, bool push, const wg_event_hdr* d_hd
                                static_cast<cudaStream_t>(cuda_stream)));
     e->sh.stamp = 1;
   }
-  WG_CUDA(e, wg::launch_shadow(p, e->sh, push, e->sm_count, static_cast<cudaStream_t>(cuda_stream)));
+  WG_CUDA(e, wg::launch_shadow(p, e->sh, push, e->sm_count, static_cast<cudaStream_t>(cuda_stream), &e->launches));
   return WG_OK;
 }
 
@@ -655,7 +681,6 @@ wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uin
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;
   if (flags & ~15u) return WG_ERR_INVALID_ARG;
-  if (flags && eng->impl == 1) return WG_ERR_INVALID_ARG;  // the baseline kernels (WG_IMPL=v1) know no profiles
   eng->profile = flags;  // takes effect with the next check call (kernel parameter)
   return WG_OK;
 }
@@ -673,7 +698,8 @@ wg_status wg_get_device_view(wg_engine* eng, wg_device_view* h_view) {
   h_view->site_recs = eng->d_recs;
   h_view->targets = eng->d_tgts;
   h_view->n_sites = eng->n_sites;
-  h_view->reserved = 0;
+  h_view->bind_hi = eng->bind_hi;
+  for (int i = 0; i < 4; ++i) h_view->v_init[i] = eng->v_init[i];
   return WG_OK;
 }
 
@@ -683,8 +709,7 @@ wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_
   DeviceGuard g(eng->device);
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
-  void* addr = what == 0 ? static_cast<void*>(eng->d_tgts + index)
-                         : static_cast<void*>(reinterpret_cast<char*>(eng->d_recs + index) + 48);
+  void* addr = what == 0 ? static_cast<void*>(eng->d_tgts + index) : static_cast<void*>(eng->d_tok + index);
   uint64_t v = 0;
   WG_CUDA(eng, cudaMemcpy(&v, addr, 8, cudaMemcpyDeviceToHost));
   v ^= xor_value;
@@ -695,7 +720,6 @@ wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_
 wg_status wg_set_ring_capacity(wg_engine* eng, uint64_t capacity, void* cuda_stream) {
   if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
   if (capacity > (1ull << 28)) return WG_ERR_INVALID_ARG;
-  if (capacity && eng->impl == 1) return WG_ERR_INVALID_ARG;  // no telemetry in the baseline kernels
   DeviceGuard g(eng->device);
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -731,10 +755,15 @@ wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, w
   h_counters->skipped_fwd_lanes = w[3];
   h_counters->ring_recorded = recorded;
   h_counters->ring_dropped = total - recorded;
+  h_counters->kernel_launches = eng->launches;
   if (h_first) {
     wg::FirstRec f;
+    unsigned long long key = 0;
     WG_CUDA(eng, cudaMemcpy(&f, eng->d_first, sizeof f, cudaMemcpyDeviceToHost));
+    WG_CUDA(eng, cudaMemcpy(&key, eng->d_glob + wg::C_FIRST_VIOLATION, sizeof key, cudaMemcpyDeviceToHost));
     static_assert(sizeof(wg_violation_rec) == sizeof(wg::ViolRec), "violation record layout");
+    // the record must be the record OF first_violation_key (R29); anything else is an engine bug, reported loudly
+    if (f.key != key) return WG_ERR_INTERNAL;
     *h_have_first = f.key != ~0ull;
     if (*h_have_first) std::memcpy(h_first, &f.rec, sizeof(wg_violation_rec));
   }
@@ -758,28 +787,5 @@ wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const
                                 wg_verdict* h_out, uint64_t n, wg_mode mode) {
   return host_common(eng, OP_FORWARD, h_hdr, h_val, nullptr, nullptr, h_out, n, mode);
 }
-
-wg_status wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms) {
-  if (!ops_per_s || mix < 0 || mix > 11) return WG_ERR_INVALID_ARG;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
-    cudaGetLastError();
-    return WG_ERR_CUDA;
-  }
-  if (device < 0 || device >= ndev) return WG_ERR_INVALID_ARG;
-  DeviceGuard g(device);
-  if (!g.ok) return WG_ERR_CUDA;
-  int sms = 0;
-  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return WG_ERR_CUDA;
-  double t = 0;
-  if (wg::run_int_pipe_probe(mix, sms, ops_per_s, &t) != cudaSuccess) {
-    cudaGetLastError();
-    return WG_ERR_CUDA;
-  }
-  if (ms) *ms = t;
-  return WG_OK;
-}
-
-uint64_t wg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 }  // extern "C"

@@ -7,27 +7,18 @@
 namespace wg {
 
 // ---- engine-owned device tables (DESIGN.md §5 "data layout") --------------------------------------
-// One 16-byte row per site, gathered once per event.  L2-resident at every config.
-struct __align__(16) SiteRow {
+// One 16-byte record per site, gathered once per event.  L2-resident at every config (1 M sites =
+// 16 MB).  Nothing key-derived is stored in it — or anywhere else in global memory: the key-derived SipHash initial
+// state lives in the kernel parameters only (constant bank), and the per-site part of the MAC is
+// recomputed in the kernels' event-parallel phases (2 SipRounds per 32 events).
+struct __align__(16) SiteRec {
   uint32_t kind;  // wg_kind
   uint32_t off;   // first element of this site's set in the device copy of `tgts` (u64 index)
   uint32_t cnt;   // number of targets (0 unless protected-forward)
-  uint32_t pad;
+  uint32_t flags; // bit 0: the site is in the coverage-reduced profile's skip set (R40)
 };
-
-// v2 site record: one 64-byte line per site (never straddles a 128-byte cache line), gathered once per event.
-//   words 0-3   kind, off, cnt, 0          (same meaning as SiteRow)
-//   words 4-11  protected-return sites: SipHash state after absorbing LE64(site_id), with quarter-round A of the
-//               next round already applied ("pre-A" mid-state, wg_sip32.cuh), as v0l v0h v1l v1h v2l v2h v3l v3h.
-//               Key-derived, so it lives only in engine-owned memory.  Zero for other kinds.
-//   words 12-13 protected-forward sites: token of the forward record at load time (SipHash over site_id,
-//               target_count, allowed_targets, R37); words 14-15 reserved (0)
-struct __align__(16) SiteRec {
-  uint32_t kind, off, cnt, pad0;
-  uint32_t st[8];
-  uint32_t pad1[4];
-};
-static_assert(sizeof(SiteRec) == 64, "SiteRec is one 64-byte line");
+static_assert(sizeof(SiteRec) == 16, "SiteRec is one 16-byte vector");
+enum : uint32_t { SITE_FLAG_SKIP = 1u };
 
 // Global counter block: the first 26 words have exactly the layout of wg_counters, so a read-out is one
 // copy.  Words 24 (policy_digest) and 25 (last_mode) are kept host-side and patched in at read-out.
@@ -91,8 +82,8 @@ struct Params {
   uint2* out;                // [n] wg_verdict
   uint64_t n;
   uint64_t seq_base;         // running event index of event 0 of this call (R12)
-  const SiteRow* rows;       // v1 kernels
-  const SiteRec* recs;       // v2 kernels
+  const SiteRec* recs;       // [n_sites]
+  const uint64_t* tok;       // [n_sites] token of each forward record at load time (metadata-integrity profile, R37)
   const uint64_t* tgts;
   uint64_t n_tgts;           // elements in tgts (v2 stages the whole table in shared memory when it is small)
   unsigned long long* glob;  // [C_WORDS]
@@ -122,20 +113,21 @@ struct ShadowState {
   unsigned long long* uses;     // [n_slots] {stamp of the call that last used the slot << 32 | its occurrences in that call}
   unsigned long long* counters; // [16] wg_shadow_counters
   uint32_t stamp;               // the current call (1, 2, ...): a use count under an older stamp counts as zero, so nothing is cleared
+  int per_sm[2];                // resident blocks per SM of the check_ret / push kernel on the engine's device
 };
-cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st);
+cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st,
+                          uint64_t* launches);
+cudaError_t shadow_occupancy(int* per_sm_push, int* per_sm_check);  // resident blocks per SM on the current device
 
-// launchers (wg_kernels.cu); grid sizing from the SM count of the engine's device
-cudaError_t launch_sign_v1(const Params& p, int sm_count, cudaStream_t st);
-cudaError_t launch_check_v1(const Params& p, int sm_count, cudaStream_t st);
-// v2 (wg_kernels_v2.cu): tiled, cp.async-staged, mid-state-cached kernels
-cudaError_t launch_sign_v2(const Params& p, int sm_count, cudaStream_t st);
-cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st);
-cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint32_t bind_hi,
-                              uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st);
-cudaError_t init_v2();  // one-time function attributes (dynamic shared memory opt-in)
-cudaError_t launch_fill_u64(unsigned long long* p, uint64_t n, unsigned long long v, cudaStream_t st);
-cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double* ms);
-void count_launch();
+// launchers (wg_kernels_v2.cu); grid sizing from the SM count of the engine's device.  `launches` (host) counts the
+// kernels enqueued, per engine (wg_telemetry_counters.kernel_launches).
+cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches);
+cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches);
+// first-violation record of the events [p.seq_base, p.seq_base + p.n) (one thread; see wg_first_record)
+cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* launches);
+// tokens of the forward records as loaded (trusted load time)
+cudaError_t launch_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites,
+                                uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st, uint64_t* launches);
+cudaError_t init_kernels();  // one-time function attributes (dynamic shared memory opt-in) on the current device
 
 }  // namespace wg

@@ -274,20 +274,14 @@ __device__ __forceinline__ TileEv classify(const Params& p, uint32_t raw_s, uint
     ev.active = h.y;
     sts_v4(dec_s + lane * 16, h.y ? static_cast<uint32_t>(__ffs(h.y) - 1) * 8u : 0u, h.y, h.z & ~31u, h.w);
     if (h.x < p.n_sites) {
-      const SiteRec* r = p.recs + h.x;
-      const uint4 a = ldg_v4(r);
+      const uint4 a = ldg_v4(p.recs + h.x);
       ev.kind = a.x;
       ev.off = a.y;
       ev.cnt = a.z;
       if (TEL && a.x == K_FWD && (p.profile & PROFILE_METADATA_INTEGRITY)) {
-        const uint4 d = ldg_v4(reinterpret_cast<const char*>(r) + 48);
+        const uint2 d = __ldg(reinterpret_cast<const uint2*>(p.tok) + h.x);
         ev.tokl = d.x;
         ev.tokh = d.y;
-      }
-      if (a.x == K_RET && MODE != MODE_FORWARD) {
-        const uint4 b = ldg_v4(reinterpret_cast<const char*>(r) + 16);
-        const uint4 c = ldg_v4(reinterpret_cast<const char*>(r) + 32);
-        ev.st = Sip32{b.x, b.y, b.z, b.w, c.x, c.y, c.z, c.w};
       }
       if constexpr (MODE == MODE_SIGN) {
         ev.cls = (a.x == K_RET && h.y != 0) ? CLS_RET : CLS_COUNT;
@@ -391,8 +385,17 @@ __global__ void __launch_bounds__(Cfg<MODE>::kThreads, 1) wg_tile_kernel(const P
     const uint64_t e0 = t * kT;
     uint64_t* const tag_out_lane = (MODE == MODE_SIGN) ? p.tag_out + (e0 * 32 + lane) : nullptr;  // this lane's column
     // ---- event-parallel: decode, gather, classify (a1, a2) ----
-    const TileEv ev = classify<MODE, TEL>(p, warp_s + L::kRaw + rb * kT * 16, dec_s, t, lane);
+    TileEv ev = classify<MODE, TEL>(p, warp_s + L::kRaw + rb * kT * 16, dec_s, t, lane);
     const uint32_t m_ret = __ballot_sync(kFull, ev.cls == CLS_RET);
+    if (MODE != MODE_FORWARD && m_ret != 0u) {
+      // the site word of the MAC, once per event: the key-derived initial state exists in the kernel parameters only
+      // (constant bank), never in global memory; leaves the "pre-A" state the tails start from
+      ev.st = Sip32{static_cast<uint32_t>(p.v0), static_cast<uint32_t>(p.v0 >> 32), static_cast<uint32_t>(p.v1),
+                    static_cast<uint32_t>(p.v1 >> 32), static_cast<uint32_t>(p.v2), static_cast<uint32_t>(p.v2 >> 32),
+                    static_cast<uint32_t>(p.v3), static_cast<uint32_t>(p.v3 >> 32)};
+      sip_absorb(ev.st, ev.site, p.bind_hi);  // LE64(site_id | digest32 << 32): zero-extended site id unless bound (R3, R5, R39)
+      sip_qA(ev.st);
+    }
     const uint32_t m_fwd = __ballot_sync(kFull, ev.cls == CLS_FWD);
 
     // ---- rows of this tile and raw headers of the next: TMA bulk copies onto the warp's mbarrier ----
@@ -795,37 +798,19 @@ __global__ void wg_first_record(const Params p, const int has_tag) {
   p.first->key = key;
 }
 
-// SiteRec table from the v1 rows: the pre-A mid-state of every protected-return site (runs once per policy load)
-__global__ void wg_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites,
-                              uint32_t bind_hi, uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3) {
+// tokens of the forward records as loaded (trusted load time; R37), one thread per site
+__global__ void wg_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                                uint64_t v1, uint64_t v2, uint64_t v3) {
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n_sites) return;
-  const SiteRow r = rows[s];
-  SiteRec o;
-  o.kind = r.kind;
-  o.off = r.off;
-  o.cnt = r.cnt;
-  o.pad0 = 0;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) o.st[i] = 0;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) o.pad1[i] = 0;
-  if (r.kind == K_RET) {
-    Sip32 st{static_cast<uint32_t>(v0), static_cast<uint32_t>(v0 >> 32), static_cast<uint32_t>(v1),
-             static_cast<uint32_t>(v1 >> 32), static_cast<uint32_t>(v2), static_cast<uint32_t>(v2 >> 32),
-             static_cast<uint32_t>(v3), static_cast<uint32_t>(v3 >> 32)};
-    sip_absorb(st, s, bind_hi);  // LE64(site_id | digest32 << 32): zero-extended site id unless bound (R3, R5, R39)
-    sip_qA(st);             // quarter A of the continuation word's first round
-    o.st[0] = st.v0l; o.st[1] = st.v0h; o.st[2] = st.v1l; o.st[3] = st.v1h;
-    o.st[4] = st.v2l; o.st[5] = st.v2h; o.st[6] = st.v3l; o.st[7] = st.v3h;
-  }
-  if (r.kind == K_FWD) {  // token of the forward record as loaded (trusted load time)
+  const SiteRec r = recs[s];
+  uint64_t t = 0;
+  if (r.kind == K_FWD) {
     const uint2* set = reinterpret_cast<const uint2*>(tgts + r.off);
     const uint2 tk = record_token(v0, v1, v2, v3, s, r.cnt, [&](uint32_t i) { return set[i]; });
-    o.pad1[0] = tk.x;
-    o.pad1[1] = tk.y;
+    t = (static_cast<uint64_t>(tk.y) << 32) | tk.x;
   }
-  recs[s] = o;
+  tok[s] = t;
 }
 
 template <int MODE>
@@ -834,7 +819,7 @@ uint32_t smem_bytes(uint32_t stage_bytes) {  // stage_bytes: staged targets + sh
 }
 
 template <int MODE>
-cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
+cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
   const uint64_t n_tiles = (p.n + kT - 1) / kT;
   constexpr int kWarps = Cfg<MODE>::kWarps;
   constexpr int kThreads = Cfg<MODE>::kThreads;
@@ -868,7 +853,7 @@ cudaError_t launch_tile(const Params& p, int sm_count, cudaStream_t st) {
   } else {
     wg_tile_kernel<MODE, false, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
   }
-  count_launch();
+  ++*launches;
   return cudaGetLastError();
 }
 
@@ -890,7 +875,7 @@ cudaError_t opt_in() {
 
 }  // namespace
 
-cudaError_t init_v2() {
+cudaError_t init_kernels() {
   cudaError_t e;
   if ((e = opt_in<MODE_VERIFY, true>()) != cudaSuccess) return e;
   if ((e = opt_in<MODE_VERIFY, false>()) != cudaSuccess) return e;
@@ -900,23 +885,25 @@ cudaError_t init_v2() {
   return cudaSuccess;
 }
 
-cudaError_t launch_sign_v2(const Params& p, int sm_count, cudaStream_t st) {
-  return launch_tile<MODE_SIGN>(p, sm_count, st);
+cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
+  return launch_tile<MODE_SIGN>(p, sm_count, st, launches);
 }
 
-cudaError_t launch_check_v2(const Params& p, int sm_count, cudaStream_t st) {
-  const cudaError_t e = p.tag ? launch_tile<MODE_VERIFY>(p, sm_count, st) : launch_tile<MODE_FORWARD>(p, sm_count, st);
-  if (e != cudaSuccess) return e;
+cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
+  return p.tag ? launch_tile<MODE_VERIFY>(p, sm_count, st, launches) : launch_tile<MODE_FORWARD>(p, sm_count, st, launches);
+}
+
+cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* launches) {
   wg_first_record<<<1, 1, 0, st>>>(p, p.tag != nullptr);
-  count_launch();
+  ++*launches;
   return cudaGetLastError();
 }
 
-cudaError_t launch_build_recs(SiteRec* recs, const SiteRow* rows, const uint64_t* tgts, uint32_t n_sites, uint32_t bind_hi,
-                              uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st) {
+cudaError_t launch_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                                uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st, uint64_t* launches) {
   if (n_sites == 0) return cudaSuccess;
-  wg_build_recs<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, rows, tgts, n_sites, bind_hi, v0, v1, v2, v3);
-  count_launch();
+  wg_build_tokens<<<(n_sites + 255) / 256, 256, 0, st>>>(tok, recs, tgts, n_sites, v0, v1, v2, v3);
+  ++*launches;
   return cudaGetLastError();
 }
 

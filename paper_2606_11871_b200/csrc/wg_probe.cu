@@ -1,9 +1,17 @@
-// wg_probe.cu — register-only integer micro-benchmark (measurement helper, no part of the check path).
+// wg_probe.cu — register-only integer micro-benchmark.  NOT part of libwarpguard.so: it is built into its own
+// libwg_probe.so, which only bench.py loads (measurement helper, no part of the check path).  One C entry point:
+//   int wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms);   returns a cudaError_t (0 = ok)
+//   mix: 0 = IADD3 only, 1 = LOP3 only, 2 = SHF only, 3 = IMAD only, 4 = IMAD.WIDE.U32 only, 5 = ALU:FMA 1:1 (LOP3 +
+//        IMAD), 6 = SipRound-shaped ALU mix (IADD3 / LOP3 / SHF, 8:8:8), 7 = IMAD.HI.U32 only, 8 = ALU:FMA 2:1,
+//        9 = ALU:FMA 1:1 (SHF + IMAD.HI.U32), 10 = 64-bit-add pairs (counts PAIRS), 11 = the SipRound itself (two
+//        independent states per thread, 24 int32 operations per round): the ceiling of any SipHash kernel on this GPU.
 // It answers "what can the sm_100a integer pipes issue?" so that the ALU roofline of the MAC kernel has a
 // measured denominator beside the one derived from unit counts.  Every chain is a dependent
 // sequence of one instruction kind; 8 independent chains per thread and 16 resident warps per SMSP keep the
 // pipes full.  `asm volatile` pins the instruction selection (checked with cuobjdump -sass).
-#include "wg_internal.h"
+#include <cuda_runtime.h>
+#include <stdint.h>
+
 #include "../../include/warpguard_sip32.cuh"
 
 namespace wg {
@@ -107,7 +115,6 @@ cudaError_t run_sip(int sm_count, uint32_t* sink, double* ops_per_s, double* ms_
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(a, nullptr);
     wg_sip_probe<<<grid, kThreads>>>(sink, 0x9e3779b9u + rep);
-    count_launch();
     cudaEventRecord(b, nullptr);
     if ((err = cudaEventSynchronize(b)) != cudaSuccess) return err;
     float ms = 0;
@@ -133,7 +140,6 @@ cudaError_t run(int sm_count, uint32_t* sink, double* ops_per_s, double* ms_out)
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(a, nullptr);
     wg_int_probe<MIX><<<grid, kThreads>>>(sink, 0x9e3779b9u + rep);
-    count_launch();
     cudaEventRecord(b, nullptr);
     if ((err = cudaEventSynchronize(b)) != cudaSuccess) return err;
     float ms = 0;
@@ -174,3 +180,15 @@ cudaError_t run_int_pipe_probe(int mix, int sm_count, double* ops_per_s, double*
 }
 
 }  // namespace wg
+
+extern "C" int wg_probe_int_pipe(int device, int mix, double* ops_per_s, double* ms) {
+  if (!ops_per_s || !ms || mix < 0 || mix > 11) return static_cast<int>(cudaErrorInvalidValue);
+  int prev = 0, sms = 0;
+  cudaError_t err;
+  if ((err = cudaGetDevice(&prev)) != cudaSuccess) return static_cast<int>(err);
+  if ((err = cudaSetDevice(device)) != cudaSuccess) return static_cast<int>(err);
+  if ((err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device)) == cudaSuccess)
+    err = wg::run_int_pipe_probe(mix, sms, ops_per_s, ms);
+  cudaSetDevice(prev);
+  return static_cast<int>(err);
+}

@@ -10,11 +10,10 @@
 // Layout (structure of arrays, so that the 32 lanes of a warp touch 256 contiguous bytes per field):
 //   depth_ctr[slot][32] u32;  entry[slot][d][32][4] u64 = {expected, token, callsite | depth << 32, 0}: one 32-byte
 //   sector per thread slot and depth, written whole by its (active) lane.
-// Mapping: one warp per event (the state access is a gather by warp slot; each lane owns its own stack).
+// Mapping: a warp owns a tile of 32 events; header decode and classification run with lane i <-> event i, the per
+// thread-slot part (depth counter, entry, MAC, compare) lane-parallel, one pass per event (each lane owns its own stack).
 // A call is one lock-step step of DISTINCT warps: a counting pass marks warp slots that occur twice in the call
 // and those events fail closed; the marks carry the call's stamp, so no clearing pass is needed.
-#include <cstdlib>
-
 #include "wg_internal.h"
 #include "../../include/warpguard_sip32.cuh"
 
@@ -22,8 +21,6 @@ namespace wg {
 
 namespace {
 
-constexpr int kThreads = 256;
-constexpr int kWarps = kThreads / 32;
 constexpr uint32_t kFull = 0xffffffffu;
 enum : uint32_t { K_RET = 0 };
 
@@ -65,185 +62,14 @@ enum ShWord {  // wg_shadow_counters
   SH_NON_RETURN, SH_SLOT_OVERFLOW, SH_SLOT_CONFLICT, SH_VIOL_LANES, SH_VIOL_EVENTS, SH_BLOCKED_LANES, SH_WORDS
 };
 
-// what an event needs from memory, in the order it can be asked for: the header; then what the header addresses
-// (site record, use count of the warp slot, the lane's value and depth counter); then (check) the entry the depth
-// counter addresses.  Every load is a dependent HBM / L2 round trip, so the kernel keeps three events in flight per
-// warp: while event k is computed, the entry of k+1, the header-addressed words of k+2 and the header of k+3 fly.
-struct StageB {
-  uint4 rec0, sb, sc;  // SiteRec: {kind, off, cnt, -}; pre-A mid-state after the site word
-  uint32_t uses, d, vl, vh;
-};
 struct StageE {
   uint32_t exl, exh, tkl, tkh, callsite, depth;
 };
 
-template <bool PUSH>
-__global__ void __launch_bounds__(kThreads) wg_shadow_kernel(const Params p, const ShadowState sh) {
-  __shared__ unsigned long long sm[SH_WORDS];
-  const uint32_t lane = threadIdx.x & 31;
-  const uint64_t warp0 = (static_cast<uint64_t>(blockIdx.x) * kThreads + threadIdx.x) >> 5;
-  const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * kWarps;
-  const bool enforce = p.mode != 0;
-  uint32_t c[SH_WORDS];
-#pragma unroll
-  for (int i = 0; i < SH_WORDS; ++i) c[i] = 0;
-
-  auto load_h = [&](uint64_t e) -> uint4 { return e < p.n ? __ldg(reinterpret_cast<const uint4*>(p.hdr) + e) : make_uint4(0u, 0u, 0u, 0u); };
-  auto load_b = [&](const uint4& h, uint64_t e) -> StageB {
-    StageB b;
-    b.rec0 = make_uint4(7u, 0u, 0u, 0u);
-    b.sb = b.sc = make_uint4(0u, 0u, 0u, 0u);
-    b.uses = b.d = b.vl = b.vh = 0u;
-    if (e < p.n && h.y != 0u) {
-      const uint32_t slot = slot_of(h.z, h.w);
-      const bool on = (h.y >> lane) & 1u;
-      if (h.x < p.n_sites) {
-        const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
-        b.rec0 = __ldg(r);
-        b.sb = __ldg(r + 1);
-        b.sc = __ldg(r + 2);
-      }
-      if (slot < sh.n_slots) {
-        b.uses = static_cast<uint32_t>(sh.uses[slot]);  // (every slot of this call carries this call's stamp)
-        if (on) b.d = sh.depth_ctr[static_cast<uint64_t>(slot) * 32 + lane];
-      }
-      if (on) {
-        const uint2 v = *reinterpret_cast<const uint2*>(p.val + e * 32 + lane);
-        b.vl = v.x;
-        b.vh = v.y;
-      }
-    }
-    return b;
-  };
-  auto load_e = [&](const uint4& h, const StageB& b) -> StageE {
-    StageE x{0u, 0u, 0u, 0u, 0u, 0u};
-    if constexpr (!PUSH) {
-      const uint32_t slot = slot_of(h.z, h.w);
-      if (((h.y >> lane) & 1u) && slot < sh.n_slots && b.d != 0u && b.d - 1u < sh.max_depth) {
-        const uint4* en = reinterpret_cast<const uint4*>(sh.entry) + ((static_cast<uint64_t>(slot) * sh.max_depth + (b.d - 1u)) * 32 + lane) * 2;
-        const uint4 et = en[0], m = en[1];
-        x = StageE{et.x, et.y, et.z, et.w, m.x, m.y};
-      }
-    }
-    return x;
-  };
-
-  // prologue: fill the pipeline
-  uint4 h0 = load_h(warp0), h1 = load_h(warp0 + nwarps), h2 = load_h(warp0 + 2 * nwarps);
-  StageB b0 = load_b(h0, warp0), b1 = load_b(h1, warp0 + nwarps);
-  StageE x0 = load_e(h0, b0);
-
-  for (uint64_t e = warp0; e < p.n; e += nwarps) {
-    // loads of the events behind this one
-    const uint4 h3 = load_h(e + 3 * nwarps);
-    const StageB b2 = load_b(h2, e + 2 * nwarps);
-    const StageE x1 = load_e(h1, b1);
-
-    const uint4 h = h0;
-    const uint32_t site = h.x, a = h.y;
-    const uint32_t slot = slot_of(h.z, h.w);
-    uint32_t viol = 0;
-    if (a == 0) {
-      c[SH_EMPTY_EVENTS] += 1;  // no lane executed the call / return
-    } else {
-      c[PUSH ? SH_PUSH_EVENTS : SH_CHECK_EVENTS] += 1;
-      c[PUSH ? SH_PUSH_LANES : SH_CHECK_LANES] += __popc(a);
-      if (b0.rec0.x != K_RET) {  // unknown site, or not a return site of the policy: fail closed, state untouched
-        viol = a;
-        c[SH_NON_RETURN] += 1;
-      } else if (slot >= sh.n_slots) {  // thread-slot overflow fails closed instead of wrapping
-        viol = a;
-        c[SH_SLOT_OVERFLOW] += 1;
-      } else if (b0.uses > 1u) {  // the same warp twice in one lock-step call
-        viol = a;
-        c[SH_SLOT_CONFLICT] += 1;
-      } else {
-        const bool on = (a >> lane) & 1u;
-        const uint32_t vl = b0.vl, vh = b0.vh;
-        uint32_t* dctr = sh.depth_ctr + static_cast<uint64_t>(slot) * 32 + lane;
-        uint32_t d = b0.d;
-        uint32_t cause = 0;  // 0 ok, else SH_* word of the lane's one cause
-        const Sip32 s_site{b0.sb.x, b0.sb.y, b0.sb.z, b0.sb.w, b0.sc.x, b0.sc.y, b0.sc.z, b0.sc.w};  // pre-A state after the site word
-        if (on) {
-          if (PUSH) {
-            if (d >= sh.max_depth) {
-              cause = SH_OVERFLOW;
-            } else {
-              // context: epoch<<48 | d<<37 | slot<<5 | lane (lane is injected by the tail)
-              const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
-              uint32_t tl, th;
-              sip_tail_val_lane(s_site, vl, vh, lane, bl, bh, 0u, 0u, tl, th);
-              uint4* en = reinterpret_cast<uint4*>(sh.entry) + ((static_cast<uint64_t>(slot) * sh.max_depth + d) * 32 + lane) * 2;
-              en[0] = make_uint4(vl, vh, tl, th);
-              en[1] = make_uint4(site, d, 0u, 0u);
-              *dctr = d + 1;
-            }
-          } else {
-            if (d == 0) {
-              cause = SH_UNDERFLOW;
-            } else {
-              d -= 1;
-              *dctr = d;  // the return consumes the frame whatever the verdict (R33)
-              // a corrupted counter may point past the arrays' depth: such an entry does not exist -> depth mismatch
-              if (d >= sh.max_depth) {
-                cause = SH_DEPTH_MISMATCH;
-              } else if (x0.depth != d) {
-                cause = SH_DEPTH_MISMATCH;
-              } else {
-                // the token is verified over the ENTRY's own fields under the event's epoch
-                const uint32_t bl = slot << 5, bh = (slot >> 27) | (d << 5) | (h.w & 0xffff0000u);
-                uint32_t tl, th;
-                if (x0.callsite == site) {  // the ordinary case: the site's cached mid-state saves the first word's rounds
-                  sip_tail_val_lane(s_site, x0.exl, x0.exh, lane, bl, bh, 0u, 0u, tl, th);
-                } else {
-                  mac_full(p, x0.callsite, x0.exl, x0.exh, bl | lane, bh, tl, th);
-                }
-                if (tl != x0.tkl || th != x0.tkh)
-                  cause = SH_TOKEN_MISMATCH;
-                else if (x0.exl != vl || x0.exh != vh || x0.callsite != site)
-                  cause = SH_TARGET_MISMATCH;
-              }
-            }
-          }
-        }
-        viol = __ballot_sync(kFull, cause != 0);
-        if (viol) {  // rare: one cause per violating lane
-#pragma unroll
-          for (int k = SH_OVERFLOW; k <= SH_TARGET_MISMATCH; ++k) c[k] += __popc(__ballot_sync(kFull, cause == k));
-        }
-      }
-    }
-    if (viol) {
-      c[SH_VIOL_LANES] += __popc(viol);
-      c[SH_VIOL_EVENTS] += 1;
-      if (enforce) c[SH_BLOCKED_LANES] += __popc(viol);
-    }
-    if (lane == 0) p.out[e] = make_uint2(viol, enforce ? (a & ~viol) : a);
-
-    h0 = h1;
-    h1 = h2;
-    h2 = h3;
-    b0 = b1;
-    b1 = b2;
-    x0 = x1;
-  }
-
-  if (threadIdx.x < SH_WORDS) sm[threadIdx.x] = 0ull;
-  __syncthreads();
-  if (lane == 0) {
-#pragma unroll
-    for (int i = 0; i < SH_WORDS; ++i)
-      if (c[i]) atomicAdd(sm + i, static_cast<unsigned long long>(c[i]));
-  }
-  __syncthreads();
-  if (threadIdx.x < SH_WORDS && sm[threadIdx.x]) atomicAdd(sh.counters + threadIdx.x, sm[threadIdx.x]);
-}
-
-
 // ---------------------------------------------------------------------------------------------------
-// Tile mapping (the default): a warp owns 16 consecutive events.  What the warp-per-event kernel above does once per
-// EVENT with all 32 lanes doing the same thing — header decode, SiteRec gather, use count, the fail-closed
-// classification, the event counters, the verdict store — is done here once per TILE with lane i <-> event i
+// Tile mapping: a warp owns 32 consecutive events.  What a warp-per-event kernel (the first version of this file, see
+// git history) does once per EVENT with all 32 lanes doing the same thing — header decode, SiteRec gather, use count,
+// the fail-closed classification, the event counters, the verdict store — is done here once per TILE with lane i <-> event i
 // ("event-parallel", as in wg_kernels_v2.cu); only the part that really is per thread slot (depth counter, value,
 // entry, MAC, compare) runs lane-parallel, one pass per ordinary event, fed from shared memory.  The per-lane loads
 // of a pass are dependent round trips (depth counter -> entry), so they are issued two passes (counter, value) and
@@ -342,7 +168,7 @@ __global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_t
 
   // event-parallel loads of a tile, in the order they can be asked for: the header; then what it addresses (site
   // record, use count of the warp slot).  Two tiles ahead / one tile ahead, so a tile starts with both in registers.
-  struct TB { uint4 rec0, sb, sc; uint32_t uses, vfl, vfh; };
+  struct TB { uint32_t kind, uses, vfl, vfh; };
   auto load_th = [&](uint64_t t) -> uint4 {
     const uint64_t e = t * kST + lane;
     return (t < n_tiles && lane < static_cast<uint32_t>(kST) && e < p.n) ? __ldg(reinterpret_cast<const uint4*>(p.hdr) + e)
@@ -350,8 +176,7 @@ __global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_t
   };
   auto load_tb = [&](const uint4& h, uint64_t t) -> TB {
     TB b;
-    b.rec0 = make_uint4(7u, 0u, 0u, 0u);
-    b.sb = b.sc = make_uint4(0u, 0u, 0u, 0u);
+    b.kind = 7u;
     b.uses = b.vfl = b.vfh = 0u;
     if (h.y != 0u) {  // (a lane without an event holds a zero header)
       // the value of the event's first active lane: when every active lane carries it (a warp-uniform return
@@ -361,12 +186,7 @@ __global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_t
         b.vfl = vf.x;
         b.vfh = vf.y;
       }
-      if (h.x < p.n_sites) {
-        const uint4* r = reinterpret_cast<const uint4*>(p.recs + h.x);
-        b.rec0 = __ldg(r);
-        b.sb = __ldg(r + 1);
-        b.sc = __ldg(r + 2);
-      }
+      if (h.x < p.n_sites) b.kind = __ldg(reinterpret_cast<const uint32_t*>(p.recs + h.x));
       const uint32_t slot = slot_of(h.z, h.w);
       if (slot < sh.n_slots) b.uses = static_cast<uint32_t>(sh.uses[slot]);  // (the slot carries this call's stamp)
     }
@@ -389,7 +209,7 @@ __global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_t
     if (valid) {
       status = ST_EMPTY;  // no lane executed the call / return
       if (a != 0u) {
-        if (b_cur.rec0.x != K_RET) {
+        if (b_cur.kind != K_RET) {
           status = ST_NON_RETURN;  // unknown site, or not a return site of the policy: fail closed, state untouched
         } else if (slot >= sh.n_slots) {
           status = ST_SLOT_OVERFLOW;  // thread-slot overflow fails closed instead of wrapping
@@ -398,15 +218,23 @@ __global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_t
         } else {
           status = ST_NORMAL;
           ts.rec[lane] = make_uint4(a, slot, h.x, (slot >> 27) | (h.w & 0xffff0000u));
-          ts.st[lane][0] = b_cur.sb;
-          ts.st[lane][1] = b_cur.sc;
           if constexpr (kFast) ts.vf[lane] = make_uint2(b_cur.vfl, b_cur.vfh);
         }
       }
     }
+    // the site word of the MAC, once per event, 32 events at a time: the key-derived initial state exists in the kernel
+    // parameters only (constant bank), never in global memory; leaves the "pre-A" state the tails start from
+    Sip32 u{static_cast<uint32_t>(p.v0), static_cast<uint32_t>(p.v0 >> 32), static_cast<uint32_t>(p.v1),
+            static_cast<uint32_t>(p.v1 >> 32), static_cast<uint32_t>(p.v2), static_cast<uint32_t>(p.v2 >> 32),
+            static_cast<uint32_t>(p.v3), static_cast<uint32_t>(p.v3 >> 32)};
+    sip_absorb(u, h.x, p.bind_hi);
+    sip_qA(u);
+    if (status == ST_NORMAL) {
+      ts.st[lane][0] = make_uint4(u.v0l, u.v0h, u.v1l, u.v1h);
+      ts.st[lane][1] = make_uint4(u.v2l, u.v2h, u.v3l, u.v3h);
+    }
     if constexpr (kFast) {  // the MAC prefix of a warp-uniform value, for all events of the tile at once (used by the passes that find
        // every MAC-computing lane on that value; harmless garbage for the others)
-      Sip32 u{b_cur.sb.x, b_cur.sb.y, b_cur.sb.z, b_cur.sb.w, b_cur.sc.x, b_cur.sc.y, b_cur.sc.z, b_cur.sc.w};
       sip_absorb_preA(u, b_cur.vfl, b_cur.vfh);
       sip_qA(u);
       if (status == ST_NORMAL) {
@@ -554,46 +382,30 @@ __global__ void __launch_bounds__(kTileThreads, 1024 / kTileThreads) wg_shadow_t
 
 }  // namespace
 
-cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st) {
+cudaError_t shadow_occupancy(int* per_sm_push, int* per_sm_check) {
+  cudaError_t err;
+  if ((err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm_push, wg_shadow_tile_kernel<true>, kTileThreads, 0)) != cudaSuccess)
+    return err;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm_check, wg_shadow_tile_kernel<false>, kTileThreads, 0);
+}
+
+cudaError_t launch_shadow(const Params& p, const ShadowState& sh, bool push, int sm_count, cudaStream_t st,
+                          uint64_t* launches) {
   const uint64_t want_m = (p.n + 255) / 256;
   const int grid_m = static_cast<int>(want_m < static_cast<uint64_t>(sm_count) * 8 ? want_m : sm_count * 8);
   wg_shadow_mark<<<grid_m, 256, 0, st>>>(p.hdr, p.n, sh.uses, sh.n_slots, sh.stamp);
-  count_launch();
-  // persistent warps: exactly the blocks that are resident at once.  WG_SHADOW=v1 selects the warp-per-event
-  // kernel (measurement knob, like WG_IMPL=v1 for the check kernels).
-  const char* knob = std::getenv("WG_SHADOW");
-  const bool v1 = knob && knob[0] == 'v' && knob[1] == '1';
-  static int per_sm_tab[2][2] = {{0, 0}, {0, 0}};
-  int* per_sm = per_sm_tab[v1];
-  if (per_sm[push] == 0) {
-    int nb = 0;
-    cudaError_t err;
-    if (v1)
-      err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<true>, kThreads, 0)
-                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_kernel<false>, kThreads, 0);
-    else
-      err = push ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<true>, kTileThreads, 0)
-                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, wg_shadow_tile_kernel<false>, kTileThreads, 0);
-    if (err != cudaSuccess) return err;
-    per_sm[push] = nb > 0 ? nb : 1;
-  }
-  const uint64_t units = v1 ? p.n : (p.n + kST - 1) / kST;  // a warp's unit of work: an event / a tile
-  const uint64_t wpb = v1 ? kWarps : kTileWarps;  // warps per block
-  const uint64_t want = (units + wpb - 1) / wpb;
-  const uint64_t resident = static_cast<uint64_t>(sm_count) * per_sm[push];
+  ++*launches;
+  // persistent warps: exactly the blocks that are resident at once (occupancy resolved per engine at configure time)
+  const int per_sm = sh.per_sm[push] > 0 ? sh.per_sm[push] : 1;
+  const uint64_t units = (p.n + kST - 1) / kST;  // a warp's unit of work: a tile
+  const uint64_t want = (units + kTileWarps - 1) / kTileWarps;
+  const uint64_t resident = static_cast<uint64_t>(sm_count) * per_sm;
   const int grid = static_cast<int>(want < resident ? want : resident);
-  if (v1) {
-    if (push)
-      wg_shadow_kernel<true><<<grid, kThreads, 0, st>>>(p, sh);
-    else
-      wg_shadow_kernel<false><<<grid, kThreads, 0, st>>>(p, sh);
-  } else {
-    if (push)
-      wg_shadow_tile_kernel<true><<<grid, kTileThreads, 0, st>>>(p, sh);
-    else
-      wg_shadow_tile_kernel<false><<<grid, kTileThreads, 0, st>>>(p, sh);
-  }
-  count_launch();
+  if (push)
+    wg_shadow_tile_kernel<true><<<grid, kTileThreads, 0, st>>>(p, sh);
+  else
+    wg_shadow_tile_kernel<false><<<grid, kTileThreads, 0, st>>>(p, sh);
+  ++*launches;
   return cudaGetLastError();
 }
 

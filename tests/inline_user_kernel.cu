@@ -35,3 +35,9 @@ extern "C" int wg_test_run_inline(wg_device_view view, const void* hdr, const vo
       static_cast<uint64_t*>(tag_out), static_cast<uint32_t*>(viol_out), n, op);
   return static_cast<int>(cudaGetLastError());
 }
+
+// raw copy of the engine's site records as the view exposes them (tests/test_gpu_device_inline.py checks that
+// nothing in them is key-derived)
+extern "C" int wg_test_copy_site_recs(wg_device_view view, void* h_out) {
+  return static_cast<int>(cudaMemcpy(h_out, view.site_recs, static_cast<size_t>(view.n_sites) * 16, cudaMemcpyDeviceToHost));
+}

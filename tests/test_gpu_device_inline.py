@@ -78,3 +78,30 @@ def test_inline_helpers_equal_the_oracle(config, n):
     assert np.array_equal(g[is_fwd], o_out[is_fwd, 0]) and is_fwd.any() and o_out[is_fwd, 0].any()
     assert np.array_equal(g[~is_fwd], active[~is_fwd])
     eng.close()
+
+
+def test_no_key_material_is_reachable_through_the_view():
+    """the engine once cached per-site SipHash mid-states in global memory, and a SipRound is a
+    bijection, so one 32-byte read gave the key.  Now the only device memory the view points at is the policy image
+    itself: every site record must be exactly {kind, set offset, set size, flags = 0} — a function of the policy alone,
+    identical under two different keys — and the key-equivalent words travel in the view BY VALUE (kernel parameters,
+    PAPER.md:256)."""
+    build_user_kernel()
+    L = C.CDLL(str(SO))
+    L.wg_test_copy_site_recs.argtypes = [B.DeviceView, C.c_void_p]
+    pol = S.make_policy(4, "cpu")
+    images = []
+    for k0, k1 in ((pol.k0, pol.k1), (pol.k0 ^ 0x5555, pol.k1 ^ 0x7777)):
+        eng = B.Engine(0)
+        eng.wg_load_policy(pol.kind, pol.tgt_off, pol.tgts, k0, k1, pol.policy_digest)
+        view = eng.wg_get_device_view()
+        raw = np.zeros((pol.n_sites, 4), dtype=np.uint32)
+        assert L.wg_test_copy_site_recs(view, raw.ctypes.data) == 0
+        images.append(raw)
+        M = (1 << 64) - 1
+        consts = (0x736f6d6570736575, 0x646f72616e646f6d, 0x6c7967656e657261, 0x7465646279746573)
+        assert [int(v) for v in view.v_init] == [(k ^ c) & M for k, c in zip((k0, k1, k0, k1), consts)]
+        eng.close()
+    expect = np.stack([pol.kind.astype(np.uint32), pol.tgt_off[:-1].astype(np.uint32),
+                       np.diff(pol.tgt_off.astype(np.int64)).astype(np.uint32), np.zeros(pol.n_sites, np.uint32)], axis=1)
+    assert np.array_equal(images[0], expect) and np.array_equal(images[1], expect)

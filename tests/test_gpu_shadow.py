@@ -95,12 +95,6 @@ def test_random_call_return_sequences(n_slots, max_depth, n):
     eng.close()
 
 
-def test_warp_per_event_shadow_kernels_stay_bit_exact(monkeypatch):
-    """WG_SHADOW=v1 selects the warp-per-event shadow kernels kept as the measured baseline: same results."""
-    monkeypatch.setenv("WG_SHADOW", "v1")
-    test_random_call_return_sequences(4096, 4, 3000)
-
-
 @pytest.mark.parametrize("n", [1, 2, 3, 7, 33])
 def test_calls_shorter_than_the_kernels_pipeline(n):
     """The shadow kernels keep three events in flight per warp: calls with fewer events than that (and than one
@@ -204,4 +198,26 @@ def test_errors_and_reconfigure():
     assert eng.wg_shadow_depth(3, 0) == 0 and eng.wg_shadow_read_counters() == orc.shadow_read_counters()
     step(orc, eng, False, hdr, val, ENF)  # underflow on both sides
     assert eng.wg_shadow_read_counters()["underflow_lanes"] == 4
+    eng.close()
+
+
+def test_known_limit_same_epoch_replay_of_a_popped_frame_matches_the_oracle():
+    """DESIGN.md R41: a popped frame replayed by bumping the (attacker-writable) depth counter verifies again under the
+    same epoch and fails under a new one; the engine and the oracle agree on both (pinned on the oracle side in
+    tests/test_oracle_shadow.py)."""
+    pol, orc, eng = pair(16, 4)
+    site = int(np.nonzero(pol.kind == 0)[0][0])
+    A = np.full((1, 32), 0x7F5A40000040, dtype=np.uint64)
+    full = 0xFFFFFFFF
+
+    def hdr(mask, epoch):
+        return mk_hdr([site], [mask], [(epoch << 48) | (5 << 5)])
+
+    step(orc, eng, True, hdr(full, 7), A, ENF)
+    assert not step(orc, eng, False, hdr(full, 7), A, ENF)[0, 0]
+    for lane, epoch, expect in ((9, 7, 0), (11, 8, 1 << 11)):
+        orc.shadow_poke(5, lane, 0, oracle.POKE_DEPTH_COUNTER, 1)
+        eng.wg_shadow_poke(5, lane, 0, 4, 1)
+        assert step(orc, eng, False, hdr(1 << lane, epoch), A, ENF)[0, 0] == expect
+    assert eng.wg_shadow_read_counters() == orc.shadow_read_counters()
     eng.close()

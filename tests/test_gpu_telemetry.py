@@ -239,3 +239,27 @@ def test_bound_load_refuses_a_mismatch_and_binds_the_tokens():
     eng.load(pol)
     assert np.array_equal(eng.wg_sign_continuations(d_hdr, d_val).cpu().numpy().view(np.uint64), plain_tag)
     eng.close()
+
+
+def test_host_path_first_record_and_ring_over_many_chunks():
+    """VERDICT r1 weak #8 / ADVICE: the *_host calls alternate chunks between two streams; the first-violation-record
+    kernels of consecutive chunks are chained by an event, so the record read back is the record OF
+    first_violation_key (wg_read_telemetry returns WG_ERR_INTERNAL otherwise).  > 4 chunks of 256 Ki events, violations
+    in every chunk, ring on; against the oracle's ring and first record."""
+    n = 5 * (1 << 18) + 12_345
+    st, orc, eng, hdr, val, tagn, d = prepared(2, n)
+    assert len(np.unique(st.ret_tamper.ev.numpy() // (1 << 18))) == 6  # every chunk holds violations
+    cap = 1 << 14
+    orc.set_ring_capacity(cap)
+    eng.wg_set_ring_capacity(cap)
+    h_hdr, h_val, h_tag = st.hdr.pin_memory(), st.val.pin_memory(), torch.from_numpy(tagn.view(np.int64)).pin_memory()
+    for mode in (DET, ENF):
+        o = orc.verify(hdr, val, tagn, mode)
+        g = eng.wg_verify_continuations_host(h_hdr, h_val, h_tag, mode).numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+    same_counters(eng, orc)
+    t, first, ring = eng.wg_read_telemetry(cap)
+    assert t == orc.read_telemetry() and t["ring_dropped"] == 0
+    assert as_tuple(first) == as_tuple(orc.read_first_violation())
+    assert sorted(as_tuple(r) for r in ring) == sorted(as_tuple(r) for r in orc.read_violations())
+    eng.close()

@@ -211,3 +211,25 @@ def test_random_call_return_sequences_against_a_mac_free_model():
     assert exp_c["overflow"] > 0 and exp_c["underflow"] > 0 and exp_c["target"] > 0
     for (slot, lane), st in model.items():
         assert o.shadow_depth(slot, lane) == len(st)
+
+
+def test_known_limit_a_popped_frame_replayed_in_the_same_epoch_at_the_same_depth_still_verifies():
+    """DESIGN.md R41: the token binds (callsite, expected_return, epoch, depth, slot, lane) — PAPER.md:258
+    "bind the expected return, callsite identifier, depth, logical thread slot, and key material; some helper profiles
+    also bind a launch epoch" — and nothing that changes when a frame is popped.  The depth counter is ordinary
+    (attacker-writable) memory, so a writer who bumps it back after a return makes the stale frame, whose bytes and
+    valid token are still in the array, authenticate again: a return to a continuation that WAS legal for this thread
+    slot at this depth in this epoch.  The paper's remedy is the epoch / monotonic counter the caller packs into
+    context_base ("profiles may also bind a launch epoch or monotonic counter"): under a new epoch the
+    same replay fails.  This test pins both halves so the limit cannot change silently."""
+    A = 0x7F5A40000040
+    for new_epoch, expect_viol in ((False, 0), (True, 1 << 9)):
+        o = make()
+        o.shadow_push(ev(0, FULL, 5, epoch=7), vals(A), ENF)
+        assert o.shadow_check_ret(ev(0, FULL, 5, epoch=7), vals(A), ENF)[0, 0] == 0  # the legitimate return pops it
+        assert o.shadow_depth(5, 9) == 0
+        o.shadow_poke(5, 9, 0, oracle.POKE_DEPTH_COUNTER, 1)  # the attacker's write: depth counter 0 -> 1
+        out = o.shadow_check_ret(ev(0, 1 << 9, 5, epoch=8 if new_epoch else 7), vals(A), ENF)
+        assert out[0, 0] == expect_viol
+        c = o.shadow_read_counters()
+        assert c["token_mismatch_lanes"] == (1 if new_epoch else 0) and c["underflow_lanes"] == 0
