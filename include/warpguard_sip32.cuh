@@ -162,6 +162,33 @@ __device__ __forceinline__ void sip_tail_val_lane(Sip32 s, uint32_t vl, uint32_t
   sip_finish(s, xl, xh, outl, outh);
 }
 
+// The two tails of the compacted consumer passes (csrc/wg_check.cu): the lane index comes from a work item, so the
+// caller hands in the whole context word (cl, ch) = (B ^ lane, B >> 32).
+// (1) warp-uniform continuation: s covers site and continuation, has quarter A of the next round applied and B folded
+//     into v3, and the caller has XORed the lane's five bits into s.v3l.
+__device__ __forceinline__ void sip_tail_ctxlane(Sip32 s, uint32_t cl, uint32_t ch, uint32_t xl, uint32_t xh,
+                                                 uint32_t& outl, uint32_t& outh) {
+  sip_qB(s);
+  sip_qC(s);
+  sip_qD(s);
+  sip_round(s);
+  s.v0l ^= cl;
+  s.v0h ^= ch;
+  sip_finish(s, xl, xh, outl, outh);
+}
+// (2) lane-divergent continuation: s is the site's pre-A state.
+__device__ __forceinline__ void sip_tail_val_ctx(Sip32 s, uint32_t vl, uint32_t vh, uint32_t cl, uint32_t ch,
+                                                 uint32_t xl, uint32_t xh, uint32_t& outl, uint32_t& outh) {
+  sip_absorb_preA(s, vl, vh);
+  s.v3l ^= cl;
+  s.v3h ^= ch;
+  sip_round(s);
+  sip_round(s);
+  s.v0l ^= cl;
+  s.v0h ^= ch;
+  sip_finish(s, xl, xh, outl, outh);
+}
+
 // per-lane tail when the event's state already covers site and continuation and has quarter A of the next round
 // applied, but the context word (cl, ch) is the lane's own in every bit (shadow stack: the depth is part of it)
 __device__ __forceinline__ void sip_tail_ctx(Sip32 s, uint32_t cl, uint32_t ch, uint32_t xl, uint32_t xh,

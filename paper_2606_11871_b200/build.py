@@ -16,7 +16,7 @@ ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libwarpguard.so"
 PROBE_LIB = PKG / "libwg_probe.so"
-SOURCES = ["wg_api.cu", "wg_kernels_v2.cu", "wg_shadow.cu"]
+SOURCES = ["wg_api.cu", "wg_check.cu", "wg_shadow.cu"]
 PROBE_SOURCES = ["wg_probe.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -160,7 +160,7 @@ wg::Params base_params(const wg_engine* e) {
   return p;
 }
 
-constexpr uint64_t kMaxLaunchEvents = 1ull << 30;
+constexpr uint64_t kMaxLaunchEvents = 1ull << 27;  // (element indices event * 32 + lane stay below 2^32 inside a launch)
 
 // rec_after: an event the first-violation-record kernel waits for (host path: the record kernel of the previous chunk,
 // which ran on the other staging stream), or nullptr

@@ -1,0 +1,868 @@
+// wg_check.cu — the check path on sm_100a: wg_sign_continuations, wg_verify_continuations, wg_check_forward.
+//
+// Steps: a1 event fetch + guard, a2 policy lookup, a3 MAC sign, a4 MAC verify + compare,
+// a5 forward membership, a6 verdicts, a7 counters, a8 first-violation record.  Paper passages: backward token
+// PAPER.md:162, 248; forward membership PAPER.md:174-178, 250-252; guards PAPER.md:190, 230; detect / enforce
+// PAPER.md:264; accounting PAPER.md:113, 127, 224.  Readings: DESIGN.md §2.  Kernel design: DESIGN.md §6.
+//
+// What bounds it (measured, profiles/): a SipRound is 20 ALU-pipe instructions (4 IADD3 with carry-out, 8 LOP3,
+// 8 SHF) + 4 IMAD.X on the FMA pipe, and every ALU-pipe instruction costs 2 issue cycles per warp on sm_100a, so a
+// round is 40 cycles per warp per SM sub-partition whatever the occupancy or ILP.  VOTE, ISETP, SEL, PRMT and LEA are
+// ALU-pipe instructions too; IMAD (FMA pipe), POPC / FLO / BREV (XU), SHFL / LDS / LDG (LSU), branches (CBU) and the
+// uniform datapath are not.  The kernel is therefore built to (1) run fewer rounds, (2) never run a round on an
+// inactive lane, and (3) spend as few ALU-pipe instructions as possible on anything else.
+//
+// Mapping.  A persistent warp walks over GROUPS of 32 consecutive events.  Per group it runs
+//   "event-parallel" phases (lane i <-> event i): header, site record (16 bytes, L2), classification, counters that
+//       need no verdict; the part of the MAC that is the same for every lane of an event — the site word always, the
+//       continuation word too when it is warp-uniform — from the key-derived initial state in the kernel parameters
+//       (nothing key-derived is ever read from memory); the membership search of warp-uniform forward targets;
+//   a "producer" loop (lane l <-> lane l, one trip per protected event): the event's value row straight from global
+//       memory (one coalesced 256-byte load, no shared-memory staging), the warp-uniformity test, and for return events
+//       the ACTIVE lanes appended, compacted, to one of two work queues in shared memory (warp-uniform /
+//       lane-divergent continuation); lane-divergent forward targets are searched here;
+//   "consumer" passes (lane j <-> queue item j): 32 queued (event, lane) items per pass, whatever events they
+//       belong to — the per-lane tail of the MAC (8 of the 12 SipRounds for a warp-uniform continuation, 10
+//       otherwise) and the compare, tags gathered from global memory.  Only FULL passes run; what is left over (< 32
+//       items per queue) is carried into the next group, so no SipRound is ever spent on an inactive lane;
+//   the event-parallel epilogue of the PREVIOUS group (its last items were consumed by this group's first passes):
+//       verdict store, violation counters, first violation.
+// The next group's rows are pulled into L2 by TMA bulk prefetches while this group is computed; when the policy's
+// whole target table is small it is staged in shared memory once per CTA by one TMA bulk copy.
+#include "wg_internal.h"
+#include "../../include/warpguard_sip32.cuh"
+
+namespace wg {
+
+namespace {
+
+enum : int { MODE_VERIFY = 0, MODE_FORWARD = 1, MODE_SIGN = 2 };
+enum : uint32_t { K_RET = 0, K_FWD = 1 };
+// what the kernel does with an event
+enum : uint32_t { CLS_NONE = 0, CLS_COUNT = 1, CLS_RET = 2, CLS_FWD = 3, CLS_FAIL = 4, CLS_SKIP_DIR = 5, CLS_SKIP_SITE = 6 };
+
+#ifndef WG_WARPS
+#define WG_WARPS 20
+#endif
+constexpr int kWarps = WG_WARPS;       // warps per CTA, one CTA per SM
+constexpr int kThreads = kWarps * 32;
+constexpr uint32_t kSmemMax = 232448;  // 227 KB opt-in shared memory per CTA on sm_100a
+constexpr uint32_t kFull = 0xffffffffu;
+constexpr uint32_t kMaxSmemSites = 1024;  // policies up to this size keep their per-site counters in shared memory
+
+// ---- shared-memory carve-up ----------------------------------------------------------------------
+// CTA part: [tgts staged: stage_bytes][per-site counters: site_bytes][cnt64: 40 x u64][bykind: 8 x u32][mbar, pad]
+// warp part: event records [2 groups][32] x 64 B, then the work queue (u32 items; warp-uniform items from the
+// front, lane-divergent items from the back)
+//   record: +0  SipHash state the event's consumer passes start from (8 words)
+//           +32 ctx lo (context_base & ~31), +36 ctx hi, +40 element base (event index * 32 - slot * 32: adding a
+//               queue item's low half gives the element index of (event, lane) in val / tag), +44 lanes whose value
+//               differs from the first active lane's (0: warp-uniform)
+//           +48 active mask, +52 meta = cls | kind << 4 | first active lane << 8, +56 violation mask, +60 site id
+constexpr uint32_t kRecBytes = 64;
+constexpr uint32_t kRecArea = 2 * 32 * kRecBytes;  // 4 KB
+constexpr uint32_t kQueueItems = 1024 + 64;        // one group adds at most 1,024 items; each queue carries < 32
+constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 4;
+constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 8 * 4 + 16 + 16;  // cnt64, bykind, mbar (+pad to 16)
+constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
+constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
+static_assert(kWarps * kWarpBytes + kCtaFixedBytes + 4096 <= kSmemMax, "too many warps for the shared memory");
+
+// ---- PTX helpers ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ uint4 ldg_v4(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+// value rows are read twice by a lane-divergent event (uniformity test, then the consumer's gather): keep them in L1
+__device__ __forceinline__ uint2 ldg_v2_keep(const void* p) {
+  uint2 r;
+  asm volatile("ld.global.ca.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+  return r;
+}
+// tags are read once
+__device__ __forceinline__ uint2 ldg_v2_stream(const void* p) {
+  uint2 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream_v2(void* p, uint32_t a, uint32_t b) {
+  asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(p), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ uint4 lds_v4(uint32_t a) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ uint2 lds_v2(uint32_t a) {
+  uint2 r;
+  asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
+  uint32_t r;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
+  uint32_t r;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(r) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ void sts_u32(uint32_t a, uint32_t x) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
+}
+__device__ __forceinline__ void sts_v4(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ void sts_v2(uint32_t a, uint32_t x, uint32_t y) {
+  asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory");
+}
+// one cache line -> L2 (the rows a later group will read; an LSU instruction, no register, no completion to wait for)
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
+}
+__device__ __forceinline__ void atoms_or(uint32_t a, uint32_t x) {
+  asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
+}
+// a * b + c on the FMA pipe (address arithmetic inside the ALU-bound loops)
+__device__ __forceinline__ uint32_t mad32(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+  return r;
+}
+// base + 8 * element as one wide multiply-add on the FMA pipe
+__device__ __forceinline__ const uint64_t* elem_ptr(const uint64_t* base, uint32_t elem) {
+  uint64_t r;
+  asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(elem), "l"(reinterpret_cast<uint64_t>(base)));
+  return reinterpret_cast<const uint64_t*>(r);
+}
+
+// TMA: 1-D bulk copy global -> shared with completion on an mbarrier (whole-table staging of the target sets), and
+// bulk prefetch global -> L2 (the next group's rows)
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(mbar)
+               : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n"
+      "WG_MBAR_WAIT:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra WG_MBAR_DONE;\n\t"
+      "bra WG_MBAR_WAIT;\n"
+      "WG_MBAR_DONE:\n\t}" ::"r"(mbar),
+      "r"(parity)
+      : "memory");
+}
+
+// exact-equality membership in a strictly ascending set: branch-free lower-bound walk, then one compare
+// (R8).  cnt >= 1 for every protected-forward site (validated at load).
+template <bool STAGED>
+__device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t off, uint32_t cnt, uint32_t vl,
+                                       uint32_t vh) {
+  const uint64_t v = (static_cast<uint64_t>(vh) << 32) | vl;
+  uint32_t lo = 0, len = cnt;
+  if constexpr (STAGED) {
+    const uint32_t base = tg_s + off * 8;
+    while (len > 1) {
+      const uint32_t half = len >> 1;
+      const uint2 m = lds_v2(base + (lo + half) * 8);
+      const uint64_t mid = (static_cast<uint64_t>(m.y) << 32) | m.x;
+      lo = (mid <= v) ? lo + half : lo;
+      len -= half;
+    }
+    const uint2 m = lds_v2(base + lo * 8);
+    return m.x == vl && m.y == vh;
+  } else {
+    const uint64_t* set = p.tgts + off;
+    // large sets live in L2 / HBM and every probe is a dependent load: quaternary steps issue three independent
+    // probes at once and halve the number of dependent rounds (config 5: sets up to 4,096 entries)
+    while (len > 8) {
+      const uint32_t q = len >> 2;
+      const uint64_t m1 = __ldg(set + lo + q), m2 = __ldg(set + lo + 2 * q), m3 = __ldg(set + lo + 3 * q);
+      if (m3 <= v) {
+        lo += 3 * q;
+        len -= 3 * q;
+      } else {
+        lo += (m2 <= v) ? 2 * q : (m1 <= v) ? q : 0u;
+        len = q;
+      }
+    }
+    while (len > 1) {
+      const uint32_t half = len >> 1;
+      const uint64_t mid = __ldg(set + lo + half);
+      lo = (mid <= v) ? lo + half : lo;
+      len -= half;
+    }
+    return __ldg(set + lo) == v;
+  }
+}
+
+__device__ __forceinline__ Sip32 init_state(const Params& p) {
+  return Sip32{static_cast<uint32_t>(p.v0), static_cast<uint32_t>(p.v0 >> 32), static_cast<uint32_t>(p.v1),
+               static_cast<uint32_t>(p.v1 >> 32), static_cast<uint32_t>(p.v2), static_cast<uint32_t>(p.v2 >> 32),
+               static_cast<uint32_t>(p.v3), static_cast<uint32_t>(p.v3 >> 32)};
+}
+
+// token of a forward record ("a MAC over site_id, target_count, and allowed_targets"; R37):
+// SipHash-2-4 over LE64(site_id) || LE64(cnt) || LE64(t_0) ... LE64(t_cnt-1), read through `load(i)`
+template <typename LoadTarget>
+__device__ __forceinline__ uint2 record_token(Sip32 s, uint32_t site, uint32_t cnt, LoadTarget load) {
+  sip_absorb(s, site, 0u);
+  sip_absorb(s, cnt, 0u);
+  for (uint32_t i = 0; i < cnt; ++i) {
+    const uint2 t = load(i);
+    sip_absorb(s, t.x, t.y);
+  }
+  uint2 out;
+  sip_finish_len(s, ((8u * (cnt + 2u)) & 0xffu) << 24, 0u, 0u, out.x, out.y);
+  return out;
+}
+
+__device__ __forceinline__ Sip32 lds_state(uint32_t a) {
+  const uint4 x = lds_v4(a), y = lds_v4(a + 16);
+  return Sip32{x.x, x.y, x.z, x.w, y.x, y.y, y.z, y.w};
+}
+
+// warp-uniform running counters of one warp (flushed once at the end)
+struct WarpCtr {
+  uint32_t total, empty, unknown, misrouted, ret_checks, fwd_checks, ret_lanes, fwd_lanes, signed_lanes, skipped;
+};
+
+// ---------------------------------------------------------------------------------------------------
+// MODE_VERIFY = wg_verify_continuations, MODE_FORWARD = wg_check_forward, MODE_SIGN = wg_sign_continuations.
+// STAGED: the whole target table sits in shared memory.  TEL: a profile flag is set or the violation ring is on
+// (compiled out of the ordinary launch).
+// ---------------------------------------------------------------------------------------------------
+template <int MODE, bool STAGED, bool TEL>
+__global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, const uint32_t stage_bytes,
+                                                                const uint32_t site_bytes) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint32_t lane, lanebit;
+  asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
+  asm volatile("shl.b32 %0, 1, %1;" : "=r"(lanebit) : "r"(lane));
+  const uint32_t ltmask = lanebit - 1u;
+  // the shuffle tells the compiler that the warp index (and what derives from it) is warp-uniform
+  const uint32_t warp = __shfl_sync(kFull, threadIdx.x >> 5, 0);
+  const uint32_t smem0 = smem_u32(smem_raw);
+  const uint32_t tg_s = smem0;
+  // small policies (site_bytes != 0): per-site counters are accumulated in shared memory as 4 x u32 per site and
+  // flushed once per CTA.  With few sites the global counter array spans only a few L2 slices and the reductions
+  // of 148 SMs would queue on them (config 3: 40 sites).
+  uint32_t* site_s = reinterpret_cast<uint32_t*>(smem_raw + stage_bytes);
+  const uint32_t cta_off = stage_bytes + site_bytes;
+  unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + cta_off);
+  uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8);
+  const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 32;
+  const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * kWarpBytes;
+  const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 4 * k
+  const uint32_t q_top = q_s + (kQueueItems - 1) * 4;        // divergent items: q_top - 4 * k
+
+  if (threadIdx.x < C_WORDS) cnt64[threadIdx.x] = 0ull;
+  for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = 0u;
+  if (threadIdx.x < 8) bykind[threadIdx.x] = 0u;
+  if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
+  __syncthreads();
+  if constexpr (STAGED) {
+    if (threadIdx.x == 0) {
+      mbar_expect_tx(mbar_cta, stage_bytes);
+      tma_bulk_g2s(tg_s, p.tgts, stage_bytes, mbar_cta);
+    }
+    mbar_wait(mbar_cta, 0);
+  }
+
+  const uint64_t n_groups = (p.n + 31) / 32;
+  const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kWarps;
+  uint64_t gi = static_cast<uint64_t>(blockIdx.x) * kWarps + warp;
+  const bool enforce = p.mode != 0;
+  const Sip32 s_init = init_state(p);
+  WarpCtr c = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  uint32_t par = 0;          // which half of the record area this group uses
+  uint32_t nu = 0, nd = 0;   // items in the uniform / divergent queue (carried items first)
+  bool have_prev = false;    // a previous group still waits for its epilogue
+  uint64_t prev_e0 = 0;
+
+  // ---- consumer passes ------------------------------------------------------------------------------
+  // one pass over 32 queue items starting at item k0 of the uniform (UNI) or divergent queue; lanes with on == false
+  // (only in the partial passes that flush a queue) do nothing
+  auto pass = [&](auto uni_tag, uint32_t k0, bool on) {
+    constexpr bool UNI = decltype(uni_tag)::value;
+    if (!on) return;
+    const uint32_t qa = UNI ? q_s + (k0 + lane) * 4u : q_top - (k0 + lane) * 4u;
+    const uint32_t item = lds_u16(qa);           // slot * 32 + lane of the event
+    const uint32_t ra = rec_s + lds_u16(qa + 2); // the event's record
+    const uint4 cx = lds_v4(ra + 32);            // ctx lo, ctx hi, element base, -
+    Sip32 s = lds_state(ra);
+    const uint32_t elem = cx.z + item;
+    uint32_t dl, dh;
+    if constexpr (MODE == MODE_SIGN) {
+      if constexpr (UNI) {
+        s.v3l ^= item & 31u;
+        sip_tail_ctxlane(s, cx.x ^ (item & 31u), cx.y, 0u, 0u, dl, dh);
+      } else {
+        const uint2 v = ldg_v2_keep(elem_ptr(p.val, elem));
+        sip_tail_val_ctx(s, v.x, v.y, cx.x ^ (item & 31u), cx.y, 0u, 0u, dl, dh);
+      }
+      st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, elem)), dl, dh);
+    } else {
+      const uint2 tg = ldg_v2_stream(elem_ptr(p.tag, elem));
+      if constexpr (UNI) {
+        s.v3l ^= item & 31u;
+        sip_tail_ctxlane(s, cx.x ^ (item & 31u), cx.y, tg.x, tg.y, dl, dh);
+      } else {
+        const uint2 v = ldg_v2_keep(elem_ptr(p.val, elem));
+        sip_tail_val_ctx(s, v.x, v.y, cx.x ^ (item & 31u), cx.y, tg.x, tg.y, dl, dh);
+      }
+      if ((dl | dh) != 0u) atoms_or(ra + 56, 1u << (item & 31u));  // rare: the lane's token does not match
+    }
+  };
+  // run every full pass of both queues, then move what is left (< 32 items each) to the queue heads.
+  // flush: also run the partial passes, leaving both queues empty.
+  auto drain = [&](bool flush_u, bool flush_d) {
+    uint32_t k = 0;
+    for (; k + 32 <= nu; k += 32) pass(std::true_type{}, k, true);
+    if (flush_u && k < nu) {
+      pass(std::true_type{}, k, k + lane < nu);
+      k = nu;
+    }
+    const uint32_t ru = nu - k;
+    uint32_t carry = 0;
+    if (ru) carry = lds_u32(q_s + (k + (lane < ru ? lane : 0u)) * 4u);
+    uint32_t kd = 0;
+    for (; kd + 32 <= nd; kd += 32) pass(std::false_type{}, kd, true);
+    if (flush_d && kd < nd) {
+      pass(std::false_type{}, kd, kd + lane < nd);
+      kd = nd;
+    }
+    const uint32_t rd = nd - kd;
+    uint32_t carry_d = 0;
+    if (rd) carry_d = lds_u32(q_top - (kd + (lane < rd ? lane : 0u)) * 4u);
+    __syncwarp();
+    if (lane < ru) sts_u32(q_s + lane * 4u, carry);
+    if (lane < rd) sts_u32(q_top - lane * 4u, carry_d);
+    nu = ru;
+    nd = rd;
+    __syncwarp();
+  };
+
+  // ---- event-parallel epilogue of a finished group: verdicts (a6), violation counters (a7), first violation (a8) ----
+  auto epilogue = [&](uint32_t rpar, uint64_t e0) {
+    if constexpr (MODE != MODE_SIGN) {
+      const uint32_t ra = rec_s + (rpar * 32u + lane) * kRecBytes;
+      const uint4 m = lds_v4(ra + 48);  // active, meta, viol, site
+      const uint32_t active = m.x, cls = m.y & 15u, kind = (m.y >> 4) & 15u, viol = m.z, site = m.w;
+      const bool valid = cls != CLS_NONE;
+      if (valid) st_stream_v2(p.out + (e0 + lane), viol, enforce ? (active & ~viol) : active);
+      // violations are rare (0.05 % of events in the paper-shaped stream): one warp-uniform branch per group
+      if (__ballot_sync(kFull, viol != 0u)) {
+        const uint32_t pv = __popc(viol);
+        const bool judged = cls == CLS_RET || cls == CLS_FWD;
+        const bool known = valid && kind < 7u;
+        const uint32_t rv = __reduce_add_sync(kFull, cls == CLS_RET ? pv : 0u);
+        const uint32_t fv = __reduce_add_sync(kFull, cls == CLS_FWD ? pv : 0u);
+        const uint32_t av = __reduce_add_sync(kFull, pv);
+        const uint32_t rve = __popc(__ballot_sync(kFull, cls == CLS_RET && viol != 0u));
+        const uint32_t fve = __popc(__ballot_sync(kFull, cls == CLS_FWD && viol != 0u));
+        const uint32_t ave = __popc(__ballot_sync(kFull, viol != 0u));
+        // first violation: smallest (seq << 5 | lane); seq = running event index (R12)
+        unsigned long long key = ~0ull;
+        if (viol) key = ((p.seq_base + e0 + lane) << 5) | static_cast<uint32_t>(__ffs(viol) - 1);
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+          const unsigned long long o = __shfl_xor_sync(kFull, key, d);
+          key = o < key ? o : key;
+        }
+        if (lane == 0) {
+          if (rv) atomicAdd(p.glob + C_RET_VIOL, static_cast<unsigned long long>(rv));
+          if (fv) atomicAdd(p.glob + C_FWD_VIOL, static_cast<unsigned long long>(fv));
+          if (rve) atomicAdd(p.glob + C_RET_VIOL_EVENTS, static_cast<unsigned long long>(rve));
+          if (fve) atomicAdd(p.glob + C_FWD_VIOL_EVENTS, static_cast<unsigned long long>(fve));
+          if (enforce) {
+            atomicAdd(p.glob + C_BLOCKED_LANES, static_cast<unsigned long long>(av));
+            atomicAdd(p.glob + C_BLOCKED_EVENTS, static_cast<unsigned long long>(ave));
+          }
+          atomicMin(p.glob + C_FIRST_VIOLATION, key);
+        }
+        if (TEL && viol && !(p.profile & PROFILE_LOW_TELEMETRY) && p.ring_cap != 0) {
+          // violation ring (R27, R28): diagnostic, bounded; a full ring drops and counts
+          const unsigned long long slot = atomicAdd(p.glob + C_RING_TOTAL, 1ull);
+          if (slot < p.ring_cap) {
+            const uint32_t fl = static_cast<uint32_t>(__ffs(viol) - 1);
+            ViolRec r;
+            r.seq = p.seq_base + e0 + lane;
+            r.site_id = site;
+            r.kind = kind;
+            r.viol_mask = viol;
+            r.active_mask = active;
+            r.lane = fl;
+            r.mode = p.mode;
+            r.observed = p.val[(e0 + lane) * 32 + fl];
+            r.stored = (MODE == MODE_VERIFY && cls == CLS_RET) ? p.tag[(e0 + lane) * 32 + fl] : 0ull;
+            p.ring[slot] = r;
+          }
+        }
+        if (viol && known && !(TEL && (p.profile & PROFILE_LOW_TELEMETRY))) {
+          if (site_bytes) {
+            if (judged) atomicAdd(&site_s[site * 4 + S_LANES_VIOLATION], pv);
+            if (enforce) atomicAdd(&site_s[site * 4 + S_LANES_BLOCKED], pv);
+          } else {
+            unsigned long long* sc = p.site + static_cast<uint64_t>(site) * 4;
+            if (judged) atomicAdd(sc + S_LANES_VIOLATION, static_cast<unsigned long long>(pv));
+            if (enforce) atomicAdd(sc + S_LANES_BLOCKED, static_cast<unsigned long long>(pv));
+          }
+        }
+      }
+    }
+  };
+
+  // ---- software pipeline of the event-parallel loads: the header two groups ahead, the site record one group ahead,
+  //      so that the rows of the NEXT group can be pulled into L2 while this group is computed ----
+  auto load_hdr = [&](uint64_t g) -> uint4 {
+    const uint64_t e = g * 32 + lane;
+    return (g < n_groups && e < p.n) ? ldg_v4(p.hdr + e) : make_uint4(0xffffffffu, 0u, 0u, 0u);
+  };
+  auto load_rec = [&](const uint4& h) -> uint4 {
+    return h.x < p.n_sites ? ldg_v4(p.recs + h.x) : make_uint4(7u, 0u, 0u, 0u);
+  };
+  uint4 h_cur = load_hdr(gi);
+  uint4 h_nxt = load_hdr(gi + stride);
+  uint4 r_cur = load_rec(h_cur);
+
+  while (gi < n_groups) {
+    const uint64_t gn = gi + stride;
+    const uint64_t e0 = gi * 32;
+    const uint4 r_nxt = load_rec(h_nxt);
+    const uint4 h_nn = load_hdr(gn + stride);
+    const uint32_t rbase = rec_s + par * (32u * kRecBytes);
+    const uint32_t ra_me = rbase + lane * kRecBytes;
+    const uint32_t slot_me = par * 32u + lane;
+    const uint32_t cu = nu, cd = nd;  // items carried over from the previous group
+
+    // ---- event-parallel: classify (a1, a2) ----
+    const bool valid = e0 + lane < p.n;
+    const uint32_t site = h_cur.x;
+    const uint32_t active = valid ? h_cur.y : 0u;
+    const bool known = valid && site < p.n_sites;
+    const uint32_t kind = known ? r_cur.x : 7u;
+    const uint32_t off = r_cur.y, cnt = r_cur.z;
+    uint32_t cls = CLS_NONE;
+    if (valid) {
+      if (known) {
+        if constexpr (MODE == MODE_SIGN) {
+          cls = (kind == K_RET && active != 0u) ? CLS_RET : CLS_COUNT;
+        } else {
+          if (active == 0u)
+            cls = CLS_COUNT;  // fully predicated off: counted, not a check (R22)
+          else if (TEL && ((kind == K_RET && (p.profile & PROFILE_SKIP_BACKWARD)) ||
+                           (kind == K_FWD && (p.profile & PROFILE_SKIP_FORWARD))))
+            cls = CLS_SKIP_DIR;   // outside this profile's protected set: separate denominator (R26)
+          else if (TEL && (kind == K_RET || kind == K_FWD) && (p.profile & PROFILE_COVERAGE_REDUCED) &&
+                   (r_cur.w & SITE_FLAG_SKIP))
+            cls = CLS_SKIP_SITE;  // a site the coverage-reduced profile leaves out: separate denominator (R40)
+          else if (kind == K_RET)
+            cls = (MODE == MODE_VERIFY) ? CLS_RET : CLS_FAIL;  // no tag at the forward entry point (R14)
+          else if (kind == K_FWD)
+            cls = CLS_FWD;
+          else
+            cls = CLS_COUNT;  // non-protected kinds are only counted (R17)
+        }
+      } else {
+        cls = (MODE == MODE_SIGN) ? CLS_COUNT : CLS_FAIL;  // unknown site: fail closed (R13)
+      }
+    }
+    const uint32_t na = __popc(active);
+    const uint32_t first = active ? static_cast<uint32_t>(__ffs(active) - 1) : 0u;
+    const uint32_t m_ret = __ballot_sync(kFull, cls == CLS_RET);
+    const uint32_t m_fwd = (MODE == MODE_SIGN) ? 0u : __ballot_sync(kFull, cls == CLS_FWD);
+    uint32_t viol = (cls == CLS_FAIL) ? active : 0u;  // fail closed (R13, R14)
+    sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, static_cast<uint32_t>(e0 + lane) * 32u - slot_me * 32u, 0u);
+    sts_v4(ra_me + 48, active, cls | (kind << 4) | (first << 8), viol, site);
+
+    if (MODE != MODE_SIGN && cls == CLS_FWD) sts_v2(ra_me + 16, off, cnt);  // (a forward event has no MAC state)
+
+    // ---- counters that need no verdict (a7) ----
+    const uint32_t judged_na = (cls == CLS_RET || cls == CLS_FWD) ? na : 0u;
+    if constexpr (MODE == MODE_SIGN) {
+      const bool is_ret = known && kind == K_RET;
+      c.signed_lanes += __reduce_add_sync(kFull, is_ret ? na : 0u);
+      c.skipped += __popc(__ballot_sync(kFull, valid && !is_ret));
+    } else {
+      c.total += __popc(__ballot_sync(kFull, valid));
+      if (__ballot_sync(kFull, valid && (!known || active == 0u || cls == CLS_FAIL))) {  // uncommon events
+        c.unknown += __popc(__ballot_sync(kFull, valid && !known));
+        c.empty += __popc(__ballot_sync(kFull, known && active == 0u));
+        c.misrouted += __popc(__ballot_sync(kFull, known && cls == CLS_FAIL));
+      }
+      c.ret_checks += __popc(m_ret);
+      c.fwd_checks += __popc(m_fwd);
+      c.ret_lanes += __reduce_add_sync(kFull, cls == CLS_RET ? na : 0u);
+      c.fwd_lanes += __reduce_add_sync(kFull, cls == CLS_FWD ? na : 0u);
+      if (known) atomicAdd(&bykind[kind], 1u);
+      if constexpr (TEL) {
+        if (p.profile & (PROFILE_SKIP_FORWARD | PROFILE_SKIP_BACKWARD | PROFILE_COVERAGE_REDUCED)) {
+          const bool sd = cls == CLS_SKIP_DIR, ss = cls == CLS_SKIP_SITE;
+          const uint32_t sr = __ballot_sync(kFull, sd && kind == K_RET);
+          const uint32_t sf = __ballot_sync(kFull, sd && kind == K_FWD);
+          const uint32_t sse = __ballot_sync(kFull, ss);
+          const uint32_t srl = __reduce_add_sync(kFull, (sd && kind == K_RET) ? na : 0u);
+          const uint32_t sfl = __reduce_add_sync(kFull, (sd && kind == K_FWD) ? na : 0u);
+          const uint32_t ssl = __reduce_add_sync(kFull, ss ? na : 0u);
+          if (lane == 0) {
+            if (sr) atomicAdd(cnt64 + C_SKIP_RET_EVENTS, static_cast<unsigned long long>(__popc(sr)));
+            if (srl) atomicAdd(cnt64 + C_SKIP_RET_LANES, static_cast<unsigned long long>(srl));
+            if (sf) atomicAdd(cnt64 + C_SKIP_FWD_EVENTS, static_cast<unsigned long long>(__popc(sf)));
+            if (sfl) atomicAdd(cnt64 + C_SKIP_FWD_LANES, static_cast<unsigned long long>(sfl));
+            if (sse) atomicAdd(cnt64 + C_SKIP_SITE_EVENTS, static_cast<unsigned long long>(__popc(sse)));
+            if (ssl) atomicAdd(cnt64 + C_SKIP_SITE_LANES, static_cast<unsigned long long>(ssl));
+          }
+        }
+      }
+      if (TEL && (p.profile & PROFILE_LOW_TELEMETRY)) {
+        // "same checked transfers with less reporting" (PAPER.md Table A2): no per-site counters
+      } else if (site_bytes) {
+        if (known) {  // per-site counters in shared memory (small policies)
+          atomicAdd(&site_s[site * 4 + S_EVENTS], 1u);
+          if (judged_na) atomicAdd(&site_s[site * 4 + S_LANES_CHECKED], judged_na);
+        }
+      } else {
+        // per-site counters in global memory, one reduction per event straight to L2 (merging equal sites of a
+        // group first costs more ALU-pipe slots than the hot site's reductions cost in L2)
+        if (known) {
+          unsigned long long* sc = p.site + static_cast<uint64_t>(site) * 4;
+          atomicAdd(sc + S_EVENTS, 1ull);
+          if (judged_na) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(judged_na));
+        }
+      }
+    }
+
+    // ---- event-parallel: the site word of the MAC, once per event; the key-derived initial state exists in the
+    //      kernel parameters only (constant bank).  Leaves the "pre-A" state the tails start from. ----
+    Sip32 st = s_init;
+    if (MODE != MODE_FORWARD && m_ret != 0u) {
+      sip_absorb(st, site, p.bind_hi);  // LE64(site_id | digest32 << 32): zero-extended site id unless bound (R3, R5, R39)
+      sip_qA(st);
+    }
+    __syncwarp();  // the records are visible to every lane
+
+    // ---- producer loop (lane-parallel), one trip per protected event: row load, warp-uniformity, queueing ----
+    {
+      const uint64_t* vrow = p.val + (e0 * 32 + lane);
+      uint64_t* trow = (MODE == MODE_SIGN) ? p.tag_out + (e0 * 32 + lane) : nullptr;
+      const uint32_t item_me = slot_me - lane;  // par * 32: the group's first slot
+      const uint32_t need = (MODE == MODE_SIGN) ? __ballot_sync(kFull, valid) : (m_ret | m_fwd);
+#pragma unroll 1
+      for (uint32_t b0 = 0; b0 < 32; b0 += 8) {
+        const uint32_t nb = (need >> b0) & 0xffu;
+        if (nb == 0u) continue;
+        uint2 v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          v[j] = make_uint2(0u, 0u);
+          if ((((MODE == MODE_SIGN) ? m_ret : need) >> (b0 + j)) & 1u) v[j] = ldg_v2_keep(vrow + (b0 + j) * 32);
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const uint32_t e = b0 + j;
+          if (!((need >> e) & 1u)) continue;
+          const uint32_t re = rbase + e * kRecBytes;
+          if (MODE == MODE_SIGN && !((m_ret >> e) & 1u)) {
+            st_stream_v2(trow + e * 32, 0u, 0u);  // not a return check: a zero row (R10)
+            continue;
+          }
+          const uint2 am = lds_v2(re + 48);  // active, meta
+          const uint32_t a = am.x, f = (am.y >> 8) & 31u;
+          const uint32_t rx = __shfl_sync(kFull, v[j].x, f), ry = __shfl_sync(kFull, v[j].y, f);
+          const uint32_t diff = __ballot_sync(kFull, v[j].x != rx || v[j].y != ry) & a;
+          const bool act = (a & lanebit) != 0u;
+          if (MODE != MODE_SIGN && ((m_fwd >> e) & 1u)) {
+            // forward event: a warp-uniform target is searched once, event-parallel, below; lane-divergent targets
+            // are searched here, per lane (per-warp checking only after proving uniformity)
+            if (diff != 0u) {
+              const uint2 oc = lds_v2(re + 16);  // off, cnt (parked in the unused state words of a forward event)
+              bool bad = false;
+              if (!(TEL && (p.profile & PROFILE_METADATA_INTEGRITY))) {
+                bad = act && !member<STAGED>(p, tg_s, oc.x, oc.y, v[j].x, v[j].y);
+                const uint32_t vb = __ballot_sync(kFull, bad);
+                if (lane == 0) sts_u32(re + 56, vb);
+              }
+            }
+            if (lane == 0) sts_u32(re + 44, diff);
+            continue;
+          }
+          // return event: append the active lanes, compacted, to the queue of its class
+          if (lane == 0) sts_u32(re + 44, diff);
+          const uint32_t rank = __popc(a & ltmask);
+          const uint32_t entry = ((e + item_me) * (kRecBytes << 16 | 32u)) + lane;  // record offset << 16 | slot * 32 + lane
+          const uint32_t nae = __popc(a);
+          if (diff == 0u) {
+            if (act) sts_u32(q_s + (nu + rank) * 4u, entry);
+            nu += nae;
+          } else {
+            if (act) sts_u32(q_top - (nd + rank) * 4u, entry);
+            nd += nae;
+          }
+          if (MODE == MODE_SIGN && !act) st_stream_v2(trow + e * 32, 0u, 0u);  // inactive lanes sign nothing (R10)
+        }
+      }
+    }
+    __syncwarp();
+
+    // ---- event-parallel: per-event part of the MAC; search of warp-uniform forward targets ----
+    {
+      const uint32_t diff = lds_u32(ra_me + 44);
+      const bool is_uni = diff == 0u;
+      uint32_t ul = 0, uh = 0;
+      if ((cls == CLS_RET || cls == CLS_FWD) && is_uni) {
+        const uint2 r = ldg_v2_keep(p.val + ((e0 + lane) * 32 + first));  // the event's one value (an L1 hit)
+        ul = r.x;
+        uh = r.y;
+      }
+      if (cls == CLS_RET) {
+        if (is_uni) {
+          sip_absorb_preA(st, ul, uh);  // the continuation word, once per event
+          sip_qA(st);                   // quarter A of the context word's first round
+          st.v3l ^= h_cur.z & ~31u;     // and the lane-independent bits of the context word
+          st.v3h ^= h_cur.w;
+        }
+        sts_v4(ra_me, st.v0l, st.v0h, st.v1l, st.v1h);
+        sts_v4(ra_me + 16, st.v2l, st.v2h, st.v3l, st.v3h);
+      }
+      if constexpr (MODE != MODE_SIGN) {
+        bool bad_rec = false;
+        if constexpr (TEL) {
+          // metadata integrity: the forward record is re-authenticated before it is used, once per
+          // event; a record that fails authorises nothing: every active lane violates
+          if (p.profile & PROFILE_METADATA_INTEGRITY) {
+            if (cls == CLS_FWD) {
+              const uint2 tok = __ldg(reinterpret_cast<const uint2*>(p.tok) + site);
+              uint2 tk;
+              if constexpr (STAGED) {
+                const uint32_t base = tg_s + off * 8;
+                tk = record_token(s_init, site, cnt, [&](uint32_t i) { return lds_v2(base + i * 8); });
+              } else {
+                const uint2* set = reinterpret_cast<const uint2*>(p.tgts + off);
+                tk = record_token(s_init, site, cnt, [&](uint32_t i) { return __ldcg(set + i); });
+              }
+              bad_rec = tk.x != tok.x || tk.y != tok.y;
+            }
+            const uint32_t m_bad = __ballot_sync(kFull, bad_rec);
+            if (m_bad && lane == 0)
+              atomicAdd(p.glob + C_META_FAIL, static_cast<unsigned long long>(__popc(m_bad)));
+            // lane-divergent forward events of an authenticated record: searched here, per lane, one event at a time
+            for (uint32_t m = m_fwd & ~m_bad & __ballot_sync(kFull, !is_uni); m; m &= m - 1) {
+              const uint32_t e = __ffs(m) - 1;
+              const uint32_t a = __shfl_sync(kFull, active, e);
+              const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
+              const uint2 v = ldg_v2_keep(p.val + ((e0 + e) * 32 + lane));
+              const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !member<STAGED>(p, tg_s, o2, c2, v.x, v.y));
+              if (lane == e) viol = vb;
+            }
+            if (cls == CLS_FWD && !is_uni && !bad_rec) sts_u32(ra_me + 56, viol);
+          }
+        }
+        if (cls == CLS_FWD && bad_rec) sts_u32(ra_me + 56, active);
+        if (cls == CLS_FWD && is_uni && !bad_rec)
+          sts_u32(ra_me + 56, member<STAGED>(p, tg_s, off, cnt, ul, uh) ? 0u : active);
+      }
+    }
+    // ---- the next group's rows -> L2: lane i pulls the two cache lines of row i of the next group, if that event
+    //      will need them (its site record has arrived by now); rows nobody will read are not fetched ----
+    if (gn < n_groups) {
+      const bool v_nxt = gn * 32 + lane < p.n && h_nxt.y != 0u;
+      const bool ret_nxt = v_nxt && r_nxt.x == K_RET, fwd_nxt = v_nxt && r_nxt.x == K_FWD;
+      const char* vr = reinterpret_cast<const char*>(p.val + (gn * 32 + lane) * 32);
+      if (MODE == MODE_FORWARD ? fwd_nxt : (MODE == MODE_SIGN ? ret_nxt : (ret_nxt || fwd_nxt))) {
+        prefetch_l2(vr);
+        prefetch_l2(vr + 128);
+      }
+      if (MODE == MODE_VERIFY && ret_nxt) {
+        const char* tr = reinterpret_cast<const char*>(p.tag + (gn * 32 + lane) * 32);
+        prefetch_l2(tr);
+        prefetch_l2(tr + 128);
+      }
+    }
+    __syncwarp();
+
+    // ---- consumer passes: every full pass; carried items of the previous group go first.  If a queue still holds
+    //      items of the previous group and cannot fill a pass, it is flushed with a partial pass (rare). ----
+    // (carried items are the oldest: any full pass consumes them; nu_carry / nd_carry < 32)
+    drain(cu != 0u && nu < 32u, cd != 0u && nd < 32u);
+    if (have_prev) epilogue(par ^ 1u, prev_e0);
+    have_prev = true;
+    prev_e0 = e0;
+    par ^= 1u;
+    gi = gn;
+    h_cur = h_nxt;
+    r_cur = r_nxt;
+    h_nxt = h_nn;
+    __syncwarp();
+  }
+  if (have_prev) {
+    drain(true, true);
+    epilogue(par ^ 1u, prev_e0);
+  }
+
+  // ---- flush: warp registers -> CTA shared memory -> one global atomic per counter per CTA ----
+  if (lane == 0) {
+    if constexpr (MODE == MODE_SIGN) {
+      if (c.signed_lanes) atomicAdd(cnt64 + C_SIGNED_LANES, static_cast<unsigned long long>(c.signed_lanes));
+      if (c.skipped) atomicAdd(cnt64 + C_SIGN_SKIPPED, static_cast<unsigned long long>(c.skipped));
+    } else {
+      if (c.total) atomicAdd(cnt64 + C_EVENTS_TOTAL, static_cast<unsigned long long>(c.total));
+      if (c.empty) atomicAdd(cnt64 + C_EVENTS_EMPTY, static_cast<unsigned long long>(c.empty));
+      if (c.unknown) atomicAdd(cnt64 + C_EVENTS_UNKNOWN, static_cast<unsigned long long>(c.unknown));
+      if (c.misrouted) atomicAdd(cnt64 + C_EVENTS_MISROUTED, static_cast<unsigned long long>(c.misrouted));
+      if (c.ret_checks) atomicAdd(cnt64 + C_RET_CHECKS, static_cast<unsigned long long>(c.ret_checks));
+      if (c.fwd_checks) atomicAdd(cnt64 + C_FWD_CHECKS, static_cast<unsigned long long>(c.fwd_checks));
+      if (c.ret_lanes) atomicAdd(cnt64 + C_RET_LANES, static_cast<unsigned long long>(c.ret_lanes));
+      if (c.fwd_lanes) atomicAdd(cnt64 + C_FWD_LANES, static_cast<unsigned long long>(c.fwd_lanes));
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < C_WORDS) {  // (words updated in global memory directly, and the host-side words, stay 0 here)
+    unsigned long long v = cnt64[threadIdx.x];
+    if (threadIdx.x >= C_BY_KIND && threadIdx.x < C_BY_KIND + 7) v = bykind[threadIdx.x - C_BY_KIND];
+    if (v) atomicAdd(p.glob + threadIdx.x, v);
+  }
+  for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) {
+    const uint32_t v = site_s[i];
+    if (v) atomicAdd(p.site + i, static_cast<unsigned long long>(v));
+  }
+}
+
+// first-violation record (R29), one thread, enqueued behind every check launch: the launch is over, so
+// the key is final for it; if the key moved into that launch's event range the full record of that event is written.
+// Deterministic, and nothing on the hot path: violations only did the atomicMin they always did.
+__global__ void wg_first_record(const Params p, const int has_tag) {
+  const unsigned long long key = p.glob[C_FIRST_VIOLATION];
+  const unsigned long long seq = key >> 5;
+  if (key == ~0ull || key == p.first->key || seq < p.seq_base || seq - p.seq_base >= p.n) return;
+  const uint64_t i = seq - p.seq_base;
+  const uint32_t fl = static_cast<uint32_t>(key & 31u);
+  const uint4 hh = p.hdr[i];
+  const uint2 o = p.out[i];
+  ViolRec r;
+  r.seq = seq;
+  r.site_id = hh.x;
+  r.kind = hh.x < p.n_sites ? p.recs[hh.x].kind : 7u;
+  r.viol_mask = o.x;
+  r.active_mask = hh.y;
+  r.lane = fl;
+  r.mode = p.mode;
+  r.observed = p.val[i * 32 + fl];
+  const bool skipped = (r.kind == K_RET && (p.profile & PROFILE_SKIP_BACKWARD)) ||
+                       (hh.x < p.n_sites && (p.profile & PROFILE_COVERAGE_REDUCED) && (p.recs[hh.x].flags & SITE_FLAG_SKIP));
+  const bool judged_ret = has_tag && r.kind == K_RET && !skipped;
+  r.stored = judged_ret ? p.tag[i * 32 + fl] : 0ull;
+  p.first->rec = r;
+  p.first->key = key;
+}
+
+// tokens of the forward records as loaded (trusted load time; R37), one thread per site
+__global__ void wg_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                                uint64_t v1, uint64_t v2, uint64_t v3) {
+  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n_sites) return;
+  const SiteRec r = recs[s];
+  uint64_t t = 0;
+  if (r.kind == K_FWD) {
+    const uint2* set = reinterpret_cast<const uint2*>(tgts + r.off);
+    const Sip32 s0{static_cast<uint32_t>(v0), static_cast<uint32_t>(v0 >> 32), static_cast<uint32_t>(v1),
+                   static_cast<uint32_t>(v1 >> 32), static_cast<uint32_t>(v2), static_cast<uint32_t>(v2 >> 32),
+                   static_cast<uint32_t>(v3), static_cast<uint32_t>(v3 >> 32)};
+    const uint2 tk = record_token(s0, s, r.cnt, [&](uint32_t i) { return set[i]; });
+    t = (static_cast<uint64_t>(tk.y) << 32) | tk.x;
+  }
+  tok[s] = t;
+}
+
+template <int MODE>
+cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
+  const uint64_t n_groups = (p.n + 31) / 32;
+  const uint64_t want = (n_groups + kWarps - 1) / kWarps;
+  const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) ? want : sm_count);
+  const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= kMaxStageTgts;
+  const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
+  // per-site counters in shared memory when the policy is small and they fit beside the staged targets
+  uint32_t site_bytes = 0;
+  if (MODE != MODE_SIGN && p.n_sites > 0 && p.n_sites <= kMaxSmemSites && stage_bytes + p.n_sites * 16u <= kLeft)
+    site_bytes = p.n_sites * 16u;
+  const uint32_t smem = stage_bytes + site_bytes + kCtaFixedBytes + kWarps * kWarpBytes;
+  const bool tel = MODE != MODE_SIGN && (p.profile != 0 || p.ring_cap != 0);
+  if (tel) {
+    if constexpr (MODE != MODE_SIGN) {
+      if (staged)
+        wg_check_kernel<MODE, true, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+      else
+        wg_check_kernel<MODE, false, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    }
+  } else if (staged) {
+    wg_check_kernel<MODE, true, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+  } else {
+    wg_check_kernel<MODE, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+  }
+  ++*launches;
+  return cudaGetLastError();
+}
+
+template <int MODE, bool STAGED>
+cudaError_t opt_in() {
+  if constexpr (MODE != MODE_SIGN) {
+    const cudaError_t e = cudaFuncSetAttribute(wg_check_kernel<MODE, STAGED, true>,
+                                               cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kSmemMax));
+    if (e != cudaSuccess) return e;
+  }
+  return cudaFuncSetAttribute(wg_check_kernel<MODE, STAGED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              static_cast<int>(kSmemMax));
+}
+
+}  // namespace
+
+cudaError_t init_kernels() {
+  cudaError_t e;
+  if ((e = opt_in<MODE_VERIFY, true>()) != cudaSuccess) return e;
+  if ((e = opt_in<MODE_VERIFY, false>()) != cudaSuccess) return e;
+  if ((e = opt_in<MODE_FORWARD, true>()) != cudaSuccess) return e;
+  if ((e = opt_in<MODE_FORWARD, false>()) != cudaSuccess) return e;
+  if ((e = opt_in<MODE_SIGN, false>()) != cudaSuccess) return e;
+  return cudaSuccess;
+}
+
+cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
+  return launch_mode<MODE_SIGN>(p, sm_count, st, launches);
+}
+
+cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
+  return p.tag ? launch_mode<MODE_VERIFY>(p, sm_count, st, launches) : launch_mode<MODE_FORWARD>(p, sm_count, st, launches);
+}
+
+cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* launches) {
+  wg_first_record<<<1, 1, 0, st>>>(p, p.tag != nullptr);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t v0,
+                                uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st, uint64_t* launches) {
+  if (n_sites == 0) return cudaSuccess;
+  wg_build_tokens<<<(n_sites + 255) / 256, 256, 0, st>>>(tok, recs, tgts, n_sites, v0, v1, v2, v3);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+}  // namespace wg

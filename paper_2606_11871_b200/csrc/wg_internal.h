@@ -51,6 +51,8 @@ enum CounterWord {
   C_RING_TOTAL = 30,  // violation records offered to the ring (recorded = min(total, capacity))
   C_SPARE31 = 31,
   C_META_FAIL = 32,   // forward records that failed their authentication (metadata-integrity profile, R37)
+  C_SKIP_SITE_EVENTS = 33,  // non-empty events at protected sites the coverage-reduced profile leaves out (R40)
+  C_SKIP_SITE_LANES = 34,
   C_WORDS = 40
 };
 
@@ -67,7 +69,7 @@ struct FirstRec {
   unsigned long long key;  // UINT64_MAX: none
 };
 enum : uint32_t { PROFILE_SKIP_FORWARD = 1, PROFILE_SKIP_BACKWARD = 2, PROFILE_LOW_TELEMETRY = 4,
-                  PROFILE_METADATA_INTEGRITY = 8 };
+                  PROFILE_METADATA_INTEGRITY = 8, PROFILE_COVERAGE_REDUCED = 16 };
 
 // Per-site counters: 4 x u64 per site, layout of wg_site_counters.
 enum SiteWord { S_EVENTS = 0, S_LANES_CHECKED = 1, S_LANES_VIOLATION = 2, S_LANES_BLOCKED = 3 };
