@@ -52,17 +52,27 @@ constexpr uint32_t kMaxSmemSites = 1024;  // policies up to this size keep their
 
 // ---- shared-memory carve-up ----------------------------------------------------------------------
 // CTA part: [tgts staged: stage_bytes][per-site counters: site_bytes][cnt64: 40 x u64][bykind: 8 x u32][mbar, pad]
-// warp part: event records [2 groups][32] x 64 B, then the work queue (u32 items; warp-uniform items from the
-// front, lane-divergent items from the back)
-//   record: +0  SipHash state the event's consumer passes start from (8 words)
+// warp part: event records [2 groups][33] x 80 B (record 32 of a group is a dummy that absorbs the padding trips of
+// the producer loop), the work queue (u32 items; warp-uniform items from the front, lane-divergent items from the
+// back), and the producer's list of the group's protected events (16 B each)
+//   record: +0  SipHash state the event's consumer passes start from (8 words); a forward event parks its set range
+//               {offset, count} at +16 instead
 //           +32 ctx lo (context_base & ~31), +36 ctx hi, +40 element base (event index * 32 - slot * 32: adding a
 //               queue item's low half gives the element index of (event, lane) in val / tag), +44 lanes whose value
 //               differs from the first active lane's (0: warp-uniform)
-//           +48 active mask, +52 meta = cls | kind << 4 | first active lane << 8, +56 violation mask, +60 site id
-constexpr uint32_t kRecBytes = 64;
-constexpr uint32_t kRecArea = 2 * 32 * kRecBytes;  // 4 KB
+//           +48 active mask, +52 queue mask (the active mask of a return check, else 0), +56 first active lane,
+//           +60 violation mask, +64 meta = cls | kind << 4, +68 site id
+constexpr uint32_t kRecBytes = 80;
+constexpr uint32_t kGroupRecs = 33;
+constexpr uint32_t kRecArea = 2 * kGroupRecs * kRecBytes;  // 5,280 B
 constexpr uint32_t kQueueItems = 1024 + 64;        // one group adds at most 1,024 items; each queue carries < 32
-constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 4;
+#ifndef WG_BATCH
+#define WG_BATCH 4
+#endif
+constexpr uint32_t kBatch = WG_BATCH;              // row loads in flight per lane in the producer loop
+constexpr uint32_t kListBytes = 40 * 16;           // up to 32 protected events, padded to a multiple of kBatch
+constexpr uint32_t kEntryMul = (kRecBytes << 16) | 32u;  // queue item of (slot, lane) = slot * kEntryMul + lane
+constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 4 + kListBytes;
 constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 8 * 4 + 16 + 16;  // cnt64, bykind, mbar (+pad to 16)
 constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
 constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
@@ -139,6 +149,13 @@ __device__ __forceinline__ const uint64_t* elem_ptr(const uint64_t* base, uint32
   uint64_t r;
   asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(elem), "l"(reinterpret_cast<uint64_t>(base)));
   return reinterpret_cast<const uint64_t*>(r);
+}
+
+// base + byte offset, likewise
+__device__ __forceinline__ const char* byte_ptr(const char* base, uint32_t off) {
+  uint64_t r;
+  asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(r) : "r"(off), "l"(reinterpret_cast<uint64_t>(base)));
+  return reinterpret_cast<const char*>(r);
 }
 
 // TMA: 1-D bulk copy global -> shared with completion on an mbarrier (whole-table staging of the target sets), and
@@ -272,6 +289,11 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * kWarpBytes;
   const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 4 * k
   const uint32_t q_top = q_s + (kQueueItems - 1) * 4;        // divergent items: q_top - 4 * k
+  const uint32_t list_s = q_s + kQueueItems * 4;
+  if (lane < 2) {  // the two dummy records: no active lane, nothing to queue
+    sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 32, 0u, 0u, 0u, 0u);
+    sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 48, 0u, 0u, 0u, 0u);
+  }
 
   if (threadIdx.x < C_WORDS) cnt64[threadIdx.x] = 0ull;
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = 0u;
@@ -328,7 +350,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         const uint2 v = ldg_v2_keep(elem_ptr(p.val, elem));
         sip_tail_val_ctx(s, v.x, v.y, cx.x ^ (item & 31u), cx.y, tg.x, tg.y, dl, dh);
       }
-      if ((dl | dh) != 0u) atoms_or(ra + 56, 1u << (item & 31u));  // rare: the lane's token does not match
+      if ((dl | dh) != 0u) atoms_or(ra + 60, 1u << (item & 31u));  // rare: the lane's token does not match
     }
   };
   // run every full pass of both queues, then move what is left (< 32 items each) to the queue heads.
@@ -363,9 +385,10 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   // ---- event-parallel epilogue of a finished group: verdicts (a6), violation counters (a7), first violation (a8) ----
   auto epilogue = [&](uint32_t rpar, uint64_t e0) {
     if constexpr (MODE != MODE_SIGN) {
-      const uint32_t ra = rec_s + (rpar * 32u + lane) * kRecBytes;
-      const uint4 m = lds_v4(ra + 48);  // active, meta, viol, site
-      const uint32_t active = m.x, cls = m.y & 15u, kind = (m.y >> 4) & 15u, viol = m.z, site = m.w;
+      const uint32_t ra = rec_s + (rpar * kGroupRecs + lane) * kRecBytes;
+      const uint4 m = lds_v4(ra + 48);   // active, queue mask, first, viol
+      const uint2 ms = lds_v2(ra + 64);  // meta, site
+      const uint32_t active = m.x, cls = ms.x & 15u, kind = (ms.x >> 4) & 15u, viol = m.w, site = ms.y;
       const bool valid = cls != CLS_NONE;
       if (valid) st_stream_v2(p.out + (e0 + lane), viol, enforce ? (active & ~viol) : active);
       // violations are rare (0.05 % of events in the paper-shaped stream): one warp-uniform branch per group
@@ -448,9 +471,9 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint64_t e0 = gi * 32;
     const uint4 r_nxt = load_rec(h_nxt);
     const uint4 h_nn = load_hdr(gn + stride);
-    const uint32_t rbase = rec_s + par * (32u * kRecBytes);
+    const uint32_t rbase = rec_s + par * (kGroupRecs * kRecBytes);
     const uint32_t ra_me = rbase + lane * kRecBytes;
-    const uint32_t slot_me = par * 32u + lane;
+    const uint32_t slot_me = par * kGroupRecs + lane;
     const uint32_t cu = nu, cd = nd;  // items carried over from the previous group
 
     // ---- event-parallel: classify (a1, a2) ----
@@ -491,9 +514,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t m_fwd = (MODE == MODE_SIGN) ? 0u : __ballot_sync(kFull, cls == CLS_FWD);
     uint32_t viol = (cls == CLS_FAIL) ? active : 0u;  // fail closed (R13, R14)
     sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, static_cast<uint32_t>(e0 + lane) * 32u - slot_me * 32u, 0u);
-    sts_v4(ra_me + 48, active, cls | (kind << 4) | (first << 8), viol, site);
-
-    if (MODE != MODE_SIGN && cls == CLS_FWD) sts_v2(ra_me + 16, off, cnt);  // (a forward event has no MAC state)
+    sts_v4(ra_me + 48, active, cls == CLS_RET ? active : 0u, first, viol);
+    sts_v2(ra_me + 64, cls | (kind << 4), site);
 
     // ---- counters that need no verdict (a7) ----
     const uint32_t judged_na = (cls == CLS_RET || cls == CLS_FWD) ? na : 0u;
@@ -550,73 +572,62 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       }
     }
 
-    // ---- event-parallel: the site word of the MAC, once per event; the key-derived initial state exists in the
-    //      kernel parameters only (constant bank).  Leaves the "pre-A" state the tails start from. ----
-    Sip32 st = s_init;
-    if (MODE != MODE_FORWARD && m_ret != 0u) {
-      sip_absorb(st, site, p.bind_hi);  // LE64(site_id | digest32 << 32): zero-extended site id unless bound (R3, R5, R39)
-      sip_qA(st);
-    }
     __syncwarp();  // the records are visible to every lane
 
-    // ---- producer loop (lane-parallel), one trip per protected event: row load, warp-uniformity, queueing ----
-    {
-      const uint64_t* vrow = p.val + (e0 * 32 + lane);
-      uint64_t* trow = (MODE == MODE_SIGN) ? p.tag_out + (e0 * 32 + lane) : nullptr;
-      const uint32_t item_me = slot_me - lane;  // par * 32: the group's first slot
-      const uint32_t need = (MODE == MODE_SIGN) ? __ballot_sync(kFull, valid) : (m_ret | m_fwd);
+    // ---- producer loop (lane-parallel), one trip per protected event: row load, warp-uniformity, queueing.
+    //      Straight-line code: the group's protected events are listed first (event-parallel), padded to a multiple
+    //      of kBatch with trips on the group's dummy record (no active lane: nothing is queued, nothing counted), so a batch
+    //      has no branch and every sync operation sees the whole warp. ----
+    const uint32_t need = (MODE == MODE_SIGN) ? m_ret : (m_ret | m_fwd);
+    if (need != 0u) {
+      const uint32_t n_need = __popc(need);
+      const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
+      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * kEntryMul, 0u);
+      if (lane < ((kBatch - n_need) & (kBatch - 1u)))
+        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * kEntryMul, 0u);
+      __syncwarp();
+      const char* vrow = reinterpret_cast<const char*>(p.val + (e0 * 32 + lane));
+      char* trow = (MODE == MODE_SIGN) ? reinterpret_cast<char*>(p.tag_out + (e0 * 32 + lane)) : nullptr;
+      uint32_t qu = q_s + nu * 4u, qd = q_top - nd * 4u;  // where the next uniform / divergent item goes
 #pragma unroll 1
-      for (uint32_t b0 = 0; b0 < 32; b0 += 8) {
-        const uint32_t nb = (need >> b0) & 0xffu;
-        if (nb == 0u) continue;
-        uint2 v[8];
+      for (uint32_t b0 = 0; b0 < n_need; b0 += kBatch) {
+        uint4 le[kBatch];
+        uint2 v[kBatch];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          v[j] = make_uint2(0u, 0u);
-          if ((((MODE == MODE_SIGN) ? m_ret : need) >> (b0 + j)) & 1u) v[j] = ldg_v2_keep(vrow + (b0 + j) * 32);
+        for (int j = 0; j < kBatch; ++j) le[j] = lds_v4(list_s + (b0 + j) * 16u);  // record, row offset, queue item base
+#pragma unroll
+        for (int j = 0; j < kBatch; ++j) v[j] = ldg_v2_keep(byte_ptr(vrow, le[j].y));
+#pragma unroll
+        for (int j = 0; j < kBatch; ++j) {
+          const uint32_t re = le[j].x;
+          const uint4 am = lds_v4(re + 48);  // active, queue mask, first active lane, -
+          const uint32_t rx = __shfl_sync(kFull, v[j].x, am.z), ry = __shfl_sync(kFull, v[j].y, am.z);
+          const uint32_t diff = __ballot_sync(kFull, v[j].x != rx || v[j].y != ry) & am.x;
+          sts_u32(re + 44, diff);  // (every lane stores the same word)
+          // a return check: its active lanes, compacted, go to the queue of its class
+          const uint32_t rank = __popc(am.y & ltmask), nae = __popc(am.y);
+          const bool div = diff != 0u, act = (am.y & lanebit) != 0u;
+          const uint32_t addr = div ? mad32(rank, 0xfffffffcu, qd) : mad32(rank, 4u, qu);
+          if (act) sts_u32(addr, le[j].z + lane);
+          qd = div ? mad32(nae, 0xfffffffcu, qd) : qd;
+          qu = div ? qu : mad32(nae, 4u, qu);
+          if (MODE == MODE_SIGN && !act && am.x != 0u) st_stream_v2(trow + le[j].y, 0u, 0u);  // inactive lanes sign nothing (R10)
         }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const uint32_t e = b0 + j;
-          if (!((need >> e) & 1u)) continue;
-          const uint32_t re = rbase + e * kRecBytes;
-          if (MODE == MODE_SIGN && !((m_ret >> e) & 1u)) {
-            st_stream_v2(trow + e * 32, 0u, 0u);  // not a return check: a zero row (R10)
-            continue;
-          }
-          const uint2 am = lds_v2(re + 48);  // active, meta
-          const uint32_t a = am.x, f = (am.y >> 8) & 31u;
-          const uint32_t rx = __shfl_sync(kFull, v[j].x, f), ry = __shfl_sync(kFull, v[j].y, f);
-          const uint32_t diff = __ballot_sync(kFull, v[j].x != rx || v[j].y != ry) & a;
-          const bool act = (a & lanebit) != 0u;
-          if (MODE != MODE_SIGN && ((m_fwd >> e) & 1u)) {
-            // forward event: a warp-uniform target is searched once, event-parallel, below; lane-divergent targets
-            // are searched here, per lane (per-warp checking only after proving uniformity)
-            if (diff != 0u) {
-              const uint2 oc = lds_v2(re + 16);  // off, cnt (parked in the unused state words of a forward event)
-              bool bad = false;
-              if (!(TEL && (p.profile & PROFILE_METADATA_INTEGRITY))) {
-                bad = act && !member<STAGED>(p, tg_s, oc.x, oc.y, v[j].x, v[j].y);
-                const uint32_t vb = __ballot_sync(kFull, bad);
-                if (lane == 0) sts_u32(re + 56, vb);
-              }
-            }
-            if (lane == 0) sts_u32(re + 44, diff);
-            continue;
-          }
-          // return event: append the active lanes, compacted, to the queue of its class
-          if (lane == 0) sts_u32(re + 44, diff);
-          const uint32_t rank = __popc(a & ltmask);
-          const uint32_t entry = ((e + item_me) * (kRecBytes << 16 | 32u)) + lane;  // record offset << 16 | slot * 32 + lane
-          const uint32_t nae = __popc(a);
-          if (diff == 0u) {
-            if (act) sts_u32(q_s + (nu + rank) * 4u, entry);
-            nu += nae;
-          } else {
-            if (act) sts_u32(q_top - (nd + rank) * 4u, entry);
-            nd += nae;
-          }
-          if (MODE == MODE_SIGN && !act) st_stream_v2(trow + e * 32, 0u, 0u);  // inactive lanes sign nothing (R10)
+      }
+      nu = (qu - q_s) >> 2;
+      nd = (q_top - qd) >> 2;
+    }
+    if constexpr (MODE == MODE_SIGN) {
+      // every event that is not a return check gets a zero row (R10): non-return sites, empty masks; written as
+      // 16-byte stores: a half-warp covers one 256-byte row, one instruction covers two events
+      const uint32_t zmask = __ballot_sync(kFull, valid && cls != CLS_RET);
+      if (zmask) {
+        const uint32_t half = lane >> 4, chunk = lane & 15u;
+#pragma unroll 4
+        for (int j = 0; j < 16; ++j) {
+          const uint32_t e = 2u * j + half;
+          if ((zmask >> e) & 1u)
+            asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%1,%1,%1};" ::"l"(p.tag_out + ((e0 + e) * 32 + chunk * 2)), "r"(0u) : "memory");
         }
       }
     }
@@ -624,23 +635,30 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
 
     // ---- event-parallel: per-event part of the MAC; search of warp-uniform forward targets ----
     {
-      const uint32_t diff = lds_u32(ra_me + 44);
-      const bool is_uni = diff == 0u;
+      const bool judged = cls == CLS_RET || cls == CLS_FWD;
+      const bool is_uni = judged && lds_u32(ra_me + 44) == 0u;
       uint32_t ul = 0, uh = 0;
-      if ((cls == CLS_RET || cls == CLS_FWD) && is_uni) {
+      if (is_uni) {
         const uint2 r = ldg_v2_keep(p.val + ((e0 + lane) * 32 + first));  // the event's one value (an L1 hit)
         ul = r.x;
         uh = r.y;
       }
-      if (cls == CLS_RET) {
+      if (MODE != MODE_FORWARD && m_ret != 0u) {
+        // the site word of the MAC, once per event; the key-derived initial state exists in the kernel parameters only
+        // (constant bank).  Leaves the "pre-A" state the lane-divergent tails start from.
+        Sip32 st = s_init;
+        sip_absorb(st, site, p.bind_hi);  // LE64(site_id | digest32 << 32): zero-extended site id unless bound (R3, R5, R39)
+        sip_qA(st);
         if (is_uni) {
           sip_absorb_preA(st, ul, uh);  // the continuation word, once per event
           sip_qA(st);                   // quarter A of the context word's first round
           st.v3l ^= h_cur.z & ~31u;     // and the lane-independent bits of the context word
           st.v3h ^= h_cur.w;
         }
-        sts_v4(ra_me, st.v0l, st.v0h, st.v1l, st.v1h);
-        sts_v4(ra_me + 16, st.v2l, st.v2h, st.v3l, st.v3h);
+        if (cls == CLS_RET) {
+          sts_v4(ra_me, st.v0l, st.v0h, st.v1l, st.v1h);
+          sts_v4(ra_me + 16, st.v2l, st.v2h, st.v3l, st.v3h);
+        }
       }
       if constexpr (MODE != MODE_SIGN) {
         bool bad_rec = false;
@@ -663,21 +681,26 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
             const uint32_t m_bad = __ballot_sync(kFull, bad_rec);
             if (m_bad && lane == 0)
               atomicAdd(p.glob + C_META_FAIL, static_cast<unsigned long long>(__popc(m_bad)));
-            // lane-divergent forward events of an authenticated record: searched here, per lane, one event at a time
-            for (uint32_t m = m_fwd & ~m_bad & __ballot_sync(kFull, !is_uni); m; m &= m - 1) {
-              const uint32_t e = __ffs(m) - 1;
-              const uint32_t a = __shfl_sync(kFull, active, e);
-              const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
-              const uint2 v = ldg_v2_keep(p.val + ((e0 + e) * 32 + lane));
-              const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !member<STAGED>(p, tg_s, o2, c2, v.x, v.y));
-              if (lane == e) viol = vb;
-            }
-            if (cls == CLS_FWD && !is_uni && !bad_rec) sts_u32(ra_me + 56, viol);
           }
         }
-        if (cls == CLS_FWD && bad_rec) sts_u32(ra_me + 56, active);
-        if (cls == CLS_FWD && is_uni && !bad_rec)
-          sts_u32(ra_me + 56, member<STAGED>(p, tg_s, off, cnt, ul, uh) ? 0u : active);
+        // lane-divergent forward targets are searched per lane, one event at a time (per-warp checking
+        // only after proving uniformity); a warp-uniform target is searched once, by the event's lane
+        uint32_t fviol = 0;
+        for (uint32_t m = __ballot_sync(kFull, cls == CLS_FWD && !is_uni && !bad_rec); m; m &= m - 1) {
+          const uint32_t e = __ffs(m) - 1;
+          const uint32_t a = __shfl_sync(kFull, active, e);
+          const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
+          const uint2 v = ldg_v2_keep(p.val + ((e0 + e) * 32 + lane));
+          const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !member<STAGED>(p, tg_s, o2, c2, v.x, v.y));
+          if (lane == e) fviol = vb;
+        }
+        if (cls == CLS_FWD) {
+          if (bad_rec)
+            fviol = active;
+          else if (is_uni)
+            fviol = member<STAGED>(p, tg_s, off, cnt, ul, uh) ? 0u : active;
+          sts_u32(ra_me + 60, fviol);
+        }
       }
     }
     // ---- the next group's rows -> L2: lane i pulls the two cache lines of row i of the next group, if that event
