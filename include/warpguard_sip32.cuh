@@ -189,6 +189,67 @@ __device__ __forceinline__ void sip_tail_val_ctx(Sip32 s, uint32_t vl, uint32_t 
   sip_finish(s, xl, xh, outl, outh);
 }
 
+// The same two tails for TWO independent items per thread, interleaved quarter by quarter so that the instruction
+// stream offers the scheduler two dependent chains instead of one.
+__device__ __forceinline__ void sip_round2(Sip32& a, Sip32& b) {
+  sip_qA(a); sip_qA(b);
+  sip_qB(a); sip_qB(b);
+  sip_qC(a); sip_qC(b);
+  sip_qD(a); sip_qD(b);
+}
+// one message word into two pre-A states (quarter A of the first round already applied)
+__device__ __forceinline__ void sip_absorb_preA2(Sip32& a, Sip32& b, uint32_t mal, uint32_t mah, uint32_t mbl, uint32_t mbh) {
+  a.v3l ^= mal; a.v3h ^= mah; b.v3l ^= mbl; b.v3h ^= mbh;
+  sip_qB(a); sip_qB(b);
+  sip_qC(a); sip_qC(b);
+  sip_qD(a); sip_qD(b);
+  sip_round2(a, b);
+  a.v0l ^= mal; a.v0h ^= mah; b.v0l ^= mbl; b.v0h ^= mbh;
+}
+__device__ __forceinline__ void sip_finish2(Sip32& a, Sip32& b, uint32_t xal, uint32_t xah, uint32_t xbl, uint32_t xbh,
+                                            uint32_t& oal, uint32_t& oah, uint32_t& obl, uint32_t& obh) {
+  a.v3h ^= kLenHi; b.v3h ^= kLenHi;
+  sip_round2(a, b);
+  sip_round2(a, b);
+  a.v0h ^= kLenHi; b.v0h ^= kLenHi;
+  a.v2l ^= 0xffu; b.v2l ^= 0xffu;
+  sip_round2(a, b);
+  sip_round2(a, b);
+  sip_round2(a, b);
+  sip_round2(a, b);
+  oal = a.v0l ^ a.v1l ^ a.v2l ^ a.v3l ^ xal;
+  oah = a.v0h ^ a.v1h ^ a.v2h ^ a.v3h ^ xah;
+  obl = b.v0l ^ b.v1l ^ b.v2l ^ b.v3l ^ xbl;
+  obh = b.v0h ^ b.v1h ^ b.v2h ^ b.v3h ^ xbh;
+}
+__device__ __forceinline__ void sip_tail_ctxlane2(Sip32 a, Sip32 b, uint32_t cal, uint32_t cah, uint32_t cbl, uint32_t cbh,
+                                                  uint32_t xal, uint32_t xah, uint32_t xbl, uint32_t xbh,
+                                                  uint32_t& oal, uint32_t& oah, uint32_t& obl, uint32_t& obh) {
+  sip_qB(a); sip_qB(b);
+  sip_qC(a); sip_qC(b);
+  sip_qD(a); sip_qD(b);
+  sip_round2(a, b);
+  a.v0l ^= cal; a.v0h ^= cah;
+  b.v0l ^= cbl; b.v0h ^= cbh;
+  sip_finish2(a, b, xal, xah, xbl, xbh, oal, oah, obl, obh);
+}
+__device__ __forceinline__ void sip_tail_val_ctx2(Sip32 a, Sip32 b, uint32_t val, uint32_t vah, uint32_t vbl, uint32_t vbh,
+                                                  uint32_t cal, uint32_t cah, uint32_t cbl, uint32_t cbh,
+                                                  uint32_t xal, uint32_t xah, uint32_t xbl, uint32_t xbh,
+                                                  uint32_t& oal, uint32_t& oah, uint32_t& obl, uint32_t& obh) {
+  a.v3l ^= val; a.v3h ^= vah; b.v3l ^= vbl; b.v3h ^= vbh;
+  sip_qB(a); sip_qB(b);
+  sip_qC(a); sip_qC(b);
+  sip_qD(a); sip_qD(b);
+  sip_round2(a, b);
+  a.v0l ^= val; a.v0h ^= vah; b.v0l ^= vbl; b.v0h ^= vbh;
+  a.v3l ^= cal; a.v3h ^= cah; b.v3l ^= cbl; b.v3h ^= cbh;
+  sip_round2(a, b);
+  sip_round2(a, b);
+  a.v0l ^= cal; a.v0h ^= cah; b.v0l ^= cbl; b.v0h ^= cbh;
+  sip_finish2(a, b, xal, xah, xbl, xbh, oal, oah, obl, obh);
+}
+
 // per-lane tail when the event's state already covers site and continuation and has quarter A of the next round
 // applied, but the context word (cl, ch) is the lane's own in every bit (shadow stack: the depth is part of it)
 __device__ __forceinline__ void sip_tail_ctx(Sip32 s, uint32_t cl, uint32_t ch, uint32_t xl, uint32_t xh,

@@ -65,7 +65,7 @@ constexpr uint32_t kMaxSmemSites = 1024;  // policies up to this size keep their
 constexpr uint32_t kRecBytes = 80;
 constexpr uint32_t kGroupRecs = 33;
 constexpr uint32_t kRecArea = 2 * kGroupRecs * kRecBytes;  // 5,280 B
-constexpr uint32_t kQueueItems = 1024 + 64;        // one group adds at most 1,024 items; each queue carries < 32
+constexpr uint32_t kQueueItems = 1024 + 128;       // one group adds at most 1,024 items; each queue carries < 64
 #ifndef WG_BATCH
 #define WG_BATCH 4
 #endif
@@ -144,14 +144,15 @@ __device__ __forceinline__ uint32_t mad32(uint32_t a, uint32_t b, uint32_t c) {
   asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
   return r;
 }
-// base + 8 * element as one wide multiply-add on the FMA pipe
+// base + 8 * element (ptxas turns it into a shift pair on the FMA pipe and a 64-bit add on the ALU pipe; passing the
+// multiplier in a register, so that it has to stay an IMAD.WIDE, was measured: the array base lives in uniform registers,
+// which IMAD.WIDE cannot take as its addend, so the 64-bit add stays and the kernel gets slower, 13.37 -> 13.72 ms)
 __device__ __forceinline__ const uint64_t* elem_ptr(const uint64_t* base, uint32_t elem) {
   uint64_t r;
   asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(elem), "l"(reinterpret_cast<uint64_t>(base)));
   return reinterpret_cast<const uint64_t*>(r);
 }
-
-// base + byte offset, likewise
+// base + byte offset
 __device__ __forceinline__ const char* byte_ptr(const char* base, uint32_t off) {
   uint64_t r;
   asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(r) : "r"(off), "l"(reinterpret_cast<uint64_t>(base)));
@@ -258,7 +259,7 @@ __device__ __forceinline__ Sip32 lds_state(uint32_t a) {
 
 // warp-uniform running counters of one warp (flushed once at the end)
 struct WarpCtr {
-  uint32_t total, empty, unknown, misrouted, ret_checks, fwd_checks, ret_lanes, fwd_lanes, signed_lanes, skipped;
+  uint32_t ret_checks, fwd_checks, ret_lanes, fwd_lanes;  // sign: ret_lanes = signed lanes, fwd_checks = skipped events
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -308,82 +309,92 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     mbar_wait(mbar_cta, 0);
   }
 
-  const uint64_t n_groups = (p.n + 31) / 32;
-  const uint64_t stride = static_cast<uint64_t>(gridDim.x) * kWarps;
-  uint64_t gi = static_cast<uint64_t>(blockIdx.x) * kWarps + warp;
+  // a launch covers at most 2^27 events (wg_api.cu), so event and element indices (event * 32 + lane) fit 32 bits
+  const uint32_t n_ev = static_cast<uint32_t>(p.n);
+  const uint32_t n_groups = (n_ev + 31u) / 32u;
+  const uint32_t stride = gridDim.x * kWarps;
+  uint32_t gi = blockIdx.x * kWarps + warp;
   const bool enforce = p.mode != 0;
   const Sip32 s_init = init_state(p);
-  WarpCtr c = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  WarpCtr c = {0, 0, 0, 0};
   uint32_t par = 0;          // which half of the record area this group uses
   uint32_t nu = 0, nd = 0;   // items in the uniform / divergent queue (carried items first)
   bool have_prev = false;    // a previous group still waits for its epilogue
-  uint64_t prev_e0 = 0;
+  uint32_t prev_e0 = 0;
 
   // ---- consumer passes ------------------------------------------------------------------------------
-  // one pass over 32 queue items starting at item k0 of the uniform (UNI) or divergent queue; lanes with on == false
-  // (only in the partial passes that flush a queue) do nothing
-  auto pass = [&](auto uni_tag, uint32_t k0, bool on) {
-    constexpr bool UNI = decltype(uni_tag)::value;
-    if (!on) return;
-    const uint32_t qa = UNI ? q_s + (k0 + lane) * 4u : q_top - (k0 + lane) * 4u;
-    const uint32_t item = lds_u16(qa);           // slot * 32 + lane of the event
-    const uint32_t ra = rec_s + lds_u16(qa + 2); // the event's record
-    const uint4 cx = lds_v4(ra + 32);            // ctx lo, ctx hi, element base, -
-    Sip32 s = lds_state(ra);
-    const uint32_t elem = cx.z + item;
-    uint32_t dl, dh;
+  // One pass = 64 queue items, two per lane (items k0 + lane and k0 + 32 + lane of the uniform or of the divergent
+  // queue): twice the instruction-level parallelism of the dependent SipRound chains for the same instruction count.
+  // ONE copy of this code serves both queues and the partial passes that flush them (on_a / on_b; a lane with on_b
+  // false works on item a twice and drops the second result): with the producer and the event-parallel phases it has
+  // to fit the 32 KB instruction cache — a version with one specialised copy per case ran at half speed on
+  // no_instruction stalls.
+  auto pass2 = [&](bool div, uint32_t k0, bool on_a, bool on_b) __attribute__((always_inline)) {
+    if (!on_a) return;
+    const uint32_t kb = on_b ? k0 + 32u : k0;
+    const uint32_t qa = div ? mad32(k0 + lane, 0xfffffffcu, q_top) : mad32(k0 + lane, 4u, q_s);
+    const uint32_t qb = div ? mad32(kb + lane, 0xfffffffcu, q_top) : mad32(kb + lane, 4u, q_s);
+    const uint32_t ia = lds_u16(qa), ib = lds_u16(qb);            // slot * 32 + lane of the event
+    const uint32_t ra = rec_s + lds_u16(qa + 2), rb = rec_s + lds_u16(qb + 2);  // the events' records
+    const uint4 ca = lds_v4(ra + 32), cb = lds_v4(rb + 32);        // ctx lo, ctx hi, element base, -
+    Sip32 sa = lds_state(ra), sb = lds_state(rb);
+    const uint32_t ea = ca.z + ia, eb = cb.z + ib;
+    const uint32_t la = ia & 31u, lb = ib & 31u;
+    uint2 ta = make_uint2(0u, 0u), tb = make_uint2(0u, 0u);
+    if constexpr (MODE != MODE_SIGN) {
+      ta = ldg_v2_stream(elem_ptr(p.tag, ea));
+      tb = ldg_v2_stream(elem_ptr(p.tag, eb));
+    }
+    if (div) {
+      // lane-divergent continuation: the states are the sites' pre-A states; absorb each item's own value, then bring
+      // the states to where a warp-uniform event's state starts (B folded into v3, quarter A of the next round done)
+      const uint2 va = ldg_v2_keep(elem_ptr(p.val, ea)), vb = ldg_v2_keep(elem_ptr(p.val, eb));
+      sip_absorb_preA2(sa, sb, va.x, va.y, vb.x, vb.y);
+      sip_qA(sa);
+      sip_qA(sb);
+      sa.v3l ^= ca.x; sa.v3h ^= ca.y;
+      sb.v3l ^= cb.x; sb.v3h ^= cb.y;
+    }
+    uint32_t al, ah, bl, bh;
+    sa.v3l ^= la;
+    sb.v3l ^= lb;
+    sip_tail_ctxlane2(sa, sb, ca.x ^ la, ca.y, cb.x ^ lb, cb.y, ta.x, ta.y, tb.x, tb.y, al, ah, bl, bh);
     if constexpr (MODE == MODE_SIGN) {
-      if constexpr (UNI) {
-        s.v3l ^= item & 31u;
-        sip_tail_ctxlane(s, cx.x ^ (item & 31u), cx.y, 0u, 0u, dl, dh);
-      } else {
-        const uint2 v = ldg_v2_keep(elem_ptr(p.val, elem));
-        sip_tail_val_ctx(s, v.x, v.y, cx.x ^ (item & 31u), cx.y, 0u, 0u, dl, dh);
-      }
-      st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, elem)), dl, dh);
+      st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, ea)), al, ah);
+      if (on_b) st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, eb)), bl, bh);
     } else {
-      const uint2 tg = ldg_v2_stream(elem_ptr(p.tag, elem));
-      if constexpr (UNI) {
-        s.v3l ^= item & 31u;
-        sip_tail_ctxlane(s, cx.x ^ (item & 31u), cx.y, tg.x, tg.y, dl, dh);
-      } else {
-        const uint2 v = ldg_v2_keep(elem_ptr(p.val, elem));
-        sip_tail_val_ctx(s, v.x, v.y, cx.x ^ (item & 31u), cx.y, tg.x, tg.y, dl, dh);
+      if ((al | ah | bl | bh) != 0u) {  // rare: a lane's token does not match
+        if ((al | ah) != 0u) atoms_or(ra + 60, 1u << la);
+        if ((bl | bh) != 0u) atoms_or(rb + 60, 1u << lb);  // (with on_b false this repeats item a's bit: harmless)
       }
-      if ((dl | dh) != 0u) atoms_or(ra + 60, 1u << (item & 31u));  // rare: the lane's token does not match
     }
   };
-  // run every full pass of both queues, then move what is left (< 32 items each) to the queue heads.
-  // flush: also run the partial passes, leaving both queues empty.
-  auto drain = [&](bool flush_u, bool flush_d) {
-    uint32_t k = 0;
-    for (; k + 32 <= nu; k += 32) pass(std::true_type{}, k, true);
-    if (flush_u && k < nu) {
-      pass(std::true_type{}, k, k + lane < nu);
-      k = nu;
+  // run every full pass of both queues, then move what is left (< 64 items each) to the queue heads.
+  // flush: also run a partial pass, leaving the queue empty.
+  auto drain = [&](bool flush_u, bool flush_d) __attribute__((always_inline)) {
+#pragma unroll 1
+    for (uint32_t cl = 0; cl < 2u; ++cl) {
+      const bool div = cl != 0u;
+      const uint32_t n = div ? nd : nu;
+      const bool flush = div ? flush_d : flush_u;
+      uint32_t k = 0;
+#pragma unroll 1
+      for (; k + 64u <= n || (flush && k < n); k += 64u) pass2(div, k, k + lane < n, k + 32u + lane < n);
+      k = k < n ? k : n;
+      const uint32_t r = n - k;  // < 64 items stay: two per lane
+      uint32_t c0 = 0, c1 = 0;
+      if (lane < r) c0 = lds_u32(div ? q_top - (k + lane) * 4u : q_s + (k + lane) * 4u);
+      if (lane + 32u < r) c1 = lds_u32(div ? q_top - (k + 32u + lane) * 4u : q_s + (k + 32u + lane) * 4u);
+      __syncwarp();
+      if (lane < r) sts_u32(div ? q_top - lane * 4u : q_s + lane * 4u, c0);
+      if (lane + 32u < r) sts_u32(div ? q_top - (32u + lane) * 4u : q_s + (32u + lane) * 4u, c1);
+      if (div) nd = r; else nu = r;
     }
-    const uint32_t ru = nu - k;
-    uint32_t carry = 0;
-    if (ru) carry = lds_u32(q_s + (k + (lane < ru ? lane : 0u)) * 4u);
-    uint32_t kd = 0;
-    for (; kd + 32 <= nd; kd += 32) pass(std::false_type{}, kd, true);
-    if (flush_d && kd < nd) {
-      pass(std::false_type{}, kd, kd + lane < nd);
-      kd = nd;
-    }
-    const uint32_t rd = nd - kd;
-    uint32_t carry_d = 0;
-    if (rd) carry_d = lds_u32(q_top - (kd + (lane < rd ? lane : 0u)) * 4u);
-    __syncwarp();
-    if (lane < ru) sts_u32(q_s + lane * 4u, carry);
-    if (lane < rd) sts_u32(q_top - lane * 4u, carry_d);
-    nu = ru;
-    nd = rd;
     __syncwarp();
   };
 
   // ---- event-parallel epilogue of a finished group: verdicts (a6), violation counters (a7), first violation (a8) ----
-  auto epilogue = [&](uint32_t rpar, uint64_t e0) {
+  auto epilogue = [&](uint32_t rpar, uint32_t e0) __attribute__((always_inline)) {
     if constexpr (MODE != MODE_SIGN) {
       const uint32_t ra = rec_s + (rpar * kGroupRecs + lane) * kRecBytes;
       const uint4 m = lds_v4(ra + 48);   // active, queue mask, first, viol
@@ -404,7 +415,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         const uint32_t ave = __popc(__ballot_sync(kFull, viol != 0u));
         // first violation: smallest (seq << 5 | lane); seq = running event index (R12)
         unsigned long long key = ~0ull;
-        if (viol) key = ((p.seq_base + e0 + lane) << 5) | static_cast<uint32_t>(__ffs(viol) - 1);
+        if (viol) key = ((p.seq_base + (e0 + lane)) << 5) | static_cast<uint32_t>(__ffs(viol) - 1);
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) {
           const unsigned long long o = __shfl_xor_sync(kFull, key, d);
@@ -427,15 +438,15 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           if (slot < p.ring_cap) {
             const uint32_t fl = static_cast<uint32_t>(__ffs(viol) - 1);
             ViolRec r;
-            r.seq = p.seq_base + e0 + lane;
+            r.seq = p.seq_base + (e0 + lane);
             r.site_id = site;
             r.kind = kind;
             r.viol_mask = viol;
             r.active_mask = active;
             r.lane = fl;
             r.mode = p.mode;
-            r.observed = p.val[(e0 + lane) * 32 + fl];
-            r.stored = (MODE == MODE_VERIFY && cls == CLS_RET) ? p.tag[(e0 + lane) * 32 + fl] : 0ull;
+            r.observed = p.val[(e0 + lane) * 32u + fl];
+            r.stored = (MODE == MODE_VERIFY && cls == CLS_RET) ? p.tag[(e0 + lane) * 32u + fl] : 0ull;
             p.ring[slot] = r;
           }
         }
@@ -455,20 +466,25 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
 
   // ---- software pipeline of the event-parallel loads: the header two groups ahead, the site record one group ahead,
   //      so that the rows of the NEXT group can be pulled into L2 while this group is computed ----
-  auto load_hdr = [&](uint64_t g) -> uint4 {
-    const uint64_t e = g * 32 + lane;
-    return (g < n_groups && e < p.n) ? ldg_v4(p.hdr + e) : make_uint4(0xffffffffu, 0u, 0u, 0u);
+  auto load_hdr = [&](uint32_t g) __attribute__((always_inline)) -> uint4 {  // (g runs past n_groups by at most two strides: no 32-bit wrap)
+    const uint32_t e = g * 32u + lane;
+    return (g < n_groups && e < n_ev) ? ldg_v4(p.hdr + e) : make_uint4(0xffffffffu, 0u, 0u, 0u);
   };
-  auto load_rec = [&](const uint4& h) -> uint4 {
+  auto load_rec = [&](const uint4& h) __attribute__((always_inline)) -> uint4 {
     return h.x < p.n_sites ? ldg_v4(p.recs + h.x) : make_uint4(7u, 0u, 0u, 0u);
   };
   uint4 h_cur = load_hdr(gi);
   uint4 h_nxt = load_hdr(gi + stride);
   uint4 r_cur = load_rec(h_cur);
 
-  while (gi < n_groups) {
-    const uint64_t gn = gi + stride;
-    const uint64_t e0 = gi * 32;
+  // One trip per group of this warp, plus one last trip over an empty group (no valid event) that flushes the queues and
+  // runs the last real group's epilogue: the drain / epilogue code exists once (the kernel must stay small enough for
+  // the instruction cache: a version that inlined it twice ran at half speed on no_instruction stalls).
+  bool last = gi >= n_groups;
+  if (!last) do {
+    last = gi >= n_groups;
+    const uint32_t gn = gi + stride;
+    const uint32_t e0 = gi * 32u;
     const uint4 r_nxt = load_rec(h_nxt);
     const uint4 h_nn = load_hdr(gn + stride);
     const uint32_t rbase = rec_s + par * (kGroupRecs * kRecBytes);
@@ -477,7 +493,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t cu = nu, cd = nd;  // items carried over from the previous group
 
     // ---- event-parallel: classify (a1, a2) ----
-    const bool valid = e0 + lane < p.n;
+    const bool valid = e0 + lane < n_ev;
     const uint32_t site = h_cur.x;
     const uint32_t active = valid ? h_cur.y : 0u;
     const bool known = valid && site < p.n_sites;
@@ -513,22 +529,48 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t m_ret = __ballot_sync(kFull, cls == CLS_RET);
     const uint32_t m_fwd = (MODE == MODE_SIGN) ? 0u : __ballot_sync(kFull, cls == CLS_FWD);
     uint32_t viol = (cls == CLS_FAIL) ? active : 0u;  // fail closed (R13, R14)
-    sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, static_cast<uint32_t>(e0 + lane) * 32u - slot_me * 32u, 0u);
+    sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, (e0 + lane) * 32u - slot_me * 32u, 0u);
     sts_v4(ra_me + 48, active, cls == CLS_RET ? active : 0u, first, viol);
     sts_v2(ra_me + 64, cls | (kind << 4), site);
+
+    // ---- the producer's list of the group's protected events (event-parallel), padded to a multiple of kBatch with
+    //      trips on the group's dummy record (no active lane: nothing is queued, nothing counted), so that a batch is
+    //      straight-line code and every sync operation in it sees the whole warp ----
+    const uint32_t need = (MODE == MODE_SIGN) ? m_ret : (m_ret | m_fwd);
+    const uint32_t n_need = __popc(need);
+    if (need != 0u) {
+      const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
+      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * kEntryMul, lane * 32u);
+      if (lane < ((kBatch - n_need) & (kBatch - 1u)))
+        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * kEntryMul, 0u);
+    }
+    __syncwarp();  // the records and the list are visible to every lane
+    // value rows, straight from global memory: one coalesced 256-byte load per event, kBatch in flight per lane; the
+    // first batch is issued now and lands while the counters below are updated
+    const char* vrow = reinterpret_cast<const char*>(elem_ptr(p.val, e0 * 32u + lane));
+    uint2 va[kBatch], vb[kBatch];
+    auto load_batch = [&](uint2 (&v)[kBatch], uint32_t b0) {
+#pragma unroll
+      for (int j = 0; j < static_cast<int>(kBatch); ++j) v[j] = ldg_v2_keep(byte_ptr(vrow, lds_u32(list_s + (b0 + j) * 16u + 4u)));
+    };
+    if (need != 0u) load_batch(va, 0u);
 
     // ---- counters that need no verdict (a7) ----
     const uint32_t judged_na = (cls == CLS_RET || cls == CLS_FWD) ? na : 0u;
     if constexpr (MODE == MODE_SIGN) {
       const bool is_ret = known && kind == K_RET;
-      c.signed_lanes += __reduce_add_sync(kFull, is_ret ? na : 0u);
-      c.skipped += __popc(__ballot_sync(kFull, valid && !is_ret));
+      c.ret_lanes += __reduce_add_sync(kFull, is_ret ? na : 0u);           // signed lanes
+      c.fwd_checks += __popc(__ballot_sync(kFull, valid && !is_ret));      // events that sign nothing
     } else {
-      c.total += __popc(__ballot_sync(kFull, valid));
       if (__ballot_sync(kFull, valid && (!known || active == 0u || cls == CLS_FAIL))) {  // uncommon events
-        c.unknown += __popc(__ballot_sync(kFull, valid && !known));
-        c.empty += __popc(__ballot_sync(kFull, known && active == 0u));
-        c.misrouted += __popc(__ballot_sync(kFull, known && cls == CLS_FAIL));
+        const uint32_t u = __popc(__ballot_sync(kFull, valid && !known));
+        const uint32_t em = __popc(__ballot_sync(kFull, known && active == 0u));
+        const uint32_t mr = __popc(__ballot_sync(kFull, known && cls == CLS_FAIL));
+        if (lane == 0) {
+          if (u) atomicAdd(cnt64 + C_EVENTS_UNKNOWN, static_cast<unsigned long long>(u));
+          if (em) atomicAdd(cnt64 + C_EVENTS_EMPTY, static_cast<unsigned long long>(em));
+          if (mr) atomicAdd(cnt64 + C_EVENTS_MISROUTED, static_cast<unsigned long long>(mr));
+        }
       }
       c.ret_checks += __popc(m_ret);
       c.fwd_checks += __popc(m_fwd);
@@ -572,46 +614,37 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       }
     }
 
-    __syncwarp();  // the records are visible to every lane
-
-    // ---- producer loop (lane-parallel), one trip per protected event: row load, warp-uniformity, queueing.
-    //      Straight-line code: the group's protected events are listed first (event-parallel), padded to a multiple
-    //      of kBatch with trips on the group's dummy record (no active lane: nothing is queued, nothing counted), so a batch
-    //      has no branch and every sync operation sees the whole warp. ----
-    const uint32_t need = (MODE == MODE_SIGN) ? m_ret : (m_ret | m_fwd);
+    // ---- producer loop (lane-parallel), one trip per protected event: warp-uniformity of the row just loaded, and
+    //      for a return check the active lanes appended, compacted, to the queue of its class.  Double-buffered: the
+    //      next batch's rows are requested before this batch is looked at. ----
     if (need != 0u) {
-      const uint32_t n_need = __popc(need);
-      const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
-      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * kEntryMul, 0u);
-      if (lane < ((kBatch - n_need) & (kBatch - 1u)))
-        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * kEntryMul, 0u);
-      __syncwarp();
-      const char* vrow = reinterpret_cast<const char*>(p.val + (e0 * 32 + lane));
-      char* trow = (MODE == MODE_SIGN) ? reinterpret_cast<char*>(p.tag_out + (e0 * 32 + lane)) : nullptr;
       uint32_t qu = q_s + nu * 4u, qd = q_top - nd * 4u;  // where the next uniform / divergent item goes
-#pragma unroll 1
-      for (uint32_t b0 = 0; b0 < n_need; b0 += kBatch) {
-        uint4 le[kBatch];
-        uint2 v[kBatch];
+      auto consume_batch = [&](const uint2 (&v)[kBatch], uint32_t b0) {
 #pragma unroll
-        for (int j = 0; j < kBatch; ++j) le[j] = lds_v4(list_s + (b0 + j) * 16u);  // record, row offset, queue item base
-#pragma unroll
-        for (int j = 0; j < kBatch; ++j) v[j] = ldg_v2_keep(byte_ptr(vrow, le[j].y));
-#pragma unroll
-        for (int j = 0; j < kBatch; ++j) {
-          const uint32_t re = le[j].x;
-          const uint4 am = lds_v4(re + 48);  // active, queue mask, first active lane, -
+        for (int j = 0; j < static_cast<int>(kBatch); ++j) {
+          const uint4 le = lds_v4(list_s + (b0 + j) * 16u);  // record, row byte offset, queue item base, row element offset
+          const uint4 am = lds_v4(le.x + 48);                // active, queue mask, first active lane, -
           const uint32_t rx = __shfl_sync(kFull, v[j].x, am.z), ry = __shfl_sync(kFull, v[j].y, am.z);
           const uint32_t diff = __ballot_sync(kFull, v[j].x != rx || v[j].y != ry) & am.x;
-          sts_u32(re + 44, diff);  // (every lane stores the same word)
-          // a return check: its active lanes, compacted, go to the queue of its class
+          sts_u32(le.x + 44, diff);  // (every lane stores the same word)
           const uint32_t rank = __popc(am.y & ltmask), nae = __popc(am.y);
           const bool div = diff != 0u, act = (am.y & lanebit) != 0u;
           const uint32_t addr = div ? mad32(rank, 0xfffffffcu, qd) : mad32(rank, 4u, qu);
-          if (act) sts_u32(addr, le[j].z + lane);
+          if (act) sts_u32(addr, le.z + lane);
           qd = div ? mad32(nae, 0xfffffffcu, qd) : qd;
           qu = div ? qu : mad32(nae, 4u, qu);
-          if (MODE == MODE_SIGN && !act && am.x != 0u) st_stream_v2(trow + le[j].y, 0u, 0u);  // inactive lanes sign nothing (R10)
+          if (MODE == MODE_SIGN && !act && am.x != 0u)  // inactive lanes sign nothing (R10)
+            st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, e0 * 32u + lane + le.w)), 0u, 0u);
+        }
+      };
+#pragma unroll 1
+      for (uint32_t b0 = 0; b0 < n_need; b0 += 2u * kBatch) {
+        const bool more = b0 + kBatch < n_need;
+        if (more) load_batch(vb, b0 + kBatch);
+        consume_batch(va, b0);
+        if (more) {
+          if (b0 + 2u * kBatch < n_need) load_batch(va, b0 + 2u * kBatch);
+          consume_batch(vb, b0 + kBatch);
         }
       }
       nu = (qu - q_s) >> 2;
@@ -627,7 +660,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         for (int j = 0; j < 16; ++j) {
           const uint32_t e = 2u * j + half;
           if ((zmask >> e) & 1u)
-            asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%1,%1,%1};" ::"l"(p.tag_out + ((e0 + e) * 32 + chunk * 2)), "r"(0u) : "memory");
+            asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%1,%1,%1};" ::"l"(elem_ptr(p.tag_out, (e0 + e) * 32u + chunk * 2u)), "r"(0u) : "memory");
         }
       }
     }
@@ -639,7 +672,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       const bool is_uni = judged && lds_u32(ra_me + 44) == 0u;
       uint32_t ul = 0, uh = 0;
       if (is_uni) {
-        const uint2 r = ldg_v2_keep(p.val + ((e0 + lane) * 32 + first));  // the event's one value (an L1 hit)
+        const uint2 r = ldg_v2_keep(elem_ptr(p.val, (e0 + lane) * 32u + first));  // the event's one value (an L1 hit)
         ul = r.x;
         uh = r.y;
       }
@@ -690,7 +723,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           const uint32_t e = __ffs(m) - 1;
           const uint32_t a = __shfl_sync(kFull, active, e);
           const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
-          const uint2 v = ldg_v2_keep(p.val + ((e0 + e) * 32 + lane));
+          const uint2 v = ldg_v2_keep(elem_ptr(p.val, (e0 + e) * 32u + lane));
           const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !member<STAGED>(p, tg_s, o2, c2, v.x, v.y));
           if (lane == e) fviol = vb;
         }
@@ -706,15 +739,15 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     // ---- the next group's rows -> L2: lane i pulls the two cache lines of row i of the next group, if that event
     //      will need them (its site record has arrived by now); rows nobody will read are not fetched ----
     if (gn < n_groups) {
-      const bool v_nxt = gn * 32 + lane < p.n && h_nxt.y != 0u;
+      const bool v_nxt = gn * 32u + lane < n_ev && h_nxt.y != 0u;
       const bool ret_nxt = v_nxt && r_nxt.x == K_RET, fwd_nxt = v_nxt && r_nxt.x == K_FWD;
-      const char* vr = reinterpret_cast<const char*>(p.val + (gn * 32 + lane) * 32);
+      const char* vr = reinterpret_cast<const char*>(elem_ptr(p.val, (gn * 32u + lane) * 32u));
       if (MODE == MODE_FORWARD ? fwd_nxt : (MODE == MODE_SIGN ? ret_nxt : (ret_nxt || fwd_nxt))) {
         prefetch_l2(vr);
         prefetch_l2(vr + 128);
       }
       if (MODE == MODE_VERIFY && ret_nxt) {
-        const char* tr = reinterpret_cast<const char*>(p.tag + (gn * 32 + lane) * 32);
+        const char* tr = reinterpret_cast<const char*>(elem_ptr(p.tag, (gn * 32u + lane) * 32u));
         prefetch_l2(tr);
         prefetch_l2(tr + 128);
       }
@@ -723,8 +756,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
 
     // ---- consumer passes: every full pass; carried items of the previous group go first.  If a queue still holds
     //      items of the previous group and cannot fill a pass, it is flushed with a partial pass (rare). ----
-    // (carried items are the oldest: any full pass consumes them; nu_carry / nd_carry < 32)
-    drain(cu != 0u && nu < 32u, cd != 0u && nd < 32u);
+    // (carried items are the oldest: any full pass consumes them; fewer than 64 are carried per queue)
+    drain(last || (cu != 0u && nu < 64u), last || (cd != 0u && nd < 64u));
     if (have_prev) epilogue(par ^ 1u, prev_e0);
     have_prev = true;
     prev_e0 = e0;
@@ -734,28 +767,22 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     r_cur = r_nxt;
     h_nxt = h_nn;
     __syncwarp();
-  }
-  if (have_prev) {
-    drain(true, true);
-    epilogue(par ^ 1u, prev_e0);
-  }
+  } while (!last);
 
   // ---- flush: warp registers -> CTA shared memory -> one global atomic per counter per CTA ----
   if (lane == 0) {
     if constexpr (MODE == MODE_SIGN) {
-      if (c.signed_lanes) atomicAdd(cnt64 + C_SIGNED_LANES, static_cast<unsigned long long>(c.signed_lanes));
-      if (c.skipped) atomicAdd(cnt64 + C_SIGN_SKIPPED, static_cast<unsigned long long>(c.skipped));
+      if (c.ret_lanes) atomicAdd(cnt64 + C_SIGNED_LANES, static_cast<unsigned long long>(c.ret_lanes));
+      if (c.fwd_checks) atomicAdd(cnt64 + C_SIGN_SKIPPED, static_cast<unsigned long long>(c.fwd_checks));
     } else {
-      if (c.total) atomicAdd(cnt64 + C_EVENTS_TOTAL, static_cast<unsigned long long>(c.total));
-      if (c.empty) atomicAdd(cnt64 + C_EVENTS_EMPTY, static_cast<unsigned long long>(c.empty));
-      if (c.unknown) atomicAdd(cnt64 + C_EVENTS_UNKNOWN, static_cast<unsigned long long>(c.unknown));
-      if (c.misrouted) atomicAdd(cnt64 + C_EVENTS_MISROUTED, static_cast<unsigned long long>(c.misrouted));
       if (c.ret_checks) atomicAdd(cnt64 + C_RET_CHECKS, static_cast<unsigned long long>(c.ret_checks));
       if (c.fwd_checks) atomicAdd(cnt64 + C_FWD_CHECKS, static_cast<unsigned long long>(c.fwd_checks));
       if (c.ret_lanes) atomicAdd(cnt64 + C_RET_LANES, static_cast<unsigned long long>(c.ret_lanes));
       if (c.fwd_lanes) atomicAdd(cnt64 + C_FWD_LANES, static_cast<unsigned long long>(c.fwd_lanes));
     }
   }
+  // every event of the launch is counted once (the kernel walks all of them)
+  if (MODE != MODE_SIGN && blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(cnt64 + C_EVENTS_TOTAL, static_cast<unsigned long long>(p.n));
   __syncthreads();
   if (threadIdx.x < C_WORDS) {  // (words updated in global memory directly, and the host-side words, stay 0 here)
     unsigned long long v = cnt64[threadIdx.x];
