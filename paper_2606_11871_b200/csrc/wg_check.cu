@@ -57,11 +57,13 @@ constexpr uint32_t kMaxSmemSites = 1024;  // policies up to this size keep their
 // back), and the producer's list of the group's protected events (16 B each)
 //   record: +0  SipHash state the event's consumer passes start from (8 words); a forward event parks its set range
 //               {offset, count} at +16 instead
-//           +32 ctx lo (context_base & ~31), +36 ctx hi, +40 element base (event index * 32 - slot * 32: adding a
-//               queue item's low half gives the element index of (event, lane) in val / tag), +44 lanes whose value
-//               differs from the first active lane's (0: warp-uniform)
-//           +48 active mask, +52 queue mask (the active mask of a return check, else 0), +56 first active lane,
-//           +60 violation mask, +64 meta = cls | kind << 4, +68 site id
+//           +32 ctx lo (context_base & ~31), +36 ctx hi, +40 (8 B) pointer to the event's tag row (sign: the row to
+//               write) minus 8 * 32 * slot, so that pointer + 8 * (queue item's low half = slot * 32 + lane) is the
+//               lane's element: one IMAD.WIDE on the FMA pipe, no 64-bit add on the ALU pipe
+//           +48 active mask, +52 queue mask (the active mask of a return check, else 0), +56 violation mask,
+//           +60 lanes whose value differs from the first active lane's (0: warp-uniform)
+//           +64 meta = cls | kind << 4, +68 site id, +72 (8 B) pointer to the event's value row, biased the same way
+//   (80 bytes: every 16-byte field stays 16-byte aligned)
 constexpr uint32_t kRecBytes = 80;
 constexpr uint32_t kGroupRecs = 33;
 constexpr uint32_t kRecArea = 2 * kGroupRecs * kRecBytes;  // 5,280 B
@@ -150,6 +152,12 @@ __device__ __forceinline__ uint32_t mad32(uint32_t a, uint32_t b, uint32_t c) {
 __device__ __forceinline__ const uint64_t* elem_ptr(const uint64_t* base, uint32_t elem) {
   uint64_t r;
   asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(elem), "l"(reinterpret_cast<uint64_t>(base)));
+  return reinterpret_cast<const uint64_t*>(r);
+}
+// biased row pointer (two 32-bit halves from a record) + 8 * queue item: the address of the item's element
+__device__ __forceinline__ const uint64_t* item_ptr(uint32_t lo, uint32_t hi, uint32_t item) {
+  uint64_t r;
+  asm("{ .reg .b64 b; mov.b64 b, {%2, %3}; mad.wide.u32 %0, %1, 8, b; }" : "=l"(r) : "r"(item), "r"(lo), "r"(hi));
   return reinterpret_cast<const uint64_t*>(r);
 }
 // base + byte offset
@@ -336,19 +344,21 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t qb = div ? mad32(kb + lane, 0xfffffffcu, q_top) : mad32(kb + lane, 4u, q_s);
     const uint32_t ia = lds_u16(qa), ib = lds_u16(qb);            // slot * 32 + lane of the event
     const uint32_t ra = rec_s + lds_u16(qa + 2), rb = rec_s + lds_u16(qb + 2);  // the events' records
-    const uint4 ca = lds_v4(ra + 32), cb = lds_v4(rb + 32);        // ctx lo, ctx hi, element base, -
+    const uint4 ca = lds_v4(ra + 32), cb = lds_v4(rb + 32);        // ctx lo, ctx hi, biased tag row pointer
     Sip32 sa = lds_state(ra), sb = lds_state(rb);
-    const uint32_t ea = ca.z + ia, eb = cb.z + ib;
+    const uint64_t* pa = item_ptr(ca.z, ca.w, ia);
+    const uint64_t* pb = item_ptr(cb.z, cb.w, ib);
     const uint32_t la = ia & 31u, lb = ib & 31u;
     uint2 ta = make_uint2(0u, 0u), tb = make_uint2(0u, 0u);
     if constexpr (MODE != MODE_SIGN) {
-      ta = ldg_v2_stream(elem_ptr(p.tag, ea));
-      tb = ldg_v2_stream(elem_ptr(p.tag, eb));
+      ta = ldg_v2_stream(pa);
+      tb = ldg_v2_stream(pb);
     }
     if (div) {
       // lane-divergent continuation: the states are the sites' pre-A states; absorb each item's own value, then bring
       // the states to where a warp-uniform event's state starts (B folded into v3, quarter A of the next round done)
-      const uint2 va = ldg_v2_keep(elem_ptr(p.val, ea)), vb = ldg_v2_keep(elem_ptr(p.val, eb));
+      const uint2 wa = lds_v2(ra + 72), wb = lds_v2(rb + 72);  // biased value row pointers
+      const uint2 va = ldg_v2_keep(item_ptr(wa.x, wa.y, ia)), vb = ldg_v2_keep(item_ptr(wb.x, wb.y, ib));
       sip_absorb_preA2(sa, sb, va.x, va.y, vb.x, vb.y);
       sip_qA(sa);
       sip_qA(sb);
@@ -360,12 +370,12 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     sb.v3l ^= lb;
     sip_tail_ctxlane2(sa, sb, ca.x ^ la, ca.y, cb.x ^ lb, cb.y, ta.x, ta.y, tb.x, tb.y, al, ah, bl, bh);
     if constexpr (MODE == MODE_SIGN) {
-      st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, ea)), al, ah);
-      if (on_b) st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, eb)), bl, bh);
+      st_stream_v2(const_cast<uint64_t*>(pa), al, ah);
+      if (on_b) st_stream_v2(const_cast<uint64_t*>(pb), bl, bh);
     } else {
       if ((al | ah | bl | bh) != 0u) {  // rare: a lane's token does not match
-        if ((al | ah) != 0u) atoms_or(ra + 60, 1u << la);
-        if ((bl | bh) != 0u) atoms_or(rb + 60, 1u << lb);  // (with on_b false this repeats item a's bit: harmless)
+        if ((al | ah) != 0u) atoms_or(ra + 56, 1u << la);
+        if ((bl | bh) != 0u) atoms_or(rb + 56, 1u << lb);  // (with on_b false this repeats item a's bit: harmless)
       }
     }
   };
@@ -397,9 +407,9 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   auto epilogue = [&](uint32_t rpar, uint32_t e0) __attribute__((always_inline)) {
     if constexpr (MODE != MODE_SIGN) {
       const uint32_t ra = rec_s + (rpar * kGroupRecs + lane) * kRecBytes;
-      const uint4 m = lds_v4(ra + 48);   // active, queue mask, first, viol
+      const uint4 m = lds_v4(ra + 48);   // active, queue mask, viol, -
       const uint2 ms = lds_v2(ra + 64);  // meta, site
-      const uint32_t active = m.x, cls = ms.x & 15u, kind = (ms.x >> 4) & 15u, viol = m.w, site = ms.y;
+      const uint32_t active = m.x, cls = ms.x & 15u, kind = (ms.x >> 4) & 15u, viol = m.z, site = ms.y;
       const bool valid = cls != CLS_NONE;
       if (valid) st_stream_v2(p.out + (e0 + lane), viol, enforce ? (active & ~viol) : active);
       // violations are rare (0.05 % of events in the paper-shaped stream): one warp-uniform branch per group
@@ -529,8 +539,14 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t m_ret = __ballot_sync(kFull, cls == CLS_RET);
     const uint32_t m_fwd = (MODE == MODE_SIGN) ? 0u : __ballot_sync(kFull, cls == CLS_FWD);
     uint32_t viol = (cls == CLS_FAIL) ? active : 0u;  // fail closed (R13, R14)
-    sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, (e0 + lane) * 32u - slot_me * 32u, 0u);
-    sts_v4(ra_me + 48, active, cls == CLS_RET ? active : 0u, first, viol);
+    {
+      const uint64_t tp = reinterpret_cast<uint64_t>(MODE == MODE_SIGN ? p.tag_out : p.tag) + static_cast<uint64_t>(e0 + lane) * 256u -
+                          static_cast<uint64_t>(slot_me) * 256u;
+      const uint64_t vp = reinterpret_cast<uint64_t>(p.val) + static_cast<uint64_t>(e0 + lane) * 256u - static_cast<uint64_t>(slot_me) * 256u;
+      sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, static_cast<uint32_t>(tp), static_cast<uint32_t>(tp >> 32));
+      sts_v2(ra_me + 72, static_cast<uint32_t>(vp), static_cast<uint32_t>(vp >> 32));
+    }
+    sts_v4(ra_me + 48, active, cls == CLS_RET ? active : 0u, viol, 0u);
     sts_v2(ra_me + 64, cls | (kind << 4), site);
 
     // ---- the producer's list of the group's protected events (event-parallel), padded to a multiple of kBatch with
@@ -540,7 +556,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t n_need = __popc(need);
     if (need != 0u) {
       const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
-      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * kEntryMul, lane * 32u);
+      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * kEntryMul, first);
       if (lane < ((kBatch - n_need) & (kBatch - 1u)))
         sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * kEntryMul, 0u);
     }
@@ -622,11 +638,11 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       auto consume_batch = [&](const uint2 (&v)[kBatch], uint32_t b0) {
 #pragma unroll
         for (int j = 0; j < static_cast<int>(kBatch); ++j) {
-          const uint4 le = lds_v4(list_s + (b0 + j) * 16u);  // record, row byte offset, queue item base, row element offset
-          const uint4 am = lds_v4(le.x + 48);                // active, queue mask, first active lane, -
-          const uint32_t rx = __shfl_sync(kFull, v[j].x, am.z), ry = __shfl_sync(kFull, v[j].y, am.z);
+          const uint4 le = lds_v4(list_s + (b0 + j) * 16u);  // record, row byte offset, queue item base, first active lane
+          const uint2 am = lds_v2(le.x + 48);                // active, queue mask
+          const uint32_t rx = __shfl_sync(kFull, v[j].x, le.w), ry = __shfl_sync(kFull, v[j].y, le.w);
           const uint32_t diff = __ballot_sync(kFull, v[j].x != rx || v[j].y != ry) & am.x;
-          sts_u32(le.x + 44, diff);  // (every lane stores the same word)
+          sts_u32(le.x + 60, diff);  // (every lane stores the same word)
           const uint32_t rank = __popc(am.y & ltmask), nae = __popc(am.y);
           const bool div = diff != 0u, act = (am.y & lanebit) != 0u;
           const uint32_t addr = div ? mad32(rank, 0xfffffffcu, qd) : mad32(rank, 4u, qu);
@@ -634,7 +650,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           qd = div ? mad32(nae, 0xfffffffcu, qd) : qd;
           qu = div ? qu : mad32(nae, 4u, qu);
           if (MODE == MODE_SIGN && !act && am.x != 0u)  // inactive lanes sign nothing (R10)
-            st_stream_v2(const_cast<uint64_t*>(elem_ptr(p.tag_out, e0 * 32u + lane + le.w)), 0u, 0u);
+            st_stream_v2(const_cast<char*>(byte_ptr(reinterpret_cast<const char*>(elem_ptr(p.tag_out, e0 * 32u + lane)), le.y)), 0u, 0u);
         }
       };
 #pragma unroll 1
@@ -669,7 +685,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     // ---- event-parallel: per-event part of the MAC; search of warp-uniform forward targets ----
     {
       const bool judged = cls == CLS_RET || cls == CLS_FWD;
-      const bool is_uni = judged && lds_u32(ra_me + 44) == 0u;
+      const bool is_uni = judged && lds_u32(ra_me + 60) == 0u;
       uint32_t ul = 0, uh = 0;
       if (is_uni) {
         const uint2 r = ldg_v2_keep(elem_ptr(p.val, (e0 + lane) * 32u + first));  // the event's one value (an L1 hit)
@@ -732,7 +748,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
             fviol = active;
           else if (is_uni)
             fviol = member<STAGED>(p, tg_s, off, cnt, ul, uh) ? 0u : active;
-          sts_u32(ra_me + 60, fviol);
+          sts_u32(ra_me + 56, fviol);
         }
       }
     }
