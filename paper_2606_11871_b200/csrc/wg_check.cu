@@ -51,7 +51,7 @@ constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxCacheSlots = 2048;  // slots of the per-site counter cache in shared memory (12 bytes each)
 
 // ---- shared-memory carve-up ----------------------------------------------------------------------
-// CTA part: [tgts staged: stage_bytes][per-site counter cache: site_bytes][cnt64: 40 x u64][bykind: 8 x u32][mbar, pad]
+// CTA part: [tgts staged: stage_bytes][per-site counter cache: site_bytes][cnt64: 40 x u64][bykind: 12 x u32][mbar, pad]
 // warp part: event records [2 groups][33] x 80 B (record 32 of a group is a dummy that absorbs the padding trips of
 // the producer loop), the work queue (u32 items; warp-uniform items from the front, lane-divergent items from the
 // back), and the producer's list of the group's protected events (16 B each)
@@ -67,7 +67,10 @@ constexpr uint32_t kMaxCacheSlots = 2048;  // slots of the per-site counter cach
 constexpr uint32_t kRecBytes = 80;
 constexpr uint32_t kGroupRecs = 33;
 constexpr uint32_t kRecArea = 2 * kGroupRecs * kRecBytes;  // 5,280 B
-constexpr uint32_t kQueueItems = 1024 + 128;       // one group adds at most 1,024 items; each queue carries < 64
+#ifndef WG_QUEUE
+#define WG_QUEUE (1024 + 128)
+#endif
+constexpr uint32_t kQueueItems = WG_QUEUE;       // one group adds at most 1,024 items; each queue carries < 64
 #ifndef WG_BATCH
 #define WG_BATCH 4
 #endif
@@ -75,7 +78,7 @@ constexpr uint32_t kBatch = WG_BATCH;              // row loads in flight per la
 constexpr uint32_t kListBytes = 40 * 16;           // up to 32 protected events, padded to a multiple of kBatch
 constexpr uint32_t kEntryMul = (kRecBytes << 16) | 32u;  // queue item of (slot, lane) = slot * kEntryMul + lane
 constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 4 + kListBytes;
-constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 8 * 4 + 16 + 16;  // cnt64, bykind, mbar (+pad to 16)
+constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 12 * 4 + 16;  // cnt64, bykind + rare-event counts (u32), mbar
 constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
 constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
 static_assert(kWarps * kWarpBytes + kCtaFixedBytes + 4096 <= kSmemMax, "too many warps for the shared memory");
@@ -297,7 +300,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   const uint32_t smem0 = smem_u32(smem_raw);
   const uint32_t tg_s = smem0;
   // Per-site counter cache (site_bytes = 12 bytes x a power-of-two number of slots, or 0): a direct-mapped table in
-  // shared memory, slot = site & mask, {owner site, events, lanes checked}.  A slot is claimed by the first site that
+  // shared memory, two candidate slots per site, {owner site, events, lanes checked}.  A slot is claimed by the first site that
   // asks for it (one compare-and-swap) and keeps it for the whole launch; that site's per-event counts are shared-memory
   // atomics from then on, flushed once per CTA.  Sites that find their slot taken use one reduction per event
   // straight to L2, as every site did before.  Why: under Zipf(1.1) one site takes 17 % of the events, and 13 M
@@ -308,7 +311,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   const uint32_t cta_off = stage_bytes + site_bytes;
   unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + cta_off);
   uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8);
-  const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 32;
+  const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 48;
   const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * kWarpBytes;
   const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 4 * k
   const uint32_t q_top = q_s + (kQueueItems - 1) * 4;        // divergent items: q_top - 4 * k
@@ -321,7 +324,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   if (threadIdx.x < C_WORDS) cnt64[threadIdx.x] = 0ull;
   const uint32_t tbl_slots = site_bytes / 12u, tbl_mask = tbl_slots - 1u;  // site_s: [slots] owner, [slots][2] counts
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = i < tbl_slots ? 0xffffffffu : 0u;
-  if (threadIdx.x < 8) bykind[threadIdx.x] = 0u;
+  if (threadIdx.x < 12) bykind[threadIdx.x] = 0u;  // 7 by-kind counts, then unknown / empty / misrouted events
   if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
   __syncthreads();
   if constexpr (STAGED) {
@@ -363,7 +366,6 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     Sip32 sa = lds_state(ra), sb = lds_state(rb);
     const uint64_t* pa = item_ptr(ca.z, ca.w, ia);
     const uint64_t* pb = item_ptr(cb.z, cb.w, ib);
-    const uint32_t la = ia & 31u, lb = ib & 31u;
     uint2 ta = make_uint2(0u, 0u), tb = make_uint2(0u, 0u);
     if constexpr (MODE != MODE_SIGN) {
       ta = ldg_v2_stream(pa);
@@ -380,6 +382,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       sa.v3l ^= ca.x; sa.v3h ^= ca.y;
       sb.v3l ^= cb.x; sb.v3h ^= cb.y;
     }
+    const uint32_t la = ia & 31u, lb = ib & 31u;
     uint32_t al, ah, bl, bh;
     sa.v3l ^= la;
     sb.v3l ^= lb;
@@ -593,10 +596,10 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         const uint32_t u = __popc(__ballot_sync(kFull, valid && !known));
         const uint32_t em = __popc(__ballot_sync(kFull, known && active == 0u));
         const uint32_t mr = __popc(__ballot_sync(kFull, known && cls == CLS_FAIL));
-        if (lane == 0) {
-          if (u) atomicAdd(cnt64 + C_EVENTS_UNKNOWN, static_cast<unsigned long long>(u));
-          if (em) atomicAdd(cnt64 + C_EVENTS_EMPTY, static_cast<unsigned long long>(em));
-          if (mr) atomicAdd(cnt64 + C_EVENTS_MISROUTED, static_cast<unsigned long long>(mr));
+        if (lane == 0) {  // (32-bit shared-memory atomics: a 64-bit one is a compare-and-swap loop)
+          if (u) atomicAdd(&bykind[8 + 0], u);
+          if (em) atomicAdd(&bykind[8 + 1], em);
+          if (mr) atomicAdd(&bykind[8 + 2], mr);
         }
       }
       c.ret_checks += __popc(m_ret);
@@ -628,9 +631,16 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       } else if (known) {
         bool cached = false;
         if (site_bytes) {
-          const uint32_t slot = site & tbl_mask;
+          // two candidate slots per site: a hot site that finds its first slot taken by an earlier (cold) site still
+          // gets cached nearly always
+          uint32_t slot = site & tbl_mask;
           uint32_t owner = site_s[slot];
           if (owner == 0xffffffffu) owner = atomicCAS(&site_s[slot], 0xffffffffu, site);  // claim a free slot
+          if (owner != site && owner != 0xffffffffu) {
+            slot = ((site * 0x9e3779b1u) >> 16) & tbl_mask;
+            owner = site_s[slot];
+            if (owner == 0xffffffffu) owner = atomicCAS(&site_s[slot], 0xffffffffu, site);
+          }
           cached = owner == site || owner == 0xffffffffu;
           if (cached) {
             atomicAdd(&site_s[tbl_slots + 2u * slot], 1u);
@@ -659,6 +669,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           uint32_t diff, div_;
           and_test(__ballot_sync(kFull, v[j].x != rx || v[j].y != ry), am.x, diff, div_);
           sts_u32(le.x + 60, diff);  // (every lane stores the same word)
+          if (MODE == MODE_FORWARD || m_ret == 0u) continue;  // a group without return checks has nothing to queue
           const uint32_t rank = __popc(am.y & ltmask), nae = __popc(am.y);
           const bool div = div_ != 0u, act = (am.y & lanebit) != 0u;
           const uint32_t addr = div ? mad32(rank, 0xfffffffcu, qd) : mad32(rank, 4u, qu);
@@ -819,6 +830,9 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   if (threadIdx.x < C_WORDS) {  // (words updated in global memory directly, and the host-side words, stay 0 here)
     unsigned long long v = cnt64[threadIdx.x];
     if (threadIdx.x >= C_BY_KIND && threadIdx.x < C_BY_KIND + 7) v = bykind[threadIdx.x - C_BY_KIND];
+    if (threadIdx.x == C_EVENTS_UNKNOWN) v = bykind[8 + 0];
+    if (threadIdx.x == C_EVENTS_EMPTY) v = bykind[8 + 1];
+    if (threadIdx.x == C_EVENTS_MISROUTED) v = bykind[8 + 2];
     if (v) atomicAdd(p.glob + threadIdx.x, v);
   }
   for (uint32_t i = threadIdx.x; i < tbl_slots; i += blockDim.x) {  // the cached sites' counts, once per CTA
