@@ -86,6 +86,10 @@ def lib():
         L.wgo_read_counters.argtypes = [vp, vp, vp]
         L.wgo_set_profile.restype = None
         L.wgo_set_profile.argtypes = [vp, u32]
+        L.wgo_set_skip_sites.restype = None
+        L.wgo_set_skip_sites.argtypes = [vp, vp]
+        L.wgo_set_sequence_base.restype = None
+        L.wgo_set_sequence_base.argtypes = [vp, C.c_uint64]
         L.wgo_set_ring_capacity.restype = None
         L.wgo_set_ring_capacity.argtypes = [vp, u64]
         L.wgo_read_violations.restype = u64
@@ -225,6 +229,18 @@ class Oracle:
     def set_profile(self, flags: int):
         lib().wgo_set_profile(self._h, int(flags))
 
+    def set_skip_sites(self, skip=None):
+        """skip: [n_sites] array, non-zero = left out by the coverage-reduced profile (R40); None clears the set."""
+        if skip is None:
+            lib().wgo_set_skip_sites(self._h, None)
+        else:
+            a = np.ascontiguousarray(skip, dtype=np.uint8)
+            assert a.size == self.n_sites
+            lib().wgo_set_skip_sites(self._h, _ptr(a))
+
+    def set_sequence_base(self, base: int):
+        lib().wgo_set_sequence_base(self._h, int(base))
+
     def set_ring_capacity(self, capacity: int):
         lib().wgo_set_ring_capacity(self._h, int(capacity))
 
@@ -243,7 +259,7 @@ class Oracle:
             raise ValueError("policy_poke: out of range")
 
     def read_telemetry(self) -> dict:
-        t = np.zeros(7, dtype=np.uint64)
+        t = np.zeros(len(TELEMETRY_FIELDS), dtype=np.uint64)
         lib().wgo_read_telemetry(self._h, _ptr(t))
         return {k: int(v) for k, v in zip(TELEMETRY_FIELDS, t)}
 
@@ -281,11 +297,12 @@ class Oracle:
 
 
 PROFILE_SKIP_FORWARD, PROFILE_SKIP_BACKWARD, PROFILE_LOW_TELEMETRY, PROFILE_METADATA_INTEGRITY = 1, 2, 4, 8
+PROFILE_COVERAGE_REDUCED = 16
 VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
                             ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
                             ("stored", "<u8")])
 TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
-                    "ring_recorded", "ring_dropped", "fwd_meta_fail_events")
+                    "ring_recorded", "ring_dropped", "fwd_meta_fail_events", "skipped_site_events", "skipped_site_lanes")
 SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "empty_events", "overflow_lanes",
                  "underflow_lanes", "depth_mismatch_lanes", "token_mismatch_lanes", "target_mismatch_lanes",
                  "non_return_events", "slot_overflow_events", "slot_conflict_events", "viol_lanes", "viol_events",

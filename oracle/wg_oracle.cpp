@@ -75,7 +75,8 @@ struct wgo_engine {
   uint32_t profile = 0;
   uint64_t ring_capacity = 0;
   std::vector<wgo_violation_rec> ring;
-  wgo_telemetry_counters t = {0, 0, 0, 0, 0, 0, 0};
+  wgo_telemetry_counters t = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  std::vector<uint8_t> skip_site;  // per site: left out by the coverage-reduced profile (R40); empty = none
   std::vector<uint64_t> fwd_token;  // per site: token of the forward record at load time (R37)
   bool have_first = false;
   wgo_violation_rec first = {};
@@ -302,6 +303,12 @@ void wgo_check(wgo_engine* e, const wgo_event_hdr* hdr, const uint64_t* val, con
         // backward-only profile (R26)
         e->t.skipped_fwd_events += 1;
         e->t.skipped_fwd_lanes += popcount32(a);
+      } else if ((k == WGO_PROTECTED_RETURN || k == WGO_PROTECTED_FORWARD) &&
+                 (e->profile & WGO_PROFILE_COVERAGE_REDUCED) && !e->skip_site.empty() && e->skip_site[s]) {
+        // coverage-reduced profile: this protected site is left out of the protected set; not judged, reported
+        // under its own denominator (Table A2 586-587; R40)
+        e->t.skipped_site_events += 1;
+        e->t.skipped_site_lanes += popcount32(a);
       } else if (k == WGO_PROTECTED_RETURN && tag != nullptr) {
         judged_ret = true;
         for (uint32_t lane = 0; lane < 32; ++lane) {
@@ -420,6 +427,14 @@ wgo_engine* wgo_create_bound(uint32_t n_sites, const uint8_t* kind, const uint32
 }
 
 void wgo_set_profile(wgo_engine* e, uint32_t flags) { e->profile = flags; }
+
+void wgo_set_skip_sites(wgo_engine* e, const uint8_t* skip) {
+  e->skip_site.clear();
+  if (skip) e->skip_site.assign(skip, skip + e->n_sites);
+}
+
+// the sequence number the next checked event gets (R12; sharded streams: a rank's events keep their global numbers)
+void wgo_set_sequence_base(wgo_engine* e, uint64_t base) { e->seq = base; }
 
 int wgo_policy_poke(wgo_engine* e, int what, uint64_t index, uint64_t xor_value) {
   if (what == 0 && index < e->tgts.size()) {

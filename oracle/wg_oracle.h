@@ -149,8 +149,17 @@ void wgo_read_counters(const wgo_engine* e, wgo_counters* global,
  *                              computed when the policy was loaded; else every active lane violates (a forward
  *                              check with popc(active) violating lanes) and fwd_meta_fail_events counts it.
  *                              wgo_policy_poke is the attacker's write into that memory. */
+/*   WGO_PROFILE_COVERAGE_REDUCED  ("profiles that skip kernels, sites, counters, or a CFI direction
+ *                              change the protected set and are reported under separate denominators"; Table A2,
+ *                              PAPER.md:586-587 "coverage-reduced"; R40): protected sites flagged by
+ *                              wgo_set_skip_sites are left out of the protected set: a non-empty event there is not
+ *                              judged (viol 0, allow = active, at either entry point: never "misrouted"); it counts in
+ *                              events_total / events_by_kind / site.events and in skipped_site_events / _lanes, never
+ *                              in ret_* / fwd_*.  A direction skip (above) takes precedence; flags on sites of other
+ *                              kinds mean nothing; signing is unaffected.  Without the profile flag the skip set is
+ *                              ignored. */
 enum { WGO_PROFILE_SKIP_FORWARD = 1, WGO_PROFILE_SKIP_BACKWARD = 2, WGO_PROFILE_LOW_TELEMETRY = 4,
-       WGO_PROFILE_METADATA_INTEGRITY = 8 };
+       WGO_PROFILE_METADATA_INTEGRITY = 8, WGO_PROFILE_COVERAGE_REDUCED = 16 };
 typedef struct {
   uint64_t seq;
   uint32_t site_id, kind, viol_mask, active_mask, lane, mode;
@@ -160,6 +169,7 @@ typedef struct {
   uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
   uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 (ring enabled) */
   uint64_t fwd_meta_fail_events;        /* forward records that failed their authentication */
+  uint64_t skipped_site_events, skipped_site_lanes; /* coverage-reduced profile: events / lanes at skipped sites */
 } wgo_telemetry_counters;
 /* what = 0: allowed_targets[index] ^= x (index into the CSR array); what = 1: the stored token of site `index` ^= x.
  * Returns 0, or -1 when out of range.  The set may become unsorted: membership is the linear scan then. */
@@ -175,6 +185,12 @@ uint64_t wgo_policy_digest(uint32_t n_sites, const uint8_t* kind, const uint32_t
 wgo_engine* wgo_create_bound(uint32_t n_sites, const uint8_t* kind, const uint32_t* tgt_off, const uint64_t* tgts,
                              uint64_t k0, uint64_t k1, uint64_t expected_digest);
 void wgo_set_profile(wgo_engine* e, uint32_t flags);
+/* skip: [n_sites] bytes, non-zero = the site is in the coverage-reduced profile's skip set; NULL clears the set */
+void wgo_set_skip_sites(wgo_engine* e, const uint8_t* skip);
+/* The running event index (R12) the NEXT checked event gets.  wgo_reset_counters sets it to 0; a rank that
+ * checks the slice [lo, hi) of a sharded stream sets it to lo so that first-violation keys and records carry the
+ * stream's own sequence numbers. */
+void wgo_set_sequence_base(wgo_engine* e, uint64_t base);
 /* capacity 0 (default) disables the ring; the oracle keeps the FIRST `capacity` records in event order
  * (any subset of that size is a valid ring content once it overflows). */
 void wgo_set_ring_capacity(wgo_engine* e, uint64_t capacity);

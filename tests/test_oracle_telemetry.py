@@ -154,3 +154,95 @@ def test_telemetry_settings_never_change_a_verdict():
         o = oracle_for(st.policy)
         o.set_ring_capacity(cap)
         assert np.array_equal(o.verify(hdr, val, tag, ENF), a)
+
+
+def test_coverage_reduced_profile_leaves_skipped_sites_unjudged_under_their_own_denominator():
+    """DESIGN.md R40 ("profiles that skip kernels, sites, counters, or a CFI direction change the protected
+    set and are reported under separate denominators"; Table A2).  Expectations are rebuilt from the
+    headers, the policy kinds, the skip set and a FULL-profile run's verdict masks (themselves pinned by the witness):
+    events at skipped protected sites lose their verdict and move from ret_* / fwd_* to skipped_site_*; nothing else
+    changes; without the profile flag the skip set means nothing."""
+    st, orc, hdr, val, tag = signed_stream(4, 40_009, mode=ENF)
+    site, active = fields(hdr)
+    kind = st.policy.kind
+    full = orc.verify(hdr, val, tag, ENF)
+    assert np.array_equal(full[:, 0], witness.expected_viol(st))
+    g_full, s_full = orc.read_counters()
+    rng = np.random.default_rng(7)
+    skip = (rng.random(kind.size) < 0.3).astype(np.uint8)
+    hot = np.bincount(site[site < kind.size], minlength=kind.size)
+    skip[np.argsort(-hot)[:3]] = 1  # the three busiest sites too, so that violations fall into the skip set
+    in_range = site < kind.size
+    k_ev = np.where(in_range, kind[np.minimum(site, kind.size - 1)], 7)
+    skipped = in_range & (active != 0) & ((k_ev == RET) | (k_ev == FWD)) & (skip[np.minimum(site, kind.size - 1)] != 0)
+    assert skipped.sum() > 1000 and (full[skipped, 0] != 0).any()
+
+    # the flag off: the skip set is ignored
+    o1 = oracle_for(st.policy)
+    o1.set_skip_sites(skip)
+    assert np.array_equal(o1.verify(hdr, val, tag, ENF), full)
+
+    o2 = oracle_for(st.policy)
+    o2.set_skip_sites(skip)
+    o2.set_profile(oracle.PROFILE_COVERAGE_REDUCED)
+    out = o2.verify(hdr, val, tag, ENF)
+    exp_viol = np.where(skipped, 0, full[:, 0]).astype(np.uint32)
+    assert np.array_equal(out[:, 0], exp_viol) and np.array_equal(out[:, 1], active & ~exp_viol)
+    g, s = o2.read_counters()
+    t = o2.read_telemetry()
+    pc = popc(active)
+    assert t["skipped_site_events"] == int(skipped.sum()) and t["skipped_site_lanes"] == int(pc[skipped].sum())
+    sk_ret, sk_fwd = skipped & (k_ev == RET), skipped & (k_ev == FWD)
+    assert g["ret_checks"] == g_full["ret_checks"] - int(sk_ret.sum())
+    assert g["fwd_checks"] == g_full["fwd_checks"] - int(sk_fwd.sum())
+    assert g["ret_lanes"] == g_full["ret_lanes"] - int(pc[sk_ret].sum())
+    assert g["fwd_lanes"] == g_full["fwd_lanes"] - int(pc[sk_fwd].sum())
+    assert g["ret_viol"] == int(popc(exp_viol[k_ev == RET]).sum()) and g["fwd_viol"] == int(popc(exp_viol[k_ev == FWD]).sum())
+    assert g["blocked_lanes"] == int(popc(exp_viol).sum())
+    for k in ("events_total", "events_empty", "events_unknown_site", "events_misrouted") + tuple(f"events_by_kind_{i}" for i in range(7)):
+        assert g[k] == g_full[k], k
+    # per site: events unchanged; a skipped site checks no lane and has no violation
+    assert np.array_equal(s[:, 0], s_full[:, 0])
+    prot_skip = (skip != 0) & ((kind == RET) | (kind == FWD))
+    assert (s[prot_skip, 1:] == 0).all() and np.array_equal(s[~prot_skip], s_full[~prot_skip])
+    viols = np.nonzero(exp_viol)[0]
+    assert g["first_violation_key"] == ((int(viols[0]) << 5) | ctz(int(exp_viol[viols[0]])))
+
+    # a skipped return site at the FORWARD entry point is skipped, not misrouted; an unskipped one still fails closed
+    o3 = oracle_for(st.policy)
+    o3.set_skip_sites(skip)
+    o3.set_profile(oracle.PROFILE_COVERAGE_REDUCED)
+    f = o3.check_forward(hdr, val, DET)
+    ret_ev = in_range & (k_ev == RET) & (active != 0)
+    assert (f[sk_ret, 0] == 0).all() and np.array_equal(f[ret_ev & ~skipped, 0], active[ret_ev & ~skipped])
+    assert o3.read_counters()[0]["events_misrouted"] == int((ret_ev & ~skipped).sum())
+
+    # a direction skip takes precedence over the site skip
+    o4 = oracle_for(st.policy)
+    o4.set_skip_sites(skip)
+    o4.set_profile(oracle.PROFILE_COVERAGE_REDUCED | oracle.PROFILE_SKIP_BACKWARD)
+    o4.verify(hdr, val, tag, ENF)
+    t4 = o4.read_telemetry()
+    all_ret = in_range & (k_ev == RET) & (active != 0)
+    assert t4["skipped_ret_events"] == int(all_ret.sum()) and t4["skipped_site_events"] == int(sk_fwd.sum())
+
+
+def test_sequence_base_shifts_keys_and_records_and_nothing_else():
+    """DESIGN.md R12 / SURVEY.md §8(e): a rank that checks the slice [lo, hi) of a sharded stream sets its sequence base
+    to lo; first-violation key and ring records then carry the stream's own sequence numbers."""
+    st, orc, hdr, val, tag = signed_stream(4, 20_011)
+    whole = orc.verify(hdr, val, tag, ENF)
+    g_whole, _ = orc.read_counters()
+    lo = 7_003
+    o2 = oracle_for(st.policy)
+    o2.set_ring_capacity(1 << 12)
+    o2.set_sequence_base(lo)
+    part = o2.verify(hdr[lo:], val[lo:], tag[lo:], ENF)
+    assert np.array_equal(part, whole[lo:])
+    bad = np.nonzero(whole[lo:, 0])[0] + lo
+    assert bad.size > 2
+    g2, _ = o2.read_counters()
+    assert g2["first_violation_key"] == ((int(bad[0]) << 5) | ctz(int(whole[bad[0], 0])))
+    assert np.array_equal(o2.read_violations()["seq"], bad.astype(np.uint64))
+    assert int(o2.read_first_violation()["seq"]) == int(bad[0])
+    assert g2["events_total"] == hdr.shape[0] - lo
