@@ -163,6 +163,11 @@ wg_status wg_read_counters(wg_engine* eng, wg_counters* h_global, wg_site_counte
 
 /* ---- lifecycle helpers beside the five ---- */
 wg_status wg_reset_counters(wg_engine* eng, void* cuda_stream); /* also restarts the event sequence (R12) */
+/* The running event index (R12) the next checked event gets; wg_reset_counters and wg_load_policy set it to 0.  A rank
+ * that checks the slice [lo, hi) of a sharded stream ("This property is site-local")
+ * sets it to lo, so that first_violation_key, the first-violation record and the ring records carry the stream's own
+ * sequence numbers.  Takes effect with the next check call; base <= 2^58. */
+wg_status wg_set_sequence_base(wg_engine* eng, uint64_t base);
 void wg_destroy(wg_engine* eng);                                /* NULL is allowed */
 const char* wg_strerror(wg_status s);
 int wg_last_cuda_error(const wg_engine* eng); /* cudaError_t of the last WG_ERR_CUDA, 0 if none */
@@ -191,7 +196,15 @@ typedef enum {
    * SipHash-2-4_key(LE64(site_id) || LE64(target_count) || LE64(t_0) || ...) over the record as it is NOW in the
    * engine's metadata memory must equal the token computed at wg_load_policy; else every active lane violates (a
    * forward check whose lanes all violate) and fwd_meta_fail_events counts the event. */
-  WG_PROFILE_METADATA_INTEGRITY = 8
+  WG_PROFILE_METADATA_INTEGRITY = 8,
+  /* Coverage-reduced ("profiles that skip kernels, sites, counters, or a CFI direction change the protected
+   * set and are reported under separate denominators"; Table A2; R40): the protected sites
+   * flagged with wg_set_skip_sites are left out of the protected set.  A non-empty event at such a site is not judged
+   * (viol 0, allow = active) at either check entry point (it is never "misrouted"); it counts in events_total /
+   * events_by_kind / site.events and in skipped_site_events / skipped_site_lanes, never in ret_* / fwd_*.  A direction
+   * skip takes precedence; flags on sites of other kinds mean nothing; signing is unaffected; without this profile
+   * flag the skip set is ignored. */
+  WG_PROFILE_COVERAGE_REDUCED = 16
 } wg_profile_flags;
 
 /* One record per event with viol_mask != 0: lane = lowest violating lane, observed = d_val[event][lane],
@@ -207,6 +220,8 @@ typedef struct {
   uint64_t skipped_ret_events, skipped_ret_lanes, skipped_fwd_events, skipped_fwd_lanes;
   uint64_t ring_recorded, ring_dropped; /* recorded + dropped == events with viol != 0 since the ring was enabled */
   uint64_t fwd_meta_fail_events;        /* forward records that failed their authentication (metadata integrity) */
+  uint64_t skipped_site_events, skipped_site_lanes; /* coverage-reduced profile: non-empty events / their active lanes
+                                                       at protected sites of the skip set                         */
   uint64_t kernel_launches;             /* CUDA kernels this engine has enqueued since it was created (diagnostic)  */
 } wg_telemetry_counters;
 /* The attacker's write into the policy metadata, for tests (the paper treats forward records as ordinary writable
@@ -214,9 +229,11 @@ typedef struct {
  * stored token of site `index` ^= x.  Synchronises cuda_stream. */
 wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_value, void* cuda_stream);
 
-/* WG_ERR_INVALID_ARG for unknown flag bits (and for any flag / ring when the measurement baseline kernels were
- * selected with WG_IMPL=v1: they implement the five calls only).  Applies to the calls made after it returns. */
+/* WG_ERR_INVALID_ARG for unknown flag bits.  Applies to the calls made after it returns. */
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags);
+/* The coverage-reduced profile's skip set: h_skip = [n_sites] bytes in HOST memory, non-zero = skipped; NULL clears
+ * the set.  Synchronises cuda_stream; belongs to the loaded policy (the next wg_load_policy clears it). */
+wg_status wg_set_skip_sites(wg_engine* eng, const uint8_t* h_skip, void* cuda_stream);
 /* Bounded violation ring in engine-owned device memory: `capacity` records (0 = off, the default).  Synchronises
  * `cuda_stream`, reallocates, and restarts the ring empty.  When the ring is full further records are dropped and
  * counted; which records a full ring holds is unspecified (any `capacity` of the violating events), their order

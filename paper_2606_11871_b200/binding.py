@@ -23,7 +23,7 @@ WG_MODE_DETECT, WG_MODE_ENFORCE = 0, 1
 
 EXPORTS = [
     "wg_load_policy", "wg_sign_continuations", "wg_verify_continuations", "wg_check_forward", "wg_read_counters",
-    "wg_reset_counters", "wg_destroy", "wg_strerror", "wg_last_cuda_error",
+    "wg_reset_counters", "wg_set_sequence_base", "wg_set_skip_sites", "wg_destroy", "wg_strerror", "wg_last_cuda_error",
     "wg_sign_continuations_host", "wg_verify_continuations_host", "wg_check_forward_host",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
@@ -44,11 +44,12 @@ SHADOW_FIELDS = ("push_events", "push_lanes", "check_events", "check_lanes", "em
 
 WG_PROFILE_FULL, WG_PROFILE_SKIP_FORWARD, WG_PROFILE_SKIP_BACKWARD, WG_PROFILE_LOW_TELEMETRY = 0, 1, 2, 4
 WG_PROFILE_METADATA_INTEGRITY = 8
+WG_PROFILE_COVERAGE_REDUCED = 16
 VIOLATION_DTYPE = np.dtype([("seq", "<u8"), ("site_id", "<u4"), ("kind", "<u4"), ("viol_mask", "<u4"),
                             ("active_mask", "<u4"), ("lane", "<u4"), ("mode", "<u4"), ("observed", "<u8"),
                             ("stored", "<u8")])  # wg_violation_rec, 48 bytes
 TELEMETRY_FIELDS = ("skipped_ret_events", "skipped_ret_lanes", "skipped_fwd_events", "skipped_fwd_lanes",
-                    "ring_recorded", "ring_dropped", "fwd_meta_fail_events")
+                    "ring_recorded", "ring_dropped", "fwd_meta_fail_events", "skipped_site_events", "skipped_site_lanes")
 # words of wg_telemetry_counters behind TELEMETRY_FIELDS that have no counterpart in the method (engine diagnostics)
 TELEMETRY_ENGINE_FIELDS = ("kernel_launches",)
 
@@ -92,6 +93,8 @@ def lib() -> C.CDLL:
         L.wg_check_forward.argtypes = [vp, vp, vp, vp, u64, i, vp]
         L.wg_read_counters.argtypes = [vp, vp, vp, vp]
         L.wg_reset_counters.argtypes = [vp, vp]
+        L.wg_set_sequence_base.argtypes = [vp, u64]
+        L.wg_set_skip_sites.argtypes = [vp, vp, vp]
         L.wg_destroy.argtypes = [vp]
         L.wg_destroy.restype = None
         L.wg_strerror.argtypes = [i]
@@ -282,6 +285,19 @@ class Engine:
     # -- profiles and telemetry (warpguard.h; R26-R29) ----------------------------------
     def wg_set_profile(self, flags: int) -> None:
         _chk(lib().wg_set_profile(self._h, int(flags)), "wg_set_profile")
+
+    def wg_set_skip_sites(self, skip=None, stream=None) -> None:
+        """skip: [n_sites] array, non-zero = left out by the coverage-reduced profile; None clears the set."""
+        if skip is None:
+            _chk(lib().wg_set_skip_sites(self._h, None, _stream_ptr(stream)), "wg_set_skip_sites")
+            return
+        a = np.ascontiguousarray(skip, dtype=np.uint8)
+        if a.size != self.n_sites:
+            raise ValueError("skip must have n_sites entries")
+        _chk(lib().wg_set_skip_sites(self._h, a.ctypes.data, _stream_ptr(stream)), "wg_set_skip_sites")
+
+    def wg_set_sequence_base(self, base: int) -> None:
+        _chk(lib().wg_set_sequence_base(self._h, int(base)), "wg_set_sequence_base")
 
     def wg_set_tuning(self, flags: int) -> None:
         _chk(lib().wg_set_tuning(self._h, int(flags)), "wg_set_tuning")

@@ -680,8 +680,38 @@ wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uin
 
 wg_status wg_set_profile(wg_engine* eng, uint32_t flags) {
   if (!eng) return WG_ERR_NO_POLICY;
-  if (flags & ~15u) return WG_ERR_INVALID_ARG;
+  if (flags & ~31u) return WG_ERR_INVALID_ARG;
   eng->profile = flags;  // takes effect with the next check call (kernel parameter)
+  return WG_OK;
+}
+
+wg_status wg_set_skip_sites(wg_engine* eng, const uint8_t* h_skip, void* cuda_stream) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  DeviceGuard g(eng->device);
+  if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  WG_CUDA(eng, cudaStreamSynchronize(st));  // no launch may still be reading the flags
+  if (eng->n_sites == 0) return WG_OK;
+  uint8_t* d_skip = nullptr;
+  if (h_skip) {
+    WG_CUDA(eng, cudaMalloc(&d_skip, eng->n_sites));
+    cudaError_t err = cudaMemcpyAsync(d_skip, h_skip, eng->n_sites, cudaMemcpyHostToDevice, st);
+    if (err != cudaSuccess) {
+      cudaFree(d_skip);
+      return cuda_fail(eng, err);
+    }
+  }
+  cudaError_t err = wg::launch_set_site_flags(eng->d_recs, d_skip, eng->n_sites, st, &eng->launches);
+  if (err == cudaSuccess) err = cudaStreamSynchronize(st);
+  cudaFree(d_skip);
+  if (err != cudaSuccess) return cuda_fail(eng, err);
+  return WG_OK;
+}
+
+wg_status wg_set_sequence_base(wg_engine* eng, uint64_t base) {
+  if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
+  if (base > (1ull << 58)) return WG_ERR_INVALID_ARG;  // (seq << 5) must not wrap
+  eng->seq = base;
   return WG_OK;
 }
 
@@ -744,7 +774,7 @@ wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, w
   DeviceGuard g(eng->device);
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
-  unsigned long long w[7];  // words 26 .. 32
+  unsigned long long w[9];  // words 26 .. 34
   WG_CUDA(eng, cudaMemcpy(w, eng->d_glob + wg::C_SKIP_RET_EVENTS, sizeof w, cudaMemcpyDeviceToHost));
   h_counters->fwd_meta_fail_events = w[wg::C_META_FAIL - wg::C_SKIP_RET_EVENTS];
   const uint64_t total = w[4];
@@ -755,6 +785,8 @@ wg_status wg_read_telemetry(wg_engine* eng, wg_telemetry_counters* h_counters, w
   h_counters->skipped_fwd_lanes = w[3];
   h_counters->ring_recorded = recorded;
   h_counters->ring_dropped = total - recorded;
+  h_counters->skipped_site_events = w[wg::C_SKIP_SITE_EVENTS - wg::C_SKIP_RET_EVENTS];
+  h_counters->skipped_site_lanes = w[wg::C_SKIP_SITE_LANES - wg::C_SKIP_RET_EVENTS];
   h_counters->kernel_launches = eng->launches;
   if (h_first) {
     wg::FirstRec f;

@@ -892,6 +892,11 @@ __global__ void wg_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64
   tok[s] = t;
 }
 
+__global__ void wg_set_site_flags(SiteRec* recs, const uint8_t* skip, uint32_t n_sites) {
+  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n_sites) recs[s].flags = (skip && skip[s]) ? SITE_FLAG_SKIP : 0u;
+}
+
 template <int MODE>
 cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
   const uint64_t n_groups = (p.n + 31) / 32;
@@ -958,6 +963,13 @@ cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st, uint64_
 
 cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* launches) {
   wg_first_record<<<1, 1, 0, st>>>(p, p.tag != nullptr);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_set_site_flags(SiteRec* recs, const uint8_t* d_skip, uint32_t n_sites, cudaStream_t st, uint64_t* launches) {
+  if (n_sites == 0) return cudaSuccess;
+  wg_set_site_flags<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, d_skip, n_sites);
   ++*launches;
   return cudaGetLastError();
 }

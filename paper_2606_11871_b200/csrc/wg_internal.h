@@ -130,6 +130,8 @@ cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* laun
 // tokens of the forward records as loaded (trusted load time)
 cudaError_t launch_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites,
                                 uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st, uint64_t* launches);
+// SiteRec.flags bit 0 <- d_skip[site] != 0 (d_skip == nullptr: cleared), the coverage-reduced profile's skip set (R40)
+cudaError_t launch_set_site_flags(SiteRec* recs, const uint8_t* d_skip, uint32_t n_sites, cudaStream_t st, uint64_t* launches);
 cudaError_t init_kernels();  // one-time function attributes (dynamic shared memory opt-in) on the current device
 
 }  // namespace wg

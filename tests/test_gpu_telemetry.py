@@ -129,7 +129,7 @@ def test_profiles_match_the_oracle(flags, config):
 def test_bad_profile_flags_are_rejected():
     st, orc, eng, hdr, val, tag, d = prepared(1, 1000)
     with pytest.raises(B.WgError) as e:
-        eng.wg_set_profile(16)
+        eng.wg_set_profile(32)
     assert e.value.status == B.WG_ERR_INVALID_ARG
     eng.close()
 
@@ -262,4 +262,74 @@ def test_host_path_first_record_and_ring_over_many_chunks():
     assert t == orc.read_telemetry() and t["ring_dropped"] == 0
     assert as_tuple(first) == as_tuple(orc.read_first_violation())
     assert sorted(as_tuple(r) for r in ring) == sorted(as_tuple(r) for r in orc.read_violations())
+    eng.close()
+
+
+@pytest.mark.parametrize("config,n,extra", [(4, 200_003, 0), (4, 120_011, B.WG_PROFILE_SKIP_BACKWARD), (5, 60_007, 0),
+                                            (1, 65_536, B.WG_PROFILE_LOW_TELEMETRY)])
+def test_coverage_reduced_profile_matches_the_oracle(config, n, extra):
+    """DESIGN.md R40 (Table A2): a per-site skip set under its own denominator; the
+    oracle side is pinned by reconstruction in tests/test_oracle_telemetry.py."""
+    if config == 5:
+        pol = S.make_policy(5, "cpu", n_sites=5_000, max_set=512)
+        st = S.make_stream(5, "cpu", n_events=n, policy=pol, batch_index=2)
+        orc = oracle_for(pol)
+        hdr = st.hdr.numpy().view(np.uint64)
+        tag_t = torch.from_numpy(orc.sign(hdr, st.val.numpy().view(np.uint64)).view(np.int64).copy())
+        st.apply_return_tamper(tag_t)
+        orc.reset_counters()
+        eng = B.Engine(0).load(pol)
+        val, tag = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+        d = (st.hdr.to(dev()), st.val.to(dev()), tag_t.to(dev()))
+    else:
+        st, orc, eng, hdr, val, tag, d = prepared(config, n)
+    pol = st.policy
+    rng = np.random.default_rng(11 + config)
+    skip = (rng.random(pol.n_sites) < 0.35).astype(np.uint8)
+    site = (hdr[:, 0] & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    hot = np.bincount(site[site < pol.n_sites], minlength=pol.n_sites)
+    skip[np.argsort(-hot)[:2]] = 1
+    cap = 1 << 18
+    for e_ in (orc, ):
+        e_.set_skip_sites(skip); e_.set_profile(oracle.PROFILE_COVERAGE_REDUCED | extra); e_.set_ring_capacity(cap)
+    eng.wg_set_skip_sites(skip); eng.wg_set_profile(B.WG_PROFILE_COVERAGE_REDUCED | extra); eng.wg_set_ring_capacity(cap)
+    for mode in (ENF, DET):
+        o = orc.verify(hdr, val, tag, mode)
+        g = eng.wg_verify_continuations(*d, mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+    o = orc.check_forward(hdr, val, ENF)
+    g = eng.wg_check_forward(d[0], d[1], ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o)
+    same_counters(eng, orc)
+    t, first, ring = eng.wg_read_telemetry(cap)
+    ot = orc.read_telemetry()
+    assert t == ot and t["skipped_site_events"] > 0 and t["ring_dropped"] == 0
+    assert sorted(map(as_tuple, ring)) == sorted(map(as_tuple, orc.read_violations(cap)))
+    of = orc.read_first_violation()
+    assert (first is None) == (of is None) and (first is None or as_tuple(first) == as_tuple(of))
+    # sign is unaffected; clearing the set or dropping the flag restores the full profile
+    assert np.array_equal(eng.wg_sign_continuations(d[0], d[1]).cpu().numpy().view(np.uint64), orc.sign(hdr, val))
+    eng.wg_reset_counters(); orc.reset_counters()
+    eng.wg_set_skip_sites(None); orc.set_skip_sites(None)
+    assert np.array_equal(eng.wg_verify_continuations(*d, ENF).cpu().numpy().view(np.uint32), orc.verify(hdr, val, tag, ENF))
+    same_counters(eng, orc)
+    assert eng.wg_read_telemetry()[0]["skipped_site_events"] == 0
+    eng.close()
+
+
+def test_sequence_base_gives_a_slice_the_streams_own_sequence_numbers():
+    """wg_set_sequence_base (R12): verdicts of a slice equal the whole stream's; key, first record and
+    ring records carry global sequence numbers."""
+    st, orc, eng, hdr, val, tag, d = prepared(4, 150_001)
+    lo = 61_234
+    cap = 1 << 12
+    orc.set_ring_capacity(cap); eng.wg_set_ring_capacity(cap)
+    orc.set_sequence_base(lo); eng.wg_set_sequence_base(lo)
+    o = orc.verify(hdr[lo:], val[lo:], tag[lo:], ENF)
+    g = eng.wg_verify_continuations(d[0][lo:], d[1][lo:], d[2][lo:], ENF).cpu().numpy().view(np.uint32)
+    assert np.array_equal(g, o) and o[:, 0].any()
+    same_counters(eng, orc)
+    t, first, ring = eng.wg_read_telemetry(cap)
+    assert as_tuple(first) == as_tuple(orc.read_first_violation()) and int(first["seq"]) >= lo
+    assert sorted(map(as_tuple, ring)) == sorted(map(as_tuple, orc.read_violations(cap)))
     eng.close()
