@@ -14,8 +14,10 @@ A STEP is one pass of the whole hot path over that
 region, on a bounded prefix of the same stream.  `cpu_baseline` = the oracle, as it stands, single-threaded, on a
 bounded prefix of the same stream (and its verdicts are compared with the GPU's while we are at it).
 
-Under torchrun (N > 1) every rank runs its own config-4 stream (weak scaling; no data-path collective — the only
-exchange is the counter all-reduce at read-out, outside the hot loop); timing is max over ranks.
+Under torchrun (N > 1) ONE config-4 stream is sharded: rank r checks the contiguous slice shard_range(n, r, N) with
+its own engine (policy and key replicated, sequence base = slice start); no data-path collective — the only exchange is
+the counter all-reduce at read-out, outside the hot loop; timing is max over ranks; "scaling": "strong".  `--weak` gives
+every rank its own full stream instead ("scaling": "weak").
 """
 from __future__ import annotations
 
@@ -40,8 +42,34 @@ OPS_PER_MAC_VERIFY = 310   # 12 SipRounds x 24 + 13 injection + 7 finalisation +
 OPS_PER_MAC_SIGN = 308
 # bytes per event
 B_RET_VERIFY, B_RET_SIGN, B_FWD, B_NON = 536, 528, 280, 24
-# traffic of the dominant kernel from the committed ncu --set full capture (profiles/); None until captured
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 24_772_875_000  # profiles/r01_v2_tile_ncu.md: 24.2775 GB read + 0.4954 GB written, 58 M-event launch
+# DRAM traffic of the dominant kernel: read from the committed ncu --set full capture under profiles/ — never typed in
+TRAFFIC_FILE = ROOT / "profiles" / "r02_traffic.json"
+KERNEL_SOURCES = ["paper_2606_11871_b200/csrc/wg_check.cu", "paper_2606_11871_b200/csrc/wg_internal.h",
+                  "include/warpguard_sip32.cuh"]
+
+
+def kernel_source_hash() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        h.update((ROOT / f).read_bytes())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic(config: int, n_events: int):
+    """(bytes per launch, source note) of the verify kernel from profiles/r02_traffic.json, or (None, why): the capture
+    must be of THIS kernel source (hash) on this workload."""
+    if not TRAFFIC_FILE.exists():
+        return None, "no capture committed"
+    try:
+        t = json.loads(TRAFFIC_FILE.read_text())
+    except Exception:
+        return None, "profiles/r02_traffic.json unreadable"
+    if t.get("source_hash") != kernel_source_hash():
+        return None, "stale: kernel sources changed since the capture (%s, commit %s)" % (TRAFFIC_FILE.name, t.get("commit"))
+    if t.get("config") != config or t.get("events") != n_events:
+        return None, "capture is of config %s / %s events" % (t.get("config"), t.get("events"))
+    return int(t["dram_bytes_read"]) + int(t["dram_bytes_write"]), "%s: ncu --set full at commit %s" % (TRAFFIC_FILE.name, t.get("commit"))
 
 
 def parse_args():
@@ -63,8 +91,11 @@ def parse_args():
     ap.add_argument("--batches", type=int, default=0,
                     help="config 5 only: stream that many 8 M-event batches (BASELINE.json: 64 = 512 M events), "
                          "alternating detect / enforce, and report the summed kernel time")
-    ap.add_argument("--dense", action="store_true", help="wg_set_tuning(WG_TUNE_DENSE_LANES) for the timed calls")
-    ap.add_argument("--sparse", action="store_true", help="accepted for compatibility: per-tile lane compaction is the default")
+    ap.add_argument("--weak", action="store_true", help="N > 1: every rank checks its own full stream (weak scaling) "
+                    "instead of a slice of one stream")
+    ap.add_argument("--host-batches", type=int, default=4,
+                    help="config 5 stream: batches also pushed through the *_host calls (wall time including H2D / D2H)")
+    ap.add_argument("--source-hash", action="store_true", help="print the kernel source hash profiles/r02_traffic.json must carry")
     ap.add_argument("--shadow", action="store_true",
                     help="also time the stateful shadow stack (SURVEY 8(f-1)): one lock-step push + check_ret over 1 Mi warps")
     return ap.parse_args()
@@ -156,7 +187,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def forward_search_ops(st, torch) -> int:
+def forward_search_ops(st, torch, lo=0, hi=None) -> int:
     """(7 ceil(log2(n+1)) + 3) int32 ops per unique active target of every non-empty forward event
     (SURVEY.md §8(d)); unique targets = 1 for a warp-uniform event, min(popc(active), n) otherwise."""
     import numpy as np
@@ -164,14 +195,14 @@ def forward_search_ops(st, torch) -> int:
     dev = st.hdr.device
     kind = torch.from_numpy(st.policy.kind.astype(np.int64)).to(dev)
     cnt = torch.from_numpy(np.diff(st.policy.tgt_off.astype(np.int64))).to(dev)
-    site = st.site_id()
+    site = st.site_id()[lo:hi]
     sel = kind[site] == S.PROTECTED_FORWARD
     n = cnt[site[sel]].double()
-    mask = st.active_mask()[sel]
+    mask = st.active_mask()[lo:hi][sel]
     pc = torch.zeros_like(mask)
     for b in range(32):
         pc += (mask >> b) & 1
-    uniq = torch.where(st.uniform[sel], torch.ones_like(pc), torch.minimum(pc, n.long()))
+    uniq = torch.where(st.uniform[lo:hi][sel], torch.ones_like(pc), torch.minimum(pc, n.long()))
     uniq = torch.where(pc > 0, uniq, torch.zeros_like(uniq))
     per = 7 * torch.ceil(torch.log2(n + 1)) + 3
     return int((per * uniq.double()).sum().item())
@@ -254,25 +285,35 @@ def run_ours(a) -> None:
         torch.cuda.synchronize()
 
     # ---- inputs, resident in HBM before anything is timed ----
-    n_events = S.FULL_EVENTS[a.config] if a.events is None else a.events
+    n_stream = S.FULL_EVENTS[a.config] if a.events is None else a.events
     if a.config == 5 and a.events is None:
-        n_events = S.CONFIG5_BATCH
-    st = S.make_stream(a.config, dev, n_events=n_events, batch_index=rank)
+        n_stream = S.CONFIG5_BATCH
+    sharded = world > 1 and not a.weak
+    # sharded (default for N > 1): every rank builds the SAME seeded stream and keeps its contiguous slice; weak: a
+    # stream of its own per rank
+    st = S.make_stream(a.config, dev, n_events=n_stream, batch_index=0 if sharded else rank)
+    lo, hi = sharding.shard_range(n_stream, rank, world) if sharded else (0, n_stream)
+    n_events = hi - lo
     eng = B.Engine(local).load(st.policy)
-    tag = eng.wg_sign_continuations(st.hdr, st.val)          # tokens at push time (engine's own signer)
-    st.apply_return_tamper(tag)                               # then the recorded corruption
+    tag_full = eng.wg_sign_continuations(st.hdr, st.val)     # tokens at push time (engine's own signer)
+    st.apply_return_tamper(tag_full)                          # then the recorded corruption
+    hdr, val, tag = st.hdr[lo:hi], st.val[lo:hi], tag_full[lo:hi]
+    in_slice = lambda plan: int(((plan.ev >= lo) & (plan.ev < hi)).sum().item()) if len(plan) else 0  # noqa: E731
+    planned_ret, planned_fwd = in_slice(st.ret_tamper), in_slice(st.fwd_tamper)
     if a.profile:
         eng.wg_set_profile(a.profile)
-    if a.dense:
-        eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
     tag_scratch = torch.empty_like(tag)
     out = torch.empty((n_events, 2), dtype=torch.int32, device=dev)
-    fwd_ops = forward_search_ops(st, torch)
+    fwd_ops = forward_search_ops(st, torch, lo, hi)
+    # inputs smaller than the 126 MB L2 (config 1) would be re-read from L2 by every step: a 256 MB buffer is written
+    # between the timed steps then; every other config streams far more than the L2 holds per step
+    step_bytes = n_events * (B_RET_VERIFY + B_RET_SIGN)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if step_bytes < (512 << 20) else None
     torch.cuda.synchronize()
 
     def step():
-        eng.wg_sign_continuations(st.hdr, st.val, tag_scratch)
-        eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode, out)
+        eng.wg_sign_continuations(hdr, val, tag_scratch)
+        eng.wg_verify_continuations(hdr, val, tag, st.mode, out)
 
     # integer-pipe ceilings of this GPU, measured now (register-only probe)
     probes = {}
@@ -287,24 +328,32 @@ def run_ours(a) -> None:
     for _ in range(max(a.warmup, 0)):
         step()
     eng.wg_reset_counters()
+    if sharded:
+        eng.wg_set_sequence_base(lo)  # (a reset restarts the sequence; the slice keeps the stream's numbering)
     barrier()
     import datetime as _dt
     t_region0 = _dt.datetime.now()
     launches0 = eng.wg_kernel_launches()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(a.steps)]
     for k in range(a.steps):
+        if flush is not None:
+            flush.zero_()  # L2 flush, outside the event brackets
         ev[k][0].record()
-        eng.wg_sign_continuations(st.hdr, st.val, tag_scratch)
+        eng.wg_sign_continuations(hdr, val, tag_scratch)
         ev[k][1].record()
-        eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode, out)
+        eng.wg_verify_continuations(hdr, val, tag, st.mode, out)
         ev[k][2].record()
     barrier()
     sampler.window(t_region0, _dt.datetime.now())
     clocks = sampler.stop()
     launches = eng.wg_kernel_launches() - launches0
-    total_ms = ev[0][0].elapsed_time(ev[-1][2])
-    sign_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / a.steps
-    verify_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / a.steps
+    step_list = [e[0].elapsed_time(e[2]) for e in ev]       # device time of each step (CUDA events on the launch stream)
+    sign_list = [e[0].elapsed_time(e[1]) for e in ev]
+    verify_list = [e[1].elapsed_time(e[2]) for e in ev]
+    total_ms = sum(step_list)
+    sign_ms = sum(sign_list) / a.steps
+    verify_ms = sum(verify_list) / a.steps
+    med = lambda x: sorted(x)[len(x) // 2]  # noqa: E731
     g, _ = eng.wg_read_counters(per_site=False)
 
     # ---- what one step judged (counters accumulated over K identical steps) ----
@@ -315,19 +364,20 @@ def run_ours(a) -> None:
     lanes = (g["ret_lanes"] + g["fwd_lanes"]) // K
     # properties that hold at any size: every planned corruption is found, nothing else is
     if not (a.profile & 2):
-        assert g["ret_viol_events"] // K == len(st.ret_tamper), (g["ret_viol_events"], len(st.ret_tamper))
+        assert g["ret_viol_events"] // K == planned_ret, (g["ret_viol_events"], planned_ret)
     if not (a.profile & 1):
-        assert g["fwd_viol_events"] // K == len(st.fwd_tamper), (g["fwd_viol_events"], len(st.fwd_tamper))
+        assert g["fwd_viol_events"] // K == planned_fwd, (g["fwd_viol_events"], planned_fwd)
     assert g["events_total"] // K == n_events
     ret_ev, fwd_ev = g["ret_checks"] // K, g["fwd_checks"] // K
     non_ev = n_events - ret_ev - fwd_ev
 
-    t = torch.tensor([total_ms, sign_ms, verify_ms], dtype=torch.float64, device=dev)
+    t = torch.tensor([total_ms, sign_ms, verify_ms, med(step_list), min(step_list), med(verify_list), min(verify_list)],
+                     dtype=torch.float64, device=dev)
     tot = torch.tensor([checks, lanes], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    total_ms, sign_ms, verify_ms = t.tolist()
+    total_ms, sign_ms, verify_ms, step_med, step_best, verify_med, verify_best = t.tolist()
     all_checks, all_lanes = tot.tolist()
     ms_per_step = total_ms / K
     value = all_checks / (ms_per_step * 1e-3)
@@ -351,15 +401,17 @@ def run_ours(a) -> None:
     t_alu = verify_ops / alu_peak
     t_hbm = verify_bytes / (hbm_peak * 1e9)
     achieved = verify_ops / (verify_ms * 1e-3)
+    traffic, traffic_src = measured_traffic(a.config, n_events) if world == 1 else (None, "one GPU only")
     roofline = {
-        "kernel": "wg_check (wg_verify_continuations)",
+        "kernel": "wg_check_kernel<verify> (wg_verify_continuations)",
         "bound": "alu" if t_alu >= t_hbm else "hbm",
         **({"achieved": achieved / 1e12, "peak": alu_peak / 1e12, "unit": "Tint32op/s", "frac": achieved / alu_peak}
            if t_alu >= t_hbm else
            {"achieved": verify_bytes / (verify_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
             "frac": verify_bytes / (verify_ms * 1e-3) / 1e9 / hbm_peak}),
         "alu_achieved_Tops": achieved / 1e12, "alu_frac": achieved / alu_peak,
-        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH if (a.config == 4 and a.events is None) else None,
+        "traffic": traffic, "traffic_source": traffic_src,
+        "ms_per_launch_median": verify_med, "ms_per_launch_best": verify_best,
         "peak_source": ("derived: 128 lanes/SM/clk x %d SMs x %.0f MHz (DESIGN.md §6); max with the measured probes"
                         % (n_sm, sm_max_mhz)),
         "ms_per_launch": verify_ms, "algorithmic_ops_per_launch": verify_ops,
@@ -375,8 +427,8 @@ def run_ours(a) -> None:
         "sipround_ceiling": sip_ceiling / 1e12,
         "frac_of_sipround_ceiling": (achieved / sip_ceiling) if sip_ceiling else None,
         "note": ("achieved counts ALGORITHMIC int32 ops (310 per verified lane: 12 SipRounds); the kernel executes "
-                 "fewer (per-site mid-state table, warp-uniform continuations absorbed once per event), so the "
-                 "fraction of the SipRound ceiling can exceed 1; ncu (profiles/) shows the ALU pipe 96 % busy"),
+                 "fewer (site word and warp-uniform continuation word absorbed once per event, no round on an inactive "
+                 "lane), so the fraction of the SipRound ceiling can exceed 1"),
         "probes_Tops": {k: v / 1e12 for k, v in probes.items()},
     }
 
@@ -385,8 +437,8 @@ def run_ours(a) -> None:
     ne = min(a.e2e_events, n_events)
     h = {}
     if not a.no_e2e or not a.no_cpu_baseline:
-        h["hdr"] = st.hdr[:ne].cpu().pin_memory()
-        h["val"] = st.val[:ne].cpu().pin_memory()
+        h["hdr"] = hdr[:ne].cpu().pin_memory()
+        h["val"] = val[:ne].cpu().pin_memory()
         h["tag"] = tag[:ne].cpu().pin_memory()
     if not a.no_e2e:
         h_scratch = torch.empty((ne, 32), dtype=torch.int64).pin_memory()
@@ -396,6 +448,7 @@ def run_ours(a) -> None:
             eng.wg_sign_continuations_host(h["hdr"], h["val"], h_scratch)
             eng.wg_verify_continuations_host(h["hdr"], h["val"], h["tag"], st.mode, h_out)
 
+        torch.cuda.synchronize()  # (the *_host calls are not ordered after work pending on this stream)
         e2e_step()
         eng.wg_reset_counters()
         barrier()
@@ -474,20 +527,26 @@ def run_ours(a) -> None:
 
     # ---- read-out exchange (outside the hot loop): counters summed over ranks ----
     gr, _ = sharding.reduce_counters(g, None, 0, device=dev)
+    small = flush is not None
     if rank == 0:
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": a.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_per_step, "ms_per_step_median": step_med, "ms_per_step_best": step_best,
+            "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
             "dtype": "u64", "data": "synthetic",
             "lane_verdicts_per_sec": all_lanes / (ms_per_step * 1e-3),
             "verify_only_checks_per_sec": all_checks / (verify_ms * 1e-3),
-            "config": {"workload": f"config{a.config}-{S.NAMES[a.config]}", "events_per_gpu": n_events,
+            "config": {"workload": f"config{a.config}-{S.NAMES[a.config]}", "events_per_gpu": n_events, "events_total": n_stream if sharded else n_events * world,
                        "checks_per_step": int(all_checks), "lane_verdicts_per_step": int(all_lanes),
                        "n_sites": st.policy.n_sites, "mode": "enforce" if st.mode else "detect", "profile_flags": a.profile,
                        "step": "wg_sign_continuations + wg_verify_continuations over the whole stream",
-                       "l2": "inputs (%.1f GB per step) are far larger than the 126 MB L2; no flush needed"
-                             % ((verify_bytes + B_RET_SIGN * ret_ev) / 1e9),
-                       "parallelism": "1 GPU" if world == 1 else f"{world} ranks x own stream, counters all-reduced at read-out"},
+                       "l2": ("a 256 MB buffer is written between the timed steps (the step's inputs, %.0f MB, would fit the "
+                              "126 MB L2)" % ((verify_bytes + B_RET_SIGN * ret_ev) / 1e6)) if small else
+                             ("inputs (%.1f GB per step per GPU) are far larger than the 126 MB L2; no flush needed"
+                              % ((verify_bytes + B_RET_SIGN * ret_ev) / 1e9)),
+                       "parallelism": "1 GPU" if world == 1 else
+                       (f"{world} ranks, one stream of {n_stream} events sharded in contiguous slices, counters all-reduced "
+                        "at read-out" if sharded else f"{world} ranks x own stream, counters all-reduced at read-out")},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
             **({"shadow": shadow} if shadow else {}),
             "counters": {k: gr[k] for k in ("events_total", "ret_checks", "fwd_checks", "ret_viol", "fwd_viol",
@@ -511,8 +570,6 @@ def run_config5_stream(a) -> None:
     dev = torch.device("cuda", 0)
     pol = S.make_policy(5, dev)
     eng = B.Engine(0).load(pol)
-    if a.dense:
-        eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
     sign_ms = verify_ms = 0.0
     planned_ret = planned_fwd = events = 0
     out = tag = None
@@ -544,6 +601,39 @@ def run_config5_stream(a) -> None:
     assert g["events_total"] == events and g["ret_viol_events"] == planned_ret
     assert planned_fwd - 20 * a.batches <= g["fwd_viol_events"] <= planned_fwd
     checks, lanes = g["ret_checks"] + g["fwd_checks"], g["ret_lanes"] + g["fwd_lanes"]
+
+    # ---- the same stream from HOST memory: wall time including transfers (SURVEY 8(d) "Config 5 ... wall time including
+    #      transfers, double-buffered on two streams"): a few batches pushed through the *_host calls, which stage 256 Ki
+    #      event chunks alternately on two streams (H2D, kernels and D2H of consecutive chunks overlap) ----
+    host = None
+    if a.host_batches > 0:
+        hb = min(a.host_batches, a.batches)
+        wall = 0.0
+        h_checks = 0
+        h2d = d2h = 0
+        for b in range(hb):
+            st = S.make_stream(5, dev, policy=pol, batch_index=b)
+            n = st.hdr.shape[0]
+            eng.wg_sign_continuations(st.hdr, st.val, tag)
+            st.apply_return_tamper(tag)
+            torch.cuda.synchronize()
+            h_hdr, h_val, h_tag = st.hdr.cpu().pin_memory(), st.val.cpu().pin_memory(), tag.cpu().pin_memory()
+            h_scratch = torch.empty((n, 32), dtype=torch.int64).pin_memory()
+            h_out = torch.empty((n, 2), dtype=torch.int32).pin_memory()
+            eng.wg_reset_counters()
+            t0 = time.perf_counter()
+            eng.wg_sign_continuations_host(h_hdr, h_val, h_scratch)
+            eng.wg_verify_continuations_host(h_hdr, h_val, h_tag, st.mode, h_out)
+            wall += time.perf_counter() - t0
+            gh, _ = eng.wg_read_counters(per_site=False)
+            h_checks += gh["ret_checks"] + gh["fwd_checks"]
+            assert gh["ret_viol_events"] == len(st.ret_tamper)
+            h2d += n * ((16 + 256) + (16 + 256 + 256))
+            d2h += n * (256 + 8)
+            del st, h_hdr, h_val, h_tag, h_scratch, h_out
+        host = {"batches": hb, "wall_ms_total": 1e3 * wall, "checks_per_sec": h_checks / wall,
+                "h2d_bytes": h2d, "d2h_bytes": d2h, "gbytes_per_sec_both_ways": (h2d + d2h) / wall / 1e9,
+                "api": "wg_sign_continuations_host + wg_verify_continuations_host (pinned host buffers)"}
     print(json.dumps({
         "workload": "config5-stress stream", "batches": a.batches, "events": events, "checks": checks,
         "lane_verdicts": lanes, "sign_ms_total": sign_ms, "verify_ms_total": verify_ms,
@@ -551,13 +641,16 @@ def run_config5_stream(a) -> None:
         "checks_per_sec_sign_plus_verify": checks / ((sign_ms + verify_ms) * 1e-3),
         "violations_found": {"ret_events": g["ret_viol_events"], "fwd_events": g["fwd_viol_events"],
                              "planned_ret": planned_ret, "planned_fwd": planned_fwd},
-        "blocked_lanes": g["blocked_lanes"], "dense_lanes_only": bool(a.dense), "n_sites": pol.n_sites,
-        "n_targets": int(pol.tgt_off[-1])}))
+        "blocked_lanes": g["blocked_lanes"], "n_sites": pol.n_sites,
+        "n_targets": int(pol.tgt_off[-1]), "host_stream": host}))
     eng.close()
 
 
 def main():
     a = parse_args()
+    if a.source_hash:
+        print(kernel_source_hash())
+        return
     if a.impl == "reference":
         run_reference(a)
     elif a.config == 5 and a.batches > 0:

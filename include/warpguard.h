@@ -284,15 +284,6 @@ wg_status wg_shadow_poke(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint
                          uint64_t xor_value, void* cuda_stream);
 wg_status wg_shadow_depth(wg_engine* eng, uint32_t warp_slot, uint32_t lane, uint32_t* h_depth, void* cuda_stream);
 
-/* ---- tuning (never changes a result) ----
- * By default the sign / verify kernels decide per 16-event tile: when at least a quarter of the lanes of the tile's
- * return events are inactive (BASELINE config 5: 1 to 32 active lanes) the per-lane MAC passes run over a compacted
- * list of the ACTIVE (event, lane) pairs of the tile instead of one 32-lane pass per event.
- * WG_TUNE_DENSE_LANES selects the kernels without that path (one pass per event always; 0.2 % faster on dense
- * masks); WG_TUNE_SPARSE_LANES names the default explicitly. */
-typedef enum { WG_TUNE_DEFAULT = 0, WG_TUNE_SPARSE_LANES = 1, WG_TUNE_DENSE_LANES = 2 } wg_tuning_flags;
-wg_status wg_set_tuning(wg_engine* eng, uint32_t flags);
-
 /* ---- inline device form (include/warpguard_device.cuh) ----
  * What a kernel needs to run the checks at its own sites: the engine's policy tables and the key-derived SipHash
  * initial state.  Pass the view to the kernel BY VALUE — kernel parameter space is where the paper puts the key

@@ -27,10 +27,9 @@ EXPORTS = [
     "wg_sign_continuations_host", "wg_verify_continuations_host", "wg_check_forward_host",
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
-    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_set_tuning", "wg_policy_digest",
+    "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_policy_digest",
     "wg_load_policy_bound",
 ]
-WG_TUNE_DEFAULT, WG_TUNE_SPARSE_LANES, WG_TUNE_DENSE_LANES = 0, 1, 2
 
 
 class DeviceView(C.Structure):
@@ -112,7 +111,6 @@ def lib() -> C.CDLL:
         L.wg_set_profile.argtypes = [vp, C.c_uint32]
         L.wg_policy_poke.argtypes = [vp, i, u64, u64, vp]
         L.wg_get_device_view.argtypes = [vp, C.POINTER(DeviceView)]
-        L.wg_set_tuning.argtypes = [vp, C.c_uint32]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
         for name in EXPORTS:
@@ -298,9 +296,6 @@ class Engine:
 
     def wg_set_sequence_base(self, base: int) -> None:
         _chk(lib().wg_set_sequence_base(self._h, int(base)), "wg_set_sequence_base")
-
-    def wg_set_tuning(self, flags: int) -> None:
-        _chk(lib().wg_set_tuning(self._h, int(flags)), "wg_set_tuning")
 
     def wg_get_device_view(self) -> DeviceView:
         v = DeviceView()

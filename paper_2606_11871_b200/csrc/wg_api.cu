@@ -18,7 +18,6 @@ struct wg_engine {
   wg::SiteRec* d_recs = nullptr;  // site records {kind, set range, flags}, 16 B each; nothing key-derived
   uint64_t* d_tok = nullptr;       // [n_sites] forward-record tokens at load time (metadata-integrity profile, R37)
   uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
-  uint32_t tuning = 0;             // WG_TUNE_* flags
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
   wg::ViolRec* d_ring = nullptr;
@@ -145,7 +144,6 @@ wg::Params base_params(const wg_engine* e) {
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
   p.bind_hi = e->bind_hi;
-  p.sparse = (e->tuning & WG_TUNE_DENSE_LANES) ? 0u : 1u;
   p.ring = e->d_ring;
   p.ring_cap = e->d_ring ? e->ring_cap : 0;
   p.first = e->d_first;
@@ -712,13 +710,6 @@ wg_status wg_set_sequence_base(wg_engine* eng, uint64_t base) {
   if (!eng || !eng->loaded) return WG_ERR_NO_POLICY;
   if (base > (1ull << 58)) return WG_ERR_INVALID_ARG;  // (seq << 5) must not wrap
   eng->seq = base;
-  return WG_OK;
-}
-
-wg_status wg_set_tuning(wg_engine* eng, uint32_t flags) {
-  if (!eng) return WG_ERR_NO_POLICY;
-  if (flags & ~static_cast<uint32_t>(WG_TUNE_SPARSE_LANES | WG_TUNE_DENSE_LANES)) return WG_ERR_INVALID_ARG;
-  eng->tuning = flags;
   return WG_OK;
 }
 

@@ -93,7 +93,7 @@ struct Params {
   uint32_t n_sites;
   uint32_t mode;             // 0 detect, 1 enforce
   uint32_t profile;          // PROFILE_* flags (R26)
-  uint32_t sparse;           // tuning: compacted-lane MAC passes (wg_set_tuning)
+  uint32_t pad0;
   uint32_t bind_hi;          // upper half of the token's first message word: low 32 bits of the policy digest when
                              // the policy was loaded with wg_load_policy_bound (R39), else 0
   uint32_t pad1;

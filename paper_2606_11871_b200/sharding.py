@@ -4,7 +4,12 @@ one sum all-reduce over the counter words (global + per-site) and one min all-re
 key.  Events are independent given the read-only policy ("This property is site-local"), so the
 union of the ranks' verdicts is the single-GPU result and the reduced counters equal the single-GPU counters.
 
-Host logic only (no method arithmetic); covered by world_size-2 gloo tests on CPU.
+Each rank tells its engine where its slice starts (``wg_set_sequence_base(lo)``), so first-violation keys, the
+first-violation record and ring records carry the stream's own sequence numbers and need no fixing up afterwards
+(``shard_lo`` stays 0 in ``reduce_counters``; the argument remains for callers whose ranks number from 0).
+
+Host logic only (no method arithmetic); covered by world_size-2 gloo tests on CPU (tests/test_sharding_gloo.py) and, on
+the real engine, by two processes sharing cuda:0 (tests/test_gpu_sharding.py).
 """
 from __future__ import annotations
 
@@ -63,3 +68,29 @@ def reduce_counters(glob: dict, per_site: np.ndarray | None, shard_lo: int = 0, 
         dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
         site = t.cpu().numpy().view(np.uint64)
     return out, site
+
+
+def reduce_first_record(key: int, record, group=None, device: torch.device | str = "cpu"):
+    """The first-violation RECORD of the whole stream on every rank: the record of the rank that holds the smallest
+    key (``key`` = this rank's first_violation_key with global sequence numbers, ``record`` = its wg_violation_rec as a
+    numpy structured scalar, or None).  One all-gather of 56 bytes per rank.  Returns (key, record or None)."""
+    none = (1 << 64) - 1
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
+        return key, record
+    mine = np.zeros(7, dtype=np.uint64)
+    mine[0] = key if record is not None else none
+    if record is not None:
+        mine[1:] = np.frombuffer(np.asarray(record).tobytes(), dtype=np.uint64)
+    t = torch.from_numpy(mine.view(np.int64).copy()).to(device)
+    world = dist.get_world_size(group)
+    parts = [torch.empty_like(t) for _ in range(world)]
+    dist.all_gather(parts, t, group=group)
+    rows = np.stack([p_.cpu().numpy().view(np.uint64) for p_ in parts])
+    best = int(np.argmin(rows[:, 0]))
+    if rows[best, 0] == none:
+        return none, None
+    rec = np.frombuffer(rows[best, 1:].tobytes(), dtype=np.asarray(record).dtype if record is not None else _REC_DTYPE)[0]
+    return int(rows[best, 0]), rec
+
+
+from .binding import VIOLATION_DTYPE as _REC_DTYPE  # noqa: E402  (48 bytes = six u64 words)

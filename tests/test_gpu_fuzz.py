@@ -83,8 +83,6 @@ def test_random_policies_and_streams(seed, n_sites, n_tgts, n):
                  B.WG_PROFILE_SKIP_BACKWARD | B.WG_PROFILE_METADATA_INTEGRITY][trial]
         orc.set_profile(flags)
         eng.wg_set_profile(flags)
-        if trial == 1:
-            eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
         if trial >= 2:
             orc.set_ring_capacity(64)
             eng.wg_set_ring_capacity(64)

@@ -457,26 +457,6 @@ def test_config5_full_size_policy_one_batch_sampled_against_the_oracle():
     eng.close()
 
 
-@pytest.mark.parametrize("config,n", [(5, 70_001), (4, 100_003), (1, 65_536), (2, 33)])
-def test_dense_lane_tuning_changes_no_result(config, n, monkeypatch):
-    """WG_TUNE_DENSE_LANES (the kernels without the per-tile lane compaction, which is the default and is what every
-    other test runs) must give the oracle's tags, verdicts and counters too."""
-    orig_load = B.Engine.load
-
-    def load_sparse(self, policy):
-        eng = orig_load(self, policy)
-        eng.wg_set_tuning(B.WG_TUNE_DENSE_LANES)
-        return eng
-
-    monkeypatch.setattr(B.Engine, "load", load_sparse)
-    if config == 5:
-        test_config5_stress_alternating_modes_accumulate()
-    else:
-        st, orc, eng, out = run_config(config, n)
-        assert out[:, 0].any() or config == 2
-        eng.close()
-
-
 @pytest.mark.parametrize("config", [6, 7])
 def test_public_code_shaped_streams(config):
     """a 38-target family at one indirect site and a wrong-callback burst that

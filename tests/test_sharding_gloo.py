@@ -59,10 +59,12 @@ def _worker(rank: int, world: int, port: int, n_events: int, q):
         orc.reset_counters()
         lo, hi = sharding.shard_range(n_events, rank, world)
         val, tag = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+        orc.set_sequence_base(lo)  # the rank's events keep the stream's own sequence numbers
         out = orc.verify(hdr[lo:hi], val[lo:hi], tag[lo:hi], st.mode)
         g, s = orc.read_counters()
-        gr, sr = sharding.reduce_counters(g, s, lo)
-        q.put((rank, lo, hi, out, gr, sr))
+        gr, sr = sharding.reduce_counters(g, s, 0)
+        key, rec = sharding.reduce_first_record(g["first_violation_key"], orc.read_first_violation())
+        q.put((rank, lo, hi, out, gr, sr, key, None if rec is None else np.asarray(rec).tobytes()))
     finally:
         dist.destroy_process_group()
 
@@ -92,6 +94,8 @@ def test_two_gloo_ranks_equal_one_process():
     g, s = orc.read_counters()
     assert np.array_equal(np.concatenate([res[0][3], res[1][3]]), out)
     assert g["first_violation_key"] != (1 << 64) - 1
-    for _, _, _, _, gr, sr in res:  # every rank holds the reduced result
+    first = orc.read_first_violation()
+    for _, _, _, _, gr, sr, key, rec in res:  # every rank holds the reduced result
         assert gr == g, {k: (gr[k], g[k]) for k in g if gr[k] != g[k]}
         assert np.array_equal(sr, s)
+        assert key == g["first_violation_key"] and rec == np.asarray(first).tobytes()
