@@ -386,77 +386,6 @@ def test_every_lane_violates_under_the_wrong_key():
     eng.close()
 
 
-def test_config4_full_size_sampled_against_the_oracle():
-    """BASELINE.json's full config 4 (58.0 M events, 52.2 M checks) in the launch configuration bench.py times.
-    The oracle cannot run 1.5 G MACs in a test, so: (1) counters must show exactly the planned corruption and the
-    exact class counts; (2) a random sample of events plus EVERY corrupted event is re-judged by the oracle, tags
-    and verdicts compared bit for bit."""
-    st = S.make_stream(4, dev())
-    n = st.hdr.shape[0]
-    assert n == S.FULL_EVENTS[4]
-    eng = engine_for(st.policy)
-    tag = eng.wg_sign_continuations(st.hdr, st.val)
-    g = torch.Generator(device="cpu").manual_seed(99)
-    idx = torch.randint(0, n, (150_000,), generator=g)
-    idx = torch.unique(torch.cat([idx, st.ret_tamper.ev.cpu(), st.fwd_tamper.ev.cpu(),
-                                  torch.arange(0, 4096), torch.arange(n - 4096, n)])).to(dev())
-    clean_tag = tag[idx].cpu().numpy().view(np.uint64)
-    st.apply_return_tamper(tag)
-    out = eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode)
-    gc, _ = eng.wg_read_counters()
-    assert gc["events_total"] == n and gc["ret_checks"] + gc["fwd_checks"] == 52_200_000
-    assert gc["ret_checks"] == 38_300_000 and gc["fwd_checks"] == 13_900_000
-    assert gc["ret_viol_events"] == len(st.ret_tamper) and gc["fwd_viol_events"] == len(st.fwd_tamper)
-    assert gc["blocked_lanes"] == gc["ret_viol"] + gc["fwd_viol"] and gc["events_unknown_site"] == 0
-    assert int((out[:, 0] != 0).sum().item()) == len(st.ret_tamper) + len(st.fwd_tamper)
-    orc = oracle_for(st.policy)
-    hdr_s = st.hdr[idx].cpu().numpy().view(np.uint64)
-    val_s = st.val[idx].cpu().numpy().view(np.uint64)
-    tag_s = tag[idx].cpu().numpy().view(np.uint64)
-    # the recorded corruption may have touched val of sampled events after signing: sign parity uses clean rows only
-    o_tag = orc.sign(hdr_s, val_s)
-    touched = np.isin(idx.cpu().numpy(), st.ret_tamper.ev.cpu().numpy())
-    assert np.array_equal(o_tag[~touched], clean_tag[~touched])
-    o_out = orc.verify(hdr_s, val_s, tag_s, st.mode)
-    assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), o_out)
-    eng.close()
-
-
-def test_config5_full_size_policy_one_batch_sampled_against_the_oracle():
-    """BASELINE.json config 5 at its maximum sizes: 1 M protected sites, log-uniform sets up to 4,096 entries
-    (~246 M targets, searched from L2 / HBM), one 8 M-event batch with 1-32 active lanes per event.  Counters must
-    show exactly the planned corruption; a random sample plus every corrupted event is re-judged by the oracle."""
-    pol = S.make_policy(5, dev())
-    assert pol.n_sites == 1_000_000 and pol.tgt_off[-1] > 100_000_000
-    st = S.make_stream(5, dev(), policy=pol, batch_index=1)
-    n = st.hdr.shape[0]
-    eng = engine_for(pol)
-    tag = eng.wg_sign_continuations(st.hdr, st.val)
-    g = torch.Generator(device="cpu").manual_seed(5)
-    idx = torch.unique(torch.cat([torch.randint(0, n, (60_000,), generator=g), st.ret_tamper.ev.cpu(),
-                                  st.fwd_tamper.ev.cpu(), torch.arange(n - 100, n)])).to(dev())
-    clean_tag = tag[idx].cpu().numpy().view(np.uint64)
-    st.apply_return_tamper(tag)
-    out = eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode)
-    gc, _ = eng.wg_read_counters(per_site=False)
-    assert gc["events_total"] == n and gc["events_unknown_site"] == 0
-    # a flipped address bit of a legal target can land on ANOTHER member of a 4,096-entry set: such an event is no
-    # violation (the sampled oracle pass below re-judges every corrupted event, so it decides)
-    assert gc["ret_viol_events"] == len(st.ret_tamper)
-    assert len(st.fwd_tamper) - 20 <= gc["fwd_viol_events"] <= len(st.fwd_tamper)
-    assert int((out[:, 0] != 0).sum().item()) == gc["ret_viol_events"] + gc["fwd_viol_events"]
-    orc = oracle_for(pol)
-    orc.set_binary_search(True)
-    hdr_s = st.hdr[idx].cpu().numpy().view(np.uint64)
-    val_s = st.val[idx].cpu().numpy().view(np.uint64)
-    tag_s = tag[idx].cpu().numpy().view(np.uint64)
-    o_tag = orc.sign(hdr_s, val_s)
-    touched = np.isin(idx.cpu().numpy(), st.ret_tamper.ev.cpu().numpy())
-    assert np.array_equal(o_tag[~touched], clean_tag[~touched])
-    assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), orc.verify(hdr_s, val_s, tag_s, st.mode))
-    eng.close()
-
-
 @pytest.mark.parametrize("config", [6, 7])
 def test_public_code_shaped_streams(config):
     """a 38-target family at one indirect site and a wrong-callback burst that
@@ -473,37 +402,6 @@ def test_public_code_shaped_streams(config):
         assert out[b0:b0 + 64, 0].all() and not out[:b0, 0].any() and not out[b0 + 64:, 0].any()
         assert (out[b0:b0 + 64, 1] == 0).all()                      # enforce: the whole burst is blocked
         assert g["first_violation_key"] >> 5 == b0
-    eng.close()
-
-
-@pytest.mark.parametrize("config", [2, 3])
-def test_configs_2_and_3_full_size_sampled_against_the_oracle(config):
-    """BASELINE.json configs 2 (4 M backward-only events) and 3 (16 M forward-only events) at full size: counters show
-    exactly the planned corruption; a random sample plus every corrupted event is re-judged by the oracle."""
-    st = S.make_stream(config, dev())
-    n = st.hdr.shape[0]
-    assert n == S.FULL_EVENTS[config]
-    eng = engine_for(st.policy)
-    tag = eng.wg_sign_continuations(st.hdr, st.val)
-    g = torch.Generator(device="cpu").manual_seed(config)
-    idx = torch.unique(torch.cat([torch.randint(0, n, (80_000,), generator=g), st.ret_tamper.ev.cpu(),
-                                  st.fwd_tamper.ev.cpu(), torch.arange(n - 50, n)])).to(dev())
-    clean_tag = tag[idx].cpu().numpy().view(np.uint64)
-    st.apply_return_tamper(tag)
-    out = eng.wg_verify_continuations(st.hdr, st.val, tag, st.mode)
-    gc, gs = eng.wg_read_counters()
-    assert gc["events_total"] == n and gc["ret_checks"] + gc["fwd_checks"] + gc["events_empty"] == n
-    assert gc["ret_viol_events"] == len(st.ret_tamper) and gc["fwd_viol_events"] == len(st.fwd_tamper)
-    assert int(gs[:, 0].sum()) == n and int(gs[:, 1].sum()) == gc["ret_lanes"] + gc["fwd_lanes"]
-    if config == 3:
-        assert gc["blocked_lanes"] == 0 and bool((out[:, 1] == (st.hdr[:, 0] >> 32).to(torch.int32)).all())  # detect
-    orc = oracle_for(st.policy)
-    hdr_s = st.hdr[idx].cpu().numpy().view(np.uint64)
-    val_s = st.val[idx].cpu().numpy().view(np.uint64)
-    tag_s = tag[idx].cpu().numpy().view(np.uint64)
-    touched = np.isin(idx.cpu().numpy(), st.ret_tamper.ev.cpu().numpy())
-    assert np.array_equal(orc.sign(hdr_s, val_s)[~touched], clean_tag[~touched])
-    assert np.array_equal(out[idx].cpu().numpy().view(np.uint32), orc.verify(hdr_s, val_s, tag_s, st.mode))
     eng.close()
 
 
