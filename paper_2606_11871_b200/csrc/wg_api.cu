@@ -17,6 +17,8 @@ struct wg_engine {
   uint64_t n_tgts = 0;
   wg::SiteRec* d_recs = nullptr;  // site records {kind, set range, flags}, 16 B each; nothing key-derived
   uint64_t* d_tok = nullptr;       // [n_sites] forward-record tokens at load time (metadata-integrity profile, R37)
+  uint64_t* d_htab = nullptr;      // hash index of the target sets when the table is too large to stage (wg_check.cu)
+  bool htab_stale = false;         // wg_policy_poke rewrote a target: the sorted sets are searched from then on
   uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
@@ -91,6 +93,9 @@ void free_tables(wg_engine* e) {
   e->d_recs = nullptr;
   cudaFree(e->d_tok);
   e->d_tok = nullptr;
+  cudaFree(e->d_htab);
+  e->d_htab = nullptr;
+  e->htab_stale = false;
   cudaFree(e->d_tgts);
   cudaFree(e->d_glob);
   cudaFree(e->d_site);
@@ -141,6 +146,7 @@ wg::Params base_params(const wg_engine* e) {
   std::memset(&p, 0, sizeof(p));
   p.recs = e->d_recs;
   p.tok = e->d_tok;
+  p.htab = e->htab_stale ? nullptr : e->d_htab;
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
   p.bind_hi = e->bind_hi;
@@ -392,6 +398,8 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
     recs[s].off = desc->tgt_off[s];
     recs[s].cnt = desc->tgt_off[s + 1] - desc->tgt_off[s];
     recs[s].flags = 0;
+    for (uint32_t i = desc->tgt_off[s]; i < desc->tgt_off[s + 1]; ++i)
+      if (desc->tgts[i] == ~0ull) recs[s].flags |= wg::SITE_FLAG_HAS_ALLONES;
   }
   wg_engine tmp;
   tmp.device = device;
@@ -426,6 +434,14 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
     return fail(err);
   if (nt && (err = cudaMemcpy(tmp.d_tgts, desc->tgts, sizeof(uint64_t) * nt, cudaMemcpyHostToDevice)) != cudaSuccess)
     return fail(err);
+  // large policies: the hash index of the target sets (one 32-byte load per membership test instead of a binary search)
+  if (nt > wg::max_staged_targets()) {
+    const size_t slots = 2 * static_cast<size_t>(nt) + 4 * static_cast<size_t>(n);
+    if ((err = cudaMalloc(&tmp.d_htab, slots * 8)) != cudaSuccess) return fail(err);
+    if ((err = cudaMemset(tmp.d_htab, 0xff, slots * 8)) != cudaSuccess) return fail(err);
+    if ((err = wg::launch_build_hash(tmp.d_htab, tmp.d_recs, tmp.d_tgts, n, nt, nullptr, &tmp.launches)) != cudaSuccess)
+      return fail(err);
+  }
   // tokens of the forward records, computed on the device at (trusted) load time (R37)
   if ((err = wg::launch_build_tokens(tmp.d_tok, tmp.d_recs, tmp.d_tgts, n, tmp.v_init[0], tmp.v_init[1], tmp.v_init[2],
                                      tmp.v_init[3], nullptr, &tmp.launches)) != cudaSuccess)
@@ -464,6 +480,8 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
   e->n_tgts = nt;
   e->d_recs = tmp.d_recs;
   e->d_tok = tmp.d_tok;
+  e->d_htab = tmp.d_htab;
+  e->htab_stale = false;
   e->d_tgts = tmp.d_tgts;
   e->d_glob = tmp.d_glob;
   e->d_site = tmp.d_site;
@@ -731,6 +749,7 @@ wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
   void* addr = what == 0 ? static_cast<void*>(eng->d_tgts + index) : static_cast<void*>(eng->d_tok + index);
+  if (what == 0) eng->htab_stale = true;  // the hash index no longer mirrors the sorted sets: search those from now on
   uint64_t v = 0;
   WG_CUDA(eng, cudaMemcpy(&v, addr, 8, cudaMemcpyDeviceToHost));
   v ^= xor_value;

@@ -251,6 +251,42 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
   }
 }
 
+// ---- hash index of the large target sets (policies whose table is not staged in shared memory) --------------------
+// A binary search over a set in L2 / HBM is up to 12 DEPENDENT loads (7 with quaternary steps): on config 5 (sets up to
+// 4,096 entries) the check kernel spent most of its time waiting on them (ALU pipe 48 % busy).  At load time the engine
+// therefore builds, per forward site, an open-addressing hash table of the site's targets in its own memory:
+//   slots of site s: htab[2 * off(s) + 4 * s ...), 4 * nb(s) of them, nb(s) = ceil(cnt(s) / 2) buckets of 4 slots (one
+//   32-byte sector): load factor <= 1/2, tables derived from the site record alone, no extra field;
+//   a target goes to the first free slot of bucket b = mulhi(hash(v), nb), b + 1, ... (linear probing by bucket).
+// Membership is then ONE 32-byte load in the common case: found if a slot equals v, absent if the bucket has a free
+// slot, else the next bucket.  Exactly the set's membership (R8): the table holds the set's
+// elements and nothing else.  The all-ones word marks a free slot; a set that contains it carries SITE_FLAG_HAS_ALLONES.
+// The metadata-integrity profile authenticates the SORTED record, so it searches that, not the index; after
+// wg_policy_poke has rewritten a target the index is dropped (Params::htab == nullptr) and the sorted sets are searched.
+constexpr uint64_t kFree = ~0ull;
+__host__ __device__ __forceinline__ uint32_t hash_target(uint32_t lo, uint32_t hi) {
+  uint32_t h = lo * 0x9e3779b1u ^ (hi + 0x7f4a7c15u) * 0x85ebca6bu;
+  h ^= h >> 15;
+  h *= 0x2c1b3c6du;
+  h ^= h >> 13;
+  return h;
+}
+__device__ __forceinline__ bool member_hash(const Params& p, uint32_t site, uint32_t off, uint32_t cnt, uint32_t flags,
+                                            uint32_t vl, uint32_t vh) {
+  if ((vl & vh) == 0xffffffffu) return (flags & SITE_FLAG_HAS_ALLONES) != 0u;
+  const uint32_t nb = (cnt + 1u) >> 1;
+  const ulonglong2* tab = reinterpret_cast<const ulonglong2*>(p.htab + (2ull * off + 4ull * site));
+  const uint64_t v = (static_cast<uint64_t>(vh) << 32) | vl;
+  uint32_t b = __umulhi(hash_target(vl, vh), nb);
+  for (uint32_t i = 0; i < nb; ++i) {  // (terminates earlier: half of the slots are free)
+    const ulonglong2 x = __ldg(tab + 2u * b), y = __ldg(tab + 2u * b + 1u);
+    if (x.x == v || x.y == v || y.x == v || y.y == v) return true;
+    if (x.x == kFree || x.y == kFree || y.x == kFree || y.y == kFree) return false;
+    b = b + 1u == nb ? 0u : b + 1u;
+  }
+  return false;
+}
+
 __device__ __forceinline__ Sip32 init_state(const Params& p) {
   return Sip32{static_cast<uint32_t>(p.v0), static_cast<uint32_t>(p.v0 >> 32), static_cast<uint32_t>(p.v1),
                static_cast<uint32_t>(p.v1 >> 32), static_cast<uint32_t>(p.v2), static_cast<uint32_t>(p.v2 >> 32),
@@ -341,6 +377,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   const uint32_t stride = gridDim.x * kWarps;
   uint32_t gi = blockIdx.x * kWarps + warp;
   const bool enforce = p.mode != 0;
+  // large sets: the hash index, unless the metadata-integrity profile wants the authenticated sorted record searched
+  const bool use_hash = !STAGED && p.htab != nullptr && !(TEL && (p.profile & PROFILE_METADATA_INTEGRITY));
   const Sip32 s_init = init_state(p);
   WarpCtr c = {0, 0, 0, 0};
   uint32_t par = 0;          // which half of the record area this group uses
@@ -767,14 +805,20 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           const uint32_t a = __shfl_sync(kFull, active, e);
           const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
           const uint2 v = ldg_v2_keep(elem_ptr(p.val, (e0 + e) * 32u + lane));
-          const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !member<STAGED>(p, tg_s, o2, c2, v.x, v.y));
+          bool in;
+          if (!STAGED && use_hash)
+            in = member_hash(p, __shfl_sync(kFull, site, e), o2, c2, __shfl_sync(kFull, r_cur.w, e), v.x, v.y);
+          else
+            in = member<STAGED>(p, tg_s, o2, c2, v.x, v.y);
+          const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !in);
           if (lane == e) fviol = vb;
         }
         if (cls == CLS_FWD) {
           if (bad_rec)
             fviol = active;
           else if (is_uni)
-            fviol = member<STAGED>(p, tg_s, off, cnt, ul, uh) ? 0u : active;
+            fviol = ((!STAGED && use_hash) ? member_hash(p, site, off, cnt, r_cur.w, ul, uh)
+                                           : member<STAGED>(p, tg_s, off, cnt, ul, uh)) ? 0u : active;
           sts_u32(ra_me + 56, fviol);
         }
       }
@@ -892,6 +936,31 @@ __global__ void wg_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64
   tok[s] = t;
 }
 
+// hash index build (load time): one thread per target finds its site (binary search over the records' offsets) and
+// claims the first free slot of its probe sequence
+__global__ void wg_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts) {
+  const uint64_t i = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= n_tgts) return;
+  uint32_t lo = 0, len = n_sites;  // last site with off <= i that owns targets: sites without targets share offsets
+  while (len > 1) {
+    const uint32_t half = len >> 1;
+    if (recs[lo + half].off <= i) lo += half;
+    len -= half;
+  }
+  while (recs[lo].cnt == 0u || recs[lo].off + recs[lo].cnt <= i) --lo;  // (step back over empty sites at the same offset)
+  const SiteRec r = recs[lo];
+  const uint64_t v = tgts[i];
+  if (v == kFree) return;  // carried by SITE_FLAG_HAS_ALLONES
+  const uint32_t nb = (r.cnt + 1u) >> 1;
+  unsigned long long* tab = reinterpret_cast<unsigned long long*>(htab + (2ull * r.off + 4ull * lo));
+  uint32_t b = __umulhi(hash_target(static_cast<uint32_t>(v), static_cast<uint32_t>(v >> 32)), nb);
+  for (;;) {
+    for (uint32_t k = 0; k < 4u; ++k)
+      if (atomicCAS(tab + 4u * b + k, kFree, v) == kFree) return;
+    b = b + 1u == nb ? 0u : b + 1u;
+  }
+}
+
 __global__ void wg_set_site_flags(SiteRec* recs, const uint8_t* skip, uint32_t n_sites) {
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s < n_sites) recs[s].flags = (skip && skip[s]) ? SITE_FLAG_SKIP : 0u;
@@ -966,6 +1035,16 @@ cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* laun
   ++*launches;
   return cudaGetLastError();
 }
+
+cudaError_t launch_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts,
+                              cudaStream_t st, uint64_t* launches) {
+  if (n_tgts == 0) return cudaSuccess;
+  wg_build_hash<<<static_cast<unsigned>((n_tgts + 255) / 256), 256, 0, st>>>(htab, recs, tgts, n_sites, n_tgts);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+uint64_t max_staged_targets() { return kMaxStageTgts; }
 
 cudaError_t launch_set_site_flags(SiteRec* recs, const uint8_t* d_skip, uint32_t n_sites, cudaStream_t st, uint64_t* launches) {
   if (n_sites == 0) return cudaSuccess;

@@ -18,7 +18,7 @@ struct __align__(16) SiteRec {
   uint32_t flags; // bit 0: the site is in the coverage-reduced profile's skip set (R40)
 };
 static_assert(sizeof(SiteRec) == 16, "SiteRec is one 16-byte vector");
-enum : uint32_t { SITE_FLAG_SKIP = 1u };
+enum : uint32_t { SITE_FLAG_SKIP = 1u, SITE_FLAG_HAS_ALLONES = 2u };  // (2: the set contains 0xffff...f, see the hash index)
 
 // Global counter block: the first 26 words have exactly the layout of wg_counters, so a read-out is one
 // copy.  Words 24 (policy_digest) and 25 (last_mode) are kept host-side and patched in at read-out.
@@ -87,6 +87,7 @@ struct Params {
   const SiteRec* recs;       // [n_sites]
   const uint64_t* tok;       // [n_sites] token of each forward record at load time (metadata-integrity profile, R37)
   const uint64_t* tgts;
+  const uint64_t* htab;      // hash index of the target sets (policies too large to stage), or nullptr (wg_check.cu)
   uint64_t n_tgts;           // elements in tgts (v2 stages the whole table in shared memory when it is small)
   unsigned long long* glob;  // [C_WORDS]
   unsigned long long* site;  // [n_sites][4]
@@ -132,6 +133,10 @@ cudaError_t launch_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64
                                 uint64_t v0, uint64_t v1, uint64_t v2, uint64_t v3, cudaStream_t st, uint64_t* launches);
 // SiteRec.flags bit 0 <- d_skip[site] != 0 (d_skip == nullptr: cleared), the coverage-reduced profile's skip set (R40)
 cudaError_t launch_set_site_flags(SiteRec* recs, const uint8_t* d_skip, uint32_t n_sites, cudaStream_t st, uint64_t* launches);
+// hash index of large target sets: htab has 2 * n_tgts + 4 * n_sites slots, pre-filled with all-ones (wg_check.cu)
+cudaError_t launch_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts,
+                              cudaStream_t st, uint64_t* launches);
+uint64_t max_staged_targets();  // larger tables are searched in global memory (and get the hash index)
 cudaError_t init_kernels();  // one-time function attributes (dynamic shared memory opt-in) on the current device
 
 }  // namespace wg
