@@ -78,7 +78,7 @@ constexpr uint32_t kBatch = WG_BATCH;              // row loads in flight per la
 constexpr uint32_t kListBytes = 40 * 16;           // up to 32 protected events, padded to a multiple of kBatch
 constexpr uint32_t kEntryMul = (kRecBytes << 16) | 32u;  // queue item of (slot, lane) = slot * kEntryMul + lane
 constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 4 + kListBytes;
-constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 12 * 4 + 16;  // cnt64, bykind + rare-event counts (u32), mbar
+constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 16 * 4 + 16;  // cnt64, bykind + rare-event counts + group ticket (u32), mbar
 constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
 constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
 static_assert(kWarps * kWarpBytes + kCtaFixedBytes + 4096 <= kSmemMax, "too many warps for the shared memory");
@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   const uint32_t cta_off = stage_bytes + site_bytes;
   unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + cta_off);
   uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8);
-  const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 48;
+  const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 64;
   const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * kWarpBytes;
   const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 4 * k
   const uint32_t q_top = q_s + (kQueueItems - 1) * 4;        // divergent items: q_top - 4 * k
@@ -360,7 +360,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   if (threadIdx.x < C_WORDS) cnt64[threadIdx.x] = 0ull;
   const uint32_t tbl_slots = site_bytes / 12u, tbl_mask = tbl_slots - 1u;  // site_s: [slots] owner, [slots][2] counts
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = i < tbl_slots ? 0xffffffffu : 0u;
-  if (threadIdx.x < 12) bykind[threadIdx.x] = 0u;  // 7 by-kind counts, then unknown / empty / misrouted events
+  if (threadIdx.x < 13) bykind[threadIdx.x] = 0u;  // 7 by-kind counts, then unknown / empty / misrouted events, the ticket
+  uint32_t* const ticket = bykind + 12;
   if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
   __syncthreads();
   if constexpr (STAGED) {
@@ -374,8 +375,17 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   // a launch covers at most 2^27 events (wg_api.cu), so event and element indices (event * 32 + lane) fit 32 bits
   const uint32_t n_ev = static_cast<uint32_t>(p.n);
   const uint32_t n_groups = (n_ev + 31u) / 32u;
-  const uint32_t stride = gridDim.x * kWarps;
-  uint32_t gi = blockIdx.x * kWarps + warp;
+  // Groups are handed out dynamically inside the CTA: CTA b owns groups b, b + gridDim.x, ...; a warp takes the next
+  // one of them from a shared-memory ticket when it needs one (three tickets ahead: the header is loaded two groups
+  // ahead, the site record one).  A warp that waits longer on memory simply takes fewer groups, and warps on a busier
+  // sub-partition do not hold the CTA back.
+  auto claim = [&]() __attribute__((always_inline)) -> uint32_t {
+    uint32_t t = 0;
+    if (lane == 0) t = atomicAdd(ticket, 1u);
+    return blockIdx.x + __shfl_sync(kFull, t, 0) * gridDim.x;
+  };
+  uint32_t gi = claim();
+  uint32_t g_nxt = claim();
   const bool enforce = p.mode != 0;
   // large sets: the hash index, unless the metadata-integrity profile wants the authenticated sorted record searched
   const bool use_hash = !STAGED && p.htab != nullptr && !(TEL && (p.profile & PROFILE_METADATA_INTEGRITY));
@@ -528,7 +538,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
 
   // ---- software pipeline of the event-parallel loads: the header two groups ahead, the site record one group ahead,
   //      so that the rows of the NEXT group can be pulled into L2 while this group is computed ----
-  auto load_hdr = [&](uint32_t g) __attribute__((always_inline)) -> uint4 {  // (g runs past n_groups by at most two strides: no 32-bit wrap)
+  auto load_hdr = [&](uint32_t g) __attribute__((always_inline)) -> uint4 {  // (tickets run a few groups past the end: no 32-bit wrap)
     const uint32_t e = g * 32u + lane;
     return (g < n_groups && e < n_ev) ? ldg_v4(p.hdr + e) : make_uint4(0xffffffffu, 0u, 0u, 0u);
   };
@@ -536,7 +546,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     return h.x < p.n_sites ? ldg_v4(p.recs + h.x) : make_uint4(7u, 0u, 0u, 0u);
   };
   uint4 h_cur = load_hdr(gi);
-  uint4 h_nxt = load_hdr(gi + stride);
+  uint4 h_nxt = load_hdr(g_nxt);
   uint4 r_cur = load_rec(h_cur);
 
   // One trip per group of this warp, plus one last trip over an empty group (no valid event) that flushes the queues and
@@ -545,10 +555,11 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   bool last = gi >= n_groups;
   if (!last) do {
     last = gi >= n_groups;
-    const uint32_t gn = gi + stride;
+    const uint32_t gn = g_nxt;
     const uint32_t e0 = gi * 32u;
+    g_nxt = claim();
     const uint4 r_nxt = load_rec(h_nxt);
-    const uint4 h_nn = load_hdr(gn + stride);
+    const uint4 h_nn = load_hdr(g_nxt);
     const uint32_t rbase = rec_s + par * (kGroupRecs * kRecBytes);
     const uint32_t ra_me = rbase + lane * kRecBytes;
     const uint32_t slot_me = par * kGroupRecs + lane;
