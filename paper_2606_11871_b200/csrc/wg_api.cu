@@ -17,6 +17,8 @@ struct wg_engine {
   uint64_t n_tgts = 0;
   wg::SiteRec* d_recs = nullptr;  // site records {kind, set range, flags}, 16 B each; nothing key-derived
   uint64_t* d_tok = nullptr;       // [n_sites] forward-record tokens at load time (metadata-integrity profile, R37)
+  unsigned int* d_sched = nullptr; // ring of group tickets, one per launch in flight (wg_check.cu)
+  uint32_t sched_next = 0;
   uint64_t* d_htab = nullptr;      // hash index of the target sets when the table is too large to stage (wg_check.cu)
   bool htab_stale = false;         // wg_policy_poke rewrote a target: the sorted sets are searched from then on
   uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
@@ -95,6 +97,8 @@ void free_tables(wg_engine* e) {
   e->d_tok = nullptr;
   cudaFree(e->d_htab);
   e->d_htab = nullptr;
+  cudaFree(e->d_sched);
+  e->d_sched = nullptr;
   e->htab_stale = false;
   cudaFree(e->d_tgts);
   cudaFree(e->d_glob);
@@ -147,6 +151,7 @@ wg::Params base_params(const wg_engine* e) {
   p.recs = e->d_recs;
   p.tok = e->d_tok;
   p.htab = e->htab_stale ? nullptr : e->d_htab;
+  p.sched = e->d_sched;  // (the check / sign launch sites pick the ring slot)
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
   p.bind_hi = e->bind_hi;
@@ -191,6 +196,7 @@ wg_status check_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* 
     p.n = m;
     p.seq_base = e->seq;
     p.mode = static_cast<uint32_t>(mode);
+    p.sched = e->d_sched + (e->sched_next++ % wg::kSchedSlots) * 16;  // (64 bytes apart)
     WG_CUDA(e, wg::launch_check(p, e->sm_count, st, &e->launches));
     // first-violation record (R29): one thread behind the check launch; the launch is over, so the key is final for it
     if (rec_after) WG_CUDA(e, cudaStreamWaitEvent(st, rec_after, 0));
@@ -216,6 +222,7 @@ wg_status sign_common(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d
     p.val = d_val + lo * 32;
     p.tag_out = d_tag + lo * 32;
     p.n = m;
+    p.sched = e->d_sched + (e->sched_next++ % wg::kSchedSlots) * 16;
     WG_CUDA(e, wg::launch_sign(p, e->sm_count, st, &e->launches));
   }
   return WG_OK;
@@ -427,6 +434,7 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
   if ((err = cudaMemset(tmp.d_tgts, 0, sizeof(uint64_t) * (nt_pad ? nt_pad : 2))) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_recs, sizeof(wg::SiteRec) * (n ? n : 1))) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_tok, sizeof(uint64_t) * (n ? n : 1))) != cudaSuccess) return fail(err);
+  if ((err = cudaMalloc(&tmp.d_sched, wg::kSchedSlots * 64)) != cudaSuccess) return fail(err);
   if ((err = wg::init_kernels()) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_glob, sizeof(unsigned long long) * wg::C_WORDS)) != cudaSuccess) return fail(err);
   if ((err = cudaMalloc(&tmp.d_site, sizeof(unsigned long long) * 4 * (n ? n : 1))) != cudaSuccess) return fail(err);
@@ -482,6 +490,7 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
   e->d_tok = tmp.d_tok;
   e->d_htab = tmp.d_htab;
   e->htab_stale = false;
+  e->d_sched = tmp.d_sched;
   e->d_tgts = tmp.d_tgts;
   e->d_glob = tmp.d_glob;
   e->d_site = tmp.d_site;

@@ -53,8 +53,8 @@ constexpr uint32_t kMaxCacheSlots = 2048;  // slots of the per-site counter cach
 // ---- shared-memory carve-up ----------------------------------------------------------------------
 // CTA part: [tgts staged: stage_bytes][per-site counter cache: site_bytes][cnt64: 40 x u64][bykind: 12 x u32][mbar, pad]
 // warp part: event records [2 groups][33] x 80 B (record 32 of a group is a dummy that absorbs the padding trips of
-// the producer loop), the work queue (u32 items; warp-uniform items from the front, lane-divergent items from the
-// back), and the producer's list of the group's protected events (16 B each)
+// the producer loop), the work queue (u16 items = record slot * 32 + lane; warp-uniform items from the front, lane-divergent
+// items from the back), and the producer's list of the group's protected events (16 B each)
 //   record: +0  SipHash state the event's consumer passes start from (8 words); a forward event parks its set range
 //               {offset, count} at +16 instead
 //           +32 ctx lo (context_base & ~31), +36 ctx hi, +40 (8 B) pointer to the event's tag row (sign: the row to
@@ -76,8 +76,7 @@ constexpr uint32_t kQueueItems = WG_QUEUE;       // one group adds at most 1,024
 #endif
 constexpr uint32_t kBatch = WG_BATCH;              // row loads in flight per lane in the producer loop
 constexpr uint32_t kListBytes = 40 * 16;           // up to 32 protected events, padded to a multiple of kBatch
-constexpr uint32_t kEntryMul = (kRecBytes << 16) | 32u;  // queue item of (slot, lane) = slot * kEntryMul + lane
-constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 4 + kListBytes;
+constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 2 + kListBytes;
 constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 16 * 4 + 16;  // cnt64, bykind + rare-event counts + group ticket (u32), mbar
 constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
 constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
@@ -126,6 +125,9 @@ __device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
   uint32_t r;
   asm volatile("ld.shared.u16 %0, [%1];" : "=r"(r) : "r"(a));
   return r;
+}
+__device__ __forceinline__ void sts_u16(uint32_t a, uint32_t x) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"(static_cast<unsigned short>(x)) : "memory");
 }
 __device__ __forceinline__ void sts_u32(uint32_t a, uint32_t x) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
@@ -349,9 +351,9 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8);
   const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 64;
   const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * kWarpBytes;
-  const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 4 * k
-  const uint32_t q_top = q_s + (kQueueItems - 1) * 4;        // divergent items: q_top - 4 * k
-  const uint32_t list_s = q_s + kQueueItems * 4;
+  const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 2 * k
+  const uint32_t q_top = q_s + (kQueueItems - 1) * 2;        // divergent items: q_top - 2 * k
+  const uint32_t list_s = q_s + kQueueItems * 2;
   if (lane < 2) {  // the two dummy records: no active lane, nothing to queue
     sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 32, 0u, 0u, 0u, 0u);
     sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 48, 0u, 0u, 0u, 0u);
@@ -360,8 +362,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   if (threadIdx.x < C_WORDS) cnt64[threadIdx.x] = 0ull;
   const uint32_t tbl_slots = site_bytes / 12u, tbl_mask = tbl_slots - 1u;  // site_s: [slots] owner, [slots][2] counts
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = i < tbl_slots ? 0xffffffffu : 0u;
-  if (threadIdx.x < 13) bykind[threadIdx.x] = 0u;  // 7 by-kind counts, then unknown / empty / misrouted events, the ticket
-  uint32_t* const ticket = bykind + 12;
+  if (threadIdx.x < 12) bykind[threadIdx.x] = 0u;  // 7 by-kind counts, then unknown / empty / misrouted events
   if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
   __syncthreads();
   if constexpr (STAGED) {
@@ -375,14 +376,32 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   // a launch covers at most 2^27 events (wg_api.cu), so event and element indices (event * 32 + lane) fit 32 bits
   const uint32_t n_ev = static_cast<uint32_t>(p.n);
   const uint32_t n_groups = (n_ev + 31u) / 32u;
-  // Groups are handed out dynamically inside the CTA: CTA b owns groups b, b + gridDim.x, ...; a warp takes the next
-  // one of them from a shared-memory ticket when it needs one (three tickets ahead: the header is loaded two groups
-  // ahead, the site record one).  A warp that waits longer on memory simply takes fewer groups, and warps on a busier
-  // sub-partition do not hold the CTA back.
+  // Groups are handed out dynamically, to the whole grid, from one ticket counter in global memory (one of a ring of
+  // counters the engine owns, zeroed by the launcher): a warp takes four consecutive groups per ticket (one 64-bit-free atomic per 128 events; the claim is made
+  // three groups before the group is needed, so its latency is never waited for), single groups near the end of the
+  // stream so that the launch ends evenly.  A warp that waits longer on memory simply takes fewer groups; no SM, and no
+  // sub-partition with one warp more than its neighbours, holds the launch back.
+  // (A short stream — fewer than 16 groups per warp — is dealt out statically, group = warp + k * warps: the tickets of
+  // 3,000 warps that all start at once would queue on the one counter for longer than such a launch lasts.)
+  const bool dyn = n_groups >= 16u * gridDim.x * kWarps;
+  uint32_t wnext = blockIdx.x * kWarps + warp, wleft = 0;
+  const uint32_t tail_from = n_groups > 8u * gridDim.x * kWarps ? n_groups - 8u * gridDim.x * kWarps : 0u;
+  unsigned int* const sched = p.sched;
   auto claim = [&]() __attribute__((always_inline)) -> uint32_t {
-    uint32_t t = 0;
-    if (lane == 0) t = atomicAdd(ticket, 1u);
-    return blockIdx.x + __shfl_sync(kFull, t, 0) * gridDim.x;
+    if (!dyn) {
+      const uint32_t g = wnext;
+      wnext += gridDim.x * kWarps;
+      return g;
+    }
+    if (wleft == 0u) {
+      const uint32_t sz = wnext < tail_from ? 4u : 1u;
+      uint32_t t = 0;
+      if (lane == 0) t = atomicAdd(sched, sz);
+      wnext = __shfl_sync(kFull, t, 0);
+      wleft = sz;
+    }
+    --wleft;
+    return wnext++;
   };
   uint32_t gi = claim();
   uint32_t g_nxt = claim();
@@ -406,10 +425,10 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   auto pass2 = [&](bool div, uint32_t k0, bool on_a, bool on_b) __attribute__((always_inline)) {
     if (!on_a) return;
     const uint32_t kb = on_b ? k0 + 32u : k0;
-    const uint32_t qa = div ? mad32(k0 + lane, 0xfffffffcu, q_top) : mad32(k0 + lane, 4u, q_s);
-    const uint32_t qb = div ? mad32(kb + lane, 0xfffffffcu, q_top) : mad32(kb + lane, 4u, q_s);
+    const uint32_t qa = div ? mad32(k0 + lane, 0xfffffffeu, q_top) : mad32(k0 + lane, 2u, q_s);
+    const uint32_t qb = div ? mad32(kb + lane, 0xfffffffeu, q_top) : mad32(kb + lane, 2u, q_s);
     const uint32_t ia = lds_u16(qa), ib = lds_u16(qb);            // slot * 32 + lane of the event
-    const uint32_t ra = rec_s + lds_u16(qa + 2), rb = rec_s + lds_u16(qb + 2);  // the events' records
+    const uint32_t ra = mad32(ia >> 5, kRecBytes, rec_s), rb = mad32(ib >> 5, kRecBytes, rec_s);  // the events' records
     const uint4 ca = lds_v4(ra + 32), cb = lds_v4(rb + 32);        // ctx lo, ctx hi, biased tag row pointer
     Sip32 sa = lds_state(ra), sb = lds_state(rb);
     const uint64_t* pa = item_ptr(ca.z, ca.w, ia);
@@ -460,11 +479,11 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       k = k < n ? k : n;
       const uint32_t r = n - k;  // < 64 items stay: two per lane
       uint32_t c0 = 0, c1 = 0;
-      if (lane < r) c0 = lds_u32(div ? q_top - (k + lane) * 4u : q_s + (k + lane) * 4u);
-      if (lane + 32u < r) c1 = lds_u32(div ? q_top - (k + 32u + lane) * 4u : q_s + (k + 32u + lane) * 4u);
+      if (lane < r) c0 = lds_u16(div ? q_top - (k + lane) * 2u : q_s + (k + lane) * 2u);
+      if (lane + 32u < r) c1 = lds_u16(div ? q_top - (k + 32u + lane) * 2u : q_s + (k + 32u + lane) * 2u);
       __syncwarp();
-      if (lane < r) sts_u32(div ? q_top - lane * 4u : q_s + lane * 4u, c0);
-      if (lane + 32u < r) sts_u32(div ? q_top - (32u + lane) * 4u : q_s + (32u + lane) * 4u, c1);
+      if (lane < r) sts_u16(div ? q_top - lane * 2u : q_s + lane * 2u, c0);
+      if (lane + 32u < r) sts_u16(div ? q_top - (32u + lane) * 2u : q_s + (32u + lane) * 2u, c1);
       if (div) nd = r; else nu = r;
     }
     __syncwarp();
@@ -619,9 +638,9 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t n_need = __popc(need);
     if (need != 0u) {
       const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
-      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * kEntryMul, first);
+      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * 32u, first);
       if (lane < ((kBatch - n_need) & (kBatch - 1u)))
-        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * kEntryMul, 0u);
+        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * 32u, 0u);
     }
     __syncwarp();  // the records and the list are visible to every lane
     // value rows, straight from global memory: one coalesced 256-byte load per event, kBatch in flight per lane; the
@@ -708,7 +727,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     //      for a return check the active lanes appended, compacted, to the queue of its class.  Double-buffered: the
     //      next batch's rows are requested before this batch is looked at. ----
     if (need != 0u) {
-      uint32_t qu = q_s + nu * 4u, qd = q_top - nd * 4u;  // where the next uniform / divergent item goes
+      uint32_t qu = q_s + nu * 2u, qd = q_top - nd * 2u;  // where the next uniform / divergent item goes
       auto consume_batch = [&](const uint2 (&v)[kBatch], uint32_t b0) {
 #pragma unroll
         for (int j = 0; j < static_cast<int>(kBatch); ++j) {
@@ -721,10 +740,10 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           if (MODE == MODE_FORWARD || m_ret == 0u) continue;  // a group without return checks has nothing to queue
           const uint32_t rank = __popc(am.y & ltmask), nae = __popc(am.y);
           const bool div = div_ != 0u, act = (am.y & lanebit) != 0u;
-          const uint32_t addr = div ? mad32(rank, 0xfffffffcu, qd) : mad32(rank, 4u, qu);
-          if (act) sts_u32(addr, le.z + lane);
-          qd = div ? mad32(nae, 0xfffffffcu, qd) : qd;
-          qu = div ? qu : mad32(nae, 4u, qu);
+          const uint32_t addr = div ? mad32(rank, 0xfffffffeu, qd) : mad32(rank, 2u, qu);
+          if (act) sts_u16(addr, le.z + lane);
+          qd = div ? mad32(nae, 0xfffffffeu, qd) : qd;
+          qu = div ? qu : mad32(nae, 2u, qu);
           if (MODE == MODE_SIGN && !act && am.x != 0u)  // inactive lanes sign nothing (R10)
             st_stream_v2(const_cast<char*>(byte_ptr(reinterpret_cast<const char*>(elem_ptr(p.tag_out, e0 * 32u + lane)), le.y)), 0u, 0u);
         }
@@ -739,8 +758,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           consume_batch(vb, b0 + kBatch);
         }
       }
-      nu = (qu - q_s) >> 2;
-      nd = (q_top - qd) >> 2;
+      nu = (qu - q_s) >> 1;
+      nd = (q_top - qd) >> 1;
     }
     if constexpr (MODE == MODE_SIGN) {
       // every event that is not a return check gets a zero row (R10): non-return sites, empty masks; written as
@@ -994,6 +1013,10 @@ cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t
   }
   const uint32_t smem = stage_bytes + site_bytes + kCtaFixedBytes + kWarps * kWarpBytes;
   const bool tel = MODE != MODE_SIGN && (p.profile != 0 || p.ring_cap != 0);
+  {  // the launch's group ticket starts at 0
+    const cudaError_t e = cudaMemsetAsync(p.sched, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+  }
   if (tel) {
     if constexpr (MODE != MODE_SIGN) {
       if (staged)

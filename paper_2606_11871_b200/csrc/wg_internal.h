@@ -56,6 +56,10 @@ enum CounterWord {
   C_WORDS = 40
 };
 
+// Launches of one engine that may be in flight at once on different streams each need their own group ticket: the
+// engine hands out the words of a small ring in launch order (wg_api.cu)
+constexpr int kSchedSlots = 64;
+
 // Violation record, layout of wg_violation_rec (48 bytes)
 struct __align__(8) ViolRec {
   uint64_t seq;
@@ -89,6 +93,7 @@ struct Params {
   const uint64_t* tgts;
   const uint64_t* htab;      // hash index of the target sets (policies too large to stage), or nullptr (wg_check.cu)
   uint64_t n_tgts;           // elements in tgts (v2 stages the whole table in shared memory when it is small)
+  unsigned int* sched;       // this launch's group ticket (wg_check.cu): one word of the engine's ring of kSchedSlots
   unsigned long long* glob;  // [C_WORDS]
   unsigned long long* site;  // [n_sites][4]
   uint32_t n_sites;
