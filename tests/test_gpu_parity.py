@@ -434,3 +434,34 @@ def test_two_engines_on_two_streams_share_no_state():
     assert_counters_equal(eng_b, orc_b)
     eng_a.close()
     eng_b.close()
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two GPUs")
+def test_reloading_an_engine_onto_another_device_moves_everything_it_owns():
+    """a reload onto a different device once freed only the staging buffers, leaving the
+    first-violation record, the ring and the shadow arrays on the old device.  Now the engine is moved whole: tables,
+    record and ring are re-created on the new device, the shadow state is dropped."""
+    st = S.make_stream(4, "cpu", n_events=50_003)
+    orc = oracle_for(st.policy)
+    hdr, val = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64)
+    tag_t = torch.from_numpy(orc.sign(hdr, val).view(np.int64).copy())
+    st.apply_return_tamper(tag_t)
+    orc.reset_counters()
+    orc.set_ring_capacity(4096)
+    eng = B.Engine(0).load(st.policy)
+    eng.wg_set_ring_capacity(4096)
+    eng.wg_shadow_configure(64, 2)
+    d0 = torch.device("cuda", 0)
+    eng.wg_verify_continuations(st.hdr.to(d0), st.val.to(d0), tag_t.to(d0), ENF)
+    eng.device = 1
+    eng.load(st.policy)  # same handle, other device: counters restart
+    d1 = torch.device("cuda", 1)
+    with torch.cuda.device(1):
+        out = eng.wg_verify_continuations(st.hdr.to(d1), st.val.to(d1), tag_t.to(d1), ENF).cpu().numpy().view(np.uint32)
+        assert np.array_equal(out, orc.verify(hdr, st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64), ENF))
+        assert_counters_equal(eng, orc)
+        t, first, ring = eng.wg_read_telemetry(4096)
+        assert first is not None and len(ring) == t["ring_recorded"] > 0
+        with pytest.raises(B.WgError):  # the shadow state did not move: it has to be configured again
+            eng.wg_shadow_read_counters()
+    eng.close()
