@@ -20,7 +20,6 @@ struct wg_engine {
   unsigned int* d_sched = nullptr; // ring of group tickets, one per launch in flight (wg_check.cu)
   uint32_t sched_next = 0;
   uint64_t* d_htab = nullptr;      // hash index of the target sets when the table is too large to stage (wg_check.cu)
-  bool htab_stale = false;         // wg_policy_poke rewrote a target: the sorted sets are searched from then on
   uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
@@ -99,7 +98,6 @@ void free_tables(wg_engine* e) {
   e->d_htab = nullptr;
   cudaFree(e->d_sched);
   e->d_sched = nullptr;
-  e->htab_stale = false;
   cudaFree(e->d_tgts);
   cudaFree(e->d_glob);
   cudaFree(e->d_site);
@@ -150,7 +148,7 @@ wg::Params base_params(const wg_engine* e) {
   std::memset(&p, 0, sizeof(p));
   p.recs = e->d_recs;
   p.tok = e->d_tok;
-  p.htab = e->htab_stale ? nullptr : e->d_htab;
+  p.htab = e->d_htab;
   p.sched = e->d_sched;  // (the check / sign launch sites pick the ring slot)
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
@@ -169,7 +167,9 @@ wg::Params base_params(const wg_engine* e) {
   return p;
 }
 
-constexpr uint64_t kMaxLaunchEvents = 1ull << 27;  // (element indices event * 32 + lane stay below 2^32 inside a launch)
+// element indices event * 32 + lane stay below 2^32 inside a launch, and so does every 32-bit lane count a warp or a CTA
+// keeps (at most 32 lanes per event): strictly fewer than 2^27 events
+constexpr uint64_t kMaxLaunchEvents = (1ull << 27) - 32;
 
 // rec_after: an event the first-violation-record kernel waits for (host path: the record kernel of the previous chunk,
 // which ran on the other staging stream), or nullptr
@@ -489,7 +489,6 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
   e->d_recs = tmp.d_recs;
   e->d_tok = tmp.d_tok;
   e->d_htab = tmp.d_htab;
-  e->htab_stale = false;
   e->d_sched = tmp.d_sched;
   e->d_tgts = tmp.d_tgts;
   e->d_glob = tmp.d_glob;
@@ -758,11 +757,19 @@ wg_status wg_policy_poke(wg_engine* eng, int what, uint64_t index, uint64_t xor_
   if (!g.ok) return cuda_fail(eng, cudaErrorInvalidDevice);
   WG_CUDA(eng, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)));
   void* addr = what == 0 ? static_cast<void*>(eng->d_tgts + index) : static_cast<void*>(eng->d_tok + index);
-  if (what == 0) eng->htab_stale = true;  // the hash index no longer mirrors the sorted sets: search those from now on
   uint64_t v = 0;
   WG_CUDA(eng, cudaMemcpy(&v, addr, 8, cudaMemcpyDeviceToHost));
   v ^= xor_value;
   WG_CUDA(eng, cudaMemcpy(addr, &v, 8, cudaMemcpyHostToDevice));
+  if (what == 0 && eng->d_htab) {
+    // the hash index mirrors the target array: rebuild it from what the array holds now (a diagnostic hook: the cost
+    // of a full rebuild does not matter), including the all-ones flags of the site records
+    const size_t slots = 2 * static_cast<size_t>(eng->n_tgts) + 4 * static_cast<size_t>(eng->n_sites);
+    WG_CUDA(eng, cudaMemset(eng->d_htab, 0xff, slots * 8));
+    WG_CUDA(eng, wg::launch_clear_allones_flags(eng->d_recs, eng->n_sites, nullptr, &eng->launches));
+    WG_CUDA(eng, wg::launch_build_hash(eng->d_htab, eng->d_recs, eng->d_tgts, eng->n_sites, eng->n_tgts, nullptr, &eng->launches));
+    WG_CUDA(eng, cudaStreamSynchronize(nullptr));
+  }
   return WG_OK;
 }
 

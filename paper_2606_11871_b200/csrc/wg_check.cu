@@ -52,6 +52,7 @@ constexpr uint32_t kMaxCacheSlots = 2048;  // slots of the per-site counter cach
 
 // ---- shared-memory carve-up ----------------------------------------------------------------------
 // CTA part: [tgts staged: stage_bytes][per-site counter cache: site_bytes][cnt64: 40 x u64][bykind: 12 x u32][mbar, pad]
+//           [violation counts: 8 x u32][smallest first-violation key: u64, pad]
 // warp part: event records [2 groups][33] x 80 B (record 32 of a group is a dummy that absorbs the padding trips of
 // the producer loop), the work queue (u16 items = record slot * 32 + lane; warp-uniform items from the front, lane-divergent
 // items from the back), and the producer's list of the group's protected events (16 B each)
@@ -77,10 +78,13 @@ constexpr uint32_t kQueueItems = WG_QUEUE;       // one group adds at most 1,024
 constexpr uint32_t kBatch = WG_BATCH;              // row loads in flight per lane in the producer loop
 constexpr uint32_t kListBytes = 40 * 16;           // up to 32 protected events, padded to a multiple of kBatch
 constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 2 + kListBytes;
-constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 16 * 4 + 16;  // cnt64, bykind + rare-event counts + group ticket (u32), mbar
+// kernels that look forward targets up in the hash index (verify / forward, table not staged) add a queue of lookups
+constexpr uint32_t kFwdQueueItems = 512;            // drained when more than 256 wait: 8 trips add at most 256
+constexpr uint32_t kFwdQueueBytes = kFwdQueueItems * 2;
+constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 16 * 4 + 16 + 48;  // cnt64, bykind + rare-event counts (u32), mbar, violation counts (8 x u32), first-violation key
 constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
 constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
-static_assert(kWarps * kWarpBytes + kCtaFixedBytes + 4096 <= kSmemMax, "too many warps for the shared memory");
+static_assert(kWarps * (kWarpBytes + kFwdQueueBytes) + kCtaFixedBytes + 4096 <= kSmemMax, "too many warps for the shared memory");
 
 // ---- PTX helpers ---------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -141,6 +145,44 @@ __device__ __forceinline__ void sts_v2(uint32_t a, uint32_t x, uint32_t y) {
 // one cache line -> L2 (the rows a later group will read; an LSU instruction, no register, no completion to wait for)
 __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
+}
+#ifndef WG_PF
+#define WG_PF 4
+#endif
+#ifndef WG_KEEP
+#define WG_KEEP 1
+#endif
+// one 256-byte row -> L2.  A prefetch pulls 64 bytes (measured: 2 sectors per request), so a row takes four.
+__device__ __forceinline__ void prefetch_row_l2(const void* p) {
+#if WG_PF == 4
+  asm volatile("prefetch.global.L2 [%0];\n\tprefetch.global.L2 [%0+64];\n\tprefetch.global.L2 [%0+128];\n\tprefetch.global.L2 [%0+192];" ::"l"(p) : "memory");
+#elif WG_PF == 1
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], 256;" ::"l"(p) : "memory");
+#else
+  asm volatile("prefetch.global.L2 [%0];\n\tprefetch.global.L2 [%0+128];" ::"l"(p) : "memory");
+#endif
+}
+// L2 policy "evict last" for what every batch of a stream comes back to: site records and per-site counters
+__device__ __forceinline__ uint64_t l2_keep_policy() {
+  uint64_t pol;
+  asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ uint4 ldg_v4_l2keep(const void* p, uint64_t pol) {
+  uint4 r;
+#if WG_KEEP
+  asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(pol));
+#else
+  asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+#endif
+  return r;
+}
+__device__ __forceinline__ void red_add_u64_l2keep(unsigned long long* p, unsigned long long v, uint64_t pol) {
+#if WG_KEEP
+  asm volatile("red.global.add.L2::cache_hint.u64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(pol) : "memory");
+#else
+  atomicAdd(p, v);
+#endif
 }
 __device__ __forceinline__ void atoms_or(uint32_t a, uint32_t x) {
   asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
@@ -263,8 +305,8 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
 // Membership is then ONE 32-byte load in the common case: found if a slot equals v, absent if the bucket has a free
 // slot, else the next bucket.  Exactly the set's membership (R8): the table holds the set's
 // elements and nothing else.  The all-ones word marks a free slot; a set that contains it carries SITE_FLAG_HAS_ALLONES.
-// The metadata-integrity profile authenticates the SORTED record, so it searches that, not the index; after
-// wg_policy_poke has rewritten a target the index is dropped (Params::htab == nullptr) and the sorted sets are searched.
+// The metadata-integrity profile authenticates the SORTED record, so it searches that, not the index; wg_policy_poke
+// rebuilds the index from the rewritten array.
 constexpr uint64_t kFree = ~0ull;
 __host__ __device__ __forceinline__ uint32_t hash_target(uint32_t lo, uint32_t hi) {
   uint32_t h = lo * 0x9e3779b1u ^ (hi + 0x7f4a7c15u) * 0x85ebca6bu;
@@ -273,20 +315,29 @@ __host__ __device__ __forceinline__ uint32_t hash_target(uint32_t lo, uint32_t h
   h ^= h >> 13;
   return h;
 }
-__device__ __forceinline__ bool member_hash(const Params& p, uint32_t site, uint32_t off, uint32_t cnt, uint32_t flags,
-                                            uint32_t vl, uint32_t vh) {
+// the same lookup in two halves, so that a pass can have the first bucket of several lookups in flight at once
+struct HashProbe {
+  const ulonglong2* tab;
+  uint32_t nb, b;
+};
+__device__ __forceinline__ HashProbe hash_probe(const Params& p, uint32_t site, uint32_t off, uint32_t cnt, uint32_t vl,
+                                                uint32_t vh) {
+  HashProbe h;
+  h.nb = (cnt + 1u) >> 1;
+  h.tab = reinterpret_cast<const ulonglong2*>(p.htab + (2ull * off + 4ull * site));
+  h.b = __umulhi(hash_target(vl, vh), h.nb);
+  return h;
+}
+__device__ __forceinline__ bool hash_resolve(HashProbe h, uint32_t flags, uint32_t vl, uint32_t vh, ulonglong2 x, ulonglong2 y) {
   if ((vl & vh) == 0xffffffffu) return (flags & SITE_FLAG_HAS_ALLONES) != 0u;
-  const uint32_t nb = (cnt + 1u) >> 1;
-  const ulonglong2* tab = reinterpret_cast<const ulonglong2*>(p.htab + (2ull * off + 4ull * site));
   const uint64_t v = (static_cast<uint64_t>(vh) << 32) | vl;
-  uint32_t b = __umulhi(hash_target(vl, vh), nb);
-  for (uint32_t i = 0; i < nb; ++i) {  // (terminates earlier: half of the slots are free)
-    const ulonglong2 x = __ldg(tab + 2u * b), y = __ldg(tab + 2u * b + 1u);
+  for (uint32_t i = 1;; ++i) {
     if (x.x == v || x.y == v || y.x == v || y.y == v) return true;
-    if (x.x == kFree || x.y == kFree || y.x == kFree || y.y == kFree) return false;
-    b = b + 1u == nb ? 0u : b + 1u;
+    if (x.x == kFree || x.y == kFree || y.x == kFree || y.y == kFree || i >= h.nb) return false;
+    h.b = h.b + 1u == h.nb ? 0u : h.b + 1u;  // (rare: a full bucket without the value)
+    x = __ldg(h.tab + 2u * h.b);
+    y = __ldg(h.tab + 2u * h.b + 1u);
   }
-  return false;
 }
 
 __device__ __forceinline__ Sip32 init_state(const Params& p) {
@@ -350,10 +401,17 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   unsigned long long* cnt64 = reinterpret_cast<unsigned long long*>(smem_raw + cta_off);
   uint32_t* bykind = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8);
   const uint32_t mbar_cta = smem0 + cta_off + C_WORDS * 8 + 64;
-  const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * kWarpBytes;
+  // violation counts of this CTA (ret lanes, fwd lanes, ret events, fwd events, blocked lanes, blocked events) and its
+  // smallest first-violation key: a stream with 1 % violating events (config 5) sent 7 same-address reductions per
+  // violating group to L2, where they queue behind one another (10 % of the launch, measured); once per CTA instead
+  uint32_t* viol_s = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8 + 80);
+  unsigned long long* key_s = reinterpret_cast<unsigned long long*>(smem_raw + cta_off + C_WORDS * 8 + 112);
+  constexpr bool FQ = MODE != MODE_SIGN && !STAGED;  // forward lookups go through the hash index and its queue
+  const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * (kWarpBytes + (FQ ? kFwdQueueBytes : 0u));
   const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 2 * k
   const uint32_t q_top = q_s + (kQueueItems - 1) * 2;        // divergent items: q_top - 2 * k
   const uint32_t list_s = q_s + kQueueItems * 2;
+  const uint32_t fq_s = list_s + kListBytes;                // forward lookups (FQ): fq_s + 2 * k
   if (lane < 2) {  // the two dummy records: no active lane, nothing to queue
     sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 32, 0u, 0u, 0u, 0u);
     sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 48, 0u, 0u, 0u, 0u);
@@ -363,6 +421,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   const uint32_t tbl_slots = site_bytes / 12u, tbl_mask = tbl_slots - 1u;  // site_s: [slots] owner, [slots][2] counts
   for (uint32_t i = threadIdx.x; i < site_bytes / 4; i += blockDim.x) site_s[i] = i < tbl_slots ? 0xffffffffu : 0u;
   if (threadIdx.x < 12) bykind[threadIdx.x] = 0u;  // 7 by-kind counts, then unknown / empty / misrouted events
+  if (threadIdx.x < 8) viol_s[threadIdx.x] = 0u;
+  if (threadIdx.x == 0) *key_s = ~0ull;
   if (threadIdx.x == 0) mbar_init(mbar_cta, 1);
   __syncthreads();
   if constexpr (STAGED) {
@@ -407,7 +467,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   uint32_t g_nxt = claim();
   const bool enforce = p.mode != 0;
   // large sets: the hash index, unless the metadata-integrity profile wants the authenticated sorted record searched
-  const bool use_hash = !STAGED && p.htab != nullptr && !(TEL && (p.profile & PROFILE_METADATA_INTEGRITY));
+  const bool use_hash = FQ && !(TEL && (p.profile & PROFILE_METADATA_INTEGRITY));
   const Sip32 s_init = init_state(p);
   WarpCtr c = {0, 0, 0, 0};
   uint32_t par = 0;          // which half of the record area this group uses
@@ -489,6 +549,28 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     __syncwarp();
   };
 
+  // ---- forward lookups in the hash index (FQ): 64 queue items, two per lane, so that a lane has the buckets of two
+  //      lookups in flight and the warp waits once per 64 lookups — not once per lane-divergent event plus once for the
+  //      group's warp-uniform targets (config 5: 2.6 waits on DRAM per group, 25 % of the launch).  A target outside its
+  //      set sets the lane's bit in the record's violation word; the event's own lane widens that to the whole active
+  //      mask for a warp-uniform target afterwards. ----
+  auto fpass = [&](uint32_t k0, uint32_t n) __attribute__((always_inline)) {
+    if constexpr (FQ) {
+      const uint32_t ka = k0 + lane < n ? k0 + lane : k0, kb = k0 + 32u + lane < n ? k0 + 32u + lane : k0;
+      const uint32_t ia = lds_u16(fq_s + ka * 2u), ib = lds_u16(fq_s + kb * 2u);  // (past the end: item k0 once more)
+      const uint32_t ra = mad32(ia >> 5, kRecBytes, rec_s), rb = mad32(ib >> 5, kRecBytes, rec_s);
+      const uint2 wa = lds_v2(ra + 72), wb = lds_v2(rb + 72);  // biased value row pointers
+      const uint2 va = ldg_v2_keep(item_ptr(wa.x, wa.y, ia)), vb = ldg_v2_keep(item_ptr(wb.x, wb.y, ib));
+      const uint4 fa = lds_v4(ra), fb = lds_v4(rb);            // offset, count, flags of the events' sets
+      const HashProbe ha = hash_probe(p, lds_u32(ra + 68), fa.x, fa.y, va.x, va.y);
+      const HashProbe hb = hash_probe(p, lds_u32(rb + 68), fb.x, fb.y, vb.x, vb.y);
+      const ulonglong2 xa = __ldg(ha.tab + 2u * ha.b), ya = __ldg(ha.tab + 2u * ha.b + 1u);
+      const ulonglong2 xb = __ldg(hb.tab + 2u * hb.b), yb = __ldg(hb.tab + 2u * hb.b + 1u);
+      if (!hash_resolve(ha, fa.z, va.x, va.y, xa, ya)) atoms_or(ra + 56, 1u << (ia & 31u));
+      if (!hash_resolve(hb, fb.z, vb.x, vb.y, xb, yb)) atoms_or(rb + 56, 1u << (ib & 31u));
+    }
+  };
+
   // ---- event-parallel epilogue of a finished group: verdicts (a6), violation counters (a7), first violation (a8) ----
   auto epilogue = [&](uint32_t rpar, uint32_t e0) __attribute__((always_inline)) {
     if constexpr (MODE != MODE_SIGN) {
@@ -517,16 +599,16 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           const unsigned long long o = __shfl_xor_sync(kFull, key, d);
           key = o < key ? o : key;
         }
-        if (lane == 0) {
-          if (rv) atomicAdd(p.glob + C_RET_VIOL, static_cast<unsigned long long>(rv));
-          if (fv) atomicAdd(p.glob + C_FWD_VIOL, static_cast<unsigned long long>(fv));
-          if (rve) atomicAdd(p.glob + C_RET_VIOL_EVENTS, static_cast<unsigned long long>(rve));
-          if (fve) atomicAdd(p.glob + C_FWD_VIOL_EVENTS, static_cast<unsigned long long>(fve));
+        if (lane == 0) {  // (32-bit shared-memory atomics; a launch has fewer than 2^27 events, so no count wraps)
+          if (rv) atomicAdd(&viol_s[0], rv);
+          if (fv) atomicAdd(&viol_s[1], fv);
+          if (rve) atomicAdd(&viol_s[2], rve);
+          if (fve) atomicAdd(&viol_s[3], fve);
           if (enforce) {
-            atomicAdd(p.glob + C_BLOCKED_LANES, static_cast<unsigned long long>(av));
-            atomicAdd(p.glob + C_BLOCKED_EVENTS, static_cast<unsigned long long>(ave));
+            atomicAdd(&viol_s[4], av);
+            atomicAdd(&viol_s[5], ave);
           }
-          atomicMin(p.glob + C_FIRST_VIOLATION, key);
+          if (key < *reinterpret_cast<volatile unsigned long long*>(key_s)) atomicMin(key_s, key);  // (settles quickly)
         }
         if (TEL && viol && !(p.profile & PROFILE_LOW_TELEMETRY) && p.ring_cap != 0) {
           // violation ring (R27, R28): diagnostic, bounded; a full ring drops and counts
@@ -562,7 +644,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     return (g < n_groups && e < n_ev) ? ldg_v4(p.hdr + e) : make_uint4(0xffffffffu, 0u, 0u, 0u);
   };
   auto load_rec = [&](const uint4& h) __attribute__((always_inline)) -> uint4 {
-    return h.x < p.n_sites ? ldg_v4(p.recs + h.x) : make_uint4(7u, 0u, 0u, 0u);
+    return h.x < p.n_sites ? ldg_v4_l2keep(p.recs + h.x, l2_keep_policy()) : make_uint4(7u, 0u, 0u, 0u);
   };
   uint4 h_cur = load_hdr(gi);
   uint4 h_nxt = load_hdr(g_nxt);
@@ -630,6 +712,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     }
     sts_v4(ra_me + 48, active, cls == CLS_RET ? active : 0u, viol, 0u);
     sts_v2(ra_me + 64, cls | (kind << 4), site);
+    if (FQ && cls == CLS_FWD) sts_v4(ra_me, off, cnt, r_cur.w, 0u);  // the set a queued lookup searches
 
     // ---- the producer's list of the group's protected events (event-parallel), padded to a multiple of kBatch with
     //      trips on the group's dummy record (no active lane: nothing is queued, nothing counted), so that a batch is
@@ -638,7 +721,9 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     const uint32_t n_need = __popc(need);
     if (need != 0u) {
       const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
-      if (need & lanebit) sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * 32u, first);
+      // (bit 5 of the last word: a forward event; the shuffle that takes this word as its source lane reads bits 0-4)
+      if (need & lanebit)
+        sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * 32u, first | ((FQ && cls == CLS_FWD) ? 32u : 0u));
       if (lane < ((kBatch - n_need) & (kBatch - 1u)))
         sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * 32u, 0u);
     }
@@ -717,8 +802,8 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         }
         if (!cached) {  // one reduction per event straight to L2
           unsigned long long* sc = p.site + static_cast<uint64_t>(site) * 4;
-          atomicAdd(sc + S_EVENTS, 1ull);
-          if (judged_na) atomicAdd(sc + S_LANES_CHECKED, static_cast<unsigned long long>(judged_na));
+          red_add_u64_l2keep(sc + S_EVENTS, 1ull, l2_keep_policy());
+          if (judged_na) red_add_u64_l2keep(sc + S_LANES_CHECKED, static_cast<unsigned long long>(judged_na), l2_keep_policy());
         }
       }
     }
@@ -728,6 +813,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     //      next batch's rows are requested before this batch is looked at. ----
     if (need != 0u) {
       uint32_t qu = q_s + nu * 2u, qd = q_top - nd * 2u;  // where the next uniform / divergent item goes
+      uint32_t qf = fq_s;                                  // ... and the next forward lookup
       auto consume_batch = [&](const uint2 (&v)[kBatch], uint32_t b0) {
 #pragma unroll
         for (int j = 0; j < static_cast<int>(kBatch); ++j) {
@@ -737,6 +823,13 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
           uint32_t diff, div_;
           and_test(__ballot_sync(kFull, v[j].x != rx || v[j].y != ry), am.x, diff, div_);
           sts_u32(le.x + 60, diff);  // (every lane stores the same word)
+          if (FQ && use_hash && (le.w & 32u)) {
+            // a forward event: one lookup for a warp-uniform target (the first active lane's), else one per active lane
+            const uint32_t fm = div_ != 0u ? am.x : (1u << (le.w & 31u));
+            if (fm & lanebit) sts_u16(mad32(__popc(fm & ltmask), 2u, qf), le.z + lane);
+            qf = mad32(__popc(fm), 2u, qf);
+            continue;
+          }
           if (MODE == MODE_FORWARD || m_ret == 0u) continue;  // a group without return checks has nothing to queue
           const uint32_t rank = __popc(am.y & ltmask), nae = __popc(am.y);
           const bool div = div_ != 0u, act = (am.y & lanebit) != 0u;
@@ -749,7 +842,21 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         }
       };
 #pragma unroll 1
-      for (uint32_t b0 = 0; b0 < n_need; b0 += 2u * kBatch) {
+      for (uint32_t b0 = 0;; b0 += 2u * kBatch) {
+        const bool done = b0 >= n_need;
+        if (FQ && use_hash) {
+          // the queued forward lookups: all of them once the group's events are through, or when the next two batches
+          // might not fit (one copy of this code: it sits at the loop head, which the last, empty trip also reaches)
+          const uint32_t nf = (qf - fq_s) >> 1;
+          if (nf != 0u && (done || nf > kFwdQueueItems - 2u * kBatch * 32u)) {
+            __syncwarp();
+#pragma unroll 1
+            for (uint32_t k = 0; k < nf; k += 64u) fpass(k, nf);
+            qf = fq_s;
+            __syncwarp();
+          }
+        }
+        if (done) break;
         const bool more = b0 + kBatch < n_need;
         if (more) load_batch(vb, b0 + kBatch);
         consume_batch(va, b0);
@@ -782,7 +889,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       const bool judged = cls == CLS_RET || cls == CLS_FWD;
       const bool is_uni = judged && lds_u32(ra_me + 60) == 0u;
       uint32_t ul = 0, uh = 0;
-      if (is_uni) {
+      if (is_uni && !(use_hash && cls == CLS_FWD)) {
         const uint2 r = ldg_v2_keep(elem_ptr(p.val, (e0 + lane) * 32u + first));  // the event's one value (an L1 hit)
         ul = r.x;
         uh = r.y;
@@ -830,26 +937,29 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         // lane-divergent forward targets are searched per lane, one event at a time (per-warp checking
         // only after proving uniformity); a warp-uniform target is searched once, by the event's lane
         uint32_t fviol = 0;
-        for (uint32_t m = __ballot_sync(kFull, cls == CLS_FWD && !is_uni && !bad_rec); m; m &= m - 1) {
-          const uint32_t e = __ffs(m) - 1;
-          const uint32_t a = __shfl_sync(kFull, active, e);
-          const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
-          const uint2 v = ldg_v2_keep(elem_ptr(p.val, (e0 + e) * 32u + lane));
-          bool in;
-          if (!STAGED && use_hash)
-            in = member_hash(p, __shfl_sync(kFull, site, e), o2, c2, __shfl_sync(kFull, r_cur.w, e), v.x, v.y);
-          else
-            in = member<STAGED>(p, tg_s, o2, c2, v.x, v.y);
-          const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !in);
-          if (lane == e) fviol = vb;
-        }
-        if (cls == CLS_FWD) {
-          if (bad_rec)
-            fviol = active;
-          else if (is_uni)
-            fviol = ((!STAGED && use_hash) ? member_hash(p, site, off, cnt, r_cur.w, ul, uh)
-                                           : member<STAGED>(p, tg_s, off, cnt, ul, uh)) ? 0u : active;
-          sts_u32(ra_me + 56, fviol);
+        if (use_hash) {
+          // the lookups went through the queue; a warp-uniform target outside the set fails every active lane
+          if (cls == CLS_FWD) {
+            const uint32_t v = lds_u32(ra_me + 56);
+            sts_u32(ra_me + 56, is_uni ? (v != 0u ? active : 0u) : v);
+          }
+        } else {
+          for (uint32_t m = __ballot_sync(kFull, cls == CLS_FWD && !is_uni && !bad_rec); m; m &= m - 1) {
+            const uint32_t e = __ffs(m) - 1;
+            const uint32_t a = __shfl_sync(kFull, active, e);
+            const uint32_t o2 = __shfl_sync(kFull, off, e), c2 = __shfl_sync(kFull, cnt, e);
+            const uint2 v = ldg_v2_keep(elem_ptr(p.val, (e0 + e) * 32u + lane));
+            const bool in = member<STAGED>(p, tg_s, o2, c2, v.x, v.y);
+            const uint32_t vb = __ballot_sync(kFull, (a & lanebit) && !in);
+            if (lane == e) fviol = vb;
+          }
+          if (cls == CLS_FWD) {
+            if (bad_rec)
+              fviol = active;
+            else if (is_uni)
+              fviol = member<STAGED>(p, tg_s, off, cnt, ul, uh) ? 0u : active;
+            sts_u32(ra_me + 56, fviol);
+          }
         }
       }
     }
@@ -860,13 +970,11 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
       const bool ret_nxt = v_nxt && r_nxt.x == K_RET, fwd_nxt = v_nxt && r_nxt.x == K_FWD;
       const char* vr = reinterpret_cast<const char*>(elem_ptr(p.val, (gn * 32u + lane) * 32u));
       if (MODE == MODE_FORWARD ? fwd_nxt : (MODE == MODE_SIGN ? ret_nxt : (ret_nxt || fwd_nxt))) {
-        prefetch_l2(vr);
-        prefetch_l2(vr + 128);
+        prefetch_row_l2(vr);
       }
       if (MODE == MODE_VERIFY && ret_nxt) {
         const char* tr = reinterpret_cast<const char*>(elem_ptr(p.tag, (gn * 32u + lane) * 32u));
-        prefetch_l2(tr);
-        prefetch_l2(tr + 128);
+        prefetch_row_l2(tr);
       }
     }
     __syncwarp();
@@ -907,8 +1015,15 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     if (threadIdx.x == C_EVENTS_UNKNOWN) v = bykind[8 + 0];
     if (threadIdx.x == C_EVENTS_EMPTY) v = bykind[8 + 1];
     if (threadIdx.x == C_EVENTS_MISROUTED) v = bykind[8 + 2];
+    if (threadIdx.x == C_RET_VIOL) v = viol_s[0];
+    if (threadIdx.x == C_FWD_VIOL) v = viol_s[1];
+    if (threadIdx.x == C_RET_VIOL_EVENTS) v = viol_s[2];
+    if (threadIdx.x == C_FWD_VIOL_EVENTS) v = viol_s[3];
+    if (threadIdx.x == C_BLOCKED_LANES) v = viol_s[4];
+    if (threadIdx.x == C_BLOCKED_EVENTS) v = viol_s[5];
     if (v) atomicAdd(p.glob + threadIdx.x, v);
   }
+  if (MODE != MODE_SIGN && threadIdx.x == 0 && *key_s != ~0ull) atomicMin(p.glob + C_FIRST_VIOLATION, *key_s);
   for (uint32_t i = threadIdx.x; i < tbl_slots; i += blockDim.x) {  // the cached sites' counts, once per CTA
     const uint32_t owner = site_s[i];
     if (owner != 0xffffffffu) {
@@ -968,7 +1083,7 @@ __global__ void wg_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64
 
 // hash index build (load time): one thread per target finds its site (binary search over the records' offsets) and
 // claims the first free slot of its probe sequence
-__global__ void wg_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts) {
+__global__ void wg_build_hash(uint64_t* htab, SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts) {
   const uint64_t i = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (i >= n_tgts) return;
   uint32_t lo = 0, len = n_sites;  // last site with off <= i that owns targets: sites without targets share offsets
@@ -980,7 +1095,10 @@ __global__ void wg_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_
   while (recs[lo].cnt == 0u || recs[lo].off + recs[lo].cnt <= i) --lo;  // (step back over empty sites at the same offset)
   const SiteRec r = recs[lo];
   const uint64_t v = tgts[i];
-  if (v == kFree) return;  // carried by SITE_FLAG_HAS_ALLONES
+  if (v == kFree) {  // the free-slot marker cannot be stored: the site's record carries a flag instead
+    atomicOr(&recs[lo].flags, SITE_FLAG_HAS_ALLONES);
+    return;
+  }
   const uint32_t nb = (r.cnt + 1u) >> 1;
   unsigned long long* tab = reinterpret_cast<unsigned long long*>(htab + (2ull * r.off + 4ull * lo));
   uint32_t b = __umulhi(hash_target(static_cast<uint32_t>(v), static_cast<uint32_t>(v >> 32)), nb);
@@ -993,7 +1111,12 @@ __global__ void wg_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_
 
 __global__ void wg_set_site_flags(SiteRec* recs, const uint8_t* skip, uint32_t n_sites) {
   const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
-  if (s < n_sites) recs[s].flags = (skip && skip[s]) ? SITE_FLAG_SKIP : 0u;
+  if (s < n_sites) recs[s].flags = (recs[s].flags & ~SITE_FLAG_SKIP) | ((skip && skip[s]) ? SITE_FLAG_SKIP : 0u);
+}
+
+__global__ void wg_clear_allones_flags(SiteRec* recs, uint32_t n_sites) {
+  const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < n_sites) recs[s].flags &= ~SITE_FLAG_HAS_ALLONES;
 }
 
 template <int MODE>
@@ -1005,13 +1128,15 @@ cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t
   const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
   // the per-site counter cache: the largest power-of-two slot count <= kMaxCacheSlots that fits beside the staged
   // targets (and no more than twice the policy needs); sign keeps no per-site counters
+  const uint32_t warp_bytes = kWarpBytes + ((MODE != MODE_SIGN && !staged) ? kFwdQueueBytes : 0u);  // (the kernel's FQ)
   uint32_t site_bytes = 0;
   if (MODE != MODE_SIGN && p.n_sites > 0) {
+    const uint32_t left = kSmemMax - kCtaFixedBytes - kWarps * warp_bytes;
     uint32_t slots = kMaxCacheSlots;
-    while (slots >= 64u && (stage_bytes + slots * 12u > kLeft || slots / 2u >= p.n_sites)) slots /= 2u;
+    while (slots >= 64u && (stage_bytes + slots * 12u > left || slots / 2u >= p.n_sites)) slots /= 2u;
     if (slots >= 64u) site_bytes = slots * 12u;
   }
-  const uint32_t smem = stage_bytes + site_bytes + kCtaFixedBytes + kWarps * kWarpBytes;
+  const uint32_t smem = stage_bytes + site_bytes + kCtaFixedBytes + kWarps * warp_bytes;
   const bool tel = MODE != MODE_SIGN && (p.profile != 0 || p.ring_cap != 0);
   {  // the launch's group ticket starts at 0
     const cudaError_t e = cudaMemsetAsync(p.sched, 0, sizeof(unsigned int), st);
@@ -1070,7 +1195,14 @@ cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* laun
   return cudaGetLastError();
 }
 
-cudaError_t launch_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts,
+cudaError_t launch_clear_allones_flags(SiteRec* recs, uint32_t n_sites, cudaStream_t st, uint64_t* launches) {
+  if (n_sites == 0) return cudaSuccess;
+  wg_clear_allones_flags<<<(n_sites + 255) / 256, 256, 0, st>>>(recs, n_sites);
+  ++*launches;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_build_hash(uint64_t* htab, SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts,
                               cudaStream_t st, uint64_t* launches) {
   if (n_tgts == 0) return cudaSuccess;
   wg_build_hash<<<static_cast<unsigned>((n_tgts + 255) / 256), 256, 0, st>>>(htab, recs, tgts, n_sites, n_tgts);

@@ -139,8 +139,9 @@ cudaError_t launch_build_tokens(uint64_t* tok, const SiteRec* recs, const uint64
 // SiteRec.flags bit 0 <- d_skip[site] != 0 (d_skip == nullptr: cleared), the coverage-reduced profile's skip set (R40)
 cudaError_t launch_set_site_flags(SiteRec* recs, const uint8_t* d_skip, uint32_t n_sites, cudaStream_t st, uint64_t* launches);
 // hash index of large target sets: htab has 2 * n_tgts + 4 * n_sites slots, pre-filled with all-ones (wg_check.cu)
-cudaError_t launch_build_hash(uint64_t* htab, const SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts,
+cudaError_t launch_build_hash(uint64_t* htab, SiteRec* recs, const uint64_t* tgts, uint32_t n_sites, uint64_t n_tgts,
                               cudaStream_t st, uint64_t* launches);
+cudaError_t launch_clear_allones_flags(SiteRec* recs, uint32_t n_sites, cudaStream_t st, uint64_t* launches);
 uint64_t max_staged_targets();  // larger tables are searched in global memory (and get the hash index)
 cudaError_t init_kernels();  // one-time function attributes (dynamic shared memory opt-in) on the current device
 
