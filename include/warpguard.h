@@ -52,7 +52,8 @@ typedef enum {
   WG_ERR_NO_POLICY = 3,   /* engine handle is NULL or holds no policy                                */
   WG_ERR_CUDA = 4,        /* a CUDA runtime call failed (wg_last_cuda_error gives the code)          */
   WG_ERR_OOM = 5,         /* host or device allocation failed                                        */
-  WG_ERR_INTERNAL = 6     /* an engine invariant does not hold (a bug): nothing returned may be trusted      */
+  WG_ERR_INTERNAL = 6,    /* an engine invariant does not hold (a bug): nothing returned may be trusted      */
+  WG_ERR_STATIC_LIMIT = 7 /* wg_verify_continuations_static: more sites or events than its static scratch holds */
 } wg_status;
 
 /* Site outcome kinds: PAPER.md:145-154 (Table 2), "protected" split by edge direction. */
@@ -309,6 +310,34 @@ wg_status wg_verify_continuations_host(wg_engine* eng, const wg_event_hdr* h_hdr
                                        const uint64_t* h_tag, wg_verdict* h_out, uint64_t n, wg_mode mode);
 wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const uint64_t* h_val,
                                 wg_verdict* h_out, uint64_t n, wg_mode mode);
+
+/* ---- allocation-free verify ----
+ * For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * wg_verify_continuations (same dispatch, same verdicts) with the kernel's scratch memory —
+ * the launch's group ticket, the counter words it adds into, the first-violation key, the per-site counters — in ONE
+ * static device array of the library (2,098,176 bytes, held by every GPU that loads the library until the process
+ * exits) instead of the engine's allocations.  The call performs no cudaMalloc / cudaFree and no allocating library
+ * call: memsets, one kernel launch and device-to-device copies, all on `cuda_stream`, nothing synchronous.  The first
+ * call on a device also resolves the array's address (cudaGetSymbolAddress: no allocation, but make that call outside
+ * graph capture).
+ *   STATELESS: the engine's cumulative counters, event sequence (R12), violation ring and first-violation record
+ *   are neither read nor changed.  The counters of THIS call alone are returned:
+ *   d_counters  DEVICE pointer, out (may be NULL): wg_counters of this call; first_violation_key numbers events from
+ *               this call's first event (seq = index into d_hdr); policy_digest and last_mode are 0 in this copy.
+ *   d_per_site  DEVICE pointer, out (may be NULL): [n_sites] wg_site_counters of this call.
+ *   d_hdr / d_val / d_tag / d_out: as wg_verify_continuations (DEVICE, caller-owned).  The engine's profile flags apply.
+ *   n == 0 writes zero counters (key UINT64_MAX) and launches nothing.
+ * Limits: the loaded policy has at most WG_STATIC_MAX_SITES sites and n <= WG_STATIC_MAX_EVENTS (one launch), else
+ * WG_ERR_STATIC_LIMIT and nothing is written.  Other errors as wg_verify_continuations.
+ * SHARED: every call, of every engine and every thread, uses the same array on a device, and the array keeps the last
+ * call's contents (each call clears what it needs).  Two calls that overlap on the GPU (different streams, or the same
+ * graph launched twice concurrently) race on it: order them on one stream.  d_counters / d_per_site are valid once the
+ * stream reaches the end of the call's work. */
+#define WG_STATIC_MAX_SITES 65536u
+#define WG_STATIC_MAX_EVENTS 134217696ull /* 2^27 - 32 */
+wg_status wg_verify_continuations_static(wg_engine* eng, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                                         const uint64_t* d_tag, wg_verdict* d_out, wg_counters* d_counters,
+                                         wg_site_counters* d_per_site, uint64_t n, wg_mode mode, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -19,6 +19,8 @@ _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libwarpguard.so"
 
 WG_OK, WG_ERR_INVALID_ARG, WG_ERR_BAD_POLICY, WG_ERR_NO_POLICY, WG_ERR_CUDA, WG_ERR_OOM, WG_ERR_INTERNAL = range(7)
+WG_ERR_STATIC_LIMIT = 7
+WG_STATIC_MAX_SITES, WG_STATIC_MAX_EVENTS = 65536, (1 << 27) - 32  # wg_verify_continuations_static
 WG_MODE_DETECT, WG_MODE_ENFORCE = 0, 1
 
 EXPORTS = [
@@ -28,7 +30,7 @@ EXPORTS = [
     "wg_set_profile", "wg_set_ring_capacity", "wg_read_telemetry",
     "wg_shadow_configure", "wg_shadow_push", "wg_shadow_check_ret", "wg_shadow_read_counters", "wg_shadow_poke",
     "wg_shadow_depth", "wg_policy_poke", "wg_get_device_view", "wg_policy_digest",
-    "wg_load_policy_bound",
+    "wg_load_policy_bound", "wg_verify_continuations_static",
 ]
 
 
@@ -113,6 +115,7 @@ def lib() -> C.CDLL:
         L.wg_get_device_view.argtypes = [vp, C.POINTER(DeviceView)]
         L.wg_set_ring_capacity.argtypes = [vp, u64, vp]
         L.wg_read_telemetry.argtypes = [vp, vp, vp, C.POINTER(C.c_int), vp, u64, C.POINTER(u64), vp]
+        L.wg_verify_continuations_static.argtypes = [vp, vp, vp, vp, vp, vp, vp, u64, i, vp]
         for name in EXPORTS:
             if name not in ("wg_destroy", "wg_strerror"):
                 getattr(L, name).restype = i
@@ -203,6 +206,37 @@ class Engine:
                                            _dev(tag, "tag", 32, 8), _dev(out, "out", 2, 4), n, int(mode),
                                            _stream_ptr(stream)), "wg_verify_continuations")
         return out
+
+    def wg_verify_continuations_static(self, hdr, val, tag, mode: int, out=None, counters=None, per_site=None,
+                                       stream=None):
+        """The allocation-free verify (warpguard.h): scratch in the library's static device array, stateless.
+        out [n, 2] int32, counters [26] int64, per_site [n_sites, 4] int64: CUDA tensors the CALLER passes (the library
+        allocates nothing; tensors left out are made here, by torch).  Returns (out, counters, per_site); all three are
+        valid once `stream` has passed the call's work — counter_dict() synchronises and decodes."""
+        n = hdr.shape[0]
+        dev = hdr.device
+        if out is None:
+            out = torch.empty((n, 2), dtype=torch.int32, device=dev)
+        if counters is None:
+            counters = torch.empty(26, dtype=torch.int64, device=dev)
+        if per_site is None:
+            per_site = torch.empty((self.n_sites, 4), dtype=torch.int64, device=dev)
+        if not (counters.is_cuda and counters.is_contiguous() and counters.numel() == 26 and counters.element_size() == 8):
+            raise ValueError("counters: expected a contiguous CUDA tensor of 26 8-byte words")
+        if not (per_site.is_cuda and per_site.is_contiguous() and tuple(per_site.shape) == (self.n_sites, 4)
+                and per_site.element_size() == 8):
+            raise ValueError(f"per_site: expected a contiguous CUDA [{self.n_sites}, 4] tensor of 8-byte words")
+        _chk(lib().wg_verify_continuations_static(
+            self._h, _dev(hdr, "hdr", 2, 8), _dev(val, "val", 32, 8), _dev(tag, "tag", 32, 8), _dev(out, "out", 2, 4),
+            C.c_void_p(counters.data_ptr()), C.c_void_p(per_site.data_ptr() if self.n_sites else None), n, int(mode),
+            _stream_ptr(stream)), "wg_verify_continuations_static")
+        return out, counters, per_site
+
+    @staticmethod
+    def counter_dict(counters: torch.Tensor) -> dict:
+        """Decodes the 26 words wg_verify_continuations_static wrote (synchronises through the copy to the host)."""
+        g = counters.cpu().numpy().view(np.uint64)
+        return {k: int(v) for k, v in zip(COUNTER_FIELDS, g)}
 
     def wg_check_forward(self, hdr, val, mode: int, out=None, stream=None) -> torch.Tensor:
         n = hdr.shape[0]

@@ -585,6 +585,7 @@ const char* wg_strerror(wg_status s) {
     case WG_ERR_CUDA: return "CUDA runtime error (no device or call failed)";
     case WG_ERR_OOM: return "out of memory";
     case WG_ERR_INTERNAL: return "engine invariant violated";
+    case WG_ERR_STATIC_LIMIT: return "beyond the limits of the allocation-free entry point (WG_STATIC_MAX_SITES / WG_STATIC_MAX_EVENTS)";
   }
   return "unknown status";
 }
@@ -847,3 +848,91 @@ wg_status wg_check_forward_host(wg_engine* eng, const wg_event_hdr* h_hdr, const
 }
 
 }  // extern "C"
+
+// ---- wg_verify_continuations_static: the verify kernel with its scratch memory in a static device array ------------
+// The check kernel's scratch memory — the launch's group ticket, the global counter words it adds into (with the
+// first-violation key) and the per-site counters — normally lives in cudaMalloc'ed arrays the engine owns and
+// accumulates over calls.  Here it lives in ONE file-scope device array of the library: the call allocates nothing
+// (no cudaMalloc / cudaFree, no allocating library routine; only memsets, the launch and device-to-device copies on
+// the caller's stream), and it leaves the engine's own counters, sequence numbers, ring and first-violation record
+// untouched.  Every GPU that loads the library holds the array (2,098,176 bytes) until the process exits.
+namespace {
+
+constexpr uint32_t kStaticMaxSites = WG_STATIC_MAX_SITES;
+struct StaticScratch {
+  unsigned int ticket[64];                               // the launch's group ticket (256 bytes: its own cache lines)
+  unsigned long long glob[64];                           // C_WORDS global counter words, padded
+  unsigned long long site[4ull * kStaticMaxSites];       // [n_sites][4] per-site counters
+};
+static_assert(wg::C_WORDS <= 64, "global counter words");
+static_assert(sizeof(StaticScratch) == 256 + 512 + 32ull * kStaticMaxSites, "static scratch layout");
+static_assert(WG_STATIC_MAX_EVENTS == kMaxLaunchEvents, "one launch");
+
+// In host code this name is a host-side stand-in for the array, NOT its device address: the address is resolved once
+// per device with cudaGetSymbolAddress (that device current) and it is that pointer the kernel is given.
+static __device__ __align__(256) unsigned char wg_static_scratch[sizeof(StaticScratch)];
+
+constexpr int kStaticMaxDevices = 64;
+StaticScratch* g_static_ptr[kStaticMaxDevices] = {};
+
+// the calling thread's current device must be `device` (the caller holds a DeviceGuard)
+cudaError_t static_scratch_for(int device, StaticScratch** out) {
+  if (device < 0 || device >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+  StaticScratch* ptr = __atomic_load_n(&g_static_ptr[device], __ATOMIC_ACQUIRE);
+  if (!ptr) {
+    void* a = nullptr;
+    const cudaError_t err = cudaGetSymbolAddress(&a, wg_static_scratch);
+    if (err != cudaSuccess) return err;
+    if (!a) return cudaErrorInvalidSymbol;
+    ptr = static_cast<StaticScratch*>(a);
+    __atomic_store_n(&g_static_ptr[device], ptr, __ATOMIC_RELEASE);  // (two threads resolve the same address)
+  }
+  *out = ptr;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" wg_status wg_verify_continuations_static(wg_engine* e, const wg_event_hdr* d_hdr, const uint64_t* d_val,
+                                                    const uint64_t* d_tag, wg_verdict* d_out, wg_counters* d_counters,
+                                                    wg_site_counters* d_per_site, uint64_t n, wg_mode mode,
+                                                    void* cuda_stream) {
+  if (!e || !e->loaded) return WG_ERR_NO_POLICY;
+  if (mode != WG_MODE_DETECT && mode != WG_MODE_ENFORCE) return WG_ERR_INVALID_ARG;
+  if (e->n_sites > kStaticMaxSites || n > WG_STATIC_MAX_EVENTS) return WG_ERR_STATIC_LIMIT;
+  if (n != 0 && (!d_hdr || !d_val || !d_tag || !d_out)) return WG_ERR_INVALID_ARG;
+  if (!aligned(d_hdr, 16) || !aligned(d_val, 16) || !aligned(d_tag, 16) || !aligned(d_out, 8) ||
+      !aligned(d_counters, 8) || !aligned(d_per_site, 8))
+    return WG_ERR_INVALID_ARG;
+  DeviceGuard g(e->device);
+  if (!g.ok) return cuda_fail(e, cudaErrorInvalidDevice);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  StaticScratch* sc = nullptr;
+  WG_CUDA(e, static_scratch_for(e->device, &sc));
+  // the array keeps the last call's contents: everything the kernel adds into starts at zero (the key at all-ones)
+  WG_CUDA(e, cudaMemsetAsync(sc->glob, 0, sizeof(sc->glob), st));
+  WG_CUDA(e, cudaMemsetAsync(sc->glob + wg::C_FIRST_VIOLATION, 0xff, sizeof(unsigned long long), st));
+  if (e->n_sites) WG_CUDA(e, cudaMemsetAsync(sc->site, 0, sizeof(unsigned long long) * 4 * e->n_sites, st));
+  if (n != 0) {
+    wg::Params p = base_params(e);
+    p.hdr = reinterpret_cast<const uint4*>(d_hdr);
+    p.val = d_val;
+    p.tag = d_tag;
+    p.out = reinterpret_cast<uint2*>(d_out);
+    p.n = n;
+    p.seq_base = 0;  // the call's own event numbering: first_violation_key counts from this call's first event
+    p.mode = static_cast<uint32_t>(mode);
+    p.sched = sc->ticket;  // (zeroed by the launcher)
+    p.glob = sc->glob;
+    p.site = sc->site;
+    p.ring = nullptr;  // no violation ring, no first-violation record: diagnostics of the engine's own calls
+    p.ring_cap = 0;
+    p.first = nullptr;
+    WG_CUDA(e, wg::launch_check(p, e->sm_count, st, &e->launches));
+  }
+  static_assert(sizeof(wg_counters) == 26 * 8 && sizeof(wg_site_counters) == 32, "counter layouts");
+  if (d_counters) WG_CUDA(e, cudaMemcpyAsync(d_counters, sc->glob, sizeof(wg_counters), cudaMemcpyDeviceToDevice, st));
+  if (d_per_site && e->n_sites)
+    WG_CUDA(e, cudaMemcpyAsync(d_per_site, sc->site, sizeof(wg_site_counters) * e->n_sites, cudaMemcpyDeviceToDevice, st));
+  return WG_OK;
+}
