@@ -309,8 +309,10 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
 // A binary search over a set in L2 / HBM is up to 12 DEPENDENT loads (7 with quaternary steps): on config 5 (sets up to
 // 4,096 entries) the check kernel spent most of its time waiting on them (ALU pipe 48 % busy).  At load time the engine
 // therefore builds, per forward site, an open-addressing hash table of the site's targets in its own memory:
-//   slots of site s: htab[2 * off(s) + 4 * s ...), 4 * nb(s) of them, nb(s) = ceil(cnt(s) / 2) buckets of 4 slots (one
-//   32-byte sector): load factor <= 1/2, tables derived from the site record alone, no extra field;
+//   slots of site s: htab[(2 * off(s) + 4 * s + 2) & ~3 ...), 4 * nb(s) of them, nb(s) = ceil(cnt(s) / 2) buckets of 4
+//   slots: load factor <= 1/2, tables derived from the site record alone, no extra field; the rounding makes every
+//   bucket ONE aligned 32-byte sector (without it the buckets of a site with an odd offset straddled two sectors, often
+//   in two DRAM bursts: measured 105 bytes of DRAM traffic per lookup on config 5) and still fits the 2 T + 4 S slots;
 //   a target goes to the first free slot of bucket b = mulhi(hash(v), nb), b + 1, ... (linear probing by bucket).
 // Membership is then ONE 32-byte load in the common case: found if a slot equals v, absent if the bucket has a free
 // slot, else the next bucket.  Exactly the set's membership (R8): the table holds the set's
@@ -318,6 +320,9 @@ __device__ __forceinline__ bool member(const Params& p, uint32_t tg_s, uint32_t 
 // The metadata-integrity profile authenticates the SORTED record, so it searches that, not the index; wg_policy_poke
 // rebuilds the index from the rewritten array.
 constexpr uint64_t kFree = ~0ull;
+__host__ __device__ __forceinline__ uint64_t hash_base(uint32_t site, uint32_t off) {
+  return (2ull * off + 4ull * site + 2ull) & ~3ull;
+}
 __host__ __device__ __forceinline__ uint32_t hash_target(uint32_t lo, uint32_t hi) {
   uint32_t h = lo * 0x9e3779b1u ^ (hi + 0x7f4a7c15u) * 0x85ebca6bu;
   h ^= h >> 15;
@@ -334,7 +339,7 @@ __device__ __forceinline__ HashProbe hash_probe(const Params& p, uint32_t site, 
                                                 uint32_t vh) {
   HashProbe h;
   h.nb = (cnt + 1u) >> 1;
-  h.tab = reinterpret_cast<const ulonglong2*>(p.htab + (2ull * off + 4ull * site));
+  h.tab = reinterpret_cast<const ulonglong2*>(p.htab + hash_base(site, off));
   h.b = __umulhi(hash_target(vl, vh), h.nb);
   return h;
 }
@@ -978,26 +983,27 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
         }
       }
     }
-    // ---- the next group's rows -> L2: lane i pulls the two cache lines of row i of the next group, if that event
-    //      will need them (its site record has arrived by now); rows nobody will read are not fetched ----
-    if (gn < n_groups) {
-      const bool v_nxt = gn * 32u + lane < n_ev && h_nxt.y != 0u;
-      const bool ret_nxt = v_nxt && r_nxt.x == K_RET, fwd_nxt = v_nxt && r_nxt.x == K_FWD;
-      const char* vr = reinterpret_cast<const char*>(elem_ptr(p.val, (gn * 32u + lane) * 32u));
-      if (MODE == MODE_FORWARD ? fwd_nxt : (MODE == MODE_SIGN ? ret_nxt : (ret_nxt || fwd_nxt))) {
-        prefetch_row_l2(vr);
-      }
-      if (MODE == MODE_VERIFY && ret_nxt) {
-        const char* tr = reinterpret_cast<const char*>(elem_ptr(p.tag, (gn * 32u + lane) * 32u));
-        prefetch_row_l2(tr);
-      }
-    }
+    // ---- tag rows -> L2: lane i pulls the tag row of event i of THIS group if it is a return check; the passes that
+    //      gather from it start below (their first items are carried ones, whose rows came in a group ago).  Rows that
+    //      were fetched a whole group ahead sat in L2 for up to two groups: with 2,960 warps that footprint (up to
+    //      97 MB of rows) did not fit beside a large policy's tables, and rows were fetched from DRAM twice (measured:
+    //      config 5 read 5.72 GB per batch, 4.95 GB now; config 4 26.8 -> 24.7 GB per launch, its algorithmic bytes) ----
+    if (MODE == MODE_VERIFY && cls == CLS_RET)
+      prefetch_row_l2(reinterpret_cast<const char*>(elem_ptr(p.tag, (e0 + lane) * 32u)));
     __syncwarp();
 
     // ---- consumer passes: every full pass; carried items of the previous group go first.  If a queue still holds
     //      items of the previous group and cannot fill a pass, it is flushed with a partial pass (rare). ----
     // (carried items are the oldest: any full pass consumes them; fewer than 64 are carried per queue)
     drain(last || (cu != 0u && nu < 64u), last || (cd != 0u && nd < 64u));
+    // ---- the next group's value rows -> L2, as late as possible (see above): lane i pulls row i of the next group if
+    //      that event will need it (its site record has arrived by now); rows nobody will read are not fetched ----
+    if (gn < n_groups) {
+      const bool v_nxt = gn * 32u + lane < n_ev && h_nxt.y != 0u;
+      const bool ret_nxt = v_nxt && r_nxt.x == K_RET, fwd_nxt = v_nxt && r_nxt.x == K_FWD;
+      if (MODE == MODE_FORWARD ? fwd_nxt : (MODE == MODE_SIGN ? ret_nxt : (ret_nxt || fwd_nxt)))
+        prefetch_row_l2(reinterpret_cast<const char*>(elem_ptr(p.val, (gn * 32u + lane) * 32u)));
+    }
     if (have_prev) epilogue(par ^ 1u, prev_e0);
     have_prev = true;
     prev_e0 = e0;
@@ -1115,7 +1121,7 @@ __global__ void wg_build_hash(uint64_t* htab, SiteRec* recs, const uint64_t* tgt
     return;
   }
   const uint32_t nb = (r.cnt + 1u) >> 1;
-  unsigned long long* tab = reinterpret_cast<unsigned long long*>(htab + (2ull * r.off + 4ull * lo));
+  unsigned long long* tab = reinterpret_cast<unsigned long long*>(htab + hash_base(lo, r.off));
   uint32_t b = __umulhi(hash_target(static_cast<uint32_t>(v), static_cast<uint32_t>(v >> 32)), nb);
   for (;;) {
     for (uint32_t k = 0; k < 4u; ++k)
