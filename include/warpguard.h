@@ -31,7 +31,9 @@
  *  - Sign / verify / check enqueue work on `cuda_stream` and return without waiting.  Counters accumulate across
  *    calls until wg_reset_counters (synchronous) or the next successful wg_load_policy.  The *_host calls are
  *    synchronous and run on the engine's own streams: they are not ordered after work still pending on a caller
- *    stream, so synchronise that stream first when both forms are mixed.
+ *    stream, so synchronise that stream first when both forms are mixed.  Calls of one engine may be in flight on
+ *    several caller streams at once (each launch takes its own group ticket from a ring of 64): keep fewer than 64
+ *    launches of one engine pending across streams; on a single stream there is no limit.
  *  - There is no CPU fallback: without a CUDA device every call that needs one returns WG_ERR_CUDA.
  */
 #ifndef WARPGUARD_H

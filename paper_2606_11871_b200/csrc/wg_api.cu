@@ -1,7 +1,7 @@
 // wg_api.cu — the C-ABI of include/warpguard.h: argument checks, policy validation (a bad
 // policy loads nothing), engine-owned device tables, launches, counter read-out, and the HOST-buffer entry
 // points that stream events through a double-buffered device staging area.  No verdict, MAC or membership
-// arithmetic happens on the host: every step of the path runs in the kernels of wg_kernels.cu.
+// arithmetic happens on the host: every step of the path runs in the kernels of wg_check.cu and wg_shadow.cu.
 #include <cstring>
 #include <new>
 #include <vector>
@@ -234,12 +234,17 @@ constexpr uint64_t kBytesPerStagedEvent = 16 + 256 + 256 + 8;
 
 wg_status ensure_staging(wg_engine* e) {
   if (e->stage_cap) return WG_OK;
-  for (int i = 0; i < 2; ++i) {
-    WG_CUDA(e, cudaMalloc(&e->d_stage[i], kStageEvents * kBytesPerStagedEvent));
-    WG_CUDA(e, cudaStreamCreateWithFlags(&e->st[i], cudaStreamNonBlocking));
-    WG_CUDA(e, cudaEventCreateWithFlags(&e->ev_done[i], cudaEventDisableTiming));
+  cudaError_t err = cudaSuccess;
+  for (int i = 0; i < 2 && err == cudaSuccess; ++i) {
+    if ((err = cudaMalloc(&e->d_stage[i], kStageEvents * kBytesPerStagedEvent)) != cudaSuccess) break;
+    if ((err = cudaStreamCreateWithFlags(&e->st[i], cudaStreamNonBlocking)) != cudaSuccess) break;
+    err = cudaEventCreateWithFlags(&e->ev_done[i], cudaEventDisableTiming);
   }
-  WG_CUDA(e, cudaEventCreateWithFlags(&e->ev_rec, cudaEventDisableTiming));
+  if (err == cudaSuccess) err = cudaEventCreateWithFlags(&e->ev_rec, cudaEventDisableTiming);
+  if (err != cudaSuccess) {
+    free_staging(e);  // all or nothing: a half-built staging area is not kept (the next call starts over)
+    return cuda_fail(e, err);
+  }
   e->stage_cap = kStageEvents;
   return WG_OK;
 }
@@ -281,29 +286,32 @@ wg_status host_common(wg_engine* e, HostOp op, const wg_event_hdr* h_hdr, const 
   // in chunk order by one kernel at a time, and the last writer is the chunk that holds the final minimum key.
   int buf = 0;
   bool rec_pending = false;
-  for (uint64_t lo = 0; lo < n; lo += kStageEvents, buf ^= 1) {
+  auto chunk = [&](uint64_t lo, cudaStream_t st, const StageView& v) -> wg_status {
     const uint64_t m = (n - lo < kStageEvents) ? (n - lo) : kStageEvents;
-    cudaStream_t st = e->st[buf];
-    StageView v = stage_view(e->d_stage[buf]);
     // the previous use of this buffer (two chunks ago) finished when its stream's D2H did: same stream, in order
     WG_CUDA(e, cudaMemcpyAsync(v.hdr, h_hdr + lo, m * 16, cudaMemcpyHostToDevice, st));
     WG_CUDA(e, cudaMemcpyAsync(v.val, h_val + lo * 32, m * 256, cudaMemcpyHostToDevice, st));
     if (op == OP_VERIFY)
       WG_CUDA(e, cudaMemcpyAsync(v.tag, h_tag_in + lo * 32, m * 256, cudaMemcpyHostToDevice, st));
     if (op == OP_SIGN) {
-      s = sign_common(e, v.hdr, v.val, v.tag, m, st);
-      if (s != WG_OK) return s;
+      const wg_status s2 = sign_common(e, v.hdr, v.val, v.tag, m, st);
+      if (s2 != WG_OK) return s2;
       WG_CUDA(e, cudaMemcpyAsync(h_tag_out + lo * 32, v.tag, m * 256, cudaMemcpyDeviceToHost, st));
     } else {
-      s = check_common(e, v.hdr, v.val, v.tag, op == OP_VERIFY, v.out, m, mode, st, rec_pending ? e->ev_rec : nullptr);
-      if (s != WG_OK) return s;
+      const wg_status s2 = check_common(e, v.hdr, v.val, v.tag, op == OP_VERIFY, v.out, m, mode, st, rec_pending ? e->ev_rec : nullptr);
+      if (s2 != WG_OK) return s2;
       WG_CUDA(e, cudaEventRecord(e->ev_rec, st));
       rec_pending = true;
       WG_CUDA(e, cudaMemcpyAsync(h_out + lo, v.out, m * 8, cudaMemcpyDeviceToHost, st));
     }
-  }
-  WG_CUDA(e, cudaStreamSynchronize(e->st[0]));
-  WG_CUDA(e, cudaStreamSynchronize(e->st[1]));
+    return WG_OK;
+  };
+  for (uint64_t lo = 0; lo < n && s == WG_OK; lo += kStageEvents, buf ^= 1) s = chunk(lo, e->st[buf], stage_view(e->d_stage[buf]));
+  // whatever happened, nothing of this call may still be copying from or into the caller's host buffers on return
+  const cudaError_t e0 = cudaStreamSynchronize(e->st[0]), e1 = cudaStreamSynchronize(e->st[1]);
+  if (s != WG_OK) return s;
+  if (e0 != cudaSuccess) return cuda_fail(e, e0);
+  if (e1 != cudaSuccess) return cuda_fail(e, e1);
   return WG_OK;
 }
 

@@ -27,8 +27,9 @@
 //       items per queue) is carried into the next group, so no SipRound is ever spent on an inactive lane;
 //   the event-parallel epilogue of the PREVIOUS group (its last items were consumed by this group's first passes):
 //       verdict store, violation counters, first violation.
-// The next group's rows are pulled into L2 by TMA bulk prefetches while this group is computed; when the policy's
-// whole target table is small it is staged in shared memory once per CTA by one TMA bulk copy.
+// Rows are pulled into L2 by `prefetch.global.L2` shortly before they are read (value rows of the next group behind this
+// group's passes, tag rows at the head of the group's own passes); when the policy's whole target table is small it is
+// staged in shared memory once per CTA by one TMA bulk copy.
 #include "wg_internal.h"
 #include "../../include/warpguard_sip32.cuh"
 
@@ -142,25 +143,10 @@ __device__ __forceinline__ void sts_v4(uint32_t a, uint32_t x, uint32_t y, uint3
 __device__ __forceinline__ void sts_v2(uint32_t a, uint32_t x, uint32_t y) {
   asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(a), "r"(x), "r"(y) : "memory");
 }
-// one cache line -> L2 (the rows a later group will read; an LSU instruction, no register, no completion to wait for)
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-  asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
-}
-#ifndef WG_PF
-#define WG_PF 4
-#endif
-#ifndef WG_KEEP
-#define WG_KEEP 1
-#endif
-// one 256-byte row -> L2.  A prefetch pulls 64 bytes (measured: 2 sectors per request), so a row takes four.
+// one 256-byte row -> L2.  A prefetch pulls 64 bytes (measured: 2 sectors per request), so a row takes four (one
+// `cp.async.bulk.prefetch.L2` of 256 bytes and two prefetches 128 bytes apart were measured: slower / rows half fetched).
 __device__ __forceinline__ void prefetch_row_l2(const void* p) {
-#if WG_PF == 4
   asm volatile("prefetch.global.L2 [%0];\n\tprefetch.global.L2 [%0+64];\n\tprefetch.global.L2 [%0+128];\n\tprefetch.global.L2 [%0+192];" ::"l"(p) : "memory");
-#elif WG_PF == 1
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], 256;" ::"l"(p) : "memory");
-#else
-  asm volatile("prefetch.global.L2 [%0];\n\tprefetch.global.L2 [%0+128];" ::"l"(p) : "memory");
-#endif
 }
 // L2 policy "evict last" for what every batch of a stream comes back to: site records and per-site counters
 __device__ __forceinline__ uint64_t l2_keep_policy() {
@@ -170,11 +156,7 @@ __device__ __forceinline__ uint64_t l2_keep_policy() {
 }
 __device__ __forceinline__ uint4 ldg_v4_l2keep(const void* p, uint64_t pol) {
   uint4 r;
-#if WG_KEEP
   asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(pol));
-#else
-  asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-#endif
   return r;
 }
 // {kind, off, cnt} of a site record, without the flags word: a kernel that never reads the flags would leave the fourth
@@ -188,11 +170,7 @@ __device__ __forceinline__ uint4 ldg_rec3_l2keep(const void* p, uint64_t pol) {
   return r;
 }
 __device__ __forceinline__ void red_add_u64_l2keep(unsigned long long* p, unsigned long long v, uint64_t pol) {
-#if WG_KEEP
   asm volatile("red.global.add.L2::cache_hint.u64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(pol) : "memory");
-#else
-  atomicAdd(p, v);
-#endif
 }
 __device__ __forceinline__ void atoms_or(uint32_t a, uint32_t x) {
   asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(a), "r"(x) : "memory");
@@ -233,8 +211,7 @@ __device__ __forceinline__ const char* byte_ptr(const char* base, uint32_t off) 
   return reinterpret_cast<const char*>(r);
 }
 
-// TMA: 1-D bulk copy global -> shared with completion on an mbarrier (whole-table staging of the target sets), and
-// bulk prefetch global -> L2 (the next group's rows)
+// TMA: 1-D bulk copy global -> shared with completion on an mbarrier (whole-table staging of the target sets)
 __device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -246,9 +223,6 @@ __device__ __forceinline__ void tma_bulk_g2s(uint32_t dst, const void* src, uint
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                "l"(src), "r"(bytes), "r"(mbar)
                : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_l2(const void* src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
   asm volatile(
@@ -659,10 +633,7 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
     return (g < n_groups && e < n_ev) ? ldg_v4(p.hdr + e) : make_uint4(0xffffffffu, 0u, 0u, 0u);
   };
   auto load_rec = [&](const uint4& h) __attribute__((always_inline)) -> uint4 {
-#ifndef WG_REC3
-#define WG_REC3 1
-#endif
-    if (WG_REC3 && !FQ && !TEL)  // (the flags: hash index and coverage-reduced profile only)
+    if (!FQ && !TEL)  // (the flags: hash index and coverage-reduced profile only)
       return h.x < p.n_sites ? ldg_rec3_l2keep(p.recs + h.x, l2_keep_policy()) : make_uint4(7u, 0u, 0u, 0u);
     return h.x < p.n_sites ? ldg_v4_l2keep(p.recs + h.x, l2_keep_policy()) : make_uint4(7u, 0u, 0u, 0u);
   };
