@@ -465,3 +465,67 @@ def test_reloading_an_engine_onto_another_device_moves_everything_it_owns():
         with pytest.raises(B.WgError):  # the shadow state did not move: it has to be configured again
             eng.wg_shadow_read_counters()
     eng.close()
+
+
+@pytest.mark.parametrize("n_big", [8, 3000])
+def test_a_target_equal_to_the_all_ones_word_is_an_ordinary_member(n_big):
+    """Degenerate case of the large-policy encoding: the hash index of the target sets (wg_check.cu) marks a free slot
+    with the all-ones word, so a set that CONTAINS 0xFFFF_FFFF_FFFF_FFFF cannot store it and carries a flag instead.
+    Membership must still be exactly the set's: all-ones is allowed at the site that lists it and
+    nowhere else, as a warp-uniform target and as one lane's target, before and after wg_policy_poke rewrites that
+    element (the index is rebuilt, the flag follows).  n_big = 8: the staged table (no hash index); 3000: the hash
+    index (more than 2,048 targets)."""
+    rng = np.random.default_rng(77 + n_big)
+    # sites: 0 return, 1 forward with all-ones as its last element, 2 forward without, 3 forward with one element
+    base = np.uint64(0x7F5A40000000)
+    set1 = np.concatenate([np.sort(rng.choice(1 << 20, n_big, replace=False).astype(np.uint64)) * np.uint64(16) + base,
+                           np.array([U64MAX], dtype=np.uint64)])
+    set2 = np.sort(rng.choice(1 << 20, 5, replace=False).astype(np.uint64)) * np.uint64(16) + base + np.uint64(8)
+    set3 = np.array([0x1234], dtype=np.uint64)
+    kind = np.array([0, 1, 1, 1], dtype=np.uint8)
+    off = np.array([0, 0, len(set1), len(set1) + len(set2), len(set1) + len(set2) + 1], dtype=np.uint32)
+    tg = np.concatenate([set1, set2, set3])
+    k0, k1 = 0x0123456789ABCDEF, 0x0FEDCBA987654321
+    orc = oracle.Oracle(kind, off, tg, k0, k1, 5)
+    eng = B.Engine(0)
+    eng.wg_load_policy(kind, off, tg, k0, k1, 5)
+
+    n = 4096 + 7
+    site = rng.integers(1, 4, n).astype(np.uint64)
+    mask = rng.integers(1, 1 << 32, n, dtype=np.uint64)
+    ctx = rng.integers(0, 1 << 63, n, dtype=np.uint64)
+    val = np.empty((n, 32), dtype=np.uint64)
+    sets = {1: set1, 2: set2, 3: set3}
+    for e in range(n):
+        members = sets[int(site[e])]
+        val[e, :] = members[rng.integers(0, len(members))] if rng.random() < 0.5 else members[rng.integers(0, len(members), 32)]
+        r = rng.random()
+        if r < 0.3:
+            val[e, :] = U64MAX              # warp-uniform all-ones: legal at site 1 only
+        elif r < 0.6:
+            val[e, rng.integers(0, 32)] = U64MAX  # one lane all-ones
+    hdr = mk_hdr(site, mask, ctx)
+    d_hdr, d_val = to_dev(hdr), to_dev(val)
+
+    def compare():
+        for mode in (DET, ENF):
+            o = orc.check_forward(hdr, val, mode)
+            g = eng.wg_check_forward(d_hdr, d_val, mode).cpu().numpy().view(np.uint32)
+            bad = np.nonzero((g != o).any(1))[0]
+            assert bad.size == 0, (mode, bad[:5], g[bad[:5]], o[bad[:5]], site[bad[:5]])
+        return o
+
+    o = compare()
+    at1 = (site == 1) & (val == U64MAX).all(1)
+    assert at1.any() and not o[at1, 0].any(), "all-ones is a member of site 1's set"
+    at2 = (site != 1) & (val == U64MAX).all(1)
+    assert at2.any() and (o[at2, 0] == (mask[at2] & np.uint64(FULL)).astype(np.uint32)).all(), "and of no other set"
+    # the attacker-write hook turns the all-ones element into another address (still ascending) and back
+    idx = len(set1) - 1
+    x = int(U64MAX) ^ int(set1[-2] + np.uint64(1))
+    for _ in range(2):
+        orc.policy_poke(0, idx, x)
+        eng.wg_policy_poke(0, idx, x)
+        compare()
+    assert_counters_equal(eng, orc)
+    eng.close()
