@@ -95,3 +95,69 @@ def test_config5_full_size_policy_one_whole_batch_against_the_oracle():
     assert g["ret_viol_events"] == len(st.ret_tamper)
     assert len(st.fwd_tamper) - 20 <= g["fwd_viol_events"] <= len(st.fwd_tamper)  # (a flipped bit can hit another member)
     eng.close()
+
+
+def test_one_call_longer_than_one_launch_tiles_a_pattern_the_oracle_judged():
+    """Maximum sizes: a launch covers at most 2^27 - 32 events (element indices event * 32 + lane stay below 2^32), a CALL
+    may be longer and is cut into launches by the C-ABI layer (pointer offsets, sequence base, ticket slots).  The stream
+    is a 4,096-event config-4 pattern repeated 32,769.x times (134,221,829 events, 34 GB of values): the oracle judges
+    the pattern (and its ragged tail) once; every tag and verdict of the long call must equal the pattern's, the
+    counters must be the pattern's times the number of repeats plus the tail's, and the first-violation key the
+    pattern's own (sequence numbers run through the call, R12)."""
+    P = 4096
+    n = (1 << 27) - 32 + P + 5
+    full, tail = divmod(n, P)
+    free, _ = torch.cuda.mem_get_info(0)
+    if free < 90 * (1 << 30):
+        pytest.skip("needs ~80 GB of device memory")
+    st = S.make_stream(4, "cpu", n_events=P, mode=S.ENFORCE)
+    pol = st.policy
+    from tests.util import oracle_for
+    hdr_p, val_p = st.hdr.numpy().view(np.uint64), st.val.numpy().view(np.uint64).copy()
+    orc = oracle_for(pol)
+    tag_p = orc.sign(hdr_p, val_p)
+    tag_t = torch.from_numpy(tag_p.view(np.int64).copy())
+    st.apply_return_tamper(tag_t)  # (values and tags, as the recorded plan says)
+    val_c, tag_c = st.val.numpy().view(np.uint64), tag_t.numpy().view(np.uint64)
+    orc = oracle_for(pol)
+    out_p = orc.verify(hdr_p, val_c, tag_c, S.ENFORCE)
+    g_p, s_p = orc.read_counters()
+    first_p = g_p["first_violation_key"]
+    orc_t = oracle_for(pol)
+    orc_t.verify(hdr_p[:tail], val_c[:tail], tag_c[:tail], S.ENFORCE)
+    g_t, s_t = orc_t.read_counters()
+    assert out_p[:, 0].any() and first_p != (1 << 64) - 1
+
+    def tiled(a):  # the pattern, repeated to n rows on the device (no temporary of the full size)
+        t = a.to(dev())
+        big = torch.empty((n, t.shape[1]), dtype=t.dtype, device=dev())
+        big[: full * P].view(full, P, -1).copy_(t.view(1, P, -1).expand(full, P, -1))
+        big[full * P:].copy_(t[:tail])
+        return big
+
+    def equals_pattern(big, pat):
+        pat = pat.to(dev())
+        ok = bool((big[: full * P].view(full, P, -1) == pat.view(1, P, -1)).all())
+        return ok and bool((big[full * P:] == pat[:tail]).all())
+
+    eng = B.Engine(0).load(pol)
+    d_hdr = tiled(st.hdr)
+    d_val = tiled(torch.from_numpy(val_p.view(np.int64)))
+    g_tag = eng.wg_sign_continuations(d_hdr, d_val)
+    assert equals_pattern(g_tag, torch.from_numpy(tag_p.view(np.int64))), "tags of the long call differ from the pattern's"
+    del g_tag, d_val
+    d_val = tiled(st.val)
+    d_tag = tiled(tag_t)
+    eng.wg_reset_counters()
+    out = eng.wg_verify_continuations(d_hdr, d_val, d_tag, S.ENFORCE)
+    assert equals_pattern(out, torch.from_numpy(out_p.view(np.int32))), "verdicts of the long call differ from the pattern's"
+    gg, gs = eng.wg_read_counters()
+    skip = ("first_violation_key", "policy_digest", "last_mode", "signed_lanes", "sign_skipped_events")
+    for k in g_p:
+        if k not in skip:
+            assert gg[k] == full * g_p[k] + g_t[k], (k, gg[k], g_p[k], g_t[k])
+    assert gg["first_violation_key"] == first_p
+    assert np.array_equal(gs, np.uint64(full) * s_p + s_t)
+    eng.close()
+    del d_hdr, d_val, d_tag, out
+    torch.cuda.empty_cache()  # (the other GPU tests, some of them in child processes, get the 70 GB back)
