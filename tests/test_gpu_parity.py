@@ -529,3 +529,36 @@ def test_a_target_equal_to_the_all_ones_word_is_an_ordinary_member(n_big):
         compare()
     assert_counters_equal(eng, orc)
     eng.close()
+
+
+def test_a_policy_without_sites_fails_every_event_closed():
+    """Degenerate policy: no site at all (what the policy does not list is not authorised).  Every event
+    names an unknown site: verify and the forward entry point fail its active lanes closed (R13), sign writes zero rows,
+    nothing enters a protected-site denominator, and the per-site array is empty."""
+    kind, off, tg = np.zeros(0, dtype=np.uint8), np.zeros(1, dtype=np.uint32), np.zeros(0, dtype=np.uint64)
+    orc = oracle.Oracle(kind, off, tg, 11, 12, 13)
+    eng = B.Engine(0)
+    eng.wg_load_policy(kind, off, tg, 11, 12, 13)
+    rng = np.random.default_rng(3)
+    n = 20 * 32 * 5 + 3
+    site = rng.choice(np.array([0, 1, 7, 0xFFFFFFFF], dtype=np.uint64), n)
+    mask = rng.integers(0, 1 << 32, n, dtype=np.uint64)
+    mask[::7] = 0
+    hdr = mk_hdr(site, mask, rng.integers(0, 1 << 63, n, dtype=np.uint64))
+    val = rng.integers(0, 1 << 63, size=(n, 32), dtype=np.uint64)
+    tag = rng.integers(0, 1 << 63, size=(n, 32), dtype=np.uint64)
+    d_hdr, d_val, d_tag = to_dev(hdr), to_dev(val), to_dev(tag)
+    g_tag = eng.wg_sign_continuations(d_hdr, d_val).cpu().numpy().view(np.uint64)
+    assert np.array_equal(g_tag, orc.sign(hdr, val)) and not g_tag.any()
+    for mode in (ENF, DET):
+        o = orc.verify(hdr, val, tag, mode)
+        g = eng.wg_verify_continuations(d_hdr, d_val, d_tag, mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o) and np.array_equal(g[:, 0], mask.astype(np.uint32))
+        o = orc.check_forward(hdr, val, mode)
+        g = eng.wg_check_forward(d_hdr, d_val, mode).cpu().numpy().view(np.uint32)
+        assert np.array_equal(g, o)
+    gg, gs = eng.wg_read_counters()
+    og, os_ = orc.read_counters()
+    assert gg == og and gs.shape == os_.shape == (0, 4)
+    assert gg["ret_checks"] == gg["fwd_checks"] == 0 and gg["events_unknown_site"] == 4 * n
+    eng.close()
