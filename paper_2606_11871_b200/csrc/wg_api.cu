@@ -21,6 +21,7 @@ struct wg_engine {
   uint32_t sched_next = 0;
   uint64_t* d_htab = nullptr;      // hash index of the target sets when the table is too large to stage (wg_check.cu)
   uint32_t bind_hi = 0;            // digest32 folded into the tokens (wg_load_policy_bound), else 0
+  bool has_ret = false;            // the policy lists a protected-return site
   uint32_t profile = 0;            // WG_PROFILE_* flags (configuration: survives resets and policy loads)
   uint64_t ring_cap = 0;           // violation ring capacity in records (0 = off)
   wg::ViolRec* d_ring = nullptr;
@@ -153,6 +154,7 @@ wg::Params base_params(const wg_engine* e) {
   p.n_tgts = e->n_tgts;
   p.profile = e->profile;
   p.bind_hi = e->bind_hi;
+  p.has_ret = e->has_ret ? 1u : 0u;
   p.ring = e->d_ring;
   p.ring_cap = e->d_ring ? e->ring_cap : 0;
   p.first = e->d_first;
@@ -505,6 +507,8 @@ static wg_status load_common(wg_engine** eng, int device, const wg_policy_desc* 
   for (int i = 0; i < 4; ++i) e->v_init[i] = tmp.v_init[i];
   e->digest = desc->policy_digest;
   e->bind_hi = bind_hi;
+  e->has_ret = false;
+  for (uint32_t s2 = 0; s2 < n; ++s2) e->has_ret = e->has_ret || desc->kind[s2] == WG_KIND_PROTECTED_RETURN;
   if (new_first) e->d_first = new_first;
   e->loaded = true;
   *eng = e;

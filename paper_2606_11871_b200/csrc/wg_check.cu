@@ -45,8 +45,15 @@ enum : uint32_t { CLS_NONE = 0, CLS_COUNT = 1, CLS_RET = 2, CLS_FWD = 3, CLS_FAI
 #ifndef WG_WARPS
 #define WG_WARPS 20
 #endif
-constexpr int kWarps = WG_WARPS;       // warps per CTA, one CTA per SM
+constexpr int kWarps = WG_WARPS;       // warps per CTA, one CTA per SM (sign / verify: the 96-register pass code)
 constexpr int kThreads = kWarps * 32;
+// The forward entry point (and a verify over a policy without return sites: the same decisions) has no MAC pass: its
+// warps wait on shared-memory and shuffle latencies with nothing else to issue, so it wants more of them — 64
+// registers, no work queue in shared memory.
+#ifndef WG_WARPS_FWD
+#define WG_WARPS_FWD 32
+#endif
+constexpr int kWarpsFwd = WG_WARPS_FWD;
 constexpr uint32_t kSmemMax = 232448;  // 227 KB opt-in shared memory per CTA on sm_100a
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kMaxCacheSlots = 2048;  // slots of the per-site counter cache in shared memory (12 bytes each)
@@ -79,6 +86,7 @@ constexpr uint32_t kQueueItems = WG_QUEUE;       // one group adds at most 1,024
 constexpr uint32_t kBatch = WG_BATCH;              // row loads in flight per lane in the producer loop
 constexpr uint32_t kListBytes = 40 * 16;           // up to 32 protected events, padded to a multiple of kBatch
 constexpr uint32_t kWarpBytes = kRecArea + kQueueItems * 2 + kListBytes;
+constexpr uint32_t kWarpBytesFwd = kRecArea + kListBytes;  // the forward kernels queue nothing
 // kernels that look forward targets up in the hash index (verify / forward, table not staged) add a queue of lookups
 constexpr uint32_t kFwdQueueItems = 512;            // drained when more than 256 wait: 8 trips add at most 256
 constexpr uint32_t kFwdQueueBytes = kFwdQueueItems * 2;
@@ -86,6 +94,8 @@ constexpr uint32_t kCtaFixedBytes = C_WORDS * 8 + 16 * 4 + 16 + 48;  // cnt64, b
 constexpr uint32_t kLeft = kSmemMax - kCtaFixedBytes - kWarps * kWarpBytes;
 constexpr uint32_t kMaxStageTgts = (kLeft / 16 * 2) < 2048 ? (kLeft / 16 * 2) : 2048;
 static_assert(kWarps * (kWarpBytes + kFwdQueueBytes) + kCtaFixedBytes + 4096 <= kSmemMax, "too many warps for the shared memory");
+static_assert(kWarpsFwd * (kWarpBytesFwd + kFwdQueueBytes) + kCtaFixedBytes + 4096 <= kSmemMax, "too many forward warps for the shared memory");
+static_assert(kWarpsFwd * kWarpBytesFwd + kCtaFixedBytes + 2048 * 8 + 64 * 12 <= kSmemMax, "the staged table must fit beside the forward warps");
 
 // ---- PTX helpers ---------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -366,8 +376,9 @@ struct WarpCtr {
 // (compiled out of the ordinary launch).
 // ---------------------------------------------------------------------------------------------------
 template <int MODE, bool STAGED, bool TEL>
-__global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, const uint32_t stage_bytes,
-                                                                const uint32_t site_bytes) {
+__global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 32, 1)
+    wg_check_kernel(const Params p, const uint32_t stage_bytes, const uint32_t site_bytes) {
+  constexpr uint32_t kW = MODE == MODE_FORWARD ? kWarpsFwd : kWarps;  // warps of this CTA
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint32_t lane, lanebit;
   asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
@@ -396,10 +407,11 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   uint32_t* viol_s = reinterpret_cast<uint32_t*>(smem_raw + cta_off + C_WORDS * 8 + 80);
   unsigned long long* key_s = reinterpret_cast<unsigned long long*>(smem_raw + cta_off + C_WORDS * 8 + 112);
   constexpr bool FQ = MODE != MODE_SIGN && !STAGED;  // forward lookups go through the hash index and its queue
-  const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * (kWarpBytes + (FQ ? kFwdQueueBytes : 0u));
+  constexpr uint32_t kQBytes = MODE == MODE_FORWARD ? 0u : kQueueItems * 2u;  // (the forward kernels have no work queue)
+  const uint32_t rec_s = smem0 + cta_off + kCtaFixedBytes + warp * (kRecArea + kQBytes + kListBytes + (FQ ? kFwdQueueBytes : 0u));
   const uint32_t q_s = rec_s + kRecArea;                    // uniform items: q_s + 2 * k
   const uint32_t q_top = q_s + (kQueueItems - 1) * 2;        // divergent items: q_top - 2 * k
-  const uint32_t list_s = q_s + kQueueItems * 2;
+  const uint32_t list_s = q_s + kQBytes;
   const uint32_t fq_s = list_s + kListBytes;                // forward lookups (FQ): fq_s + 2 * k
   if (lane < 2) {  // the two dummy records: no active lane, nothing to queue
     sts_v4(rec_s + (lane * kGroupRecs + 32u) * kRecBytes + 32, 0u, 0u, 0u, 0u);
@@ -432,14 +444,14 @@ __global__ void __launch_bounds__(kThreads, 1) wg_check_kernel(const Params p, c
   // sub-partition with one warp more than its neighbours, holds the launch back.
   // (A short stream — fewer than 16 groups per warp — is dealt out statically, group = warp + k * warps: the tickets of
   // 3,000 warps that all start at once would queue on the one counter for longer than such a launch lasts.)
-  const bool dyn = n_groups >= 16u * gridDim.x * kWarps;
-  uint32_t wnext = blockIdx.x * kWarps + warp, wleft = 0;
-  const uint32_t tail_from = n_groups > 8u * gridDim.x * kWarps ? n_groups - 8u * gridDim.x * kWarps : 0u;
+  const bool dyn = n_groups >= 16u * gridDim.x * kW;
+  uint32_t wnext = blockIdx.x * kW + warp, wleft = 0;
+  const uint32_t tail_from = n_groups > 8u * gridDim.x * kW ? n_groups - 8u * gridDim.x * kW : 0u;
   unsigned int* const sched = p.sched;
   auto claim = [&]() __attribute__((always_inline)) -> uint32_t {
     if (!dyn) {
       const uint32_t g = wnext;
-      wnext += gridDim.x * kWarps;
+      wnext += gridDim.x * kW;
       return g;
     }
     if (wleft == 0u) {
@@ -1114,21 +1126,23 @@ __global__ void wg_clear_allones_flags(SiteRec* recs, uint32_t n_sites) {
 template <int MODE>
 cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
   const uint64_t n_groups = (p.n + 31) / 32;
-  const uint64_t want = (n_groups + kWarps - 1) / kWarps;
+  constexpr uint32_t W = MODE == MODE_FORWARD ? kWarpsFwd : kWarps;
+  const uint64_t want = (n_groups + W - 1) / W;
   const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) ? want : sm_count);
   const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= kMaxStageTgts;
   const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
   // the per-site counter cache: the largest power-of-two slot count <= kMaxCacheSlots that fits beside the staged
   // targets (and no more than twice the policy needs); sign keeps no per-site counters
-  const uint32_t warp_bytes = kWarpBytes + ((MODE != MODE_SIGN && !staged) ? kFwdQueueBytes : 0u);  // (the kernel's FQ)
+  const uint32_t warp_bytes = (MODE == MODE_FORWARD ? kWarpBytesFwd : kWarpBytes) +
+                              ((MODE != MODE_SIGN && !staged) ? kFwdQueueBytes : 0u);  // (the kernel's FQ)
   uint32_t site_bytes = 0;
   if (MODE != MODE_SIGN && p.n_sites > 0) {
-    const uint32_t left = kSmemMax - kCtaFixedBytes - kWarps * warp_bytes;
+    const uint32_t left = kSmemMax - kCtaFixedBytes - W * warp_bytes;
     uint32_t slots = kMaxCacheSlots;
     while (slots >= 64u && (stage_bytes + slots * 12u > left || slots / 2u >= p.n_sites)) slots /= 2u;
     if (slots >= 64u) site_bytes = slots * 12u;
   }
-  const uint32_t smem = stage_bytes + site_bytes + kCtaFixedBytes + kWarps * warp_bytes;
+  const uint32_t smem = stage_bytes + site_bytes + kCtaFixedBytes + W * warp_bytes;
   const bool tel = MODE != MODE_SIGN && (p.profile != 0 || p.ring_cap != 0);
   {  // the launch's group ticket starts at 0
     const cudaError_t e = cudaMemsetAsync(p.sched, 0, sizeof(unsigned int), st);
@@ -1137,14 +1151,14 @@ cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t
   if (tel) {
     if constexpr (MODE != MODE_SIGN) {
       if (staged)
-        wg_check_kernel<MODE, true, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+        wg_check_kernel<MODE, true, true><<<grid, W * 32, smem, st>>>(p, stage_bytes, site_bytes);
       else
-        wg_check_kernel<MODE, false, true><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+        wg_check_kernel<MODE, false, true><<<grid, W * 32, smem, st>>>(p, stage_bytes, site_bytes);
     }
   } else if (staged) {
-    wg_check_kernel<MODE, true, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    wg_check_kernel<MODE, true, false><<<grid, W * 32, smem, st>>>(p, stage_bytes, site_bytes);
   } else {
-    wg_check_kernel<MODE, false, false><<<grid, kThreads, smem, st>>>(p, stage_bytes, site_bytes);
+    wg_check_kernel<MODE, false, false><<<grid, W * 32, smem, st>>>(p, stage_bytes, site_bytes);
   }
   ++*launches;
   return cudaGetLastError();
@@ -1178,7 +1192,9 @@ cudaError_t launch_sign(const Params& p, int sm_count, cudaStream_t st, uint64_t
 }
 
 cudaError_t launch_check(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
-  return p.tag ? launch_mode<MODE_VERIFY>(p, sm_count, st, launches) : launch_mode<MODE_FORWARD>(p, sm_count, st, launches);
+  // without a return site in the policy no event can be a return check: the verify decides exactly what the forward entry
+  // point decides (unknown sites fail closed in both) and runs its leaner, wider kernel
+  return (p.tag && p.has_ret) ? launch_mode<MODE_VERIFY>(p, sm_count, st, launches) : launch_mode<MODE_FORWARD>(p, sm_count, st, launches);
 }
 
 cudaError_t launch_first_record(const Params& p, cudaStream_t st, uint64_t* launches) {

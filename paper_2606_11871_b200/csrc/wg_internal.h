@@ -102,7 +102,8 @@ struct Params {
   uint32_t pad0;
   uint32_t bind_hi;          // upper half of the token's first message word: low 32 bits of the policy digest when
                              // the policy was loaded with wg_load_policy_bound (R39), else 0
-  uint32_t pad1;
+  uint32_t has_ret;          // the policy lists at least one protected-return site (else a verify decides what the forward
+                             // entry point decides, and runs its kernel)
   ViolRec* ring;             // violation ring or nullptr
   uint64_t ring_cap;         // its capacity in records
   FirstRec* first;           // first-violation record
