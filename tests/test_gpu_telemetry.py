@@ -43,7 +43,7 @@ def as_tuple(r):
     return tuple(int(r[f]) for f in B.VIOLATION_DTYPE.names)
 
 
-@pytest.mark.parametrize("config,n", [(4, 250_003), (1, 65_536), (5, 40_001)])
+@pytest.mark.parametrize("config,n", [(4, 250_003), (1, 65_536), (5, 40_001), (3, 120_007)])  # (3: no return site in the policy: the verify runs the forward kernel)
 def test_ring_and_first_record_equal_the_oracle(config, n):
     if config == 5:
         pol = S.make_policy(5, "cpu", n_sites=5_000, max_set=512)
@@ -98,7 +98,7 @@ def test_full_ring_drops_and_counts_and_keeps_valid_records():
 @pytest.mark.parametrize("flags", [B.WG_PROFILE_SKIP_FORWARD, B.WG_PROFILE_SKIP_BACKWARD, B.WG_PROFILE_LOW_TELEMETRY,
                                    B.WG_PROFILE_SKIP_FORWARD | B.WG_PROFILE_LOW_TELEMETRY,
                                    B.WG_PROFILE_SKIP_FORWARD | B.WG_PROFILE_SKIP_BACKWARD])
-@pytest.mark.parametrize("config", [4, 1])
+@pytest.mark.parametrize("config", [4, 1, 3])
 def test_profiles_match_the_oracle(flags, config):
     st, orc, eng, hdr, val, tag, d = prepared(config, 120_011)
     orc.set_profile(flags)
