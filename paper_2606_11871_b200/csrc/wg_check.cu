@@ -710,8 +710,12 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
       const uint64_t tp = reinterpret_cast<uint64_t>(MODE == MODE_SIGN ? p.tag_out : p.tag) + static_cast<uint64_t>(e0 + lane) * 256u -
                           static_cast<uint64_t>(slot_me) * 256u;
       const uint64_t vp = reinterpret_cast<uint64_t>(p.val) + static_cast<uint64_t>(e0 + lane) * 256u - static_cast<uint64_t>(slot_me) * 256u;
-      sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, static_cast<uint32_t>(tp), static_cast<uint32_t>(tp >> 32));
-      sts_v2(ra_me + 72, static_cast<uint32_t>(vp), static_cast<uint32_t>(vp >> 32));
+      // (the forward kernels run no MAC pass: nobody reads the context or the tag row there, and only the hash-index
+      // lookups read the value-row pointer; their warps queue on the shared-memory unit, so what is not read is not written)
+      if constexpr (MODE != MODE_FORWARD)
+        sts_v4(ra_me + 32, h_cur.z & ~31u, h_cur.w, static_cast<uint32_t>(tp), static_cast<uint32_t>(tp >> 32));
+      if constexpr (MODE != MODE_FORWARD || FQ)
+        sts_v2(ra_me + 72, static_cast<uint32_t>(vp), static_cast<uint32_t>(vp >> 32));
     }
     sts_v4(ra_me + 48, active, cls == CLS_RET ? active : 0u, viol, 0u);
     sts_v2(ra_me + 64, cls | (kind << 4), site);
@@ -814,6 +818,7 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
     // ---- producer loop (lane-parallel), one trip per protected event: warp-uniformity of the row just loaded, and
     //      for a return check the active lanes appended, compacted, to the queue of its class.  Double-buffered: the
     //      next batch's rows are requested before this batch is looked at. ----
+    uint32_t divbits = 0;  // forward kernels: bit e = event e of the group has lane-divergent targets (warp-uniform word)
     if (need != 0u) {
       uint32_t qu = q_s + nu * 2u, qd = q_top - nd * 2u;  // where the next uniform / divergent item goes
       uint32_t qf = fq_s;                                  // ... and the next forward lookup
@@ -825,7 +830,10 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
           const uint32_t rx = __shfl_sync(kFull, v[j].x, le.w), ry = __shfl_sync(kFull, v[j].y, le.w);
           uint32_t diff, div_;
           and_test(__ballot_sync(kFull, v[j].x != rx || v[j].y != ry), am.x, diff, div_);
-          sts_u32(le.x + 60, diff);  // (every lane stores the same word)
+          if constexpr (MODE == MODE_FORWARD)
+            divbits |= div_ << ((le.y >> 8) & 31u);  // (kept in a register: one shared-memory store less per event)
+          else
+            sts_u32(le.x + 60, diff);  // (every lane stores the same word)
           if (FQ && use_hash && (le.w & 32u)) {
             // a forward event: one lookup for a warp-uniform target (the first active lane's), else one per active lane
             const uint32_t fm = div_ != 0u ? am.x : (1u << (le.w & 31u));
@@ -890,7 +898,7 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
     // ---- event-parallel: per-event part of the MAC; search of warp-uniform forward targets ----
     {
       const bool judged = cls == CLS_RET || cls == CLS_FWD;
-      const bool is_uni = judged && lds_u32(ra_me + 60) == 0u;
+      const bool is_uni = judged && (MODE == MODE_FORWARD ? ((divbits >> lane) & 1u) == 0u : lds_u32(ra_me + 60) == 0u);
       uint32_t ul = 0, uh = 0;
       if (is_uni && !(use_hash && cls == CLS_FWD)) {
         const uint2 r = ldg_v2_keep(elem_ptr(p.val, (e0 + lane) * 32u + first));  // the event's one value (an L1 hit)
