@@ -730,9 +730,12 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
       const uint32_t row0 = static_cast<uint32_t>(__ffs(need) - 1) * 256u;  // a row that is read anyway (padding trips)
       // (bit 5 of the last word: a forward event; the shuffle that takes this word as its source lane reads bits 0-4)
       if (need & lanebit)
-        sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, slot_me * 32u, first | ((FQ && cls == CLS_FWD) ? 32u : 0u));
+        // (third word: the queue item base; a forward kernel without the hash index queues nothing and carries the
+        // event's active mask there instead, which saves the producer one shared-memory load per event)
+        sts_v4(list_s + __popc(need & ltmask) * 16u, ra_me, lane * 256u, (MODE == MODE_FORWARD && !FQ) ? active : slot_me * 32u,
+               first | ((FQ && cls == CLS_FWD) ? 32u : 0u));
       if (lane < ((kBatch - n_need) & (kBatch - 1u)))
-        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (slot_me - lane + 32u) * 32u, 0u);
+        sts_v4(list_s + (n_need + lane) * 16u, rbase + 32u * kRecBytes, row0, (MODE == MODE_FORWARD && !FQ) ? 0u : (slot_me - lane + 32u) * 32u, 0u);
     }
     __syncwarp();  // the records and the list are visible to every lane
     // value rows, straight from global memory: one coalesced 256-byte load per event, kBatch in flight per lane; the
@@ -826,7 +829,11 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
 #pragma unroll
         for (int j = 0; j < static_cast<int>(kBatch); ++j) {
           const uint4 le = lds_v4(list_s + (b0 + j) * 16u);  // record, row byte offset, queue item base, first active lane
-          const uint2 am = lds_v2(le.x + 48);                // active, queue mask
+          uint2 am;                                          // active, queue mask
+          if constexpr (MODE == MODE_FORWARD && !FQ)
+            am = make_uint2(le.z, 0u);
+          else
+            am = lds_v2(le.x + 48);
           const uint32_t rx = __shfl_sync(kFull, v[j].x, le.w), ry = __shfl_sync(kFull, v[j].y, le.w);
           uint32_t diff, div_;
           and_test(__ballot_sync(kFull, v[j].x != rx || v[j].y != ry), am.x, diff, div_);
