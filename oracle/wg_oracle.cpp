@@ -193,7 +193,7 @@ void wgo_reset_counters(wgo_engine* e) {
   std::fill(e->site.begin(), e->site.end(), wgo_site_counters{0, 0, 0, 0});
   e->seq = 0;
   e->ring.clear();  // profile and ring capacity are configuration and stay
-  e->t = wgo_telemetry_counters{0, 0, 0, 0, 0, 0, 0};
+  e->t = wgo_telemetry_counters{};  // every field zero
   e->have_first = false;
 }
 
