@@ -445,7 +445,7 @@ __global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 
   // (A short stream — fewer than 16 groups per warp — is dealt out statically, group = warp + k * warps: the tickets of
   // 3,000 warps that all start at once would queue on the one counter for longer than such a launch lasts.)
   const bool dyn = n_groups >= 16u * gridDim.x * kW;
-  uint32_t wnext = blockIdx.x * kW + warp, wleft = 0;
+  uint32_t wnext = warp * gridDim.x + blockIdx.x, wleft = 0;  // (static dealing: consecutive groups go to different SMs)
   const uint32_t tail_from = n_groups > 8u * gridDim.x * kW ? n_groups - 8u * gridDim.x * kW : 0u;
   unsigned int* const sched = p.sched;
   auto claim = [&]() __attribute__((always_inline)) -> uint32_t {
@@ -1142,7 +1142,7 @@ template <int MODE>
 cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
   const uint64_t n_groups = (p.n + 31) / 32;
   constexpr uint32_t W = MODE == MODE_FORWARD ? kWarpsFwd : kWarps;
-  const uint64_t want = (n_groups + W - 1) / W;
+  const uint64_t want = n_groups;  // a short stream is spread over all SMs, a few warps each, not packed into a few full CTAs
   const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) ? want : sm_count);
   const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= kMaxStageTgts;
   const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
