@@ -376,9 +376,12 @@ struct WarpCtr {
 // (compiled out of the ordinary launch).
 // ---------------------------------------------------------------------------------------------------
 template <int MODE, bool STAGED, bool TEL>
-__global__ void __launch_bounds__((MODE == MODE_FORWARD ? kWarpsFwd : kWarps) * 32, 1)
+__global__ void __launch_bounds__(((MODE == MODE_FORWARD && STAGED) ? kWarpsFwd : kWarps) * 32, 1)
     wg_check_kernel(const Params p, const uint32_t stage_bytes, const uint32_t site_bytes) {
-  constexpr uint32_t kW = MODE == MODE_FORWARD ? kWarpsFwd : kWarps;  // warps of this CTA
+  // warps of this CTA.  (The forward kernel that looks targets up in the hash index keeps the 20-warp shape: at 64
+  // registers it spills, and its lookups wait on DRAM, not on the shared-memory unit — measured on config 5's forward
+  // entry: 0.80 ms with 20 warps, 0.90 ms with 32.)
+  constexpr uint32_t kW = (MODE == MODE_FORWARD && STAGED) ? kWarpsFwd : kWarps;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint32_t lane, lanebit;
   asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
@@ -1141,10 +1144,10 @@ __global__ void wg_clear_allones_flags(SiteRec* recs, uint32_t n_sites) {
 template <int MODE>
 cudaError_t launch_mode(const Params& p, int sm_count, cudaStream_t st, uint64_t* launches) {
   const uint64_t n_groups = (p.n + 31) / 32;
-  constexpr uint32_t W = MODE == MODE_FORWARD ? kWarpsFwd : kWarps;
   const uint64_t want = n_groups;  // a short stream is spread over all SMs, a few warps each, not packed into a few full CTAs
   const int grid = static_cast<int>(want < static_cast<uint64_t>(sm_count) ? want : sm_count);
   const bool staged = MODE != MODE_SIGN && p.n_tgts > 0 && p.n_tgts <= kMaxStageTgts;
+  const uint32_t W = (MODE == MODE_FORWARD && staged) ? kWarpsFwd : kWarps;  // (the kernel's kW)
   const uint32_t stage_bytes = staged ? static_cast<uint32_t>((p.n_tgts * 8 + 15) & ~15ull) : 0u;
   // the per-site counter cache: the largest power-of-two slot count <= kMaxCacheSlots that fits beside the staged
   // targets (and no more than twice the policy needs); sign keeps no per-site counters
