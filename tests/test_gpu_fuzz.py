@@ -112,3 +112,43 @@ def test_random_policies_and_streams(seed, n_sites, n_tgts, n):
         if first is not None:
             assert all(int(first[f]) == int(of[f]) for f in B.VIOLATION_DTYPE.names)
         eng.close()
+
+
+@pytest.mark.parametrize("seed,n_sites,n_tgts,n", [(21, 300, 900, 20_011), (22, 4000, 9000, 20_011)])
+def test_random_policies_without_a_return_site(seed, n_sites, n_tgts, n):
+    """No protected-return site in the policy: wg_verify_continuations runs the forward kernel and must
+    still decide what the oracle's verify decides — unknown sites and empty masks included, tags ignored — on the staged
+    table (900 targets) and on the hash index (9,000), in every profile."""
+    rng = np.random.default_rng(seed)
+    kind, off, tg = random_policy(rng, n_sites, n_tgts)
+    ret = np.nonzero(kind == 0)[0]
+    kind[ret] = rng.choice(np.array([2, 3, 4, 5, 6], dtype=np.uint8), len(ret))  # (return sites own no targets: relabel freely)
+    assert not (kind == 0).any() and (kind == 1).any()
+    k0, k1 = int(rng.integers(0, 1 << 63)), int(rng.integers(0, 1 << 63))
+    hdr, val = random_events(rng, kind, off, tg, n)
+    tag = rng.integers(0, 1 << 63, size=(n, 32), dtype=np.uint64)
+    d_hdr, d_val, d_tag = to_dev(hdr), to_dev(val), to_dev(tag)
+    for flags in (0, B.WG_PROFILE_LOW_TELEMETRY, B.WG_PROFILE_SKIP_FORWARD, B.WG_PROFILE_SKIP_BACKWARD | B.WG_PROFILE_METADATA_INTEGRITY):
+        orc = oracle.Oracle(kind, off, tg, k0, k1, seed)
+        eng = B.Engine(0)
+        eng.wg_load_policy(kind, off, tg, k0, k1, seed)
+        orc.set_profile(flags)
+        eng.wg_set_profile(flags)
+        orc.set_ring_capacity(256)
+        eng.wg_set_ring_capacity(256)
+        assert not eng.wg_sign_continuations(d_hdr, d_val).any() and not orc.sign(hdr, val).any()
+        for mode in (1, 0):
+            o = orc.verify(hdr, val, tag, mode)
+            g = eng.wg_verify_continuations(d_hdr, d_val, d_tag, mode).cpu().numpy().view(np.uint32)
+            assert np.array_equal(g, o), (seed, flags, mode, np.nonzero((g != o).any(1))[0][:5])
+        gg, gs = eng.wg_read_counters()
+        og, os_ = orc.read_counters()
+        assert gg == og, {k: (gg[k], og[k]) for k in og if gg[k] != og[k]}
+        assert np.array_equal(gs, os_)
+        t, first, ring = eng.wg_read_telemetry(256)
+        assert t == orc.read_telemetry()
+        of = orc.read_first_violation()
+        assert (first is None) == (of is None)
+        if first is not None:
+            assert all(int(first[f]) == int(of[f]) for f in B.VIOLATION_DTYPE.names)
+        eng.close()
